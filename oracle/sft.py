@@ -1,0 +1,54 @@
+"""Oracle data SFTs by direct DFT and the plain inner products, fp64.  Test infrastructure.
+
+* ``sft_direct``        – Eq.(26): ``x~_a[k] = dt sum_j x_a[j] exp(-i 2 pi tau_j f_k)``,
+  ``tau_j = j dt``, ``f_k = k / T_SFT``, by explicit summation (a dense matrix product
+  with the exponent table, no FFT).
+* ``split_segments``    – P:157: disjoint segments of ``n_SFT = T_SFT/dt`` samples; a trailing
+  partial segment is dropped (reading A13).
+* ``time_domain_product`` – Eq.(1)/(14) P:20, P:149 for a flat PSD: ``(2 dt/S) sum_j x_j h_j``.
+* ``full_band_product`` – Eq.(1) discretised per SFT: ``4 df Re sum_k x~*_k h~_k / S_k`` over
+  ``1 <= k <= n/2-1`` (reading A6), optionally with DC and Nyquist at half weight,
+  which makes it equal to the time-domain product exactly (Parseval, pin P2).
+Pins: tests/test_oracle_sft.py (P1, P2, P4).
+"""
+import numpy as np
+
+
+def split_segments(x, n_sft):
+    """[N] -> [N_SFT][n_sft]; drops the trailing ``N mod n_sft`` samples (reading A13)."""
+    x = np.asarray(x, dtype=np.float64)
+    n_seg = x.shape[-1] // n_sft
+    return x[..., : n_seg * n_sft].reshape(x.shape[:-1] + (n_seg, n_sft))
+
+
+def dft_table(n, ks):
+    """exp(-2 pi i j k / n), j<n, k in ks; the exponent is reduced with exact integers."""
+    j = np.arange(n, dtype=np.int64)[:, None]
+    k = np.asarray(ks, dtype=np.int64)[None, :]
+    jk = (j * k) % n
+    return np.exp(-2j * np.pi * jk.astype(np.float64) / n)
+
+
+def sft_direct(segments, ks, dt):
+    """Eq.(26): [..., n] real segments -> [..., len(ks)] complex SFT bins (units: x * s)."""
+    segments = np.asarray(segments, dtype=np.float64)
+    n = segments.shape[-1]
+    return dt * (segments.astype(np.complex128) @ dft_table(n, ks))
+
+
+def time_domain_product(x, h, dt, S_flat):
+    """(2 dt / S) sum_j x_j h_j: Eq.(1) for a flat one-sided PSD, written in the time domain."""
+    return 2.0 * dt / S_flat * float(np.dot(np.asarray(x, np.float64), np.asarray(h, np.float64)))
+
+
+def full_band_product(xs, hs, S, df, ks, n, half_weight_edges=False):
+    """4 df Re sum_k conj(xs_k) hs_k / S_k over bins ``ks`` of an n-sample segment.
+
+    ``half_weight_edges=False`` keeps ``1 <= k <= n/2-1`` (reading A6);
+    ``True`` also takes k=0 and k=n/2 at half weight (the exact Parseval partner).
+    """
+    ks = np.asarray(ks)
+    w = np.where((ks >= 1) & (ks <= n // 2 - 1), 1.0, 0.0)
+    if half_weight_edges:
+        w = np.where((ks == 0) | (ks == n // 2), 0.5, w)
+    return 4.0 * df * float(np.sum(w * np.real(np.conj(xs) * hs) / S))
