@@ -1,0 +1,156 @@
+/* sft.h - C ABI of libsft_b200.so: the SFT inner product of arXiv:2502.11823 on one B200.
+ *
+ * Citations "P:NNN" are line numbers of the paper text; "DESIGN" is DESIGN.md in
+ * this repository (readings of the paper where it is silent or garbled).
+ *
+ * What the library computes (Eq.(20)-(35); discretised Eq.(1)):
+ *
+ *   ([x,h]) = 4 df Re sum_{c,a,k in B_a} conj(x~_{c,a,k}) h~_{c,a,k} / S_{c,a}(f_k)
+ *   ([h,h]) = 4 df    sum_{c,a,k in B_a} |h~_{c,a,k}|^2            / S_{c,a}(f_k)
+ *   h~_{c,a,k} = 1/2 T A_a R_{c,a} e^{i phi_a} F((f_a - f_k) T, fdot_a T^2)
+ *   F(a,b)     = int_0^1 exp(i pi (2 a s + b s^2)) ds          (Eq.(28), dimensionless)
+ *
+ * c = channel, a = SFT index (start t_a = t0 + a T), k = frequency bin (f_k = k/T,
+ * P:191), B_a = {k_c-K .. k_c+K} the truncated band around the signal, {A, phi, f,
+ * fdot}_a the four numbers per SFT of P:164 from a restricted TaylorT3 inspiral (0PN or
+ * 0PN+1PN; DESIGN W1), R_{c,a} the per-SFT complex detector response with
+ * Lambda z = Re[R z] (Eq.(5)-(6) P:80-85), S_{c,a}(f_k) = s_{c,a} S_c(f_k) the per-SFT noise
+ * PSD, gaps = missing SFTs.  Every step runs in CUDA kernels on the plan's
+ * device; there is no CPU fallback.
+ *
+ * Conventions: all functions return an sft_status and never throw, abort or touch errno.
+ * On error the outputs are untouched and sft_last_error(plan) describes the failure.
+ * The caller owns every pointer it passes; the plan copies what it keeps.  A plan is not
+ * thread-safe; distinct plans are independent.  Work is ordered on the plan's stream; calls
+ * with host pointers return after the results are on the host, calls with device pointers
+ * return after enqueueing (call sft_plan_sync or synchronise the stream yourself).
+ */
+#ifndef SFT_B200_H
+#define SFT_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SFT_MAX_CHANNELS 4
+#define SFT_NPARAM 8   /* doubles per template row, see sft_inner_products */
+#define SFT_MAX_K 128  /* largest accepted half-width of the band */
+
+typedef struct sft_plan sft_plan; /* opaque; owns all its device memory */
+
+typedef enum {
+  SFT_OK = 0,
+  SFT_EINVAL = 1,       /* NULL pointer or out-of-range argument            */
+  SFT_ESHAPE = 2,       /* inconsistent sizes (t_sft*fs not an integer, ..) */
+  SFT_ENODATA = 3,      /* a channel has not been loaded yet                */
+  SFT_EUNSUPPORTED = 4, /* valid request this build does not implement      */
+  SFT_ECUDA = 5,        /* CUDA runtime error (message in sft_last_error)   */
+  SFT_ENOMEM = 6        /* host or device allocation failed                 */
+} sft_status;
+
+enum { SFT_KERNEL_DIRICHLET = 0, /* F(a,0) = e^{i pi a} sinc(a), Eq.(B2)          */
+       SFT_KERNEL_FRESNEL = 1 }; /* F(a,b), Eq.(28)-(32) P:215-236                      */
+enum { SFT_WF_PN0 = 0,           /* Newtonian restricted TaylorT3 inspiral              */
+       SFT_WF_PN1 = 1 };         /* + 1PN phase and frequency terms                     */
+enum { SFT_PHASE_FP64 = 0,       /* phase/frequency track evaluated in fp64             */
+       SFT_PHASE_SPLIT32 = 1 };  /* track evaluated in double-float (2 x fp32) arithmetic */
+enum { SFT_RESP_NONE = 0,        /* R = 1                                               */
+       SFT_RESP_TABLE = 1,       /* R_{c,a} from sft_load_data's `response`             */
+       SFT_RESP_ANNUAL = 2 };    /* R_{c,a} = [1 + depth cos(2 pi t_a/period + psi_c + lambda)]
+                                    e^{i (chi_c + beta)}, (lambda, beta) per template    */
+enum { SFT_MEM_HOST = 0, SFT_MEM_DEVICE = 1 };
+
+/* Analysis set-up.  Zero-initialise, then fill. */
+typedef struct {
+  int32_t n_channels;  /* 1..SFT_MAX_CHANNELS                                            */
+  int64_t n_sft;       /* SFT slots per channel, gaps included                   */
+  double t_sft;        /* T_SFT [s]; t_sft*fs must be an integer n (samples per SFT)     */
+  double fs;           /* sampling rate [Hz]; bins k<1 and k>=n/2 never contribute (DESIGN A6) */
+  double t0;           /* start time of SFT 0 [s]                                        */
+  int32_t k_lo, k_hi;  /* stored band: bins k_lo <= k < k_hi                             */
+  int32_t K;           /* band half-width, 2K+1 bins per SFT; 0..SFT_MAX_K       */
+  int32_t kernel;      /* SFT_KERNEL_*                                                   */
+  int32_t waveform;    /* SFT_WF_*                                                       */
+  int32_t phase_path;  /* SFT_PHASE_*                                                    */
+  int32_t response;    /* SFT_RESP_*                                                     */
+  double f_lo, f_hi;   /* pair active iff f_lo <= f_a, f_a + fdot_a T <= f_hi, t_a + T < t_c (DESIGN A12) */
+  double f_ref;        /* amplitude reference: A_a = amp (f_a/f_ref)^(2/3)       */
+  double resp_period;  /* SFT_RESP_ANNUAL: modulation period [s]                          */
+  double resp_depth;   /* SFT_RESP_ANNUAL: modulation depth                               */
+  double resp_psi[SFT_MAX_CHANNELS]; /* SFT_RESP_ANNUAL: amplitude-modulation phase per channel */
+  double resp_chi[SFT_MAX_CHANNELS]; /* SFT_RESP_ANNUAL: response phase per channel             */
+  int32_t device;      /* CUDA device ordinal                                             */
+  void *stream;        /* cudaStream_t to order work on, or NULL for the legacy default stream */
+} sft_plan_desc;
+
+/* Creates a plan: validates `desc`, selects the device, allocates the (empty) data-SFT store
+ * [n_channels][n_sft][k_hi-k_lo] complex64 + weight tables in device memory (SFTs are
+ * "computed once ... reused").  *out is set only on SFT_OK. */
+sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out);
+
+/* Frees the plan and all device memory it owns.  NULL is accepted. */
+sft_status sft_plan_destroy(sft_plan *plan);
+
+/* Loads one channel of data SFTs (Eq.(26)) and its noise description, and whitens it
+ * on the device (Eq.(15) P:153 moves 1/S onto the data):
+ *   sft_bins   complex64 interleaved (re,im), [n_sft][k_hi-k_lo], bin fastest, units strain*s
+ *   psd_scale  [n_sft] s_{c,a} of S_{c,a}(f_k) = s_{c,a} S_c(f_k); <= 0 or non-finite => gap
+ *   psd_shape  [k_hi-k_lo] S_c(f_k) > 0 (one-sided PSD); NULL => 1
+ *   response   complex64 interleaved [n_sft] R_{c,a}; required iff plan response == SFT_RESP_TABLE, else ignored/NULL
+ *   mem        SFT_MEM_HOST or SFT_MEM_DEVICE: where ALL the non-NULL pointers of this call live
+ * May be called again for the same channel to replace its data. */
+sft_status sft_load_data(sft_plan *plan, int32_t channel, const float *sft_bins,
+                         const double *psd_scale, const double *psd_shape,
+                         const float *response, int32_t mem);
+
+/* ([x,h]) and ([h,h]) for n_templates templates (Eq.(35) P:259 with ONE df, DESIGN A1).
+ *   params  [n_templates][SFT_NPARAM] doubles, row-major:
+ *           m_chirp [Msun], eta, t_c [s], phi_c [rad], amp, lambda [rad], beta [rad], reserved(0)
+ *   xh, hh  [n_templates] doubles (required)
+ *   xh_im   [n_templates] or NULL: imaginary part of the complex sum (for the phase-maximised
+ *           statistic Eq.(7)-(9) P:97-101)
+ *   kc_out  [n_templates][n_channels][n_sft] int32 or NULL: the selected central bin k_c of
+ *           every active pair whose SFT is present, -1 otherwise (DESIGN A5)
+ *   mem     where params and all outputs live (SFT_MEM_HOST / SFT_MEM_DEVICE)
+ * n_templates == 0 is SFT_OK and touches nothing.  SFT_ENODATA unless every channel is loaded. */
+sft_status sft_inner_products(sft_plan *plan, int64_t n_templates, const double *params,
+                              double *xh, double *hh, double *xh_im, int32_t *kc_out,
+                              int32_t mem);
+
+/* Early-warning variant ("accumulating the result over time"): inclusive prefix
+ * sums over the SFT index of the per-SFT terms (summed over channels; gaps and inactive SFTs
+ * add 0), carried in fp64 and stored in fp32:
+ *   snr     [n_templates][n_sft] floats, SFT index fastest: cum_xh / sqrt(cum_hh), 0 where cum_hh == 0
+ *   cum_xh, cum_hh  same shape, or NULL
+ * At least one of the three outputs must be non-NULL. */
+sft_status sft_cumulative_snr(sft_plan *plan, int64_t n_templates, const double *params,
+                              float *snr, float *cum_xh, float *cum_hh, int32_t mem);
+
+/* Blocks until all work enqueued on the plan's stream has finished. */
+sft_status sft_plan_sync(sft_plan *plan);
+
+/* Number of kernels this plan has launched so far (for launch accounting in benchmarks). */
+int64_t sft_plan_launch_count(const sft_plan *plan);
+
+/* Duration [ms] of the most recent main (fused waveform+coefficient+contraction) kernel launch
+ * of this plan, from CUDA events recorded on the plan's stream around that launch; blocks
+ * until that launch has finished.  < 0 if nothing has been launched. */
+double sft_plan_last_kernel_ms(sft_plan *plan);
+
+/* Tuning knob: SFTs per block along the time axis (0 = automatic).  Results do not depend on it
+ * beyond fp64 summation order. */
+sft_status sft_plan_set_chunk(sft_plan *plan, int32_t sfts_per_block);
+
+/* Message for the last error of this plan ("" if none).  With plan == NULL: the message of the
+ * last failed sft_plan_create in this thread.  The pointer stays valid until the next call. */
+const char *sft_last_error(const sft_plan *plan);
+
+/* Library version string. */
+const char *sft_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SFT_B200_H */

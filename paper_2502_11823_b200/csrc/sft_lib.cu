@@ -1,0 +1,436 @@
+// sft_lib.cu - host side of libsft_b200.so: the C ABI of include/sft.h.  Argument checking,
+// device-memory ownership, launch geometry; all arithmetic of the method is in sft_kernels.cuh.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+#include "../../include/sft.h"
+#include "sft_kernels.cuh"
+
+#define SFT_API extern "C" __attribute__((visibility("default")))
+
+using sftk::KParams;
+
+struct sft_plan {
+  sft_plan_desc d;
+  int nb = 0;             // stored bins per SFT
+  int n_samp = 0;         // samples per SFT
+  int kv_lo = 0, kv_hi = 0;
+  cudaStream_t stream = nullptr;
+  float2 *D = nullptr;    // [C][n_sft][nb]
+  float *ub2 = nullptr;   // [C][nb]
+  float *us2 = nullptr;   // [C][n_sft]
+  float2 *rtab = nullptr; // [C][n_sft]
+  double sigma[SFT_MAX_CHANNELS] = {0, 0, 0, 0};
+  bool loaded[SFT_MAX_CHANNELS] = {false, false, false, false};
+  // scratch, grown on demand
+  double *part = nullptr; size_t part_bytes = 0;
+  double *d_params = nullptr; size_t params_bytes = 0;
+  void *d_out = nullptr; size_t out_bytes = 0;         // staging for host outputs
+  float *loc = nullptr; size_t loc_bytes = 0;          // cumulative: chunk-local prefixes
+  int chunk_user = 0;
+  long long launches = 0;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool timed = false;
+  char err[512] = {0};
+};
+
+static thread_local char g_create_err[512] = {0};
+
+static sft_status fail(sft_plan *p, sft_status st, const char *fmt, ...) {
+  char *buf = p ? p->err : g_create_err;
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, 512, fmt, ap);
+  va_end(ap);
+  return st;
+}
+
+#define CU(p, call)                                                                         \
+  do {                                                                                      \
+    cudaError_t e_ = (call);                                                                \
+    if (e_ != cudaSuccess)                                                                  \
+      return fail(p, e_ == cudaErrorMemoryAllocation ? SFT_ENOMEM : SFT_ECUDA, "%s: %s", #call, \
+                  cudaGetErrorString(e_));                                                  \
+  } while (0)
+
+static sft_status grow(sft_plan *p, void **ptr, size_t *have, size_t need) {
+  if (*have >= need) return SFT_OK;
+  if (*ptr) { CU(p, cudaFree(*ptr)); *ptr = nullptr; *have = 0; }
+  CU(p, cudaMalloc(ptr, need));
+  *have = need;
+  return SFT_OK;
+}
+
+SFT_API const char *sft_version(void) { return "sft_b200 0.1 (sm_100a)"; }
+
+SFT_API const char *sft_last_error(const sft_plan *plan) { return plan ? plan->err : g_create_err; }
+
+SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
+  g_create_err[0] = 0;
+  if (!desc || !out) return fail(nullptr, SFT_EINVAL, "sft_plan_create: NULL argument");
+  const sft_plan_desc &d = *desc;
+  if (d.n_channels < 1 || d.n_channels > SFT_MAX_CHANNELS)
+    return fail(nullptr, SFT_EINVAL, "n_channels=%d outside 1..%d", d.n_channels, SFT_MAX_CHANNELS);
+  if (d.n_sft < 1 || d.n_sft > (1ll << 30)) return fail(nullptr, SFT_EINVAL, "n_sft=%lld out of range", (long long)d.n_sft);
+  if (!(d.t_sft > 0.0) || !(d.fs > 0.0) || !isfinite(d.t0)) return fail(nullptr, SFT_EINVAL, "t_sft, fs must be > 0 and t0 finite");
+  const double n = d.t_sft * d.fs;
+  if (fabs(n - nearbyint(n)) > 1e-9 * fmax(1.0, n) || n < 2.0 || n > 2e9)
+    return fail(nullptr, SFT_ESHAPE, "t_sft*fs = %.12g is not an integer number of samples (P:157)", n);
+  if (d.k_lo < 0 || d.k_hi <= d.k_lo) return fail(nullptr, SFT_ESHAPE, "stored band [k_lo=%d, k_hi=%d) is empty or negative", d.k_lo, d.k_hi);
+  if (d.K < 0 || d.K > SFT_MAX_K) return fail(nullptr, SFT_EINVAL, "K=%d outside 0..%d", d.K, SFT_MAX_K);
+  if (d.kernel != SFT_KERNEL_DIRICHLET && d.kernel != SFT_KERNEL_FRESNEL) return fail(nullptr, SFT_EINVAL, "unknown kernel %d", d.kernel);
+  if (d.waveform != SFT_WF_PN0 && d.waveform != SFT_WF_PN1) return fail(nullptr, SFT_EINVAL, "unknown waveform %d", d.waveform);
+  if (d.phase_path != SFT_PHASE_FP64 && d.phase_path != SFT_PHASE_SPLIT32) return fail(nullptr, SFT_EINVAL, "unknown phase_path %d", d.phase_path);
+  if (d.phase_path == SFT_PHASE_SPLIT32) return fail(nullptr, SFT_EUNSUPPORTED, "SFT_PHASE_SPLIT32 is not implemented in this build");
+  if (d.response < SFT_RESP_NONE || d.response > SFT_RESP_ANNUAL) return fail(nullptr, SFT_EINVAL, "unknown response %d", d.response);
+  if (!(d.f_ref > 0.0)) return fail(nullptr, SFT_EINVAL, "f_ref must be > 0");
+  if (!(d.f_hi >= d.f_lo)) return fail(nullptr, SFT_EINVAL, "need f_lo <= f_hi");
+  if (d.response == SFT_RESP_ANNUAL && !(d.resp_period > 0.0)) return fail(nullptr, SFT_EINVAL, "resp_period must be > 0");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess) return fail(nullptr, SFT_ECUDA, "cudaGetDeviceCount: %s", cudaGetErrorString(e));
+  if (d.device < 0 || d.device >= ndev) return fail(nullptr, SFT_EINVAL, "device %d not in 0..%d", d.device, ndev - 1);
+  e = cudaSetDevice(d.device);
+  if (e != cudaSuccess) return fail(nullptr, SFT_ECUDA, "cudaSetDevice: %s", cudaGetErrorString(e));
+
+  sft_plan *p = new (std::nothrow) sft_plan();
+  if (!p) return fail(nullptr, SFT_ENOMEM, "out of host memory");
+  p->d = d;
+  p->nb = d.k_hi - d.k_lo;
+  p->n_samp = (int)nearbyint(n);
+  p->kv_lo = d.k_lo > 1 ? d.k_lo : 1;                                   // DESIGN A6: 1 <= k <= n/2-1
+  p->kv_hi = d.k_hi < p->n_samp / 2 ? d.k_hi : p->n_samp / 2;
+  p->stream = (cudaStream_t)d.stream;
+  const size_t C = d.n_channels, N = d.n_sft, nb = p->nb;
+  sft_status st = SFT_OK;
+  auto alloc = [&](void **ptr, size_t bytes) {
+    if (st != SFT_OK) return;
+    cudaError_t e2 = cudaMalloc(ptr, bytes);
+    if (e2 != cudaSuccess) st = fail(nullptr, SFT_ENOMEM, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e2));
+  };
+  alloc((void **)&p->D, C * N * nb * sizeof(float2));
+  alloc((void **)&p->ub2, C * nb * sizeof(float));
+  alloc((void **)&p->us2, C * N * sizeof(float));
+  alloc((void **)&p->rtab, C * N * sizeof(float2));
+  if (st == SFT_OK) {
+    cudaError_t e2 = cudaEventCreate(&p->ev0);
+    if (e2 == cudaSuccess) e2 = cudaEventCreate(&p->ev1);
+    if (e2 != cudaSuccess) st = fail(nullptr, SFT_ECUDA, "cudaEventCreate: %s", cudaGetErrorString(e2));
+  }
+  if (st == SFT_OK && d.response == SFT_RESP_ANNUAL) {
+    for (size_t c = 0; c < C; ++c) {
+      sftk::sft_annual_table_kernel<<<(unsigned)((N + 255) / 256), 256, 0, p->stream>>>(
+          (int)N, d.t0, d.t_sft, d.resp_period, d.resp_psi[c], p->rtab + c * N);
+      p->launches++;
+    }
+    cudaError_t e2 = cudaGetLastError();
+    if (e2 != cudaSuccess) st = fail(nullptr, SFT_ECUDA, "annual table launch: %s", cudaGetErrorString(e2));
+  }
+  if (st != SFT_OK) {
+    char keep[512];
+    memcpy(keep, g_create_err, 512);
+    sft_plan_destroy(p);
+    memcpy(g_create_err, keep, 512);
+    return st;
+  }
+  *out = p;
+  return SFT_OK;
+}
+
+SFT_API sft_status sft_plan_destroy(sft_plan *p) {
+  if (!p) return SFT_OK;
+  cudaSetDevice(p->d.device);
+  cudaStreamSynchronize(p->stream);
+  cudaFree(p->D); cudaFree(p->ub2); cudaFree(p->us2); cudaFree(p->rtab);
+  cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->loc);
+  if (p->ev0) cudaEventDestroy(p->ev0);
+  if (p->ev1) cudaEventDestroy(p->ev1);
+  delete p;
+  return SFT_OK;
+}
+
+SFT_API sft_status sft_plan_sync(sft_plan *p) {
+  if (!p) return SFT_EINVAL;
+  CU(p, cudaSetDevice(p->d.device));
+  CU(p, cudaStreamSynchronize(p->stream));
+  return SFT_OK;
+}
+
+SFT_API int64_t sft_plan_launch_count(const sft_plan *p) { return p ? p->launches : 0; }
+
+SFT_API double sft_plan_last_kernel_ms(sft_plan *p) {
+  if (!p || !p->timed) return -1.0;
+  if (cudaSetDevice(p->d.device) != cudaSuccess) return -1.0;
+  if (cudaEventSynchronize(p->ev1) != cudaSuccess) return -1.0;
+  float ms = -1.f;
+  if (cudaEventElapsedTime(&ms, p->ev0, p->ev1) != cudaSuccess) return -1.0;
+  return (double)ms;
+}
+
+SFT_API sft_status sft_plan_set_chunk(sft_plan *p, int32_t c) {
+  if (!p) return SFT_EINVAL;
+  if (c < 0) return fail(p, SFT_EINVAL, "sfts_per_block must be >= 0");
+  p->chunk_user = c;
+  return SFT_OK;
+}
+
+SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_bins, const double *psd_scale,
+                                    const double *psd_shape, const float *response, int32_t mem) {
+  if (!p) return SFT_EINVAL;
+  p->err[0] = 0;
+  if (channel < 0 || channel >= p->d.n_channels) return fail(p, SFT_EINVAL, "channel %d outside 0..%d", channel, p->d.n_channels - 1);
+  if (!sft_bins || !psd_scale) return fail(p, SFT_EINVAL, "sft_bins and psd_scale are required");
+  if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(p, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
+  if (p->d.response == SFT_RESP_TABLE && !response) return fail(p, SFT_EINVAL, "response table required by SFT_RESP_TABLE");
+  CU(p, cudaSetDevice(p->d.device));
+  const size_t N = p->d.n_sft, nb = p->nb;
+  // PSD shape on the host: reference level S_ref = min S over the valid stored bins
+  std::vector<double> shape;
+  double S_ref = 1.0;
+  if (psd_shape) {
+    shape.resize(nb);
+    if (mem == SFT_MEM_DEVICE) {
+      CU(p, cudaMemcpyAsync(shape.data(), psd_shape, nb * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+      CU(p, cudaStreamSynchronize(p->stream));
+    } else {
+      memcpy(shape.data(), psd_shape, nb * sizeof(double));
+    }
+    S_ref = INFINITY;
+    for (size_t j = 0; j < nb; ++j) {
+      const int k = p->d.k_lo + (int)j;
+      if (k < p->kv_lo || k >= p->kv_hi) continue;
+      if (!(shape[j] > 0.0) || !isfinite(shape[j])) return fail(p, SFT_EINVAL, "psd_shape[%zu] = %g is not a positive finite PSD", j, shape[j]);
+      if (shape[j] < S_ref) S_ref = shape[j];
+    }
+    if (!isfinite(S_ref)) S_ref = 1.0;   // no valid bin in the stored band: everything contributes 0
+  }
+  const float2 *d_raw = nullptr;
+  const double *d_scale = nullptr, *d_shape = nullptr;
+  void *tmp = nullptr;
+  if (mem == SFT_MEM_HOST) {
+    const size_t b_raw = N * nb * sizeof(float2), b_scale = N * sizeof(double), b_shape = psd_shape ? nb * sizeof(double) : 0;
+    const size_t o_scale = (b_raw + 255) & ~size_t(255), o_shape = (o_scale + b_scale + 255) & ~size_t(255);
+    cudaError_t e = cudaMalloc(&tmp, o_shape + b_shape + 256);
+    if (e != cudaSuccess) return fail(p, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(e));
+    char *base = (char *)tmp;
+    cudaMemcpyAsync(base, sft_bins, b_raw, cudaMemcpyHostToDevice, p->stream);
+    cudaMemcpyAsync(base + o_scale, psd_scale, b_scale, cudaMemcpyHostToDevice, p->stream);
+    if (psd_shape) cudaMemcpyAsync(base + o_shape, psd_shape, b_shape, cudaMemcpyHostToDevice, p->stream);
+    if (p->d.response == SFT_RESP_TABLE)
+      cudaMemcpyAsync(p->rtab + (size_t)channel * N, response, N * sizeof(float2), cudaMemcpyHostToDevice, p->stream);
+    d_raw = (const float2 *)base;
+    d_scale = (const double *)(base + o_scale);
+    d_shape = psd_shape ? (const double *)(base + o_shape) : nullptr;
+  } else {
+    d_raw = (const float2 *)sft_bins;
+    d_scale = psd_scale;
+    d_shape = psd_shape;
+    if (p->d.response == SFT_RESP_TABLE)
+      cudaMemcpyAsync(p->rtab + (size_t)channel * N, response, N * sizeof(float2), cudaMemcpyDeviceToDevice, p->stream);
+  }
+  sftk::sft_whiten_kernel<<<(unsigned)N, 128, 0, p->stream>>>(d_raw, d_scale, d_shape, (int)N, (int)nb, p->d.k_lo, p->kv_lo,
+                                                             p->kv_hi, p->d.t_sft, S_ref, p->D + (size_t)channel * N * nb,
+                                                             p->us2 + (size_t)channel * N);
+  sftk::sft_ub2_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, p->stream>>>(d_shape, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi, S_ref,
+                                                                          p->ub2 + (size_t)channel * nb);
+  p->launches += 2;
+  cudaError_t e = cudaGetLastError();
+  cudaError_t e2 = cudaStreamSynchronize(p->stream);
+  if (tmp) cudaFree(tmp);
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "whiten launch: %s", cudaGetErrorString(e));
+  if (e2 != cudaSuccess) return fail(p, SFT_ECUDA, "whiten: %s", cudaGetErrorString(e2));
+  p->sigma[channel] = sqrt(p->d.t_sft / S_ref);
+  p->loaded[channel] = true;
+  return SFT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+static void fill_kparams(const sft_plan *p, KParams &k) {
+  memset(&k, 0, sizeof(k));
+  k.C = p->d.n_channels;
+  k.n_sft = (int)p->d.n_sft;
+  k.nb = p->nb;
+  k.k_lo = p->d.k_lo;
+  k.kv_lo = p->kv_lo;
+  k.kv_hi = p->kv_hi;
+  k.K = p->d.K;
+  k.kernel = p->d.kernel;
+  k.pn1 = p->d.waveform == SFT_WF_PN1;
+  k.response = p->d.response;
+  k.T = p->d.t_sft;
+  k.t0 = p->d.t0;
+  k.f_loT = p->d.f_lo * p->d.t_sft;
+  k.f_hiT = p->d.f_hi * p->d.t_sft;
+  k.inv_fref = 1.0 / p->d.f_ref;
+  for (int c = 0; c < SFT_MAX_CHANNELS; ++c) {
+    k.sigma[c] = p->sigma[c];
+    k.chi[c] = p->d.resp_chi[c];
+  }
+  k.depth = (float)p->d.resp_depth;
+  k.D = p->D;
+  k.ub2 = p->ub2;
+  k.us2 = p->us2;
+  k.rtab = p->rtab;
+}
+
+template <int MODE>
+static cudaError_t launch_main(sft_plan *p, const KParams &k) {
+  dim3 grid((unsigned)((k.nT + sftk::TILE - 1) / sftk::TILE), (unsigned)k.n_chunks);
+  dim3 block(sftk::TILE);
+  cudaEventRecord(p->ev0, p->stream);
+#define SFT_LAUNCH(KT, CT) sftk::sft_main_kernel<KT, CT, MODE><<<grid, block, 0, p->stream>>>(k)
+  const int C = k.C;
+  if (C == 1) {
+    switch (k.K) {
+      case 4: SFT_LAUNCH(4, 1); break;
+      case 8: SFT_LAUNCH(8, 1); break;
+      case 16: SFT_LAUNCH(16, 1); break;
+      default: SFT_LAUNCH(0, 1); break;
+    }
+  } else if (C == 2) {
+    switch (k.K) {
+      case 8: SFT_LAUNCH(8, 2); break;
+      case 16: SFT_LAUNCH(16, 2); break;
+      default: SFT_LAUNCH(0, 2); break;
+    }
+  } else {
+    SFT_LAUNCH(0, sftk::MAXC);
+  }
+#undef SFT_LAUNCH
+  cudaEventRecord(p->ev1, p->stream);
+  p->timed = true;
+  p->launches++;
+  return cudaGetLastError();
+}
+
+static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t mem, KParams &k, bool cumulative) {
+  for (int c = 0; c < p->d.n_channels; ++c)
+    if (!p->loaded[c]) return fail(p, SFT_ENODATA, "channel %d has no data (call sft_load_data)", c);
+  if (nT > (1ll << 31) - 1) return fail(p, SFT_EINVAL, "n_templates too large");
+  if (cumulative && (double)nT * (double)p->d.n_sft > 4.0e10) return fail(p, SFT_EINVAL, "cumulative output too large");
+  CU(p, cudaSetDevice(p->d.device));
+  fill_kparams(p, k);
+  k.nT = nT;
+  int chunk = p->chunk_user > 0 ? p->chunk_user : 64;
+  if (cumulative) chunk = ((chunk + 31) / 32) * 32;
+  if (chunk > k.n_sft) chunk = cumulative ? ((k.n_sft + 31) / 32) * 32 : k.n_sft;
+  k.chunk = chunk;
+  k.n_chunks = (k.n_sft + chunk - 1) / chunk;
+  if (k.n_chunks > 65535) {
+    k.chunk = ((k.n_sft + 65534) / 65535 + 31) / 32 * 32;
+    k.n_chunks = (k.n_sft + k.chunk - 1) / k.chunk;
+  }
+  sft_status st = grow(p, (void **)&p->part, &p->part_bytes, (size_t)k.n_chunks * 3 * nT * sizeof(double));
+  if (st != SFT_OK) return st;
+  k.part = p->part;
+  if (mem == SFT_MEM_HOST) {
+    st = grow(p, (void **)&p->d_params, &p->params_bytes, (size_t)nT * SFT_NPARAM * sizeof(double));
+    if (st != SFT_OK) return st;
+    CU(p, cudaMemcpyAsync(p->d_params, params, (size_t)nT * SFT_NPARAM * sizeof(double), cudaMemcpyHostToDevice, p->stream));
+    k.params = p->d_params;
+  } else {
+    k.params = params;
+  }
+  return SFT_OK;
+}
+
+SFT_API sft_status sft_inner_products(sft_plan *p, int64_t nT, const double *params, double *xh, double *hh,
+                                         double *xh_im, int32_t *kc_out, int32_t mem) {
+  if (!p) return SFT_EINVAL;
+  p->err[0] = 0;
+  if (nT < 0) return fail(p, SFT_EINVAL, "n_templates < 0");
+  if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(p, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
+  if (nT == 0) return SFT_OK;
+  if (!params || !xh || !hh) return fail(p, SFT_EINVAL, "params, xh and hh are required");
+  KParams k;
+  sft_status st = prepare(p, nT, params, mem, k, false);
+  if (st != SFT_OK) return st;
+  const size_t C = p->d.n_channels, N = p->d.n_sft;
+  double *d_xh = xh, *d_hh = hh, *d_xi = xh_im;
+  int *d_kc = kc_out;
+  if (mem == SFT_MEM_HOST) {
+    const size_t b_vec = (size_t)nT * sizeof(double);
+    const size_t b_kc = kc_out ? (size_t)nT * C * N * sizeof(int) : 0;
+    st = grow(p, &p->d_out, &p->out_bytes, 3 * b_vec + b_kc + 256);
+    if (st != SFT_OK) return st;
+    d_xh = (double *)p->d_out;
+    d_hh = d_xh + nT;
+    d_xi = d_hh + nT;
+    d_kc = kc_out ? (int *)(d_xi + nT) : nullptr;
+  }
+  k.kc_out = d_kc;
+  cudaError_t e = launch_main<0>(p, k);
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
+  sftk::sft_reduce_kernel<<<(unsigned)((nT + 255) / 256), 256, 0, p->stream>>>(p->part, nT, k.n_chunks, d_xh, d_hh, d_xi);
+  p->launches++;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "reduce kernel launch: %s", cudaGetErrorString(e));
+  if (mem == SFT_MEM_HOST) {
+    // results go to caller memory only after the stream finished without error
+    std::vector<double> h(3 * (size_t)nT);
+    CU(p, cudaMemcpyAsync(h.data(), d_xh, 3 * (size_t)nT * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
+    memcpy(xh, h.data(), (size_t)nT * sizeof(double));
+    memcpy(hh, h.data() + nT, (size_t)nT * sizeof(double));
+    if (xh_im) memcpy(xh_im, h.data() + 2 * nT, (size_t)nT * sizeof(double));
+    if (kc_out) {
+      CU(p, cudaMemcpyAsync(kc_out, d_kc, (size_t)nT * C * N * sizeof(int), cudaMemcpyDeviceToHost, p->stream));
+      CU(p, cudaStreamSynchronize(p->stream));
+    }
+  }
+  return SFT_OK;
+}
+
+SFT_API sft_status sft_cumulative_snr(sft_plan *p, int64_t nT, const double *params, float *snr, float *cum_xh,
+                                         float *cum_hh, int32_t mem) {
+  if (!p) return SFT_EINVAL;
+  p->err[0] = 0;
+  if (nT < 0) return fail(p, SFT_EINVAL, "n_templates < 0");
+  if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(p, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
+  if (nT == 0) return SFT_OK;
+  if (!params) return fail(p, SFT_EINVAL, "params is required");
+  if (!snr && !cum_xh && !cum_hh) return fail(p, SFT_EINVAL, "at least one of snr, cum_xh, cum_hh must be non-NULL");
+  KParams k;
+  sft_status st = prepare(p, nT, params, mem, k, true);
+  if (st != SFT_OK) return st;
+  const size_t N = p->d.n_sft, mat = (size_t)nT * N * sizeof(float);
+  // chunk-local prefixes: written into cum_xh/cum_hh when the caller gave device buffers, else scratch
+  float *d_snr = snr, *d_cx = cum_xh, *d_ch = cum_hh;
+  int n_out = (snr != nullptr) + (cum_xh != nullptr) + (cum_hh != nullptr);
+  if (mem == SFT_MEM_HOST) {
+    st = grow(p, &p->d_out, &p->out_bytes, (size_t)n_out * mat);
+    if (st != SFT_OK) return st;
+    float *q = (float *)p->d_out;
+    d_snr = snr ? q : nullptr; if (snr) q += (size_t)nT * N;
+    d_cx = cum_xh ? q : nullptr; if (cum_xh) q += (size_t)nT * N;
+    d_ch = cum_hh ? q : nullptr;
+  }
+  const int n_loc = (d_cx ? 0 : 1) + (d_ch ? 0 : 1);
+  if (n_loc) {
+    st = grow(p, (void **)&p->loc, &p->loc_bytes, (size_t)n_loc * mat);
+    if (st != SFT_OK) return st;
+  }
+  k.loc_xh = d_cx ? d_cx : p->loc;
+  k.loc_hh = d_ch ? d_ch : (d_cx ? p->loc : p->loc + (size_t)nT * N);
+  cudaError_t e = launch_main<1>(p, k);
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
+  sftk::sft_scan_chunks_kernel<<<(unsigned)((nT + 255) / 256), 256, 0, p->stream>>>(p->part, nT, k.n_chunks);
+  dim3 fgrid((unsigned)((N + 255) / 256 < 64 ? (N + 255) / 256 : 64), (unsigned)(nT < 65535 ? nT : 65535));
+  sftk::sft_fixup_kernel<<<fgrid, 256, 0, p->stream>>>(p->part, nT, (int)N, k.chunk, k.loc_xh, k.loc_hh, d_snr, d_cx, d_ch);
+  p->launches += 2;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "scan/fixup launch: %s", cudaGetErrorString(e));
+  if (mem == SFT_MEM_HOST) {
+    CU(p, cudaStreamSynchronize(p->stream));
+    if (snr) CU(p, cudaMemcpyAsync(snr, d_snr, mat, cudaMemcpyDeviceToHost, p->stream));
+    if (cum_xh) CU(p, cudaMemcpyAsync(cum_xh, d_cx, mat, cudaMemcpyDeviceToHost, p->stream));
+    if (cum_hh) CU(p, cudaMemcpyAsync(cum_hh, d_ch, mat, cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
+  }
+  return SFT_OK;
+}
