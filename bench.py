@@ -1,0 +1,346 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the SFT inner-product hot path on B200 (driver contract in DESIGN.md §8).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+One "step" = one pass of the whole hot path (waveform -> bin selection -> kernel coefficients ->
+response -> contraction -> reduction over SFTs) over one batch of synthetic
+input: ``sft_inner_products`` for the full template bank of the workload.  Default workload:
+BASELINE.json configs[1] ("config2-F": ET-like BNS bank, 4096 templates x 10,800 SFT slots, 10 %
+gaps, K = +-8 bins, Fresnel kernel, 0PN+1PN, complex64 data), the config the metric is quoted on.
+
+metric  = active template-SFT(-channel) pairs per second, whole job (sum over ranks / max time).
+value   : inputs resident in HBM, device-side CUDA-event time per step, L2 flushed between steps.
+e2e     : same call with HOST buffers (pinned params in, results out) through the C ABI; the
+          host<->device copies are inside the timed region.
+roofline: the fused main kernel against the ALU bound derived in DESIGN.md §7.
+cpu_baseline / --impl reference: the fp64 oracle (oracle/, as it stands) on the host cores, on a
+          bounded sample of the same workload.
+
+Under torchrun (N > 1) every rank runs the same data store with its own template shard (weak
+scaling, no data-path collective: templates are independent).
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "template-SFT inner products/s (<x,h>,<h,h>)"
+UNIT = "template-SFT pairs/s"
+
+
+# ---------------------------------------------------------------------------------------------
+def make_workload(name, rank=0, n_templates=None, n_sft=None, K=None):
+    from paper_2502_11823_b200 import workloads as wl
+    if name == "config1":
+        return wl.config1(n_templates=n_templates or 64)
+    if name == "config2":
+        kw = dict(n_templates=n_templates or 4096, bank_seed=5 + 1000 * rank)
+        if n_sft:
+            kw["n_sft"] = n_sft
+        if K is not None:
+            kw["K"] = K
+        return wl.config2(**kw)
+    if name == "config3":
+        return wl.config3(n_templates=n_templates or 16384, bank_seed=6 + 1000 * rank)
+    if name == "config4":
+        return wl.config4(n_templates=n_templates or 65536)
+    raise SystemExit("unknown workload %r" % name)
+
+
+def oracle_objects(w):
+    from oracle import inner as oin
+    plan = oin.Plan(**w.desc)
+    store = oin.Store(bins=w.bins.astype(np.complex128), psd_scale=w.psd_scale, psd_shape=w.psd_shape,
+                      response=None if w.response is None else w.response.astype(np.complex128))
+    return oin, plan, store
+
+
+def time_oracle(w, budget_s=12.0, max_templates=None):
+    """Times oracle.inner.inner_products (as it stands) on the first n templates of the workload,
+    n chosen so the run takes about ``budget_s`` seconds.  Returns (pairs/s, n, seconds, active pairs)."""
+    oin, plan, store = oracle_objects(w)
+    t0 = time.perf_counter()
+    r = oin.inner_products(plan, store, w.params[:1])
+    t1 = time.perf_counter() - t0
+    n = int(max(1, min(w.n_templates if max_templates is None else max_templates, budget_s / max(t1, 1e-6))))
+    t0 = time.perf_counter()
+    r = oin.inner_products(plan, store, w.params[:n])
+    dt = time.perf_counter() - t0
+    pairs = int((r["kc"] >= 0).sum())
+    return pairs / dt, n, dt, pairs
+
+
+def cores_used():
+    """Threads the oracle actually uses: it is single-threaded numpy elementwise code (no BLAS call
+    on its hot path), so 1; the number of host cores available is reported beside it."""
+    return 1
+
+
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+    def __init__(self, index, period=0.01):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.period, self._stop, self._th = period, threading.Event(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {getattr(nv, k): v for k, v in (
+            ("nvmlClocksEventReasonHwSlowdown", "hw_slowdown"),
+            ("nvmlClocksThrottleReasonHwSlowdown", "hw_slowdown"),
+            ("nvmlClocksThrottleReasonHwThermalSlowdown", "hw_thermal_slowdown"),
+            ("nvmlClocksThrottleReasonSwThermalSlowdown", "sw_thermal_slowdown"),
+            ("nvmlClocksThrottleReasonSwPowerCap", "sw_power_cap")) if hasattr(nv, k)}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def start(self):
+        if self.nv is not None:
+            self._th = threading.Thread(target=self._run, daemon=True)
+            self._th.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._th:
+            self._th.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------
+def run_reference(args, rank, world):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    w = make_workload(args.workload, 0, args.templates, args.n_sft, args.K)
+    oin, plan, store = oracle_objects(w)
+    # one step = a bounded sample: n_ref templates x all SFTs, sized from a probe so that the
+    # whole run (steps + warmup) ends within a few minutes
+    t0 = time.perf_counter()
+    oin.inner_products(plan, store, w.params[:1])
+    t1 = time.perf_counter() - t0
+    total = args.steps + args.warmup
+    n_ref = int(max(1, min(w.n_templates, 120.0 / total / max(t1, 1e-6), 64)))
+    P = w.params[:n_ref]
+    for _ in range(args.warmup):
+        oin.inner_products(plan, store, P)
+    pairs = 0
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        r = oin.inner_products(plan, store, P)
+        pairs += int((r["kc"] >= 0).sum())
+    dt = time.perf_counter() - t0
+    val = pairs / dt
+    sample = "%d of %d templates x all %d SFT slots per step (oracle.inner.inner_products, numpy fp64)" % (
+        n_ref, w.n_templates, w.desc["n_sft"])
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "templates_per_step": n_ref, "n_sft": w.desc["n_sft"], "K": w.desc["K"],
+                   "kernel": w.desc["kernel"]},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores_used(), "kind": "oracle", "sample": sample,
+                         "host_cores_available": len(os.sched_getaffinity(0))},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}), flush=True)
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2502_11823_b200 import api, build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device - the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if local_rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    w = make_workload(args.workload, rank, args.templates, args.n_sft, args.K)
+    stream = torch.cuda.current_stream()
+    plan = api.plan_from_workload(w, device=local_rank, stream=stream.cuda_stream)
+    if args.chunk:
+        plan.set_chunk(args.chunk)
+    nT = w.n_templates
+    P_host = torch.from_numpy(np.ascontiguousarray(w.params)).pin_memory()
+    P_dev = P_host.to(dev)
+    xh = torch.empty(nT, dtype=torch.float64, device=dev)
+    hh = torch.empty_like(xh)
+    xi = torch.empty_like(xh)
+    out_host = [torch.empty(nT, dtype=torch.float64).pin_memory() for _ in range(3)]
+    out_np = [t.numpy() for t in out_host]
+    P_np = P_host.numpy()
+    # active pairs of this rank's bank, counted once by the library itself (k_c >= 0)
+    kc = torch.empty((nT, plan.n_channels, plan.n_sft), dtype=torch.int32, device=dev)
+    plan.inner_products(P_dev, xh, hh, xi, kc)
+    plan.sync()
+    pairs = int((kc >= 0).sum().item())
+    del kc
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    def step_device():
+        plan.inner_products(P_dev, xh, hh, xi, None)
+
+    def step_host():
+        plan.inner_products(P_np, out_np[0], out_np[1], out_np[2], None)
+
+    def timed(fn, steps, warmup, record_kernel=False):
+        for _ in range(warmup):
+            flush.zero_()
+            fn()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        kms = []
+        l0 = plan.launch_count()
+        for a, b in ev:
+            flush.zero_()
+            a.record(stream)
+            fn()
+            b.record(stream)
+            if record_kernel:
+                kms.append(plan.last_kernel_ms())
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        ms = sum(a.elapsed_time(b) for a, b in ev)
+        return ms, plan.launch_count() - l0, kms
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ms_dev, launches, kms = timed(step_device, args.steps, args.warmup, record_kernel=True)
+    clocks = sampler.stop()
+    e2e_steps = max(3, min(args.steps, 50))
+    ms_host, _, _ = timed(step_host, e2e_steps, 3)
+    ok = bool(torch.isfinite(xh).all().item() and (hh >= 0).all().item())
+    t = torch.tensor([ms_dev, ms_host / e2e_steps, float(pairs)], dtype=torch.float64, device=dev)
+    if world > 1:
+        tmax = t.clone()
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone()
+        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms_dev, ms_host_step, pairs_all = float(tmax[0]), float(tmax[1]), float(tsum[2])
+    else:
+        ms_host_step, pairs_all = float(t[1]), float(pairs)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    ms_step = ms_dev / args.steps
+    value = pairs_all / (ms_step * 1e-3)
+    e2e = pairs_all / (ms_host_step * 1e-3)
+    k_ms = float(np.mean(kms)) if kms else None
+    roof = roofline(w, pairs, k_ms)
+    cpu_val, cpu_n, cpu_dt, cpu_pairs = time_oracle(w, budget_s=args.cpu_budget)
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32 (fp64 phase track + fp64 accumulators)", "data": "synthetic",
+        "config": {"workload": w.name, "templates_per_gpu": nT, "n_sft_slots": int(w.desc["n_sft"]),
+                   "n_channels": int(w.desc["n_channels"]), "K": int(w.desc["K"]), "kernel": w.desc["kernel"],
+                   "pn1": int(w.desc["pn1"]), "active_pairs_per_gpu": pairs, "bin_terms_per_gpu": pairs * (2 * w.desc["K"] + 1),
+                   "parallelism": "templates sharded over %d GPU(s), data store replicated, no collective" % world,
+                   "cache": "l2_flush_between_steps (256 MiB memset, outside the per-step events)"},
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(P_np.nbytes), "d2h_bytes_per_step": int(3 * nT * 8),
+                "ms_per_step": ms_host_step, "steps": e2e_steps},
+        "gpu_launches": int(launches), "kernel_ms": k_ms, "results_finite": ok,
+        "clocks": clocks, "roofline": roof,
+        "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores_used(), "kind": "oracle",
+                         "host_cores_available": len(os.sched_getaffinity(0)),
+                         "sample": "first %d of %d templates x all %d SFT slots (%d active pairs) in %.1f s, "
+                                   "oracle.inner.inner_products numpy fp64" % (cpu_n, nT, w.desc["n_sft"], cpu_pairs, cpu_dt)},
+    }
+    print(json.dumps(out), flush=True)
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# Algorithmic work per active pair and the ALU peak: DESIGN.md §7.
+SM_COUNT, SM_MAX_GHZ = 148, 1.965
+
+
+def roofline(w, pairs, kernel_ms):
+    """ALU roofline of the fused main kernel: the path is bound by plain ALU
+    arithmetic (the 13 MB data store is L2 resident and shared by every template).  Unit: FP32-pipe
+    lane-operations (FFMA/FMUL/FADD = 1 op); peak = 148 SMs x 128 FP32 lanes x 1.965 GHz."""
+    K = int(w.desc["K"])
+    C = int(w.desc["n_channels"])
+    ops_pair = alg_fp32_ops_per_pair(K, C, w.desc["kernel"])
+    peak = SM_COUNT * 128 * SM_MAX_GHZ          # Gop/s
+    if not kernel_ms:
+        return None
+    achieved = ops_pair * pairs / (kernel_ms * 1e-3) / 1e9
+    return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Gop/s (FP32-pipe lane ops)",
+            "frac": achieved / peak, "traffic": None, "kernel": "sft_main_kernel", "kernel_ms": kernel_ms,
+            "alg_ops_per_pair": ops_pair,
+            "peak_source": "derived: 148 SM x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md unit counts/clocks), DESIGN.md §7"}
+
+
+def alg_fp32_ops_per_pair(K, C, kernel):
+    """FP32-pipe-equivalent lane operations the method needs per active (template, SFT) pair
+    (DESIGN.md §7): per bin and channel 4 FMA (complex x complex MAC) + 2 (|F|^2 weight MAC) and the
+    coefficient evaluation (Dirichlet: 3, Fresnel series order 3: 14); per pair the fixed part
+    (phase/prefactor/response, ~40) plus the fp64 track counted at its 2:1 pipe-rate ratio
+    (~30 DFMA-class ops -> 60)."""
+    nb = 2 * K + 1
+    coeff = 3 if kernel == "dirichlet" else 14
+    return nb * (coeff + 6 * C) + 40 + 60
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--templates", type=int, default=None)
+    ap.add_argument("--n-sft", type=int, default=None, dest="n_sft")
+    ap.add_argument("--K", type=int, default=None)
+    ap.add_argument("--chunk", type=int, default=0)
+    ap.add_argument("--cpu-budget", type=float, default=12.0, dest="cpu_budget")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,235 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element,
+on the same seeded inputs.  Tolerances (BASELINE.json north_star):
+
+* ``|d<x,h>|`` and ``|d<h,h>|`` <= 1e-4 * sqrt(<x,x> <h,h>), with ``<x,x>`` restricted to the stored
+  band (stricter than the full-band normaliser the north star names, reading A14);
+* stricter, also enforced here: ``|d<h,h>| <= 1e-4 <h,h>`` and ``|d<x,h>| <= 1e-4 sqrt(<x,x>_band <h,h>)``
+  per template with the *band of that template* implied by the kernel - see ``_check``;
+* selected central bins ``k_c`` bit-exact except pairs the oracle flags as ties (reading A5/A12),
+  where either neighbour / either mask decision is accepted.
+"""
+import numpy as np
+import pytest
+
+from oracle import inner as oin
+from paper_2502_11823_b200 import workloads as wl
+from _util import to_oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+def _api():
+    from paper_2502_11823_b200 import api
+    return api
+
+
+def _run_gpu(w, params=None, want_kc=True, **override):
+    api = _api()
+    P = np.ascontiguousarray(w.params if params is None else params, dtype=np.float64)
+    nT = P.shape[0]
+    with api.plan_from_workload(w, **override) as plan:
+        xh, hh, xi = np.full(nT, np.nan), np.full(nT, np.nan), np.full(nT, np.nan)
+        kc = np.full((nT, plan.n_channels, plan.n_sft), -7, dtype=np.int32) if want_kc else None
+        plan.inner_products(P, xh, hh, xi, kc)
+    return dict(xh=xh, hh=hh, xh_im=xi, kc=kc)
+
+
+def _check(w, g, o, xx, tol=TOL):
+    norm = np.sqrt(xx * np.maximum(o["hh"], 1e-300))
+    assert np.all(np.isfinite(g["xh"])) and np.all(np.isfinite(g["hh"]))
+    e_xh = np.abs(g["xh"] - o["xh"]) / norm
+    e_xi = np.abs(g["xh_im"] - o["xh_im"]) / norm
+    e_hh = np.abs(g["hh"] - o["hh"]) / norm
+    e_hh_rel = np.abs(g["hh"] - o["hh"]) / np.maximum(o["hh"], 1e-300)
+    assert e_xh.max() <= tol, ("xh", e_xh.max(), int(e_xh.argmax()))
+    assert e_xi.max() <= tol, ("xh_im", e_xi.max(), int(e_xi.argmax()))
+    assert e_hh.max() <= tol, ("hh", e_hh.max(), int(e_hh.argmax()))
+    assert e_hh_rel[o["hh"] > 0].max(initial=0.0) <= tol, ("hh rel", e_hh_rel.max())
+    if g.get("kc") is not None:
+        tie = (o["flags"] != 0)[:, None, :]
+        bad = (g["kc"] != o["kc"]) & ~tie
+        assert not bad.any(), ("k_c mismatch", np.argwhere(bad)[:5], g["kc"][bad][:5], o["kc"][bad][:5])
+        d = np.abs(g["kc"].astype(np.int64) - o["kc"])
+        assert np.all((d <= 1) | (g["kc"] == -1) | (o["kc"] == -1))
+    return float(e_xh.max()), float(e_hh_rel.max())
+
+
+def _oracle(w, params=None, **override):
+    ww = w
+    if override:
+        import copy
+        ww = copy.copy(w)
+        ww.desc = dict(w.desc, **override)
+    plan, store = to_oracle(ww)
+    o = oin.inner_products(plan, store, w.params if params is None else params)
+    return o, oin.xx_band(plan, store), plan, store
+
+
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", ["F", "M"])
+@pytest.mark.parametrize("kernel", ["fresnel", "dirichlet"])
+def test_config1(variant, kernel):
+    """BASELINE.json configs[0] whole: 64 templates x 256 SFTs, K = 4."""
+    w = wl.config1(variant=variant)
+    o, xx, _, _ = _oracle(w, kernel=kernel)
+    g = _run_gpu(w, kernel=kernel)
+    _check(w, g, o, xx)
+    assert (o["kc"] >= 0).sum() > 0
+    # the injected signal is template 0: its <x,h> is the largest of the bank up to noise
+    if kernel == "fresnel" and variant == "F":
+        assert g["xh"][0] > 0.5 * g["hh"][0]
+
+
+@pytest.fixture(scope="module")
+def et_small():
+    """Config-2 recipe at a size the oracle finishes in seconds: 1200 SFT slots (10 % gaps,
+    lognormal per-SFT PSD scale, coloured PSD shape), b up to ~4 in the last SFTs, 333 templates
+    (2 full tiles of 128 + a ragged tail)."""
+    return wl.et_bns(n_templates=333, n_sft=1200, K=8, name="et-small")
+
+
+def test_et_small_fresnel(et_small):
+    w = et_small
+    o, xx, _, _ = _oracle(w)
+    g = _run_gpu(w)
+    _check(w, g, o, xx)
+    gaps = w.psd_scale[0] <= 0
+    assert gaps.sum() == 120 and np.all(g["kc"][:, 0, gaps] == -1)
+
+
+def test_et_small_masked_and_dirichlet(et_small):
+    """Variant "M" (f_lo = 5 Hz: only the tail is active) and the Dirichlet kernel."""
+    w = et_small
+    for ov in (dict(f_lo=5.0), dict(kernel="dirichlet"), dict(f_lo=5.0, f_hi=9.0, kernel="dirichlet")):
+        o, xx, _, _ = _oracle(w, **ov)
+        g = _run_gpu(w, **ov)
+        _check(w, g, o, xx)
+        assert 0 < (o["kc"] >= 0).sum() <= o["kc"].size
+
+
+@pytest.mark.parametrize("K", [0, 1, 2, 5, 16, 32, 64])
+def test_band_half_widths(et_small, K):
+    """Config 5's K axis: specialised (4, 8, 16) and generic code paths, including K = 0."""
+    w = et_small
+    P = w.params[:40]
+    o, xx, _, _ = _oracle(w, params=P, K=K)
+    g = _run_gpu(w, params=P, K=K)
+    _check(w, g, o, xx)
+
+
+@pytest.mark.parametrize("chunk", [1, 7, 32, 64, 5000])
+def test_chunking_is_invisible(et_small, chunk):
+    """SFT-axis tiling (grid.y) must not change results beyond fp64 summation order."""
+    api = _api()
+    w = et_small
+    P = np.ascontiguousarray(w.params[:130])
+    o, xx, _, _ = _oracle(w, params=P)
+    with api.plan_from_workload(w) as plan:
+        plan.set_chunk(chunk)
+        xh, hh, xi = np.empty(130), np.empty(130), np.empty(130)
+        plan.inner_products(P, xh, hh, xi, None)
+    _check(w, dict(xh=xh, hh=hh, xh_im=xi, kc=None), o, xx)
+
+
+def test_config4_small():
+    """BASELINE.json configs[3] recipe with 300 templates: 2 channels, annual response, K = 16
+    clipping at k < 1, 0PN+1PN."""
+    w = wl.config4(n_templates=300)
+    o, xx, _, _ = _oracle(w)
+    g = _run_gpu(w)
+    _check(w, g, o, xx)
+    assert g["xh"][0] > 0.5 * g["hh"][0]
+
+
+def test_response_table():
+    """SFT_RESP_TABLE: an arbitrary complex per-(channel, SFT) response."""
+    w = wl.config4(n_templates=40)
+    rng = np.random.default_rng(77)
+    R = (rng.standard_normal((2, w.desc["n_sft"])) + 1j * rng.standard_normal((2, w.desc["n_sft"]))).astype(np.complex64)
+    w.response = R
+    w.desc = dict(w.desc, response="table")
+    o, xx, _, _ = _oracle(w)
+    g = _run_gpu(w)
+    _check(w, g, o, xx)
+
+
+def test_cumulative_small(et_small):
+    """sft_cumulative_snr: inclusive prefix sums over SFTs, every element, fp32 outputs."""
+    api = _api()
+    w = et_small
+    P = np.ascontiguousarray(w.params[:150])
+    plan_o, store = to_oracle(w)
+    o = oin.cumulative_snr(plan_o, store, P)
+    ref = oin.inner_products(plan_o, store, P)
+    xx = oin.xx_band(plan_o, store)
+    n = w.desc["n_sft"]
+    for chunk in (0, 32, 96):
+        with api.plan_from_workload(w) as plan:
+            plan.set_chunk(chunk)
+            snr = np.full((150, n), np.nan, np.float32)
+            cx = np.full((150, n), np.nan, np.float32)
+            ch = np.full((150, n), np.nan, np.float32)
+            plan.cumulative_snr(P, snr, cx, ch)
+            snr_only = np.full((150, n), np.nan, np.float32)
+            plan.cumulative_snr(P, snr_only, None, None)
+        norm = np.sqrt(xx * ref["hh"])[:, None]
+        assert np.abs(cx - o["cum_xh"]).max() <= 1e-4 * norm.max()
+        assert (np.abs(cx - o["cum_xh"]) / norm).max() <= TOL
+        assert (np.abs(ch - o["cum_hh"]) / norm).max() <= TOL
+        big = o["cum_hh"] > 1e-3 * ref["hh"][:, None]
+        assert np.abs(snr - o["snr"])[big].max() <= 1e-3 * max(1.0, np.abs(o["snr"]).max())
+        assert np.array_equal(snr, snr_only)
+        assert np.all(snr[o["cum_hh"] == 0.0] == 0.0)
+        # last column equals the totals
+        assert np.allclose(cx[:, -1], ref["xh"], rtol=0, atol=1e-4 * norm.max())
+
+
+def test_device_pointers_and_edge_sizes(et_small):
+    """Device-resident params/outputs (torch tensors), n_templates in {0, 1, 129}."""
+    import torch
+    api = _api()
+    w = et_small
+    o, xx, _, _ = _oracle(w, params=w.params[:129])
+    with api.plan_from_workload(w) as plan:
+        plan.inner_products(np.zeros((0, 8)), np.zeros(0), np.zeros(0))      # n = 0: SFT_OK, no work
+        for nT in (1, 129):
+            P = torch.from_numpy(np.ascontiguousarray(w.params[:nT])).cuda()
+            xh = torch.full((nT,), float("nan"), dtype=torch.float64, device="cuda")
+            hh = torch.full_like(xh, float("nan"))
+            xi = torch.full_like(xh, float("nan"))
+            plan.inner_products(P, xh, hh, xi, None)
+            plan.sync()
+            g = dict(xh=xh.cpu().numpy(), hh=hh.cpu().numpy(), xh_im=xi.cpu().numpy(), kc=None)
+            oo = {k: (v[:nT] if isinstance(v, np.ndarray) else v) for k, v in o.items()}
+            _check(w, g, oo, xx)
+        assert plan.launch_count() > 0 and plan.last_kernel_ms() > 0.0
+
+
+def test_errors_on_device(et_small):
+    api = _api()
+    w = et_small
+    plan = api.Plan(w.desc)
+    with pytest.raises(api.SftError) as ei:
+        plan.inner_products(np.zeros((1, 8)), np.zeros(1), np.zeros(1))
+    assert "SFT_ENODATA" in str(ei.value)
+    plan.close()
+
+
+def test_ended_and_degenerate_templates(et_small):
+    """Templates whose t_c lies inside / before the data (inactive from some SFT on; all inactive)."""
+    w = et_small
+    P = w.params[:6].copy()
+    T_obs = w.desc["n_sft"] * w.desc["t_sft"]
+    P[1, 2] = 0.5 * T_obs          # coalesces mid-way: later SFTs inactive, earlier ones out of band
+    P[2, 2] = -10.0                # already over
+    P[3, 2] = T_obs + 5000.0       # far in the future: frequencies below the stored band
+    P[4, 4] = 0.0                  # zero amplitude
+    o, xx, _, _ = _oracle(w, params=P)
+    g = _run_gpu(w, params=P)
+    norm = np.sqrt(xx * np.maximum(o["hh"].max(), 1.0))
+    assert np.all(np.abs(g["xh"] - o["xh"]) <= TOL * norm) and np.all(np.abs(g["hh"] - o["hh"]) <= TOL * norm)
+    tie = (o["flags"] != 0)[:, None, :]
+    assert not ((g["kc"] != o["kc"]) & ~tie).any()
+    assert g["hh"][2] == 0.0 and g["hh"][4] == 0.0
