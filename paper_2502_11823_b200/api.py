@@ -43,7 +43,7 @@ class PlanDesc(C.Structure):
 
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
-           "sft_plan_set_chunk", "sft_last_error", "sft_version"]
+           "sft_plan_set_chunk", "sft_last_error", "sft_version", "sft_measure_alu_peaks"]
 
 _lib = None
 
@@ -69,6 +69,8 @@ def load_library(path=None):
     lib.sft_plan_last_kernel_ms.argtypes = [vp]
     lib.sft_plan_last_kernel_ms.restype = dbl
     lib.sft_plan_set_chunk.argtypes = [vp, i32]
+    lib.sft_measure_alu_peaks.argtypes = [i32, C.POINTER(dbl), i32]
+    lib.sft_measure_alu_peaks.restype = i32
     lib.sft_last_error.argtypes = [vp]
     lib.sft_last_error.restype = C.c_char_p
     lib.sft_version.restype = C.c_char_p
@@ -227,6 +229,16 @@ def plan_from_workload(w, device=0, stream=None, **override):
                        np.ascontiguousarray(w.psd_scale[c], dtype=np.float64),
                        np.ascontiguousarray(w.psd_shape[c], dtype=np.float64), resp)
     return plan
+
+
+def measure_alu_peaks(device=0):
+    """``sft_measure_alu_peaks``: dict of measured pipe rates in Gop/s (lane operations)."""
+    lib = load_library()
+    out = (C.c_double * 5)()
+    st = lib.sft_measure_alu_peaks(int(device), out, 5)
+    if st != 0:
+        raise SftError(st, lib.sft_last_error(None).decode())
+    return dict(zip(("ffma", "ffma2", "dfma", "mufu_rcp", "ffma_mufu_mix"), [float(v) for v in out]))
 
 
 def version():

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsft_b200.so")
 SOURCES = [os.path.join(CSRC, "sft_lib.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "sft_kernels.cuh"), os.path.join(CSRC, "fresnel_aux_coeffs.h"),
+DEPS = SOURCES + [os.path.join(CSRC, "sft_kernels.cuh"), os.path.join(CSRC, "fresnel_aux_coeffs.h"), os.path.join(CSRC, "alu_peaks.cuh"),
                   os.path.join(os.path.dirname(HERE), "include", "sft.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",

@@ -1,11 +1,20 @@
 // sft_kernels.cuh - device code of libsft_b200.so (sm_100a).  See include/sft.h for the maths
 // and DESIGN.md for the layout; "P:NNN" cites the paper text, "DESIGN xx" a reading in DESIGN.md.
 //
-// One thread owns one template and walks a chunk of consecutive SFTs; a warp therefore holds 32
-// templates at the SAME SFT, so that (i) every data-bin load is a warp-wide broadcast of the same
-// few addresses (templates of a bank tile select the same k_c to within a bin), (ii) the branch on
-// the chirp parameter b = fdot T^2 (series vs Fresnel form) is warp-uniform, and (iii) the sum over
-// SFTs needs no cross-lane traffic at all: it is a private fp64 accumulator per thread.
+// Mapping.  One thread owns one template and walks a chunk of consecutive SFTs; a warp therefore
+// holds 32 templates at the SAME SFT, so that (i) every data load is a warp-wide broadcast of the
+// same one or two 128-byte lines (templates of a bank tile select the same k_c to within a bin),
+// (ii) the branch on the chirp parameter b = fdot T^2 (series order / Fresnel form) is made
+// warp-uniform, and (iii) the sum over SFTs needs no cross-lane traffic at all: it is a private
+// accumulator per thread (fp32 over 8 SFTs, flushed into fp64).
+//
+// Inner loop.  The 2K+1 bins of a pair are processed two adjacent bins at a time with the packed
+// fp32x2 instructions of sm_100 (FADD2/FMUL2/FFMA2: one issue slot, two lanes).  The store keeps
+// the whitened data "pair-planar", {re_j, re_j+1, im_j, im_j+1} per 16 bytes, in two copies (pairs
+// starting at even / odd bins), so that ONE aligned 128-bit load delivers both packed operands of a
+// bin pair whatever the parity of the window start k_c - K; rows are zero-padded by 2K+2 bins on
+// both sides, so no per-bin band-edge test exists.  One MUFU reciprocal serves both bins of a pair
+// (1/a = (a-1)/(a(a-1))).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -15,26 +24,30 @@ namespace sftk {
 
 constexpr int TILE = 128;            // templates (= threads) per block
 constexpr int MAXC = 4;              // SFT_MAX_CHANNELS
+constexpr int FLUSH = 8;             // SFTs summed in fp32 before the fp64 accumulators are touched
 constexpr double GMSUN_S = 4.925491025543576e-6;   // G Msun / c^3 [s]
 constexpr float PI_F = 3.14159265358979f;
+constexpr float INV_2PI_F = 0.15915494309189535f;
 
 // b = fdot T^2 thresholds of the coefficient evaluator (DESIGN "kernel evaluator"): the power
 // series in b about the SFT mid-point truncated after order n has error <= (pi b)^(n+1) /
 // ((n+1)! 4^(n+1) (2n+3)); the bounds below keep that under 2e-6.
 constexpr float B_ORDER1 = 0.0057f;  // |b| <= : order 1
+constexpr float B_ORDER2 = 0.056f;   // |b| <= : order 2
 constexpr float B_ORDER3 = 0.18f;    // |b| <= : order 3; above: closed Fresnel form
 
 struct KParams {
-  int C, n_sft, nb, k_lo, kv_lo, kv_hi, K;
+  int C, n_sft, nb, k_lo, kv_lo, kv_hi, K, PAD, npair;
   int kernel, pn1, response;
   double T, t0, f_loT, f_hiT, inv_fref;
   double sigma[MAXC];      // sqrt(T / S_ref,c)
   double chi[MAXC];        // SFT_RESP_ANNUAL response phase per channel
   float depth;
-  const float2 *D;         // [C][n_sft][nb]   2 conj(x~) sqrt(S_ref) / (sqrt(T) s_a S_k)
-  const float *ub2;        // [C][nb]          S_ref / S_k   (0 for invalid bins)
-  const float *us2;        // [C][n_sft]       1 / s_a       (0 for gaps)
-  const float2 *rtab;      // [C][n_sft]       TABLE: R_{c,a}; ANNUAL: (cos, sin)(2 pi t_a/P + psi_c)
+  const float4 *Dp;        // [2][C][n_sft][npair]  {re_j, re_j+1, im_j, im_j+1} of
+                           //                        2 conj(x~) sqrt(S_ref) / (sqrt(T) s_a S_k), padded index j = 2i+copy
+  const float2 *ubp;       // [2][C][npair]         {u_j, u_j+1}, u = S_ref / S_k (0 for invalid bins)
+  const float *us2;        // [C][n_sft]            1 / s_a       (0 for gaps)
+  const float2 *rtab;      // [C][n_sft]            TABLE: R_{c,a}; ANNUAL: (cos, sin)(2 pi t_a/P + psi_c)
   const double *params;    // [nT][8]
   long long nT;
   int chunk, n_chunks;
@@ -48,6 +61,33 @@ __device__ __forceinline__ float rcp_approx(float x) {
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
   return r;
 }
+__device__ __forceinline__ float rsqrt_approx(float x) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float sqrt_approx(float x) {
+  float r;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float lg2_approx(float x) {
+  float r;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float ex2_approx(float x) {
+  float r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+// (sin, cos)(pi t) for |t| <= 1 on the MUFU (absolute error ~5e-7 over [-pi, pi])
+__device__ __forceinline__ void sincospi_fast(float t, float &s, float &c) {
+  const float a = PI_F * t;
+  s = __sinf(a);
+  c = __cosf(a);
+}
+__device__ __forceinline__ float2 bc(float v) { return make_float2(v, v); }
 
 template <int N>
 __device__ __forceinline__ float horner(const float *c, float s) {
@@ -133,90 +173,161 @@ struct Track {
   float amp;     // (f_a / F0)^(2/3) = Theta^(-1/4) (1 + cf Theta^(-1/4))^(2/3)
 };
 
-__device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, int alpha, Track &tr) {
-  const double ta = p.t0 + (double)alpha * p.T;
+// fp64 track.  Theta^(-1/8) comes from an fp32 MUFU seed (relative error e ~ 5e-7) refined by one
+// second-order Newton step in fp64:  with r = 1 - Theta y^8,  Theta^(-1/8) = y (1-r)^(-1/8)
+// = y (1 + r/8 + 9 r^2/128 + O(r^3));  r ~ 8e, so the result is good to ~0.05 (8e)^3 ~ 3e-18 (+ rounding).
+__device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, double dalpha, Track &tr) {
+  const double ta = __dadd_rn(p.t0, __dmul_rn(dalpha, p.T));   // t_a = t0 + a T, rounded as written
   const double tau = tm.tc - ta;
   tr.active = false;
   tr.kc = -1;
   if (!tm.ok || !(tau > p.T)) return;
   const double theta = tm.cTheta * tau;
-  const double q = rsqrt(sqrt(sqrt(theta)));      // Theta^(-1/8)
+  const float y0 = ex2_approx(-0.125f * lg2_approx((float)theta));
+  const double y = (double)y0;
+  const double y2 = y * y, y4 = y2 * y2, y8 = y4 * y4;
+  const double r = fma(-theta, y8, 1.0);
+  const double s = fma(r, 9.0 / 128.0, 0.125) * r;
+  const double q = fma(y, s, y);                  // Theta^(-1/8)
   const double q2 = q * q, q3 = q2 * q, q4 = q2 * q2, q8 = q4 * q4;
-  const double ph = tm.phic_cyc - tm.cphase * (theta * q3) * fma(tm.cphi, q2, 1.0);   // cycles
+  const double ph = fma(-tm.cphase * (theta * q3), fma(tm.cphi, q2, 1.0), tm.phic_cyc);   // cycles
   const double fT = tm.F0T * q3 * fma(tm.cf, q2, 1.0);
   const double b = tm.bscale * (q8 * q3) * fma(0.625 * tm.cf, q2, 0.375);
-  const double y = (p.kernel == 1) ? fma(0.5, b, fT) : fT;   // Fresnel: centre of the swept band
-  const double kcd = floor(y + 0.5);
+  const double yy = (p.kernel == 1) ? fma(0.5, b, fT) : fT;   // Fresnel: centre of the swept band
+  double kcd = floor(yy + 0.5);
   if (!(fT >= p.f_loT) || !(fT + b <= p.f_hiT)) return;
   tr.active = true;
-  tr.kc = (int)kcd;
   tr.x = (float)(fT - kcd);
+  kcd = fmin(fmax(kcd, -1073741824.0), 1073741824.0);
+  tr.kc = (int)kcd;
   tr.b = (float)b;
   tr.frac = (float)(ph - rint(ph));
   const float q2f = (float)q2;
   float a = q2f;
-  if (p.pn1) {
-    const float e = fmaf(tm.cf32, q2f, 1.0f);
-    a *= cbrtf(e * e);
-  }
+  if (p.pn1) a *= ex2_approx((2.0f / 3.0f) * lg2_approx(fmaf(tm.cf32, q2f, 1.0f)));
   tr.amp = a;
 }
 
 // ---------------------------------------------------------------------------------------------
-// Coefficient evaluator + contraction for one (template, SFT): accumulates, per channel,
-//   S1 = sum_m D_{k_c+m} I_m     (complex)      S2 = sum_m ub2_{k_c+m} |I_m|^2
-// where F(x-m, b) = pref * I_m and `pref` (unit modulus times a real scale) is returned through
-// (pr, pi, scale):  F_m = scale * (pr + i pi) * I_m.
-//
-// Series form (|b| <= B_ORDER3), about the SFT mid-point (DESIGN "kernel evaluator"):
-//   F(x-m,b) = e^{i pi (x-m+b/4)} int_{-1/2}^{1/2} e^{i pi (2 a' v + b v^2)} dv,  a' = x + b/2 - m
-//            = e^{i pi (x+b/4)} sum_n (i pi b)^n / n! * r_2n(a'),
-//   (-1)^m r_j from the forward recurrence of int v^j e^{i w v} dv (w = 2 pi a'), which is stable
-//   for |a'| >= 1/2; the central bin (|a'| < 1/2) uses the Taylor series in (pi a')^2.
-// b = 0 is the Dirichlet kernel e^{i pi a} sinc(a), Eq.(B2) P:451.
+// Coefficient evaluator.  F(x-m, b) = e^{i pi (x + b/4)} J_m with (DESIGN "kernel evaluator")
+//   J_m = (-1)^m int_{-1/2}^{1/2} e^{i (w v + pi b v^2)} dv,  w = 2 pi a',  a' = x + b/2 - m
+//       = sum_n (i pi b)^n / n! r_2n(a'),   r_j = (-1)^m int v^j e^{i w v} dv,
+// expanded about the SFT mid-point.  Far bins (m != 0, |a'| >= 1/2) use the forward recurrence
+//   r_0 = 2 S w', q_1 = (r_0 - C) w', r_2 = (S/2 - 2 q_1) w', q_3 = (3 r_2 - C/4) w', ...   w' = 1/w,
+// with S = sin(pi xp), C = cos(pi xp), xp = x + b/2 (the (-1)^m of sin/cos(pi a') cancels the one in
+// J_m).  The central bin (m = 0, |a'| <= 1/2 by construction of k_c, DESIGN A5) uses the Taylor
+// series in z = (pi a')^2.  b = 0 is the Dirichlet kernel e^{i pi a} sinc(a), Eq.(B2) P:451.
 // ---------------------------------------------------------------------------------------------
-template <int ORDER>
-__device__ __forceinline__ void series_central(float xp, float pb, float &Ir, float &Ii) {
-  // r_2n(w) = 4^-n sum_p (-1)^p z^p / ((2p)! (2n+2p+1)),  z = (pi xp)^2 <= (pi/2)^2
-  const float z = (PI_F * xp) * (PI_F * xp);
-  auto tay = [&](int n) {
-    float acc = 0.f;
-    float fact[8] = {1.f, 2.f, 24.f, 720.f, 40320.f, 3628800.f, 479001600.f, 87178291200.f};
-#pragma unroll
-    for (int pp = 7; pp >= 0; --pp) {
-      const float c = ((pp & 1) ? -1.f : 1.f) / (fact[pp] * (float)(2 * n + 2 * pp + 1));
-      acc = fmaf(acc, z, c);
-    }
-    return acc;
-  };
-  const float r0 = tay(0);
-  Ir = r0;
-  Ii = 0.f;
-  if (ORDER >= 1) Ii = pb * (0.25f * tay(1));
-  if (ORDER >= 3) {
-    Ir = fmaf(-0.5f * pb * pb, 0.0625f * tay(2), Ir);
-    Ii = fmaf(-(1.0f / 6.0f) * pb * pb * pb, 0.015625f * tay(3), Ii);
+template <int ORD>
+struct SeriesK {           // per-(template, SFT) constants, broadcast into both packed lanes
+  float2 S2, mC, c_i1, c_i0;            // order >= 1 : 2S, -C, and  J_i = (c_i0 + c_i1 q_1) w'  (order 1)
+  float2 Sh, mC4, S8, mC16, S32;        // higher orders
+  float2 pb, mpb2h, mpb3s;              // pi b, -(pi b)^2/2, -(pi b)^3/6
+  float S, C, pbs;
+};
+
+template <int ORD>
+__device__ __forceinline__ void series_setup(float xp, float b, SeriesK<ORD> &k) {
+  float S, C;
+  sincospi_fast(xp, S, C);
+  const float pb = PI_F * b;
+  k.S = S; k.C = C; k.pbs = pb;
+  k.S2 = bc(2.0f * S);
+  k.mC = bc(-C);
+  if (ORD == 1) {
+    k.c_i1 = bc(-2.0f * pb);
+    k.c_i0 = bc(0.5f * pb * S);
+  }
+  if (ORD >= 2) {
+    k.Sh = bc(0.5f * S);
+    k.mC4 = bc(-0.25f * C);
+    k.S8 = bc(0.125f * S);
+    k.pb = bc(pb);
+    k.mpb2h = bc(-0.5f * pb * pb);
+  }
+  if (ORD >= 3) {
+    k.mC16 = bc(-0.0625f * C);
+    k.S32 = bc(0.03125f * S);
+    k.mpb3s = bc(-(1.0f / 6.0f) * pb * pb * pb);
   }
 }
 
-template <int ORDER>
-__device__ __forceinline__ void series_far(float ap, float S, float C, float pb, float &Ir, float &Ii) {
-  const float w = rcp_approx(2.0f * PI_F * ap);   // 1 / omega
-  const float r0 = 2.0f * S * w;
-  Ir = r0;
-  Ii = 0.f;
-  if (ORDER >= 1) {
-    const float q1 = (r0 - C) * w;
-    const float r2 = fmaf(0.5f, S, -2.0f * q1) * w;
-    Ii = pb * r2;
-    if (ORDER >= 3) {
-      const float q3 = fmaf(3.0f, r2, -0.25f * C) * w;
-      const float r4 = fmaf(0.125f, S, -4.0f * q3) * w;
-      const float q5 = fmaf(5.0f, r4, -0.0625f * C) * w;
-      const float r6 = fmaf(0.03125f, S, -6.0f * q5) * w;
-      Ir = fmaf(-0.5f * pb * pb, r4, Ir);
-      Ii = fmaf(-(1.0f / 6.0f) * pb * pb * pb, r6, Ii);
+// two far bins at once; w = {1/(2 pi a_lo), 1/(2 pi a_hi)}
+template <int ORD>
+__device__ __forceinline__ void series_far2(const SeriesK<ORD> &k, float2 w, float2 &Jr, float2 &Ji) {
+  const float2 r0 = __fmul2_rn(k.S2, w);
+  Jr = r0;
+  if (ORD == 0) {
+    Ji = make_float2(0.f, 0.f);
+  } else if (ORD == 1) {
+    const float2 q1 = __fmul2_rn(__fadd2_rn(r0, k.mC), w);
+    Ji = __fmul2_rn(__ffma2_rn(k.c_i1, q1, k.c_i0), w);
+  } else {
+    const float2 q1 = __fmul2_rn(__fadd2_rn(r0, k.mC), w);
+    const float2 r2 = __fmul2_rn(__ffma2_rn(bc(-2.0f), q1, k.Sh), w);
+    const float2 q3 = __fmul2_rn(__ffma2_rn(bc(3.0f), r2, k.mC4), w);
+    const float2 r4 = __fmul2_rn(__ffma2_rn(bc(-4.0f), q3, k.S8), w);
+    Jr = __ffma2_rn(k.mpb2h, r4, r0);
+    Ji = __fmul2_rn(k.pb, r2);
+    if (ORD >= 3) {
+      const float2 q5 = __fmul2_rn(__ffma2_rn(bc(5.0f), r4, k.mC16), w);
+      const float2 r6 = __fmul2_rn(__ffma2_rn(bc(-6.0f), q5, k.S32), w);
+      Ji = __ffma2_rn(k.mpb3s, r6, Ji);
     }
+  }
+}
+
+// one far bin (scalar twin of series_far2)
+template <int ORD>
+__device__ __forceinline__ void series_far1(const SeriesK<ORD> &k, float a, float &Jr, float &Ji) {
+  const float w = rcp_approx(2.0f * PI_F * a);
+  const float r0 = 2.0f * k.S * w;
+  Jr = r0;
+  Ji = 0.f;
+  if (ORD >= 1) {
+    const float q1 = (r0 - k.C) * w;
+    const float r2 = fmaf(-2.0f, q1, 0.5f * k.S) * w;
+    Ji = k.pbs * r2;
+    if (ORD >= 2) {
+      const float q3 = fmaf(3.0f, r2, -0.25f * k.C) * w;
+      const float r4 = fmaf(-4.0f, q3, 0.125f * k.S) * w;
+      Jr = fmaf(-0.5f * k.pbs * k.pbs, r4, r0);
+      if (ORD >= 3) {
+        const float q5 = fmaf(5.0f, r4, -0.0625f * k.C) * w;
+        const float r6 = fmaf(-6.0f, q5, 0.03125f * k.S) * w;
+        Ji = fmaf(-(1.0f / 6.0f) * k.pbs * k.pbs * k.pbs, r6, Ji);
+      }
+    }
+  }
+}
+
+// Taylor coefficients of r_2n(a') = 4^-n sum_p (-1)^p z^p / ((2p)! (2n+2p+1)),  z = (pi a')^2 <= (pi/2)^2;
+// 7 terms: truncation < 5e-10.  Packed as {r_0, r_2} and {r_4, r_6}.
+__device__ __forceinline__ constexpr float tay_c(int n, int pp) {
+  double f = 1.0;
+  for (int i = 2; i <= 2 * pp; ++i) f *= (double)i;
+  double s = (pp & 1) ? -1.0 : 1.0;
+  double four = 1.0;
+  for (int i = 0; i < n; ++i) four *= 4.0;
+  return (float)(s / (f * (double)(2 * n + 2 * pp + 1) * four));
+}
+
+template <int ORD>
+__device__ __forceinline__ void series_central(const SeriesK<ORD> &k, float a, float &Jr, float &Ji) {
+  const float t = PI_F * a;
+  const float2 z = bc(t * t);
+  float2 lo = make_float2(tay_c(0, 6), tay_c(1, 6));
+#pragma unroll
+  for (int pp = 5; pp >= 0; --pp) lo = __ffma2_rn(lo, z, make_float2(tay_c(0, pp), tay_c(1, pp)));
+  Jr = lo.x;                 // r_0
+  Ji = k.pbs * lo.y;         // pi b r_2
+  if (ORD == 0) Ji = 0.f;
+  if (ORD >= 2) {
+    float2 hi = make_float2(tay_c(2, 6), tay_c(3, 6));
+#pragma unroll
+    for (int pp = 5; pp >= 0; --pp) hi = __ffma2_rn(hi, z, make_float2(tay_c(2, pp), tay_c(3, pp)));
+    Jr = fmaf(-0.5f * k.pbs * k.pbs, hi.x, Jr);
+    if (ORD >= 3) Ji = fmaf(-(1.0f / 6.0f) * k.pbs * k.pbs * k.pbs, hi.y, Ji);
   }
 }
 
@@ -224,126 +335,158 @@ __device__ __forceinline__ void series_far(float ap, float S, float C, float pb,
 // large phase pi a^2/b cancels analytically (DESIGN "kernel evaluator"):  with l = a sqrt(2/b),
 // u = l + sqrt(2b), w(t) = g(t) + i f(t), E = e^{i pi (2x+b)},
 //   sqrt(2b) F(a,b) = sgn(l) w(|l|) - E sgn(u) w(|u|) + [l < 0 <= u] (1+i) e^{-i pi a^2/b}.
-__device__ __forceinline__ void fresnel_bin(float a, float c1, float c2, float inv_b, float Er, float Ei,
-                                            float &Yr, float &Yi) {
-  const float l = a * c1;
-  const float u = l + c2;
+struct FresK {
+  float c1, c2, inv_b, Er, Ei, xs;
+  bool neg;
+};
+__device__ __forceinline__ void fresnel_bin(const FresK &k, int m, float &Yr, float &Yi) {
+  // b < 0: F(a,-|b|) = conj F(-a,|b|)  (DESIGN A10)
+  const float a = k.neg ? -(k.xs - (float)m) : (k.xs - (float)m);
+  const float l = a * k.c1;
+  const float u = l + k.c2;
   float gl, fl, gu, fu;
   fresnel_w(fabsf(l), gl, fl);
   fresnel_w(fabsf(u), gu, fu);
   const float sl = (l >= 0.f) ? 1.f : -1.f;
   const float su = (u >= 0.f) ? 1.f : -1.f;
-  // E * w(|u|)
-  const float er = Er * gu - Ei * fu;
-  const float ei = Er * fu + Ei * gu;
+  const float er = k.Er * gu - k.Ei * fu;       // E * w(|u|)
+  const float ei = k.Er * fu + k.Ei * gu;
   Yr = sl * gl - su * er;
   Yi = sl * fl - su * ei;
   if (l < 0.f && u >= 0.f) {
     float s, c;
-    sincospif(a * a * inv_b, &s, &c);     // e^{-i pi a^2/b} = c - i s ;  (1+i)(c - i s) = (c+s) + i(c-s)
+    sincospif(a * a * k.inv_b, &s, &c);     // e^{-i pi a^2/b} = c - i s ;  (1+i)(c - i s) = (c+s) + i(c-s)
     Yr += c + s;
     Yi += c - s;
+  }
+  if (k.neg) Yi = -Yi;
+}
+
+// Per-channel packed accumulators of the contraction over the bins of one (template, SFT):
+//   A = sum Dre J_r,  B = sum Dim J_i,  I = sum (Dre J_i + Dim J_r),  W = sum u |J|^2   (lane = bin parity)
+struct Acc {
+  float2 A, B, I, W;
+};
+
+template <int CT>
+__device__ __forceinline__ void mac_pair(const KParams &p, const float4 *Drow, const float2 *urow, size_t dstride,
+                                         size_t ustride, int q, float2 Jr, float2 Ji, Acc (&acc)[CT]) {
+  const float2 mag = __ffma2_rn(Ji, Ji, __fmul2_rn(Jr, Jr));
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+    {
+      const float4 d = __ldg(Drow + c * dstride + q);
+      const float2 u = __ldg(urow + c * ustride + q);
+      const float2 dre = make_float2(d.x, d.y), dim = make_float2(d.z, d.w);
+      acc[c].A = __ffma2_rn(dre, Jr, acc[c].A);
+      acc[c].B = __ffma2_rn(dim, Ji, acc[c].B);
+      acc[c].I = __ffma2_rn(dre, Ji, acc[c].I);
+      acc[c].I = __ffma2_rn(dim, Jr, acc[c].I);
+      acc[c].W = __ffma2_rn(u, mag, acc[c].W);
+    }
+  }
+}
+
+// Series path of one (template, SFT): all K+1 bin pairs.  Pair q holds m = -K+2q (lo) and -K+2q+1 (hi);
+// the hi lane of the last pair (m = K+1) is outside the band and gets J = 0.
+template <int ORD, int KT, int CT>
+__device__ __forceinline__ void series_pairs(const KParams &p, float xp, float b, const float4 *Drow, const float2 *urow,
+                                             size_t dstride, size_t ustride, Acc (&acc)[CT]) {
+  const int K = KT > 0 ? KT : p.K;
+  SeriesK<ORD> k;
+  series_setup<ORD>(xp, b, k);
+  const int qc = K >> 1;                 // pair holding m = 0 (lo lane if K even, hi lane if K odd)
+  const float a0 = xp + (float)K;        // a' of m = -K
+#pragma unroll
+  for (int q = 0; q <= K; ++q) {
+    float2 Jr, Ji;
+    const float a_lo = a0 - (float)(2 * q), a_hi = a_lo - 1.0f;
+    if (q == qc || q == K) {
+      const int m_lo = -K + 2 * q, m_hi = m_lo + 1;
+      if (m_lo == 0) series_central<ORD>(k, a_lo, Jr.x, Ji.x);
+      else series_far1<ORD>(k, a_lo, Jr.x, Ji.x);
+      if (m_hi == 0) series_central<ORD>(k, a_hi, Jr.y, Ji.y);
+      else if (m_hi > K) { Jr.y = 0.f; Ji.y = 0.f; }
+      else series_far1<ORD>(k, a_hi, Jr.y, Ji.y);
+    } else {
+      const float rp = rcp_approx(a_lo * a_hi) * INV_2PI_F;
+      series_far2<ORD>(k, make_float2(a_hi * rp, a_lo * rp), Jr, Ji);
+    }
+    mac_pair<CT>(p, Drow, urow, dstride, ustride, q, Jr, Ji, acc);
   }
 }
 
 template <int KT, int CT>
-__device__ __forceinline__ void pair_contract(const KParams &p, int alpha, const Track &tr,
-                                              float (&S1r)[CT], float (&S1i)[CT], float (&S2)[CT],
-                                              float &pr, float &pi_, float &scale) {
+__device__ __forceinline__ void fresnel_pairs(const KParams &p, float x, float b, const float4 *Drow, const float2 *urow,
+                                              size_t dstride, size_t ustride, Acc (&acc)[CT], float &scale) {
   const int K = KT > 0 ? KT : p.K;
-  const int C = p.C;
-#pragma unroll
-  for (int c = 0; c < CT; ++c) { S1r[c] = 0.f; S1i[c] = 0.f; S2[c] = 0.f; }
-  const bool fres = (p.kernel == 1);
-  const float b = fres ? tr.b : 0.f;
-  const float x = tr.x;
-  const int col0 = tr.kc - p.k_lo;                    // column of the central bin in the store
-  const int mlo = max(-K, p.kv_lo - tr.kc), mhi = min(K, p.kv_hi - 1 - tr.kc);
-  const float2 *Drow = p.D + (size_t)alpha * p.nb + col0;
-  const float *ubrow = p.ub2 + col0;
-  const size_t Dstride = (size_t)p.n_sft * p.nb;
-
-  auto accum = [&](int m, float Ir, float Ii) {
-    const float mag = fmaf(Ir, Ir, Ii * Ii);
-#pragma unroll
-    for (int c = 0; c < CT; ++c) {
-      if (c < C) {
-        const float2 d = __ldg(Drow + c * Dstride + m);
-        const float w2 = __ldg(ubrow + c * p.nb + m);
-        S1r[c] = fmaf(d.x, Ir, fmaf(-d.y, Ii, S1r[c]));
-        S1i[c] = fmaf(d.x, Ii, fmaf(d.y, Ir, S1i[c]));
-        S2[c] = fmaf(w2, mag, S2[c]);
-      }
-    }
-  };
-
-  if (fabsf(b) <= B_ORDER3) {
-    const float xp = fmaf(0.5f, b, x);
-    const float pb = PI_F * b;
-    float S, Cc;
-    sincospif(xp, &S, &Cc);
-    const int ord = (b == 0.f) ? 0 : (fabsf(b) <= B_ORDER1 ? 1 : 3);
-    // prefactor e^{i pi (x + b/4)}
-    sincospif(fmaf(0.25f, b, x), &pi_, &pr);
-    scale = 1.0f;
-#pragma unroll
-    for (int m = -K; m <= K; ++m) {
-      if (m < mlo || m > mhi) continue;
-      float Ir, Ii;
-      const float ap = xp - (float)m;
-      if (fabsf(ap) < 0.5f) {
-        if (ord == 0) series_central<0>(ap, pb, Ir, Ii);
-        else if (ord == 1) series_central<1>(ap, pb, Ir, Ii);
-        else series_central<3>(ap, pb, Ir, Ii);
-        // Taylor form carries no (-1)^m; the far form's S, C are those of xp, i.e. include it
-        if (m & 1) { Ir = -Ir; Ii = -Ii; }
-      } else {
-        if (ord == 0) series_far<0>(ap, S, Cc, pb, Ir, Ii);
-        else if (ord == 1) series_far<1>(ap, S, Cc, pb, Ir, Ii);
-        else series_far<3>(ap, S, Cc, pb, Ir, Ii);
-      }
-      accum(m, Ir, Ii);
-    }
-  } else {
-    // closed Fresnel form; b < 0: F(a,-|b|) = conj F(-a,|b|)  (DESIGN A10)
-    const bool neg = b < 0.f;
-    const float ab = fabsf(b);
-    const float c1 = sqrtf(2.0f / ab), c2 = sqrtf(2.0f * ab), inv_b = 1.0f / ab;
-    const float xs = neg ? -x : x;
-    float Er, Ei;
-    sincospif(fmaf(2.0f, xs, ab), &Ei, &Er);
-    pr = 1.0f;
-    pi_ = 0.0f;
-    scale = 1.0f / c2;
-#pragma unroll
-    for (int m = -K; m <= K; ++m) {
-      if (m < mlo || m > mhi) continue;
-      float Yr, Yi;
-      const float a = neg ? -(x - (float)m) : (x - (float)m);
-      fresnel_bin(a, c1, c2, inv_b, Er, Ei, Yr, Yi);
-      if (neg) Yi = -Yi;
-      accum(m, Yr, Yi);
-    }
+  FresK k;
+  k.neg = b < 0.f;
+  const float ab = fabsf(b);
+  k.c1 = sqrtf(2.0f / ab);
+  k.c2 = sqrtf(2.0f * ab);
+  k.inv_b = 1.0f / ab;
+  k.xs = x;
+  const float xs = k.neg ? -x : x;
+  sincospif(fmaf(2.0f, xs, ab), &k.Ei, &k.Er);
+  scale = 1.0f / k.c2;
+#pragma unroll 1
+  for (int q = 0; q <= K; ++q) {
+    float2 Jr, Ji;
+    const int m_lo = -K + 2 * q;
+    fresnel_bin(k, m_lo, Jr.x, Ji.x);
+    if (m_lo + 1 > K) { Jr.y = 0.f; Ji.y = 0.f; }
+    else fresnel_bin(k, m_lo + 1, Jr.y, Ji.y);
+    mac_pair<CT>(p, Drow, urow, dstride, ustride, q, Jr, Ji, acc);
   }
 }
 
 // Z_c = Re/Im of the per-(SFT, channel) complex term, H_c its <h,h> term (include/sft.h).
+// `bmax` is the warp-wide max |b| of the pairs being evaluated: it selects the series order for the
+// whole warp (a higher order than a lane needs is still correct for that lane).
 template <int KT, int CT>
-__device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int alpha, const Track &tr,
+__device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int alpha, const Track &tr, float bmax,
                                            const float (&us2)[CT], float &zr, float &zi, float &hh) {
-  float S1r[CT], S1i[CT], S2[CT];
-  float pr, pi_, scale;
-  pair_contract<KT, CT>(p, alpha, tr, S1r, S1i, S2, pr, pi_, scale);
-  // e^{i phi_a} * (pr + i pi)
-  float sp, cp;
-  sincospif(2.0f * tr.frac, &sp, &cp);
-  const float er = (cp * pr - sp * pi_) * scale * tr.amp;
-  const float ei = (cp * pi_ + sp * pr) * scale * tr.amp;
-  const float a2 = tr.amp * tr.amp * scale * scale;
+  const int K = KT > 0 ? KT : p.K;
   zr = 0.f; zi = 0.f; hh = 0.f;
+  // window start in the zero-padded row; windows that miss the stored band entirely contribute 0
+  if (tr.kc + K < p.k_lo || tr.kc - K >= p.k_lo + p.nb) return;
+  const int j0 = tr.kc - K - p.k_lo + p.PAD;
+  const int copy = j0 & 1;
+  const size_t dstride = (size_t)p.n_sft * p.npair, ustride = (size_t)p.npair;
+  const float4 *Drow = p.Dp + (size_t)copy * CT * dstride + (size_t)alpha * p.npair + (j0 >> 1);
+  const float2 *urow = p.ubp + (size_t)copy * CT * ustride + (j0 >> 1);
+  Acc acc[CT];
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
-    if (c < p.C && us2[c] > 0.f) {
+    acc[c].A = make_float2(0.f, 0.f); acc[c].B = acc[c].A; acc[c].I = acc[c].A; acc[c].W = acc[c].A;
+  }
+  const bool fres = (p.kernel == 1);
+  const float b = fres ? tr.b : 0.f;
+  float scale = 1.0f;
+  float t;    // total phase / pi:  2 frac (= phi_a/pi) + prefactor phase / pi
+  if (bmax <= B_ORDER3 || fabsf(b) <= B_ORDER3) {
+    const float xp = fmaf(0.5f, b, tr.x);
+    if (bmax == 0.f) series_pairs<0, KT, CT>(p, xp, b, Drow, urow, dstride, ustride, acc);
+    else if (bmax <= B_ORDER1) series_pairs<1, KT, CT>(p, xp, b, Drow, urow, dstride, ustride, acc);
+    else if (bmax <= B_ORDER2) series_pairs<2, KT, CT>(p, xp, b, Drow, urow, dstride, ustride, acc);
+    else series_pairs<3, KT, CT>(p, xp, b, Drow, urow, dstride, ustride, acc);
+    t = fmaf(2.0f, tr.frac, fmaf(0.25f, b, tr.x));         // prefactor e^{i pi (x + b/4)}
+  } else {
+    fresnel_pairs<KT, CT>(p, tr.x, b, Drow, urow, dstride, ustride, acc, scale);
+    t = 2.0f * tr.frac;
+  }
+  t = fmaf(-2.0f, rintf(0.5f * t), t);                       // into [-1, 1]
+  float sp, cp;
+  sincospi_fast(t, sp, cp);
+  const float er = cp * scale * tr.amp, ei = sp * scale * tr.amp;
+  const float a2 = tr.amp * tr.amp * scale * scale;
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+    if (us2[c] > 0.f) {
+      const float S1r = (acc[c].A.x + acc[c].A.y) - (acc[c].B.x + acc[c].B.y);
+      const float S1i = acc[c].I.x + acc[c].I.y;
+      const float S2 = acc[c].W.x + acc[c].W.y;
       // response (Eq.(5)-(6) P:80-85 as Lambda z = Re[R z]; DESIGN C3/D4)
       float2 R = tm.AE[c];
       if (p.response == 1) {
@@ -355,15 +498,15 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int
         R = make_float2(R.x * am, R.y * am);
       }
       const float gr = R.x * er - R.y * ei, gi = R.x * ei + R.y * er;   // p_c = R * A e^{i phi} pref
-      zr += gr * S1r[c] - gi * S1i[c];
-      zi += gr * S1i[c] + gi * S1r[c];
-      hh += (R.x * R.x + R.y * R.y) * a2 * us2[c] * S2[c];
+      zr += gr * S1r - gi * S1i;
+      zi += gr * S1i + gi * S1r;
+      hh += (R.x * R.x + R.y * R.y) * a2 * us2[c] * S2;
     }
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-// Main fused kernel.  grid = (template tiles, SFT chunks).  MODE 0: chunk totals only.
+// Main fused kernel.  grid = (template tiles, SFT chunks); CT == number of channels (exactly).  MODE 0: chunk totals only.
 // MODE 1 (cumulative): additionally writes chunk-local inclusive prefix sums, transposed through
 // shared memory so that global stores are 128-byte rows along the SFT axis.
 // ---------------------------------------------------------------------------------------------
@@ -376,33 +519,50 @@ __global__ void __launch_bounds__(TILE) sft_main_kernel(const KParams p) {
   Tmpl tm;
   tmpl_init(p, t, tm);
   double axh = 0.0, ahh = 0.0, axi = 0.0;
+  float fxh = 0.f, fhh = 0.f, fxi = 0.f;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float *txh = tile_s + (MODE == 1 ? warp * 2 * 32 * 33 : 0);
   float *thh = txh + (MODE == 1 ? 32 * 33 : 0);
+  double dalpha = (double)a0;
 
-  for (int alpha = a0; alpha < a1; ++alpha) {
+  for (int alpha = a0; alpha < a1; ++alpha, dalpha += 1.0) {
     float us2[CT];
     bool any = false;
 #pragma unroll
     for (int c = 0; c < CT; ++c) {
-      us2[c] = (c < p.C) ? __ldg(p.us2 + (size_t)c * p.n_sft + alpha) : 0.f;
+      us2[c] = __ldg(p.us2 + (size_t)c * p.n_sft + alpha);
       any |= us2[c] > 0.f;
     }
     Track tr;
     tr.active = false;
     tr.kc = -1;
-    if (any || p.kc_out) track_eval(p, tm, alpha, tr);
-    if (any && tr.active) {
-      float zr, zi, hh;
-      pair_terms<KT, CT>(p, tm, alpha, tr, us2, zr, zi, hh);
-      axh += (double)zr;
-      axi += (double)zi;
-      ahh += (double)hh;
+    tr.b = 0.f;
+    if (any || p.kc_out) track_eval(p, tm, dalpha, tr);      // `any` is block-uniform
+    const bool go = any && tr.active;
+    if (any) {
+      const float ab = (go && p.kernel == 1) ? fabsf(tr.b) : 0.f;
+      const float bmax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(ab)));
+      if (go) {
+        float zr, zi, hh;
+        pair_terms<KT, CT>(p, tm, alpha, tr, bmax, us2, zr, zi, hh);
+        if (MODE == 1) {
+          axh += (double)zr;
+          ahh += (double)hh;
+        } else {
+          fxh += zr;
+          fxi += zi;
+          fhh += hh;
+        }
+      }
+    }
+    if (MODE == 0 && (((alpha - a0) & (FLUSH - 1)) == FLUSH - 1)) {
+      axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
+      fxh = 0.f; fxi = 0.f; fhh = 0.f;
     }
     if (p.kc_out && tm.ok) {
 #pragma unroll
       for (int c = 0; c < CT; ++c)
-        if (c < p.C) p.kc_out[((size_t)t * p.C + c) * p.n_sft + alpha] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
+        p.kc_out[((size_t)t * CT + c) * p.n_sft + alpha] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
     }
     if (MODE == 1) {
       const int j = (alpha - a0) & 31;
@@ -424,27 +584,36 @@ __global__ void __launch_bounds__(TILE) sft_main_kernel(const KParams p) {
   }
   if (tm.ok) {
     double *q = p.part + (size_t)blockIdx.y * 3 * p.nT + t;
-    q[0] = axh;
-    q[p.nT] = ahh;
-    q[2 * p.nT] = axi;
+    q[0] = axh + (double)fxh;
+    q[p.nT] = ahh + (double)fhh;
+    q[2 * p.nT] = axi + (double)fxi;
   }
 }
 
-// Sum of the chunk totals in fp64, fixed order (deterministic).
-__global__ void sft_reduce_kernel(const double *part, long long nT, int n_chunks, double *xh, double *hh,
-                                  double *xi) {
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nT) return;
+// Sum of the chunk totals in fp64, fixed order (deterministic).  block = (32 templates, 8 chunk lanes).
+__global__ void __launch_bounds__(256) sft_reduce_kernel(const double *part, long long nT, int n_chunks, double *xh,
+                                                         double *hh, double *xi) {
+  __shared__ double sm[3][8][33];
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const long long t = (long long)blockIdx.x * 32 + tx;
   double s0 = 0.0, s1 = 0.0, s2 = 0.0;
-  for (int c = 0; c < n_chunks; ++c) {
-    const double *q = part + (size_t)c * 3 * nT + t;
-    s0 += q[0];
-    s1 += q[nT];
-    s2 += q[2 * nT];
+  if (t < nT) {
+    for (int c = ty; c < n_chunks; c += 8) {
+      const double *q = part + (size_t)c * 3 * nT + t;
+      s0 += q[0];
+      s1 += q[nT];
+      s2 += q[2 * nT];
+    }
   }
-  xh[t] = s0;
-  hh[t] = s1;
-  if (xi) xi[t] = s2;
+  sm[0][ty][tx] = s0; sm[1][ty][tx] = s1; sm[2][ty][tx] = s2;
+  __syncthreads();
+  if (ty == 0 && t < nT) {
+#pragma unroll
+    for (int j = 1; j < 8; ++j) { s0 += sm[0][j][tx]; s1 += sm[1][j][tx]; s2 += sm[2][j][tx]; }
+    xh[t] = s0;
+    hh[t] = s1;
+    if (xi) xi[t] = s2;
+  }
 }
 
 // Exclusive scan of the chunk totals along the chunk axis, in place, fp64 (the carries).
@@ -479,35 +648,45 @@ __global__ void sft_fixup_kernel(const double *part, long long nT, int n_sft, in
   }
 }
 
-// Whitening of one channel at load time (Eq.(15); DESIGN "store").
+// Whitening of one channel at load time (Eq.(15); DESIGN "store"): writes both pair-planar
+// copies of the zero-padded row of SFT a.  Padded index j <-> bin k = k_lo + j - PAD.
 __global__ void sft_whiten_kernel(const float2 *raw, const double *psd_scale, const double *psd_shape, int n_sft,
-                                  int nb, int k_lo, int kv_lo, int kv_hi, double T, double S_ref, float2 *D,
-                                  float *us2) {
+                                  int nb, int k_lo, int kv_lo, int kv_hi, int PAD, int npair, double T, double S_ref,
+                                  float4 *Dp0, float4 *Dp1, float *us2) {
   const int a = blockIdx.x;
   const double s = psd_scale[a];
   const bool present = isfinite(s) && s > 0.0;
   if (threadIdx.x == 0) us2[a] = present ? (float)(1.0 / s) : 0.f;
   const double pre = present ? 2.0 * sqrt(S_ref / T) / s : 0.0;
-  for (int j = threadIdx.x; j < nb; j += blockDim.x) {
-    const int k = k_lo + j;
+  auto value = [&](int j) {
+    const int jj = j - PAD, k = k_lo + jj;
     float2 o = make_float2(0.f, 0.f);
-    if (present && k >= kv_lo && k < kv_hi) {
-      const double Sk = psd_shape ? psd_shape[j] : 1.0;
-      const float2 v = raw[(size_t)a * nb + j];
+    if (present && jj >= 0 && jj < nb && k >= kv_lo && k < kv_hi) {
+      const double Sk = psd_shape ? psd_shape[jj] : 1.0;
+      const float2 v = raw[(size_t)a * nb + jj];
       const double w = pre / Sk;
       o = make_float2((float)(w * (double)v.x), (float)(-w * (double)v.y));
     }
-    D[(size_t)a * nb + j] = o;
+    return o;
+  };
+  for (int i = threadIdx.x; i < 2 * npair; i += blockDim.x) {
+    const int copy = i >= npair, e = copy ? i - npair : i;
+    const float2 lo = value(2 * e + copy), hi = value(2 * e + copy + 1);
+    (copy ? Dp1 : Dp0)[(size_t)a * npair + e] = make_float4(lo.x, hi.x, lo.y, hi.y);
   }
 }
 
-__global__ void sft_ub2_kernel(const double *psd_shape, int nb, int k_lo, int kv_lo, int kv_hi, double S_ref,
-                               float *ub2) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= nb) return;
-  const int k = k_lo + j;
-  const double Sk = psd_shape ? psd_shape[j] : 1.0;
-  ub2[j] = (k >= kv_lo && k < kv_hi) ? (float)(S_ref / Sk) : 0.f;
+__global__ void sft_ub2_kernel(const double *psd_shape, int nb, int k_lo, int kv_lo, int kv_hi, int PAD, int npair,
+                               double S_ref, float2 *ub0, float2 *ub1) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= 2 * npair) return;
+  const int copy = i >= npair, e = copy ? i - npair : i;
+  auto value = [&](int j) {
+    const int jj = j - PAD, k = k_lo + jj;
+    if (jj < 0 || jj >= nb || k < kv_lo || k >= kv_hi) return 0.f;
+    return (float)(S_ref / (psd_shape ? psd_shape[jj] : 1.0));
+  };
+  (copy ? ub1 : ub0)[e] = make_float2(value(2 * e + copy), value(2 * e + copy + 1));
 }
 
 // SFT_RESP_ANNUAL: (cos, sin)(2 pi t_a / P + psi_c) per (channel, SFT).

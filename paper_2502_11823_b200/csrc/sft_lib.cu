@@ -10,6 +10,7 @@
 
 #include "../../include/sft.h"
 #include "sft_kernels.cuh"
+#include "alu_peaks.cuh"
 
 #define SFT_API extern "C" __attribute__((visibility("default")))
 
@@ -21,8 +22,9 @@ struct sft_plan {
   int n_samp = 0;         // samples per SFT
   int kv_lo = 0, kv_hi = 0;
   cudaStream_t stream = nullptr;
-  float2 *D = nullptr;    // [C][n_sft][nb]
-  float *ub2 = nullptr;   // [C][nb]
+  int PAD = 0, npair = 0; // zero padding (bins) on both sides of a stored row; 16-byte pair entries per row
+  float4 *Dp = nullptr;   // [2][C][n_sft][npair] pair-planar whitened data, two parities (sft_kernels.cuh)
+  float2 *ubp = nullptr;  // [2][C][npair]
   float *us2 = nullptr;   // [C][n_sft]
   float2 *rtab = nullptr; // [C][n_sft]
   double sigma[SFT_MAX_CHANNELS] = {0, 0, 0, 0};
@@ -113,8 +115,12 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
     cudaError_t e2 = cudaMalloc(ptr, bytes);
     if (e2 != cudaSuccess) st = fail(nullptr, SFT_ENOMEM, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e2));
   };
-  alloc((void **)&p->D, C * N * nb * sizeof(float2));
-  alloc((void **)&p->ub2, C * nb * sizeof(float));
+  p->PAD = 2 * d.K + 2;
+  p->npair = (p->nb + 2 * p->PAD + 1) / 2 + 1;
+  const size_t npair = p->npair;
+  (void)nb;
+  alloc((void **)&p->Dp, 2 * C * N * npair * sizeof(float4));
+  alloc((void **)&p->ubp, 2 * C * npair * sizeof(float2));
   alloc((void **)&p->us2, C * N * sizeof(float));
   alloc((void **)&p->rtab, C * N * sizeof(float2));
   if (st == SFT_OK) {
@@ -146,7 +152,7 @@ SFT_API sft_status sft_plan_destroy(sft_plan *p) {
   if (!p) return SFT_OK;
   cudaSetDevice(p->d.device);
   cudaStreamSynchronize(p->stream);
-  cudaFree(p->D); cudaFree(p->ub2); cudaFree(p->us2); cudaFree(p->rtab);
+  cudaFree(p->Dp); cudaFree(p->ubp); cudaFree(p->us2); cudaFree(p->rtab);
   cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->loc);
   if (p->ev0) cudaEventDestroy(p->ev0);
   if (p->ev1) cudaEventDestroy(p->ev1);
@@ -233,11 +239,13 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
     if (p->d.response == SFT_RESP_TABLE)
       cudaMemcpyAsync(p->rtab + (size_t)channel * N, response, N * sizeof(float2), cudaMemcpyDeviceToDevice, p->stream);
   }
-  sftk::sft_whiten_kernel<<<(unsigned)N, 128, 0, p->stream>>>(d_raw, d_scale, d_shape, (int)N, (int)nb, p->d.k_lo, p->kv_lo,
-                                                             p->kv_hi, p->d.t_sft, S_ref, p->D + (size_t)channel * N * nb,
-                                                             p->us2 + (size_t)channel * N);
-  sftk::sft_ub2_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, p->stream>>>(d_shape, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi, S_ref,
-                                                                          p->ub2 + (size_t)channel * nb);
+  const size_t C = p->d.n_channels, npair = p->npair;
+  sftk::sft_whiten_kernel<<<(unsigned)N, 128, 0, p->stream>>>(
+      d_raw, d_scale, d_shape, (int)N, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi, p->PAD, p->npair, p->d.t_sft, S_ref,
+      p->Dp + (size_t)channel * N * npair, p->Dp + (C + (size_t)channel) * N * npair, p->us2 + (size_t)channel * N);
+  sftk::sft_ub2_kernel<<<(unsigned)((2 * npair + 255) / 256), 256, 0, p->stream>>>(
+      d_shape, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi, p->PAD, p->npair, S_ref, p->ubp + (size_t)channel * npair,
+      p->ubp + (C + (size_t)channel) * npair);
   p->launches += 2;
   cudaError_t e = cudaGetLastError();
   cudaError_t e2 = cudaStreamSynchronize(p->stream);
@@ -259,6 +267,8 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.kv_lo = p->kv_lo;
   k.kv_hi = p->kv_hi;
   k.K = p->d.K;
+  k.PAD = p->PAD;
+  k.npair = p->npair;
   k.kernel = p->d.kernel;
   k.pn1 = p->d.waveform == SFT_WF_PN1;
   k.response = p->d.response;
@@ -272,8 +282,8 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
     k.chi[c] = p->d.resp_chi[c];
   }
   k.depth = (float)p->d.resp_depth;
-  k.D = p->D;
-  k.ub2 = p->ub2;
+  k.Dp = p->Dp;
+  k.ubp = p->ubp;
   k.us2 = p->us2;
   k.rtab = p->rtab;
 }
@@ -298,8 +308,10 @@ static cudaError_t launch_main(sft_plan *p, const KParams &k) {
       case 16: SFT_LAUNCH(16, 2); break;
       default: SFT_LAUNCH(0, 2); break;
     }
+  } else if (C == 3) {
+    SFT_LAUNCH(0, 3);
   } else {
-    SFT_LAUNCH(0, sftk::MAXC);
+    SFT_LAUNCH(0, 4);
   }
 #undef SFT_LAUNCH
   cudaEventRecord(p->ev1, p->stream);
@@ -366,7 +378,7 @@ SFT_API sft_status sft_inner_products(sft_plan *p, int64_t nT, const double *par
   k.kc_out = d_kc;
   cudaError_t e = launch_main<0>(p, k);
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
-  sftk::sft_reduce_kernel<<<(unsigned)((nT + 255) / 256), 256, 0, p->stream>>>(p->part, nT, k.n_chunks, d_xh, d_hh, d_xi);
+  sftk::sft_reduce_kernel<<<(unsigned)((nT + 31) / 32), 256, 0, p->stream>>>(p->part, nT, k.n_chunks, d_xh, d_hh, d_xi);
   p->launches++;
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "reduce kernel launch: %s", cudaGetErrorString(e));
@@ -432,5 +444,52 @@ SFT_API sft_status sft_cumulative_snr(sft_plan *p, int64_t nT, const double *par
     if (cum_hh) CU(p, cudaMemcpyAsync(cum_hh, d_ch, mat, cudaMemcpyDeviceToHost, p->stream));
     CU(p, cudaStreamSynchronize(p->stream));
   }
+  return SFT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+SFT_API sft_status sft_measure_alu_peaks(int32_t device, double *out, int32_t n_out) {
+  g_create_err[0] = 0;
+  if (!out || n_out < 1) return fail(nullptr, SFT_EINVAL, "sft_measure_alu_peaks: out is NULL or n_out < 1");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess) return fail(nullptr, SFT_ECUDA, "cudaGetDeviceCount: %s", cudaGetErrorString(e));
+  if (device < 0 || device >= ndev) return fail(nullptr, SFT_EINVAL, "device %d not in 0..%d", device, ndev - 1);
+  CU(nullptr, cudaSetDevice(device));
+  cudaDeviceProp prop;
+  CU(nullptr, cudaGetDeviceProperties(&prop, device));
+  float *d = nullptr;
+  CU(nullptr, cudaMalloc((void **)&d, 64));
+  cudaEvent_t e0, e1;
+  CU(nullptr, cudaEventCreate(&e0));
+  CU(nullptr, cudaEventCreate(&e1));
+  const int blocks = prop.multiProcessorCount * 8, threads = 256;
+  const double lane_ops = (double)blocks * threads * sftk::PEAK_ITERS * sftk::PEAK_ILP;
+  double res[5] = {0, 0, 0, 0, 0};
+  for (int which = 0; which < 5; ++which) {
+    float best = 1e30f;
+    for (int rep = 0; rep < 5; ++rep) {
+      cudaEventRecord(e0, 0);
+      switch (which) {
+        case 0: sftk::peak_ffma_kernel<<<blocks, threads>>>(d, 1.0000001f, 1e-9f); break;
+        case 1: sftk::peak_ffma2_kernel<<<blocks, threads>>>(d, 1.0000001f, 1e-9f); break;
+        case 2: sftk::peak_dfma_kernel<<<blocks, threads>>>(d, 1.0000001, 1e-9); break;
+        case 3: sftk::peak_mufu_kernel<<<blocks, threads>>>(d, 1.5f); break;
+        default: sftk::peak_mix_kernel<<<blocks, threads>>>(d, 1.0000001f, 1e-9f); break;
+      }
+      cudaEventRecord(e1, 0);
+      cudaError_t es = cudaEventSynchronize(e1);
+      if (es != cudaSuccess) { cudaFree(d); return fail(nullptr, SFT_ECUDA, "peak kernel: %s", cudaGetErrorString(es)); }
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, e0, e1);
+      if (rep > 0 && ms < best) best = ms;
+    }
+    const double mult = which == 1 ? 2.0 : (which == 4 ? 1.25 : 1.0);   // packed: 2 lanes; mix: 8 FFMA + 2 MUFU per 8
+    res[which] = lane_ops * mult / (best * 1e-3) / 1e9;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d);
+  for (int i = 0; i < n_out && i < 5; ++i) out[i] = res[i];
   return SFT_OK;
 }
