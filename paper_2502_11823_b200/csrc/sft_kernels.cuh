@@ -38,6 +38,8 @@ constexpr float B_ORDER3 = 0.18f;    // |b| <= : order 3; above: closed Fresnel 
 
 struct KParams {
   int C, n_sft, nb, k_lo, kv_lo, kv_hi, K, PAD, npair;
+  int kwin0, jmax;         // window start j0 = k_c - kwin0 in the padded row; in band iff 2 <= j0 <= jmax + 2
+  unsigned dstride, cstrideD, cstrideU;   // entries: per channel (n_sft*npair), per copy (C*n_sft*npair), (C*npair)
   int kernel, pn1, response;
   double T, t0, f_loT, f_hiT, inv_fref;
   double sigma[MAXC];      // sqrt(T / S_ref,c)
@@ -194,11 +196,10 @@ __device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, dou
   const double fT = tm.F0T * q3 * fma(tm.cf, q2, 1.0);
   const double b = tm.bscale * (q8 * q3) * fma(0.625 * tm.cf, q2, 0.375);
   const double yy = (p.kernel == 1) ? fma(0.5, b, fT) : fT;   // Fresnel: centre of the swept band
-  double kcd = floor(yy + 0.5);
+  const double kcd = floor(yy + 0.5);                       // |kcd| < 2^30: f_hiT is clamped by the host
   if (!(fT >= p.f_loT) || !(fT + b <= p.f_hiT)) return;
   tr.active = true;
   tr.x = (float)(fT - kcd);
-  kcd = fmin(fmax(kcd, -1073741824.0), 1073741824.0);
   tr.kc = (int)kcd;
   tr.b = (float)b;
   tr.frac = (float)(ph - rint(ph));
@@ -218,12 +219,15 @@ __device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, dou
 // J_m).  The central bin (m = 0, |a'| <= 1/2 by construction of k_c, DESIGN A5) uses the Taylor
 // series in z = (pi a')^2.  b = 0 is the Dirichlet kernel e^{i pi a} sinc(a), Eq.(B2) P:451.
 // ---------------------------------------------------------------------------------------------
+// All evaluators below return J^ = 2 pi J (the common factor kappa = 1/(2 pi) of the far recurrence is
+// applied once per (template, SFT) instead of once per bin): with u = 1/a' and X^ = X / kappa,
+//   r^_0 = 2 S u,  q^_1 = (kappa r^_0 - C) u,  r^_2 = (S/2 - 2 kappa q^_1) u,  q^_3 = (3 kappa r^_2 - C/4) u, ...
 template <int ORD>
 struct SeriesK {           // per-(template, SFT) constants, broadcast into both packed lanes
-  float2 S2, mC, c_i1, c_i0;            // order >= 1 : 2S, -C, and  J_i = (c_i0 + c_i1 q_1) w'  (order 1)
+  float2 S2, mC, c_i1, c_i0;            // 2S, -C, and for order 1:  J^_i = (c_i0 + c_i1 q^_1) u
   float2 Sh, mC4, S8, mC16, S32;        // higher orders
   float2 pb, mpb2h, mpb3s;              // pi b, -(pi b)^2/2, -(pi b)^3/6
-  float S, C, pbs;
+  float pbs;
 };
 
 template <int ORD>
@@ -231,11 +235,11 @@ __device__ __forceinline__ void series_setup(float xp, float b, SeriesK<ORD> &k)
   float S, C;
   sincospi_fast(xp, S, C);
   const float pb = PI_F * b;
-  k.S = S; k.C = C; k.pbs = pb;
+  k.pbs = pb;
   k.S2 = bc(2.0f * S);
   k.mC = bc(-C);
   if (ORD == 1) {
-    k.c_i1 = bc(-2.0f * pb);
+    k.c_i1 = bc(-2.0f * INV_2PI_F * pb);
     k.c_i0 = bc(0.5f * pb * S);
   }
   if (ORD >= 2) {
@@ -252,64 +256,47 @@ __device__ __forceinline__ void series_setup(float xp, float b, SeriesK<ORD> &k)
   }
 }
 
-// two far bins at once; w = {1/(2 pi a_lo), 1/(2 pi a_hi)}
+// two far bins at once; u = {1/a_lo, 1/a_hi}
 template <int ORD>
-__device__ __forceinline__ void series_far2(const SeriesK<ORD> &k, float2 w, float2 &Jr, float2 &Ji) {
-  const float2 r0 = __fmul2_rn(k.S2, w);
+__device__ __forceinline__ void series_far2(const SeriesK<ORD> &k, float2 u, float2 &Jr, float2 &Ji) {
+  const float2 r0 = __fmul2_rn(k.S2, u);
   Jr = r0;
   if (ORD == 0) {
     Ji = make_float2(0.f, 0.f);
-  } else if (ORD == 1) {
-    const float2 q1 = __fmul2_rn(__fadd2_rn(r0, k.mC), w);
-    Ji = __fmul2_rn(__ffma2_rn(k.c_i1, q1, k.c_i0), w);
   } else {
-    const float2 q1 = __fmul2_rn(__fadd2_rn(r0, k.mC), w);
-    const float2 r2 = __fmul2_rn(__ffma2_rn(bc(-2.0f), q1, k.Sh), w);
-    const float2 q3 = __fmul2_rn(__ffma2_rn(bc(3.0f), r2, k.mC4), w);
-    const float2 r4 = __fmul2_rn(__ffma2_rn(bc(-4.0f), q3, k.S8), w);
-    Jr = __ffma2_rn(k.mpb2h, r4, r0);
-    Ji = __fmul2_rn(k.pb, r2);
-    if (ORD >= 3) {
-      const float2 q5 = __fmul2_rn(__ffma2_rn(bc(5.0f), r4, k.mC16), w);
-      const float2 r6 = __fmul2_rn(__ffma2_rn(bc(-6.0f), q5, k.S32), w);
-      Ji = __ffma2_rn(k.mpb3s, r6, Ji);
-    }
-  }
-}
-
-// one far bin (scalar twin of series_far2)
-template <int ORD>
-__device__ __forceinline__ void series_far1(const SeriesK<ORD> &k, float a, float &Jr, float &Ji) {
-  const float w = rcp_approx(2.0f * PI_F * a);
-  const float r0 = 2.0f * k.S * w;
-  Jr = r0;
-  Ji = 0.f;
-  if (ORD >= 1) {
-    const float q1 = (r0 - k.C) * w;
-    const float r2 = fmaf(-2.0f, q1, 0.5f * k.S) * w;
-    Ji = k.pbs * r2;
-    if (ORD >= 2) {
-      const float q3 = fmaf(3.0f, r2, -0.25f * k.C) * w;
-      const float r4 = fmaf(-4.0f, q3, 0.125f * k.S) * w;
-      Jr = fmaf(-0.5f * k.pbs * k.pbs, r4, r0);
+    const float2 q1 = __fmul2_rn(__ffma2_rn(bc(INV_2PI_F), r0, k.mC), u);
+    if (ORD == 1) {
+      Ji = __fmul2_rn(__ffma2_rn(k.c_i1, q1, k.c_i0), u);
+    } else {
+      const float2 r2 = __fmul2_rn(__ffma2_rn(bc(-2.0f * INV_2PI_F), q1, k.Sh), u);
+      const float2 q3 = __fmul2_rn(__ffma2_rn(bc(3.0f * INV_2PI_F), r2, k.mC4), u);
+      const float2 r4 = __fmul2_rn(__ffma2_rn(bc(-4.0f * INV_2PI_F), q3, k.S8), u);
+      Jr = __ffma2_rn(k.mpb2h, r4, r0);
+      Ji = __fmul2_rn(k.pb, r2);
       if (ORD >= 3) {
-        const float q5 = fmaf(5.0f, r4, -0.0625f * k.C) * w;
-        const float r6 = fmaf(-6.0f, q5, 0.03125f * k.S) * w;
-        Ji = fmaf(-(1.0f / 6.0f) * k.pbs * k.pbs * k.pbs, r6, Ji);
+        const float2 q5 = __fmul2_rn(__ffma2_rn(bc(5.0f * INV_2PI_F), r4, k.mC16), u);
+        const float2 r6 = __fmul2_rn(__ffma2_rn(bc(-6.0f * INV_2PI_F), q5, k.S32), u);
+        Ji = __ffma2_rn(k.mpb3s, r6, Ji);
       }
     }
   }
 }
 
-// Taylor coefficients of r_2n(a') = 4^-n sum_p (-1)^p z^p / ((2p)! (2n+2p+1)),  z = (pi a')^2 <= (pi/2)^2;
-// 7 terms: truncation < 5e-10.  Packed as {r_0, r_2} and {r_4, r_6}.
+// {1/a, 1/b} with one MUFU reciprocal
+__device__ __forceinline__ float2 rcp2(float a, float b) {
+  const float rp = rcp_approx(a * b);
+  return make_float2(b * rp, a * rp);
+}
+
+// Taylor coefficients of 2 pi r_2n(a') = 2 pi 4^-n sum_p (-1)^p z^p / ((2p)! (2n+2p+1)),  z = (pi a')^2 <= (pi/2)^2;
+// 7 terms: truncation < 5e-10 (relative to r_0 <= 1).  Packed as {r_0, r_2} and {r_4, r_6}.
 __device__ __forceinline__ constexpr float tay_c(int n, int pp) {
   double f = 1.0;
   for (int i = 2; i <= 2 * pp; ++i) f *= (double)i;
   double s = (pp & 1) ? -1.0 : 1.0;
   double four = 1.0;
   for (int i = 0; i < n; ++i) four *= 4.0;
-  return (float)(s / (f * (double)(2 * n + 2 * pp + 1) * four));
+  return (float)(6.283185307179586 * s / (f * (double)(2 * n + 2 * pp + 1) * four));
 }
 
 template <int ORD>
@@ -319,8 +306,8 @@ __device__ __forceinline__ void series_central(const SeriesK<ORD> &k, float a, f
   float2 lo = make_float2(tay_c(0, 6), tay_c(1, 6));
 #pragma unroll
   for (int pp = 5; pp >= 0; --pp) lo = __ffma2_rn(lo, z, make_float2(tay_c(0, pp), tay_c(1, pp)));
-  Jr = lo.x;                 // r_0
-  Ji = k.pbs * lo.y;         // pi b r_2
+  Jr = lo.x;                 // r^_0
+  Ji = k.pbs * lo.y;         // pi b r^_2
   if (ORD == 0) Ji = 0.f;
   if (ORD >= 2) {
     float2 hi = make_float2(tay_c(2, 6), tay_c(3, 6));
@@ -369,56 +356,63 @@ struct Acc {
 };
 
 template <int CT>
-__device__ __forceinline__ void mac_pair(const KParams &p, const float4 *Drow, const float2 *urow, size_t dstride,
-                                         size_t ustride, int q, float2 Jr, float2 Ji, Acc (&acc)[CT]) {
+__device__ __forceinline__ void mac_pair(const KParams &p, const float4 *Drow, const float2 *urow, int q, float2 Jr,
+                                         float2 Ji, Acc (&acc)[CT]) {
   const float2 mag = __ffma2_rn(Ji, Ji, __fmul2_rn(Jr, Jr));
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
-    {
-      const float4 d = __ldg(Drow + c * dstride + q);
-      const float2 u = __ldg(urow + c * ustride + q);
-      const float2 dre = make_float2(d.x, d.y), dim = make_float2(d.z, d.w);
-      acc[c].A = __ffma2_rn(dre, Jr, acc[c].A);
-      acc[c].B = __ffma2_rn(dim, Ji, acc[c].B);
-      acc[c].I = __ffma2_rn(dre, Ji, acc[c].I);
-      acc[c].I = __ffma2_rn(dim, Jr, acc[c].I);
-      acc[c].W = __ffma2_rn(u, mag, acc[c].W);
-    }
+    const float4 d = __ldg(Drow + c * p.dstride + q);
+    const float2 u = __ldg(urow + c * p.npair + q);
+    const float2 dre = make_float2(d.x, d.y), dim = make_float2(d.z, d.w);
+    acc[c].A = __ffma2_rn(dre, Jr, acc[c].A);
+    acc[c].B = __ffma2_rn(dim, Ji, acc[c].B);
+    acc[c].I = __ffma2_rn(dre, Ji, acc[c].I);
+    acc[c].I = __ffma2_rn(dim, Jr, acc[c].I);
+    acc[c].W = __ffma2_rn(u, mag, acc[c].W);
   }
 }
 
 // Series path of one (template, SFT): all K+1 bin pairs.  Pair q holds m = -K+2q (lo) and -K+2q+1 (hi);
-// the hi lane of the last pair (m = K+1) is outside the band and gets J = 0.
+// the hi lane of the last pair (m = K+1) is outside the band and gets J = 0.  The two pairs that are not
+// "two far bins" - the one holding the central bin m = 0 (with its neighbour m_p = +1 or -1) and the last
+// one (m = K) - share one packed far evaluation {m_p, K}.
 template <int ORD, int KT, int CT>
 __device__ __forceinline__ void series_pairs(const KParams &p, float xp, float b, const float4 *Drow, const float2 *urow,
-                                             size_t dstride, size_t ustride, Acc (&acc)[CT]) {
+                                             Acc (&acc)[CT]) {
   const int K = KT > 0 ? KT : p.K;
   SeriesK<ORD> k;
   series_setup<ORD>(xp, b, k);
   const int qc = K >> 1;                 // pair holding m = 0 (lo lane if K even, hi lane if K odd)
+  const bool c_lo = (K & 1) == 0;
   const float a0 = xp + (float)K;        // a' of m = -K
+  float2 Jc_r, Jc_i, Jl_r = make_float2(0.f, 0.f), Jl_i = make_float2(0.f, 0.f);
+  {
+    float c_r, c_i;
+    series_central<ORD>(k, xp, c_r, c_i);
+    float2 Fr = make_float2(0.f, 0.f), Fi = make_float2(0.f, 0.f);
+    if (K >= 1) series_far2<ORD>(k, rcp2(c_lo ? xp - 1.0f : xp + 1.0f, xp - (float)K), Fr, Fi);
+    Jc_r = c_lo ? make_float2(c_r, Fr.x) : make_float2(Fr.x, c_r);
+    Jc_i = c_lo ? make_float2(c_i, Fi.x) : make_float2(Fi.x, c_i);
+    if (K == 0) { Jc_r.y = 0.f; Jc_i.y = 0.f; }      // single pair: hi lane is m = 1 > K
+    Jl_r.x = Fr.y;
+    Jl_i.x = Fi.y;
+  }
 #pragma unroll
   for (int q = 0; q <= K; ++q) {
     float2 Jr, Ji;
-    const float a_lo = a0 - (float)(2 * q), a_hi = a_lo - 1.0f;
-    if (q == qc || q == K) {
-      const int m_lo = -K + 2 * q, m_hi = m_lo + 1;
-      if (m_lo == 0) series_central<ORD>(k, a_lo, Jr.x, Ji.x);
-      else series_far1<ORD>(k, a_lo, Jr.x, Ji.x);
-      if (m_hi == 0) series_central<ORD>(k, a_hi, Jr.y, Ji.y);
-      else if (m_hi > K) { Jr.y = 0.f; Ji.y = 0.f; }
-      else series_far1<ORD>(k, a_hi, Jr.y, Ji.y);
-    } else {
-      const float rp = rcp_approx(a_lo * a_hi) * INV_2PI_F;
-      series_far2<ORD>(k, make_float2(a_hi * rp, a_lo * rp), Jr, Ji);
+    if (q == qc) { Jr = Jc_r; Ji = Jc_i; }
+    else if (q == K) { Jr = Jl_r; Ji = Jl_i; }
+    else {
+      const float a_lo = a0 - (float)(2 * q);
+      series_far2<ORD>(k, rcp2(a_lo, a_lo - 1.0f), Jr, Ji);
     }
-    mac_pair<CT>(p, Drow, urow, dstride, ustride, q, Jr, Ji, acc);
+    mac_pair<CT>(p, Drow, urow, q, Jr, Ji, acc);
   }
 }
 
 template <int KT, int CT>
 __device__ __forceinline__ void fresnel_pairs(const KParams &p, float x, float b, const float4 *Drow, const float2 *urow,
-                                              size_t dstride, size_t ustride, Acc (&acc)[CT], float &scale) {
+                                              Acc (&acc)[CT], float &scale) {
   const int K = KT > 0 ? KT : p.K;
   FresK k;
   k.neg = b < 0.f;
@@ -437,25 +431,30 @@ __device__ __forceinline__ void fresnel_pairs(const KParams &p, float x, float b
     fresnel_bin(k, m_lo, Jr.x, Ji.x);
     if (m_lo + 1 > K) { Jr.y = 0.f; Ji.y = 0.f; }
     else fresnel_bin(k, m_lo + 1, Jr.y, Ji.y);
-    mac_pair<CT>(p, Drow, urow, dstride, ustride, q, Jr, Ji, acc);
+    mac_pair<CT>(p, Drow, urow, q, Jr, Ji, acc);
   }
 }
 
 // Z_c = Re/Im of the per-(SFT, channel) complex term, H_c its <h,h> term (include/sft.h).
 // `bmax` is the warp-wide max |b| of the pairs being evaluated: it selects the series order for the
-// whole warp (a higher order than a lane needs is still correct for that lane).
+// whole warp (a higher order than a lane needs is still correct for that lane).  `arow` = alpha * npair.
 template <int KT, int CT>
-__device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int alpha, const Track &tr, float bmax,
-                                           const float (&us2)[CT], float &zr, float &zi, float &hh) {
-  const int K = KT > 0 ? KT : p.K;
+__device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int alpha, unsigned arow, const Track &tr,
+                                           float bmax, const float (&us2)[CT], float &zr, float &zi, float &hh) {
   zr = 0.f; zi = 0.f; hh = 0.f;
   // window start in the zero-padded row; windows that miss the stored band entirely contribute 0
-  if (tr.kc + K < p.k_lo || tr.kc - K >= p.k_lo + p.nb) return;
-  const int j0 = tr.kc - K - p.k_lo + p.PAD;
-  const int copy = j0 & 1;
-  const size_t dstride = (size_t)p.n_sft * p.npair, ustride = (size_t)p.npair;
-  const float4 *Drow = p.Dp + (size_t)copy * CT * dstride + (size_t)alpha * p.npair + (j0 >> 1);
-  const float2 *urow = p.ubp + (size_t)copy * CT * ustride + (j0 >> 1);
+  const int j0 = tr.kc - p.kwin0;                       // kwin0 = k_lo + K - PAD
+  if ((unsigned)(j0 - 2) > (unsigned)p.jmax) return;    // 2 <= j0 <= nb - 1 + PAD  <=>  window overlaps the band
+  const unsigned e0 = (unsigned)(j0 >> 1), cp = (unsigned)(j0 & 1);
+  const float4 *Drow = p.Dp + (cp * p.cstrideD + arow + e0);
+  const float2 *urow = p.ubp + (cp * p.cstrideU + e0);
+  // the same window of the next SFT will be wanted next: pull its lines into L1 now (rows are contiguous)
+  {
+    const char *nx = (const char *)(Drow + p.npair);
+#pragma unroll
+    for (int o = 0; o < (KT > 0 ? (KT + 1) * 16 + 127 : 128); o += 128)
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(nx + o));
+  }
   Acc acc[CT];
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
@@ -463,24 +462,25 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int
   }
   const bool fres = (p.kernel == 1);
   const float b = fres ? tr.b : 0.f;
-  float scale = 1.0f;
-  float t;    // total phase / pi:  2 frac (= phi_a/pi) + prefactor phase / pi
+  float scale = INV_2PI_F;     // the series evaluators return 2 pi J
+  float t;                     // total phase / pi:  2 frac (= phi_a/pi) + prefactor phase / pi
   if (bmax <= B_ORDER3 || fabsf(b) <= B_ORDER3) {
     const float xp = fmaf(0.5f, b, tr.x);
-    if (bmax == 0.f) series_pairs<0, KT, CT>(p, xp, b, Drow, urow, dstride, ustride, acc);
-    else if (bmax <= B_ORDER1) series_pairs<1, KT, CT>(p, xp, b, Drow, urow, dstride, ustride, acc);
-    else if (bmax <= B_ORDER2) series_pairs<2, KT, CT>(p, xp, b, Drow, urow, dstride, ustride, acc);
-    else series_pairs<3, KT, CT>(p, xp, b, Drow, urow, dstride, ustride, acc);
+    if (bmax == 0.f) series_pairs<0, KT, CT>(p, xp, b, Drow, urow, acc);
+    else if (bmax <= B_ORDER1) series_pairs<1, KT, CT>(p, xp, b, Drow, urow, acc);
+    else if (bmax <= B_ORDER2) series_pairs<2, KT, CT>(p, xp, b, Drow, urow, acc);
+    else series_pairs<3, KT, CT>(p, xp, b, Drow, urow, acc);
     t = fmaf(2.0f, tr.frac, fmaf(0.25f, b, tr.x));         // prefactor e^{i pi (x + b/4)}
   } else {
-    fresnel_pairs<KT, CT>(p, tr.x, b, Drow, urow, dstride, ustride, acc, scale);
+    fresnel_pairs<KT, CT>(p, tr.x, b, Drow, urow, acc, scale);
     t = 2.0f * tr.frac;
   }
   t = fmaf(-2.0f, rintf(0.5f * t), t);                       // into [-1, 1]
-  float sp, cp;
-  sincospi_fast(t, sp, cp);
-  const float er = cp * scale * tr.amp, ei = sp * scale * tr.amp;
-  const float a2 = tr.amp * tr.amp * scale * scale;
+  float sp, cp_;
+  sincospi_fast(t, sp, cp_);
+  const float as = scale * tr.amp;
+  const float er = cp_ * as, ei = sp * as;
+  const float a2 = as * as;
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
     if (us2[c] > 0.f) {
@@ -490,10 +490,10 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int
       // response (Eq.(5)-(6) P:80-85 as Lambda z = Re[R z]; DESIGN C3/D4)
       float2 R = tm.AE[c];
       if (p.response == 1) {
-        const float2 r = __ldg(p.rtab + (size_t)c * p.n_sft + alpha);
+        const float2 r = __ldg(p.rtab + (c * p.n_sft + alpha));
         R = make_float2(tm.AE[c].x * r.x, tm.AE[c].x * r.y);      // AE is real here
       } else if (p.response == 2) {
-        const float2 cs = __ldg(p.rtab + (size_t)c * p.n_sft + alpha);
+        const float2 cs = __ldg(p.rtab + (c * p.n_sft + alpha));
         const float am = fmaf(p.depth, cs.x * tm.cl - cs.y * tm.sl, 1.0f);
         R = make_float2(R.x * am, R.y * am);
       }
@@ -506,12 +506,15 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int
 }
 
 // ---------------------------------------------------------------------------------------------
-// Main fused kernel.  grid = (template tiles, SFT chunks); CT == number of channels (exactly).  MODE 0: chunk totals only.
-// MODE 1 (cumulative): additionally writes chunk-local inclusive prefix sums, transposed through
-// shared memory so that global stores are 128-byte rows along the SFT axis.
+// Main fused kernel.  grid = (template tiles, SFT chunks); CT == number of channels (exactly).
+// MODE 0: chunk totals only.  MODE 1 (cumulative): additionally writes chunk-local inclusive prefix
+// sums, transposed through shared memory so that global stores are 128-byte rows along the SFT axis.
+// The SFT loop runs in groups of GROUP: fp32 partial sums flushed into fp64 per group (MODE 0),
+// one transposed store per group (MODE 1).
 // ---------------------------------------------------------------------------------------------
 template <int KT, int CT, int MODE>
 __global__ void __launch_bounds__(TILE) sft_main_kernel(const KParams p) {
+  constexpr int GROUP = MODE == 1 ? 32 : FLUSH;
   __shared__ float tile_s[MODE == 1 ? (TILE / 32) * 2 * 32 * 33 : 1];
   const long long t = (long long)blockIdx.x * TILE + threadIdx.x;
   const int a0 = blockIdx.y * p.chunk;
@@ -519,74 +522,75 @@ __global__ void __launch_bounds__(TILE) sft_main_kernel(const KParams p) {
   Tmpl tm;
   tmpl_init(p, t, tm);
   double axh = 0.0, ahh = 0.0, axi = 0.0;
-  float fxh = 0.f, fhh = 0.f, fxi = 0.f;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float *txh = tile_s + (MODE == 1 ? warp * 2 * 32 * 33 : 0);
   float *thh = txh + (MODE == 1 ? 32 * 33 : 0);
   double dalpha = (double)a0;
+  unsigned arow = (unsigned)a0 * (unsigned)p.npair;
 
-  for (int alpha = a0; alpha < a1; ++alpha, dalpha += 1.0) {
-    float us2[CT];
-    bool any = false;
+  for (int g = a0; g < a1; g += GROUP) {
+    const int ge = min(g + GROUP, a1);
+    float fxh = 0.f, fhh = 0.f, fxi = 0.f;
+    for (int alpha = g; alpha < ge; ++alpha, dalpha += 1.0, arow += p.npair) {
+      float us2[CT];
+      bool any = false;
 #pragma unroll
-    for (int c = 0; c < CT; ++c) {
-      us2[c] = __ldg(p.us2 + (size_t)c * p.n_sft + alpha);
-      any |= us2[c] > 0.f;
-    }
-    Track tr;
-    tr.active = false;
-    tr.kc = -1;
-    tr.b = 0.f;
-    if (any || p.kc_out) track_eval(p, tm, dalpha, tr);      // `any` is block-uniform
-    const bool go = any && tr.active;
-    if (any) {
-      const float ab = (go && p.kernel == 1) ? fabsf(tr.b) : 0.f;
-      const float bmax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(ab)));
-      if (go) {
-        float zr, zi, hh;
-        pair_terms<KT, CT>(p, tm, alpha, tr, bmax, us2, zr, zi, hh);
-        if (MODE == 1) {
-          axh += (double)zr;
-          ahh += (double)hh;
-        } else {
-          fxh += zr;
-          fxi += zi;
-          fhh += hh;
-        }
+      for (int c = 0; c < CT; ++c) {
+        us2[c] = __ldg(p.us2 + (c * p.n_sft + alpha));
+        any |= us2[c] > 0.f;
       }
-    }
-    if (MODE == 0 && (((alpha - a0) & (FLUSH - 1)) == FLUSH - 1)) {
-      axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
-      fxh = 0.f; fxi = 0.f; fhh = 0.f;
-    }
-    if (p.kc_out && tm.ok) {
-#pragma unroll
-      for (int c = 0; c < CT; ++c)
-        p.kc_out[((size_t)t * CT + c) * p.n_sft + alpha] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
-    }
-    if (MODE == 1) {
-      const int j = (alpha - a0) & 31;
-      txh[lane * 33 + j] = (float)axh;
-      thh[lane * 33 + j] = (float)ahh;
-      if (j == 31 || alpha == a1 - 1) {
-        __syncwarp();
-        const int base = alpha - j;
-        for (int r = 0; r < 32; ++r) {
-          const long long tt = (long long)blockIdx.x * TILE + warp * 32 + r;
-          if (tt < p.nT && lane <= j) {
-            p.loc_xh[(size_t)tt * p.n_sft + base + lane] = txh[r * 33 + lane];
-            p.loc_hh[(size_t)tt * p.n_sft + base + lane] = thh[r * 33 + lane];
+      Track tr;
+      tr.active = false;
+      tr.kc = -1;
+      tr.b = 0.f;
+      if (any || p.kc_out) track_eval(p, tm, dalpha, tr);      // `any` is block-uniform
+      const bool go = any && tr.active;
+      if (any) {
+        const float ab = (go && p.kernel == 1) ? fabsf(tr.b) : 0.f;
+        const float bmax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(ab)));
+        if (go) {
+          float zr, zi, hh;
+          pair_terms<KT, CT>(p, tm, alpha, arow, tr, bmax, us2, zr, zi, hh);
+          if (MODE == 1) {
+            axh += (double)zr;
+            ahh += (double)hh;
+          } else {
+            fxh += zr;
+            fxi += zi;
+            fhh += hh;
           }
         }
-        __syncwarp();
       }
+      if (p.kc_out && tm.ok) {
+#pragma unroll
+        for (int c = 0; c < CT; ++c)
+          p.kc_out[((size_t)t * CT + c) * p.n_sft + alpha] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
+      }
+      if (MODE == 1) {
+        txh[lane * 33 + (alpha - g)] = (float)axh;
+        thh[lane * 33 + (alpha - g)] = (float)ahh;
+      }
+    }
+    if (MODE == 0) {
+      axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
+    } else {
+      __syncwarp();
+      const int n = ge - g;
+      for (int r = 0; r < 32; ++r) {
+        const long long tt = (long long)blockIdx.x * TILE + warp * 32 + r;
+        if (tt < p.nT && lane < n) {
+          p.loc_xh[(size_t)tt * p.n_sft + g + lane] = txh[r * 33 + lane];
+          p.loc_hh[(size_t)tt * p.n_sft + g + lane] = thh[r * 33 + lane];
+        }
+      }
+      __syncwarp();
     }
   }
   if (tm.ok) {
     double *q = p.part + (size_t)blockIdx.y * 3 * p.nT + t;
-    q[0] = axh + (double)fxh;
-    q[p.nT] = ahh + (double)fhh;
-    q[2 * p.nT] = axi + (double)fxi;
+    q[0] = axh;
+    q[p.nT] = ahh;
+    q[2 * p.nT] = axi;
   }
 }
 

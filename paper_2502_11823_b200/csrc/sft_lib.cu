@@ -119,7 +119,9 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   p->npair = (p->nb + 2 * p->PAD + 1) / 2 + 1;
   const size_t npair = p->npair;
   (void)nb;
-  alloc((void **)&p->Dp, 2 * C * N * npair * sizeof(float4));
+  if (2.0 * C * (double)N * npair + npair >= 2147483648.0)
+    st = fail(nullptr, SFT_EUNSUPPORTED, "data store of %.3g pair entries exceeds 32-bit indexing", 2.0 * C * (double)N * npair);
+  alloc((void **)&p->Dp, (2 * C * N + 1) * npair * sizeof(float4));   // + one row: the kernel prefetches one row ahead
   alloc((void **)&p->ubp, 2 * C * npair * sizeof(float2));
   alloc((void **)&p->us2, C * N * sizeof(float));
   alloc((void **)&p->rtab, C * N * sizeof(float2));
@@ -269,13 +271,18 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.K = p->d.K;
   k.PAD = p->PAD;
   k.npair = p->npair;
+  k.kwin0 = p->d.k_lo + p->d.K - p->PAD;
+  k.jmax = p->nb - 1 + p->PAD - 2;
+  k.dstride = (unsigned)(p->d.n_sft * p->npair);
+  k.cstrideD = (unsigned)(p->d.n_channels * p->d.n_sft * p->npair);
+  k.cstrideU = (unsigned)(p->d.n_channels * p->npair);
   k.kernel = p->d.kernel;
   k.pn1 = p->d.waveform == SFT_WF_PN1;
   k.response = p->d.response;
   k.T = p->d.t_sft;
   k.t0 = p->d.t0;
   k.f_loT = p->d.f_lo * p->d.t_sft;
-  k.f_hiT = p->d.f_hi * p->d.t_sft;
+  k.f_hiT = fmin(p->d.f_hi * p->d.t_sft, 1.0e9);   // keeps k_c inside int32 (bins beyond 1e9 do not exist)
   k.inv_fref = 1.0 / p->d.f_ref;
   for (int c = 0; c < SFT_MAX_CHANNELS; ++c) {
     k.sigma[c] = p->sigma[c];
