@@ -139,9 +139,17 @@ int64_t sft_plan_launch_count(const sft_plan *plan);
  * until that launch has finished.  < 0 if nothing has been launched. */
 double sft_plan_last_kernel_ms(sft_plan *plan);
 
-/* Tuning knob: SFTs per block along the time axis (0 = automatic).  Results do not depend on it
+/* Diagnostic: how the coefficient evaluator (rows A4/A6 of the hot path) was used by the most recent
+ * sft_inner_products call that had kc_out != NULL: the number of active (template, SFT, channel) pairs
+ * evaluated with the series in b = fdot T^2 about the Dirichlet kernel at order 0, 1, 2, 3 (out[0..3])
+ * and with the closed Fresnel form Eq.(29) P:219 (out[4]).  The order is chosen per warp of 32
+ * templates from the largest |b| in the warp.  Blocks until that call finished.
+ * Writes min(n_out, 5) values; host pointer. */
+sft_status sft_plan_path_counts(sft_plan *plan, int64_t *out, int32_t n_out);
+
+/* Tuning knob: SFTs per work unit along the time axis (0 = automatic).  Results do not depend on it
  * beyond fp64 summation order. */
-sft_status sft_plan_set_chunk(sft_plan *plan, int32_t sfts_per_block);
+sft_status sft_plan_set_chunk(sft_plan *plan, int32_t sfts_per_unit);
 
 /* Diagnostic: measures the plain-ALU pipe rates of `device` that bound this path (the
  * data store is L2 resident, so FP32 / FP64 / XU issue rates, not HBM, are the roofline).  Writes up

@@ -18,6 +18,7 @@ KERNEL = {"dirichlet": 0, "fresnel": 1}
 RESPONSE = {"none": 0, "table": 1, "annual": 2}
 PHASE = {"fp64": 0, "split32": 1}
 MEM_HOST, MEM_DEVICE = 0, 1
+PATHS = ("series0", "series1", "series2", "series3", "fresnel")
 STATUS = {0: "SFT_OK", 1: "SFT_EINVAL", 2: "SFT_ESHAPE", 3: "SFT_ENODATA", 4: "SFT_EUNSUPPORTED",
           5: "SFT_ECUDA", 6: "SFT_ENOMEM"}
 
@@ -43,7 +44,8 @@ class PlanDesc(C.Structure):
 
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
-           "sft_plan_set_chunk", "sft_last_error", "sft_version", "sft_measure_alu_peaks"]
+           "sft_plan_set_chunk", "sft_plan_path_counts", "sft_last_error", "sft_version",
+           "sft_measure_alu_peaks"]
 
 _lib = None
 
@@ -69,13 +71,14 @@ def load_library(path=None):
     lib.sft_plan_last_kernel_ms.argtypes = [vp]
     lib.sft_plan_last_kernel_ms.restype = dbl
     lib.sft_plan_set_chunk.argtypes = [vp, i32]
+    lib.sft_plan_path_counts.argtypes = [vp, C.POINTER(i64), i32]
     lib.sft_measure_alu_peaks.argtypes = [i32, C.POINTER(dbl), i32]
     lib.sft_measure_alu_peaks.restype = i32
     lib.sft_last_error.argtypes = [vp]
     lib.sft_last_error.restype = C.c_char_p
     lib.sft_version.restype = C.c_char_p
     for f in ("sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
-              "sft_cumulative_snr", "sft_plan_sync", "sft_plan_set_chunk"):
+              "sft_cumulative_snr", "sft_plan_sync", "sft_plan_set_chunk", "sft_plan_path_counts"):
         getattr(lib, f).restype = i32
     _lib = lib
     return lib
@@ -214,8 +217,14 @@ class Plan:
     def last_kernel_ms(self):
         return float(self.lib.sft_plan_last_kernel_ms(self._h))
 
-    def set_chunk(self, sfts_per_block):
-        self._check(self.lib.sft_plan_set_chunk(self._h, int(sfts_per_block)))
+    def set_chunk(self, sfts_per_unit):
+        self._check(self.lib.sft_plan_set_chunk(self._h, int(sfts_per_unit)))
+
+    def path_counts(self):
+        """``sft_plan_path_counts``: dict path name -> active pairs of the last call that had kc_out."""
+        out = (C.c_int64 * 5)()
+        self._check(self.lib.sft_plan_path_counts(self._h, out, 5))
+        return dict(zip(PATHS, [int(v) for v in out]))
 
 
 def plan_from_workload(w, device=0, stream=None, **override):

@@ -8,6 +8,11 @@
 // warp-uniform, and (iii) the sum over SFTs needs no cross-lane traffic at all: it is a private
 // accumulator per thread (fp32 over 8 SFTs, flushed into fp64).
 //
+// Scheduling.  The unit of work is (32 templates) x (one chunk of SFTs).  The grid is persistent
+// (SM count x resident blocks); every WARP draws work units from one global counter, latest chunks
+// (largest b, most expensive) first, so that no SM idles behind a tail of equal-sized blocks.  The
+// per-template constants are computed once per call by sft_tmpl_kernel.
+//
 // Inner loop.  The 2K+1 bins of a pair are processed two adjacent bins at a time with the packed
 // fp32x2 instructions of sm_100 (FADD2/FMUL2/FFMA2: one issue slot, two lanes).  The store keeps
 // the whitened data "pair-planar", {re_j, re_j+1, im_j, im_j+1} per 16 bytes, in two copies (pairs
@@ -51,8 +56,13 @@ struct KParams {
   const float *us2;        // [C][n_sft]            1 / s_a       (0 for gaps)
   const float2 *rtab;      // [C][n_sft]            TABLE: R_{c,a}; ANNUAL: (cos, sin)(2 pi t_a/P + psi_c)
   const double *params;    // [nT][8]
+  const double *td;        // [TD_N][nT]  per-template fp64 constants (sft_tmpl_kernel)
+  const float *tf;         // [TF_N][nT]  per-template fp32 constants
   long long nT;
   int chunk, n_chunks;
+  int n_tgroups, n_items;  // work units: n_tgroups = ceil(nT/32) template groups x n_chunks
+  int *counter;            // work-unit counter (zeroed before every launch)
+  unsigned long long *path_counts;   // nullable [PATH_N]: active pairs per evaluator path (diagnostic)
   double *part;            // [n_chunks][3][nT] chunk totals (xh, hh, xh_im)
   int *kc_out;             // [nT][C][n_sft] or null
   float *loc_xh, *loc_hh;  // cumulative mode: [nT][n_sft] chunk-local prefix sums
@@ -120,49 +130,89 @@ __device__ __forceinline__ void fresnel_w(float t, float &g, float &f) {
   }
 }
 
+// Compile-time plan flags of a kernel variant; -1 = read the flag from KParams at run time.
+template <int KERNEL_, int PN1_, int RESP_, int KC_>
+struct Cfg {
+  static constexpr int KERNEL = KERNEL_, PN1 = PN1_, RESP = RESP_, KC = KC_;
+};
+template <class CFG> __device__ __forceinline__ int cfg_kernel(const KParams &p) { return CFG::KERNEL >= 0 ? CFG::KERNEL : p.kernel; }
+template <class CFG> __device__ __forceinline__ int cfg_pn1(const KParams &p) { return CFG::PN1 >= 0 ? CFG::PN1 : p.pn1; }
+template <class CFG> __device__ __forceinline__ int cfg_resp(const KParams &p) { return CFG::RESP >= 0 ? CFG::RESP : p.response; }
+
 // Per-template constants, fp64 where the phase needs it (the template is "described by 4
 // numbers" per SFT; these are the closed-form coefficients of those 4 numbers, DESIGN W1).
+// Layout in global memory: structure of arrays, component-major with stride nT.
+enum { TD_TAU0 = 0, TD_CTHETA, TD_PHIC, TD_CPHASE, TD_CPHI, TD_CF, TD_F0T, TD_BSCALE, TD_N };
+enum { TF_CF = 0, TF_CL, TF_SL, TF_AE, TF_N = TF_AE + 2 * MAXC };
+
 struct Tmpl {
-  double tc, cTheta, phic_cyc, cphase, cphi, cf, F0T, bscale;
+  double tau0, cTheta, phic_cyc, cphase, cphi, cf, F0T, bscale;   // tau0 = t_c - t0
   float cf32, cl, sl;
   float2 AE[MAXC];   // amp (F0/f_ref)^(2/3) sigma_c e^{i(chi_c+beta)}
-  bool ok;
 };
 
-__device__ __forceinline__ void tmpl_init(const KParams &p, long long t, Tmpl &tm) {
-  tm.ok = t < p.nT;
-  const double *row = p.params + (tm.ok ? t : 0) * 8;
+// One thread per template, once per call.
+__global__ void sft_tmpl_kernel(const KParams p, double *td, float *tf) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= p.nT) return;
+  const double *row = p.params + t * 8;
   const double mc = row[0], eta = row[1], tc = row[2], phic = row[3], amp = row[4];
   const double lam = row[5], beta = row[6];
   const double M = mc * pow(eta, -0.6) * GMSUN_S;             // total mass [s]
   const double inv2pi = 0.15915494309189535;
-  tm.tc = tc;
-  tm.cTheta = eta / (5.0 * M);
-  tm.phic_cyc = phic * inv2pi;
-  tm.cphase = (2.0 / eta) * inv2pi;
-  tm.cphi = p.pn1 ? (3715.0 / 8064.0 + 55.0 / 96.0 * eta) : 0.0;
-  tm.cf = p.pn1 ? (743.0 / 2688.0 + 11.0 / 32.0 * eta) : 0.0;
+  const double cTheta = eta / (5.0 * M);
+  const double cf = p.pn1 ? (743.0 / 2688.0 + 11.0 / 32.0 * eta) : 0.0;
   const double F0 = 1.0 / (8.0 * 3.141592653589793 * M);
-  tm.F0T = F0 * p.T;
-  tm.bscale = tm.cTheta * F0 * p.T * p.T;
-  tm.cf32 = (float)tm.cf;
+  const long long n = p.nT;
+  td[TD_TAU0 * n + t] = tc - p.t0;
+  td[TD_CTHETA * n + t] = cTheta;
+  td[TD_PHIC * n + t] = phic * inv2pi;
+  td[TD_CPHASE * n + t] = (2.0 / eta) * inv2pi;
+  td[TD_CPHI * n + t] = p.pn1 ? (3715.0 / 8064.0 + 55.0 / 96.0 * eta) : 0.0;
+  td[TD_CF * n + t] = cf;
+  td[TD_F0T * n + t] = F0 * p.T;
+  td[TD_BSCALE * n + t] = cTheta * F0 * p.T * p.T;
   const double A0 = amp * cbrt((F0 * p.inv_fref) * (F0 * p.inv_fref));
   double sl, cl;
   sincos(lam, &sl, &cl);
-  tm.cl = (float)cl;
-  tm.sl = (float)sl;
-#pragma unroll
+  tf[TF_CF * n + t] = (float)cf;
+  tf[TF_CL * n + t] = (float)cl;
+  tf[TF_SL * n + t] = (float)sl;
   for (int c = 0; c < MAXC; ++c) {
+    float2 ae = make_float2(0.f, 0.f);
     if (c < p.C) {
       double s, co;
       const double ang = (p.response == 2) ? (p.chi[c] + beta) : 0.0;
       sincos(ang, &s, &co);
       const double a = A0 * p.sigma[c];
-      tm.AE[c] = make_float2((float)(a * co), (float)(a * s));
-    } else {
-      tm.AE[c] = make_float2(0.f, 0.f);
+      ae = make_float2((float)(a * co), (float)(a * s));
     }
+    tf[(TF_AE + 2 * c) * n + t] = ae.x;
+    tf[(TF_AE + 2 * c + 1) * n + t] = ae.y;
   }
+}
+
+// Lanes beyond the last template get tau0 = -1: never active.
+template <int CT>
+__device__ __forceinline__ void tmpl_load(const KParams &p, long long t, Tmpl &tm) {
+  const bool ok = t < p.nT;
+  const long long n = p.nT, tt = ok ? t : 0;
+  const double *d = p.td + tt;
+  const float *f = p.tf + tt;
+  tm.tau0 = ok ? __ldg(d + TD_TAU0 * n) : -1.0;
+  tm.cTheta = __ldg(d + TD_CTHETA * n);
+  tm.phic_cyc = __ldg(d + TD_PHIC * n);
+  tm.cphase = __ldg(d + TD_CPHASE * n);
+  tm.cphi = __ldg(d + TD_CPHI * n);
+  tm.cf = __ldg(d + TD_CF * n);
+  tm.F0T = __ldg(d + TD_F0T * n);
+  tm.bscale = __ldg(d + TD_BSCALE * n);
+  tm.cf32 = __ldg(f + TF_CF * n);
+  tm.cl = __ldg(f + TF_CL * n);
+  tm.sl = __ldg(f + TF_SL * n);
+#pragma unroll
+  for (int c = 0; c < CT; ++c)
+    tm.AE[c] = make_float2(__ldg(f + (TF_AE + 2 * c) * n), __ldg(f + (TF_AE + 2 * c + 1) * n));
 }
 
 // The four numbers of P:164 at t_a, reduced for fp32 consumption.
@@ -175,15 +225,17 @@ struct Track {
   float amp;     // (f_a / F0)^(2/3) = Theta^(-1/4) (1 + cf Theta^(-1/4))^(2/3)
 };
 
-// fp64 track.  Theta^(-1/8) comes from an fp32 MUFU seed (relative error e ~ 5e-7) refined by one
-// second-order Newton step in fp64:  with r = 1 - Theta y^8,  Theta^(-1/8) = y (1-r)^(-1/8)
+// fp64 track.  tau = t_c - t_a = (t_c - t0) - a T in one fma (t_a differs from the separately rounded
+// t0 + a T of P:157 by at most one ulp of t_a, i.e. ~1e-11 s: 1e-9 rad of phase, 1e-13 bins).
+// Theta^(-1/8) comes from an fp32 MUFU seed (relative error e ~ 5e-7) refined by one second-order
+// Newton step in fp64:  with r = 1 - Theta y^8,  Theta^(-1/8) = y (1-r)^(-1/8)
 // = y (1 + r/8 + 9 r^2/128 + O(r^3));  r ~ 8e, so the result is good to ~0.05 (8e)^3 ~ 3e-18 (+ rounding).
+template <class CFG>
 __device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, double dalpha, Track &tr) {
-  const double ta = __dadd_rn(p.t0, __dmul_rn(dalpha, p.T));   // t_a = t0 + a T, rounded as written
-  const double tau = tm.tc - ta;
+  const double tau = fma(-dalpha, p.T, tm.tau0);
   tr.active = false;
   tr.kc = -1;
-  if (!tm.ok || !(tau > p.T)) return;
+  if (!(tau > p.T)) return;
   const double theta = tm.cTheta * tau;
   const float y0 = ex2_approx(-0.125f * lg2_approx((float)theta));
   const double y = (double)y0;
@@ -192,10 +244,18 @@ __device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, dou
   const double s = fma(r, 9.0 / 128.0, 0.125) * r;
   const double q = fma(y, s, y);                  // Theta^(-1/8)
   const double q2 = q * q, q3 = q2 * q, q4 = q2 * q2, q8 = q4 * q4;
-  const double ph = fma(-tm.cphase * (theta * q3), fma(tm.cphi, q2, 1.0), tm.phic_cyc);   // cycles
-  const double fT = tm.F0T * q3 * fma(tm.cf, q2, 1.0);
-  const double b = tm.bscale * (q8 * q3) * fma(0.625 * tm.cf, q2, 0.375);
-  const double yy = (p.kernel == 1) ? fma(0.5, b, fT) : fT;   // Fresnel: centre of the swept band
+  const bool pn1 = cfg_pn1<CFG>(p) != 0;
+  double ph, fT, b;
+  if (pn1) {
+    ph = fma(-tm.cphase * (theta * q3), fma(tm.cphi, q2, 1.0), tm.phic_cyc);   // cycles
+    fT = tm.F0T * q3 * fma(tm.cf, q2, 1.0);
+    b = tm.bscale * (q8 * q3) * fma(0.625 * tm.cf, q2, 0.375);
+  } else {
+    ph = fma(-tm.cphase, theta * q3, tm.phic_cyc);
+    fT = tm.F0T * q3;
+    b = (0.375 * tm.bscale) * (q8 * q3);
+  }
+  const double yy = (cfg_kernel<CFG>(p) == 1) ? fma(0.5, b, fT) : fT;   // Fresnel: centre of the swept band
   const double kcd = floor(yy + 0.5);                       // |kcd| < 2^30: f_hiT is clamped by the host
   if (!(fT >= p.f_loT) || !(fT + b <= p.f_hiT)) return;
   tr.active = true;
@@ -205,7 +265,7 @@ __device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, dou
   tr.frac = (float)(ph - rint(ph));
   const float q2f = (float)q2;
   float a = q2f;
-  if (p.pn1) a *= ex2_approx((2.0f / 3.0f) * lg2_approx(fmaf(tm.cf32, q2f, 1.0f)));
+  if (pn1) a *= ex2_approx((2.0f / 3.0f) * lg2_approx(fmaf(tm.cf32, q2f, 1.0f)));
   tr.amp = a;
 }
 
@@ -224,7 +284,7 @@ __device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, dou
 //   r^_0 = 2 S u,  q^_1 = (kappa r^_0 - C) u,  r^_2 = (S/2 - 2 kappa q^_1) u,  q^_3 = (3 kappa r^_2 - C/4) u, ...
 template <int ORD>
 struct SeriesK {           // per-(template, SFT) constants, broadcast into both packed lanes
-  float2 S2, mC, c_i1, c_i0;            // 2S, -C, and for order 1:  J^_i = (c_i0 + c_i1 q^_1) u
+  float2 S2, mC, c_i0, c_i1, c_i2;      // 2S, -C, and for order 1:  J^_i = (c_i0 + (c_i1 + c_i2 u) u) u
   float2 Sh, mC4, S8, mC16, S32;        // higher orders
   float2 pb, mpb2h, mpb3s;              // pi b, -(pi b)^2/2, -(pi b)^3/6
   float pbs;
@@ -238,9 +298,10 @@ __device__ __forceinline__ void series_setup(float xp, float b, SeriesK<ORD> &k)
   k.pbs = pb;
   k.S2 = bc(2.0f * S);
   k.mC = bc(-C);
-  if (ORD == 1) {
-    k.c_i1 = bc(-2.0f * INV_2PI_F * pb);
+  if (ORD == 1) {       // J^_i = pi b r^_2 = pi b (S/2 - 2 kappa (2 kappa S u - C) u) u, expanded in u
     k.c_i0 = bc(0.5f * pb * S);
+    k.c_i1 = bc(2.0f * INV_2PI_F * pb * C);
+    k.c_i2 = bc(-4.0f * INV_2PI_F * INV_2PI_F * pb * S);
   }
   if (ORD >= 2) {
     k.Sh = bc(0.5f * S);
@@ -264,10 +325,10 @@ __device__ __forceinline__ void series_far2(const SeriesK<ORD> &k, float2 u, flo
   if (ORD == 0) {
     Ji = make_float2(0.f, 0.f);
   } else {
-    const float2 q1 = __fmul2_rn(__ffma2_rn(bc(INV_2PI_F), r0, k.mC), u);
     if (ORD == 1) {
-      Ji = __fmul2_rn(__ffma2_rn(k.c_i1, q1, k.c_i0), u);
+      Ji = __fmul2_rn(__ffma2_rn(__ffma2_rn(k.c_i2, u, k.c_i1), u, k.c_i0), u);
     } else {
+      const float2 q1 = __fmul2_rn(__ffma2_rn(bc(INV_2PI_F), r0, k.mC), u);
       const float2 r2 = __fmul2_rn(__ffma2_rn(bc(-2.0f * INV_2PI_F), q1, k.Sh), u);
       const float2 q3 = __fmul2_rn(__ffma2_rn(bc(3.0f * INV_2PI_F), r2, k.mC4), u);
       const float2 r4 = __fmul2_rn(__ffma2_rn(bc(-4.0f * INV_2PI_F), q3, k.S8), u);
@@ -286,6 +347,12 @@ __device__ __forceinline__ void series_far2(const SeriesK<ORD> &k, float2 u, flo
 __device__ __forceinline__ float2 rcp2(float a, float b) {
   const float rp = rcp_approx(a * b);
   return make_float2(b * rp, a * rp);
+}
+
+// {1/a, 1/(a-1)} with one MUFU reciprocal and one rounding per result:  a (a-1) = fma(a, a, -a)
+__device__ __forceinline__ float2 rcp2_adj(float a) {
+  const float rp = rcp_approx(fmaf(a, a, -a));
+  return make_float2(fmaf(a, rp, -rp), a * rp);
 }
 
 // Taylor coefficients of 2 pi r_2n(a') = 2 pi 4^-n sum_p (-1)^p z^p / ((2p)! (2n+2p+1)),  z = (pi a')^2 <= (pi/2)^2;
@@ -404,7 +471,7 @@ __device__ __forceinline__ void series_pairs(const KParams &p, float xp, float b
     else if (q == K) { Jr = Jl_r; Ji = Jl_i; }
     else {
       const float a_lo = a0 - (float)(2 * q);
-      series_far2<ORD>(k, rcp2(a_lo, a_lo - 1.0f), Jr, Ji);
+      series_far2<ORD>(k, rcp2_adj(a_lo), Jr, Ji);
     }
     mac_pair<CT>(p, Drow, urow, q, Jr, Ji, acc);
   }
@@ -435,18 +502,28 @@ __device__ __forceinline__ void fresnel_pairs(const KParams &p, float x, float b
   }
 }
 
+// Evaluator paths (warp-uniform): series order 0..3, closed Fresnel form.
+enum { PATH_ORD0 = 0, PATH_ORD1, PATH_ORD2, PATH_ORD3, PATH_FRESNEL, PATH_N };
+
+__device__ __forceinline__ int path_of(float bmax) {
+  return bmax == 0.f ? PATH_ORD0 : bmax <= B_ORDER1 ? PATH_ORD1 : bmax <= B_ORDER2 ? PATH_ORD2 : bmax <= B_ORDER3 ? PATH_ORD3
+                                                                                                               : PATH_FRESNEL;
+}
+
 // Z_c = Re/Im of the per-(SFT, channel) complex term, H_c its <h,h> term (include/sft.h).
 // `bmax` is the warp-wide max |b| of the pairs being evaluated: it selects the series order for the
-// whole warp (a higher order than a lane needs is still correct for that lane).  `arow` = alpha * npair.
-template <int KT, int CT>
-__device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int alpha, unsigned arow, const Track &tr,
-                                           float bmax, const float (&us2)[CT], float &zr, float &zi, float &hh) {
+// whole warp (a higher order than a lane needs is still correct for that lane).  `Drow0` points at the
+// padded row of SFT alpha, channel 0, copy 0.
+template <int KT, int CT, class CFG>
+__device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, const float4 *Drow0, const float2 *rt,
+                                           const Track &tr, float bmax, const float (&us2)[CT], float &zr, float &zi,
+                                           float &hh) {
   zr = 0.f; zi = 0.f; hh = 0.f;
   // window start in the zero-padded row; windows that miss the stored band entirely contribute 0
   const int j0 = tr.kc - p.kwin0;                       // kwin0 = k_lo + K - PAD
   if ((unsigned)(j0 - 2) > (unsigned)p.jmax) return;    // 2 <= j0 <= nb - 1 + PAD  <=>  window overlaps the band
   const unsigned e0 = (unsigned)(j0 >> 1), cp = (unsigned)(j0 & 1);
-  const float4 *Drow = p.Dp + (cp * p.cstrideD + arow + e0);
+  const float4 *Drow = Drow0 + (cp * p.cstrideD + e0);
   const float2 *urow = p.ubp + (cp * p.cstrideU + e0);
   // the same window of the next SFT will be wanted next: pull its lines into L1 now (rows are contiguous)
   {
@@ -460,7 +537,7 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int
   for (int c = 0; c < CT; ++c) {
     acc[c].A = make_float2(0.f, 0.f); acc[c].B = acc[c].A; acc[c].I = acc[c].A; acc[c].W = acc[c].A;
   }
-  const bool fres = (p.kernel == 1);
+  const bool fres = (cfg_kernel<CFG>(p) == 1);
   const float b = fres ? tr.b : 0.f;
   float scale = INV_2PI_F;     // the series evaluators return 2 pi J
   float t;                     // total phase / pi:  2 frac (= phi_a/pi) + prefactor phase / pi
@@ -481,19 +558,20 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int
   const float as = scale * tr.amp;
   const float er = cp_ * as, ei = sp * as;
   const float a2 = as * as;
+  const int resp = cfg_resp<CFG>(p);
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
-    if (us2[c] > 0.f) {
+    if (CT == 1 || us2[c] > 0.f) {
       const float S1r = (acc[c].A.x + acc[c].A.y) - (acc[c].B.x + acc[c].B.y);
       const float S1i = acc[c].I.x + acc[c].I.y;
       const float S2 = acc[c].W.x + acc[c].W.y;
       // response (Eq.(5)-(6) P:80-85 as Lambda z = Re[R z]; DESIGN C3/D4)
       float2 R = tm.AE[c];
-      if (p.response == 1) {
-        const float2 r = __ldg(p.rtab + (c * p.n_sft + alpha));
+      if (resp == 1) {
+        const float2 r = __ldg(rt + c * p.n_sft);
         R = make_float2(tm.AE[c].x * r.x, tm.AE[c].x * r.y);      // AE is real here
-      } else if (p.response == 2) {
-        const float2 cs = __ldg(p.rtab + (c * p.n_sft + alpha));
+      } else if (resp == 2) {
+        const float2 cs = __ldg(rt + c * p.n_sft);
         const float am = fmaf(p.depth, cs.x * tm.cl - cs.y * tm.sl, 1.0f);
         R = make_float2(R.x * am, R.y * am);
       }
@@ -506,118 +584,140 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, int
 }
 
 // ---------------------------------------------------------------------------------------------
-// Main fused kernel.  grid = (template tiles, SFT chunks); CT == number of channels (exactly).
+// Main fused kernel.  Persistent grid; every warp draws (32 templates) x (SFT chunk) work units from
+// p.counter.  CT == number of channels (exactly).
 // MODE 0: chunk totals only.  MODE 1 (cumulative): additionally writes chunk-local inclusive prefix
 // sums, transposed through shared memory so that global stores are 128-byte rows along the SFT axis.
 // The SFT loop runs in groups of GROUP: fp32 partial sums flushed into fp64 per group (MODE 0),
 // one transposed store per group (MODE 1).
 // ---------------------------------------------------------------------------------------------
-template <int KT, int CT, int MODE>
-__global__ void __launch_bounds__(TILE) sft_main_kernel(const KParams p) {
+template <int KT, int CT, int MODE, class CFG, int MINB>
+__global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
   constexpr int GROUP = MODE == 1 ? 32 : FLUSH;
   __shared__ float tile_s[MODE == 1 ? (TILE / 32) * 2 * 32 * 33 : 1];
-  const long long t = (long long)blockIdx.x * TILE + threadIdx.x;
-  const int a0 = blockIdx.y * p.chunk;
-  const int a1 = min(a0 + p.chunk, p.n_sft);
-  Tmpl tm;
-  tmpl_init(p, t, tm);
-  double axh = 0.0, ahh = 0.0, axi = 0.0;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float *txh = tile_s + (MODE == 1 ? warp * 2 * 32 * 33 : 0);
   float *thh = txh + (MODE == 1 ? 32 * 33 : 0);
-  double dalpha = (double)a0;
-  unsigned arow = (unsigned)a0 * (unsigned)p.npair;
+  const bool want_kc = CFG::KC && p.kc_out != nullptr;
 
-  for (int g = a0; g < a1; g += GROUP) {
-    const int ge = min(g + GROUP, a1);
-    float fxh = 0.f, fhh = 0.f, fxi = 0.f;
-    for (int alpha = g; alpha < ge; ++alpha, dalpha += 1.0, arow += p.npair) {
-      float us2[CT];
-      bool any = false;
+  for (;;) {
+    int item = 0;
+    if (lane == 0) item = atomicAdd(p.counter, 1);
+    item = __shfl_sync(0xffffffffu, item, 0);
+    if (item >= p.n_items) break;
+    const int ch = p.n_chunks - 1 - item / p.n_tgroups;     // latest (most expensive) chunks first
+    const int tg = item - (item / p.n_tgroups) * p.n_tgroups;
+    const long long t = (long long)tg * 32 + lane;
+    const int a0 = ch * p.chunk;
+    const int a1 = min(a0 + p.chunk, p.n_sft);
+    Tmpl tm;
+    tmpl_load<CT>(p, t, tm);
+    double axh = 0.0, ahh = 0.0, axi = 0.0;
+    double dalpha = (double)a0;
+    const float *usp = p.us2 + a0;
+    const float2 *rt = p.rtab + a0;
+    const float4 *Drow0 = p.Dp + (size_t)a0 * p.npair;
+    int *kcp = want_kc ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + a0 : nullptr;
+    unsigned long long n_path[PATH_N] = {0, 0, 0, 0, 0};
+
+    for (int g = a0; g < a1; g += GROUP) {
+      const int ge = min(g + GROUP, a1);
+      float fxh = 0.f, fhh = 0.f, fxi = 0.f;
+      for (int alpha = g; alpha < ge; ++alpha, dalpha += 1.0, ++usp, ++rt, Drow0 += p.npair) {
+        float us2[CT];
+        bool any = false;
 #pragma unroll
-      for (int c = 0; c < CT; ++c) {
-        us2[c] = __ldg(p.us2 + (c * p.n_sft + alpha));
-        any |= us2[c] > 0.f;
-      }
-      Track tr;
-      tr.active = false;
-      tr.kc = -1;
-      tr.b = 0.f;
-      if (any || p.kc_out) track_eval(p, tm, dalpha, tr);      // `any` is block-uniform
-      const bool go = any && tr.active;
-      if (any) {
-        const float ab = (go && p.kernel == 1) ? fabsf(tr.b) : 0.f;
-        const float bmax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(ab)));
-        if (go) {
-          float zr, zi, hh;
-          pair_terms<KT, CT>(p, tm, alpha, arow, tr, bmax, us2, zr, zi, hh);
-          if (MODE == 1) {
-            axh += (double)zr;
-            ahh += (double)hh;
-          } else {
-            fxh += zr;
-            fxi += zi;
-            fhh += hh;
+        for (int c = 0; c < CT; ++c) {
+          us2[c] = __ldg(usp + c * p.n_sft);
+          any |= us2[c] > 0.f;
+        }
+        Track tr;
+        tr.active = false;
+        tr.kc = -1;
+        tr.b = 0.f;
+        if (any || want_kc) track_eval<CFG>(p, tm, dalpha, tr);      // `any` is warp-uniform
+        const bool go = any && tr.active;
+        if (any) {
+          const float ab = (go && cfg_kernel<CFG>(p) == 1) ? fabsf(tr.b) : 0.f;
+          const float bmax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(ab)));
+          if (CFG::KC && p.path_counts) {
+            int n_present = 0;
+#pragma unroll
+            for (int c = 0; c < CT; ++c) n_present += us2[c] > 0.f;
+            n_path[path_of(bmax)] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * n_present);
+          }
+          if (go) {
+            float zr, zi, hh;
+            pair_terms<KT, CT, CFG>(p, tm, Drow0, rt, tr, bmax, us2, zr, zi, hh);
+            if (MODE == 1) {
+              axh += (double)zr;
+              ahh += (double)hh;
+            } else {
+              fxh += zr;
+              fxi += zi;
+              fhh += hh;
+            }
           }
         }
-      }
-      if (p.kc_out && tm.ok) {
+        if (CFG::KC && want_kc) {
+          if (t < p.nT) {
 #pragma unroll
-        for (int c = 0; c < CT; ++c)
-          p.kc_out[((size_t)t * CT + c) * p.n_sft + alpha] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
-      }
-      if (MODE == 1) {
-        txh[lane * 33 + (alpha - g)] = (float)axh;
-        thh[lane * 33 + (alpha - g)] = (float)ahh;
-      }
-    }
-    if (MODE == 0) {
-      axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
-    } else {
-      __syncwarp();
-      const int n = ge - g;
-      for (int r = 0; r < 32; ++r) {
-        const long long tt = (long long)blockIdx.x * TILE + warp * 32 + r;
-        if (tt < p.nT && lane < n) {
-          p.loc_xh[(size_t)tt * p.n_sft + g + lane] = txh[r * 33 + lane];
-          p.loc_hh[(size_t)tt * p.n_sft + g + lane] = thh[r * 33 + lane];
+            for (int c = 0; c < CT; ++c) kcp[(size_t)c * p.n_sft] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
+          }
+          ++kcp;
+        }
+        if (MODE == 1) {
+          txh[lane * 33 + (alpha - g)] = (float)axh;
+          thh[lane * 33 + (alpha - g)] = (float)ahh;
         }
       }
-      __syncwarp();
+      if (MODE == 0) {
+        axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
+      } else {
+        __syncwarp();
+        const int n = ge - g;
+        for (int r = 0; r < 32; ++r) {
+          const long long tt = (long long)tg * 32 + r;
+          if (tt < p.nT && lane < n) {
+            p.loc_xh[(size_t)tt * p.n_sft + g + lane] = txh[r * 33 + lane];
+            p.loc_hh[(size_t)tt * p.n_sft + g + lane] = thh[r * 33 + lane];
+          }
+        }
+        __syncwarp();
+      }
     }
-  }
-  if (tm.ok) {
-    double *q = p.part + (size_t)blockIdx.y * 3 * p.nT + t;
-    q[0] = axh;
-    q[p.nT] = ahh;
-    q[2 * p.nT] = axi;
+    if (t < p.nT) {
+      double *q = p.part + (size_t)ch * 3 * p.nT + t;
+      q[0] = axh;
+      q[p.nT] = ahh;
+      q[2 * p.nT] = axi;
+    }
+    if (CFG::KC && p.path_counts && lane == 0) {
+#pragma unroll
+      for (int i = 0; i < PATH_N; ++i)
+        if (n_path[i]) atomicAdd(p.path_counts + i, n_path[i]);
+    }
   }
 }
 
-// Sum of the chunk totals in fp64, fixed order (deterministic).  block = (32 templates, 8 chunk lanes).
-__global__ void __launch_bounds__(256) sft_reduce_kernel(const double *part, long long nT, int n_chunks, double *xh,
-                                                         double *hh, double *xi) {
-  __shared__ double sm[3][8][33];
-  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-  const long long t = (long long)blockIdx.x * 32 + tx;
-  double s0 = 0.0, s1 = 0.0, s2 = 0.0;
-  if (t < nT) {
-    for (int c = ty; c < n_chunks; c += 8) {
-      const double *q = part + (size_t)c * 3 * nT + t;
-      s0 += q[0];
-      s1 += q[nT];
-      s2 += q[2 * nT];
-    }
+// Sum of the chunk totals in fp64, fixed order (deterministic).  grid = (ceil(nT/64), 3 quantities).
+__global__ void __launch_bounds__(64) sft_reduce_kernel(const double *part, long long nT, int n_chunks, double *xh,
+                                                        double *hh, double *xi) {
+  const long long t = (long long)blockIdx.x * 64 + threadIdx.x;
+  double *out = blockIdx.y == 0 ? xh : blockIdx.y == 1 ? hh : xi;
+  if (t >= nT || !out) return;
+  const double *q = part + (size_t)blockIdx.y * nT + t;
+  const size_t stride = (size_t)3 * nT;
+  double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+  int c = 0;
+  for (; c + 4 <= n_chunks; c += 4) {
+    s0 += q[(size_t)c * stride];
+    s1 += q[(size_t)(c + 1) * stride];
+    s2 += q[(size_t)(c + 2) * stride];
+    s3 += q[(size_t)(c + 3) * stride];
   }
-  sm[0][ty][tx] = s0; sm[1][ty][tx] = s1; sm[2][ty][tx] = s2;
-  __syncthreads();
-  if (ty == 0 && t < nT) {
-#pragma unroll
-    for (int j = 1; j < 8; ++j) { s0 += sm[0][j][tx]; s1 += sm[1][j][tx]; s2 += sm[2][j][tx]; }
-    xh[t] = s0;
-    hh[t] = s1;
-    if (xi) xi[t] = s2;
-  }
+  for (; c < n_chunks; ++c) s0 += q[(size_t)c * stride];
+  out[t] = (s0 + s1) + (s2 + s3);
 }
 
 // Exclusive scan of the chunk totals along the chunk axis, in place, fp64 (the carries).

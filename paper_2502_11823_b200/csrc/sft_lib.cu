@@ -34,6 +34,11 @@ struct sft_plan {
   double *d_params = nullptr; size_t params_bytes = 0;
   void *d_out = nullptr; size_t out_bytes = 0;         // staging for host outputs
   float *loc = nullptr; size_t loc_bytes = 0;          // cumulative: chunk-local prefixes
+  double *td = nullptr; size_t td_bytes = 0;           // per-template constants (sft_tmpl_kernel)
+  float *tf = nullptr; size_t tf_bytes = 0;
+  int *counter = nullptr;                              // work-unit counter of the persistent main kernel
+  unsigned long long *path_counts = nullptr;           // [PATH_N] diagnostic counters
+  int n_sm = 0;
   int chunk_user = 0;
   long long launches = 0;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -125,6 +130,13 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   alloc((void **)&p->ubp, 2 * C * npair * sizeof(float2));
   alloc((void **)&p->us2, C * N * sizeof(float));
   alloc((void **)&p->rtab, C * N * sizeof(float2));
+  alloc((void **)&p->counter, sizeof(int));
+  alloc((void **)&p->path_counts, sftk::PATH_N * sizeof(unsigned long long));
+  if (st == SFT_OK) {
+    cudaError_t e2 = cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, d.device);
+    if (e2 == cudaSuccess) e2 = cudaMemsetAsync(p->path_counts, 0, sftk::PATH_N * sizeof(unsigned long long), p->stream);
+    if (e2 != cudaSuccess) st = fail(nullptr, SFT_ECUDA, "plan set-up: %s", cudaGetErrorString(e2));
+  }
   if (st == SFT_OK) {
     cudaError_t e2 = cudaEventCreate(&p->ev0);
     if (e2 == cudaSuccess) e2 = cudaEventCreate(&p->ev1);
@@ -156,6 +168,7 @@ SFT_API sft_status sft_plan_destroy(sft_plan *p) {
   cudaStreamSynchronize(p->stream);
   cudaFree(p->Dp); cudaFree(p->ubp); cudaFree(p->us2); cudaFree(p->rtab);
   cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->loc);
+  cudaFree(p->td); cudaFree(p->tf); cudaFree(p->counter); cudaFree(p->path_counts);
   if (p->ev0) cudaEventDestroy(p->ev0);
   if (p->ev1) cudaEventDestroy(p->ev1);
   delete p;
@@ -178,6 +191,17 @@ SFT_API double sft_plan_last_kernel_ms(sft_plan *p) {
   float ms = -1.f;
   if (cudaEventElapsedTime(&ms, p->ev0, p->ev1) != cudaSuccess) return -1.0;
   return (double)ms;
+}
+
+SFT_API sft_status sft_plan_path_counts(sft_plan *p, int64_t *out, int32_t n_out) {
+  if (!p) return SFT_EINVAL;
+  if (!out || n_out < 1) return fail(p, SFT_EINVAL, "sft_plan_path_counts: out is NULL or n_out < 1");
+  CU(p, cudaSetDevice(p->d.device));
+  unsigned long long h[sftk::PATH_N];
+  CU(p, cudaMemcpyAsync(h, p->path_counts, sizeof(h), cudaMemcpyDeviceToHost, p->stream));
+  CU(p, cudaStreamSynchronize(p->stream));
+  for (int i = 0; i < n_out && i < sftk::PATH_N; ++i) out[i] = (int64_t)h[i];
+  return SFT_OK;
 }
 
 SFT_API sft_status sft_plan_set_chunk(sft_plan *p, int32_t c) {
@@ -295,32 +319,49 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.rtab = p->rtab;
 }
 
+#ifndef SFT_MINB
+#define SFT_MINB 5          // resident 128-thread blocks per SM the main kernel is compiled for
+#endif
+
+// Compile-time flag sets of the hot variants (everything else takes the run-time-flag variant):
+//   CfgBNS  = Fresnel kernel, 0PN+1PN, no response      (configs 2, 3, 5)
+//   CfgNewt = Fresnel kernel, 0PN, no response          (config 1)
+//   CfgLISA = Fresnel kernel, 0PN+1PN, annual response  (config 4)
+//   CfgAny  = run-time flags, optional k_c output and path counters
+using CfgBNS = sftk::Cfg<1, 1, 0, 0>;
+using CfgNewt = sftk::Cfg<1, 0, 0, 0>;
+using CfgLISA = sftk::Cfg<1, 1, 2, 0>;
+using CfgAny = sftk::Cfg<-1, -1, -1, 1>;
+
+template <int KT, int CT, int MODE, class CFG>
+static void launch_variant(sft_plan *p, const KParams &k) {
+  auto kern = sftk::sft_main_kernel<KT, CT, MODE, CFG, SFT_MINB>;
+  int per_sm = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, sftk::TILE, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
+  long long blocks = (long long)p->n_sm * per_sm;
+  const long long need = ((long long)k.n_items + sftk::TILE / 32 - 1) / (sftk::TILE / 32);
+  if (blocks > need) blocks = need;
+  kern<<<(unsigned)blocks, sftk::TILE, 0, p->stream>>>(k);
+}
+
 template <int MODE>
 static cudaError_t launch_main(sft_plan *p, const KParams &k) {
-  dim3 grid((unsigned)((k.nT + sftk::TILE - 1) / sftk::TILE), (unsigned)k.n_chunks);
-  dim3 block(sftk::TILE);
+  cudaMemsetAsync(p->counter, 0, sizeof(int), p->stream);
   cudaEventRecord(p->ev0, p->stream);
-#define SFT_LAUNCH(KT, CT) sftk::sft_main_kernel<KT, CT, MODE><<<grid, block, 0, p->stream>>>(k)
-  const int C = k.C;
-  if (C == 1) {
-    switch (k.K) {
-      case 4: SFT_LAUNCH(4, 1); break;
-      case 8: SFT_LAUNCH(8, 1); break;
-      case 16: SFT_LAUNCH(16, 1); break;
-      default: SFT_LAUNCH(0, 1); break;
-    }
-  } else if (C == 2) {
-    switch (k.K) {
-      case 8: SFT_LAUNCH(8, 2); break;
-      case 16: SFT_LAUNCH(16, 2); break;
-      default: SFT_LAUNCH(0, 2); break;
-    }
-  } else if (C == 3) {
-    SFT_LAUNCH(0, 3);
-  } else {
-    SFT_LAUNCH(0, 4);
-  }
-#undef SFT_LAUNCH
+  const int C = k.C, K = k.K;
+  const bool diag = k.kc_out != nullptr || k.path_counts != nullptr;
+  const bool bns = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 0;
+  const bool newt = !diag && k.kernel == 1 && k.pn1 == 0 && k.response == 0;
+  const bool lisa = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 2;
+  if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS>(p, k);
+  else if (bns && C == 1 && K == 16) launch_variant<16, 1, MODE, CfgBNS>(p, k);
+  else if (bns && C == 1) launch_variant<0, 1, MODE, CfgBNS>(p, k);
+  else if (newt && C == 1 && K == 4) launch_variant<4, 1, MODE, CfgNewt>(p, k);
+  else if (lisa && C == 2 && K == 16) launch_variant<16, 2, MODE, CfgLISA>(p, k);
+  else if (C == 1) launch_variant<0, 1, MODE, CfgAny>(p, k);
+  else if (C == 2) launch_variant<0, 2, MODE, CfgAny>(p, k);
+  else if (C == 3) launch_variant<0, 3, MODE, CfgAny>(p, k);
+  else launch_variant<0, 4, MODE, CfgAny>(p, k);
   cudaEventRecord(p->ev1, p->stream);
   p->timed = true;
   p->launches++;
@@ -335,18 +376,33 @@ static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t
   CU(p, cudaSetDevice(p->d.device));
   fill_kparams(p, k);
   k.nT = nT;
-  int chunk = p->chunk_user > 0 ? p->chunk_user : 64;
+  // SFTs per work unit: enough units (>= ~16 per resident warp) for the dynamic scheduler to balance,
+  // but no more chunks than that (the chunk totals cost 24 bytes per template and chunk)
+  k.n_tgroups = (int)((nT + 31) / 32);
+  int chunk = p->chunk_user;
+  if (chunk <= 0) {
+    const long long target_units = 16ll * p->n_sm * 24;
+    long long want_chunks = (target_units + k.n_tgroups - 1) / k.n_tgroups;
+    if (want_chunks < 1) want_chunks = 1;
+    chunk = (int)((k.n_sft + want_chunks - 1) / want_chunks);
+    if (chunk < 32) chunk = 32;
+  }
   if (cumulative) chunk = ((chunk + 31) / 32) * 32;
   if (chunk > k.n_sft) chunk = cumulative ? ((k.n_sft + 31) / 32) * 32 : k.n_sft;
   k.chunk = chunk;
   k.n_chunks = (k.n_sft + chunk - 1) / chunk;
-  if (k.n_chunks > 65535) {
-    k.chunk = ((k.n_sft + 65534) / 65535 + 31) / 32 * 32;
-    k.n_chunks = (k.n_sft + k.chunk - 1) / k.chunk;
-  }
   sft_status st = grow(p, (void **)&p->part, &p->part_bytes, (size_t)k.n_chunks * 3 * nT * sizeof(double));
   if (st != SFT_OK) return st;
   k.part = p->part;
+  if ((double)k.n_tgroups * (double)k.n_chunks > 2.0e9) return fail(p, SFT_EINVAL, "too many work units: raise sfts_per_block");
+  k.n_items = k.n_tgroups * k.n_chunks;
+  k.counter = p->counter;
+  st = grow(p, (void **)&p->td, &p->td_bytes, (size_t)sftk::TD_N * nT * sizeof(double));
+  if (st != SFT_OK) return st;
+  st = grow(p, (void **)&p->tf, &p->tf_bytes, (size_t)sftk::TF_N * nT * sizeof(float));
+  if (st != SFT_OK) return st;
+  k.td = p->td;
+  k.tf = p->tf;
   if (mem == SFT_MEM_HOST) {
     st = grow(p, (void **)&p->d_params, &p->params_bytes, (size_t)nT * SFT_NPARAM * sizeof(double));
     if (st != SFT_OK) return st;
@@ -355,6 +411,10 @@ static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t
   } else {
     k.params = params;
   }
+  sftk::sft_tmpl_kernel<<<(unsigned)((nT + 127) / 128), 128, 0, p->stream>>>(k, p->td, p->tf);
+  p->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "template kernel launch: %s", cudaGetErrorString(e));
   return SFT_OK;
 }
 
@@ -383,9 +443,11 @@ SFT_API sft_status sft_inner_products(sft_plan *p, int64_t nT, const double *par
     d_kc = kc_out ? (int *)(d_xi + nT) : nullptr;
   }
   k.kc_out = d_kc;
+  k.path_counts = d_kc ? p->path_counts : nullptr;     // the diagnostic call also counts the evaluator paths
+  if (d_kc) CU(p, cudaMemsetAsync(p->path_counts, 0, sftk::PATH_N * sizeof(unsigned long long), p->stream));
   cudaError_t e = launch_main<0>(p, k);
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
-  sftk::sft_reduce_kernel<<<(unsigned)((nT + 31) / 32), 256, 0, p->stream>>>(p->part, nT, k.n_chunks, d_xh, d_hh, d_xi);
+  sftk::sft_reduce_kernel<<<dim3((unsigned)((nT + 63) / 64), 3), 64, 0, p->stream>>>(p->part, nT, k.n_chunks, d_xh, d_hh, d_xi);
   p->launches++;
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "reduce kernel launch: %s", cudaGetErrorString(e));
