@@ -38,7 +38,8 @@ def build(force=False, verbose=False, extra=()):
     """Compiles the library if it is missing or older than its sources.  Returns its path."""
     if not force and up_to_date():
         return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + list(extra) + ["-o", LIB] + SOURCES
+    extra = list(extra) + os.environ.get("SFT_NVCC_EXTRA", "").split()      # e.g. -DSFT_MINB=4
+    cmd = [nvcc()] + NVCC_FLAGS + extra + ["-o", LIB] + SOURCES
     if verbose:
         print(" ".join(cmd), flush=True)
     r = subprocess.run(cmd, capture_output=True, text=True)

@@ -93,7 +93,7 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
   return r;
 }
-// (sin, cos)(pi t) for |t| <= 1 on the MUFU (absolute error ~5e-7 over [-pi, pi])
+// (sin, cos)(pi t) for |t| <~ 2 on the MUFU (absolute error ~5e-7)
 __device__ __forceinline__ void sincospi_fast(float t, float &s, float &c) {
   const float a = PI_F * t;
   s = __sinf(a);
@@ -225,17 +225,20 @@ struct Track {
   float amp;     // (f_a / F0)^(2/3) = Theta^(-1/4) (1 + cf Theta^(-1/4))^(2/3)
 };
 
-// fp64 track.  tau = t_c - t_a = (t_c - t0) - a T in one fma (t_a differs from the separately rounded
-// t0 + a T of P:157 by at most one ulp of t_a, i.e. ~1e-11 s: 1e-9 rad of phase, 1e-13 bins).
+// fp64 track, branch-free (so that it can be scheduled into the straight-line code of the bin loop of
+// the previous SFT).  tau = t_c - t_a = (t_c - t0) - a T in one fma (t_a differs from the separately
+// rounded t0 + a T of P:157 by at most one ulp of t_a, i.e. ~1e-11 s: 1e-9 rad of phase, 1e-13 bins).
 // Theta^(-1/8) comes from an fp32 MUFU seed (relative error e ~ 5e-7) refined by one second-order
 // Newton step in fp64:  with r = 1 - Theta y^8,  Theta^(-1/8) = y (1-r)^(-1/8)
 // = y (1 + r/8 + 9 r^2/128 + O(r^3));  r ~ 8e, so the result is good to ~0.05 (8e)^3 ~ 3e-18 (+ rounding).
+// tau <= 0 gives NaNs, which fail every comparison of the activity mask.  Rounding to the nearest
+// integer is done by adding 1.5 * 2^52 (|values| < 2^31): k_c = rint(y) equals floor(y + 1/2) except
+// for y exactly half-way between two bins, which DESIGN A5 flags as a tie anyway.
+constexpr double RND_MAGIC = 6755399441055744.0;   // 1.5 * 2^52
+
 template <class CFG>
 __device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, double dalpha, Track &tr) {
   const double tau = fma(-dalpha, p.T, tm.tau0);
-  tr.active = false;
-  tr.kc = -1;
-  if (!(tau > p.T)) return;
   const double theta = tm.cTheta * tau;
   const float y0 = ex2_approx(-0.125f * lg2_approx((float)theta));
   const double y = (double)y0;
@@ -256,16 +259,26 @@ __device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, dou
     b = (0.375 * tm.bscale) * (q8 * q3);
   }
   const double yy = (cfg_kernel<CFG>(p) == 1) ? fma(0.5, b, fT) : fT;   // Fresnel: centre of the swept band
-  const double kcd = floor(yy + 0.5);                       // |kcd| < 2^30: f_hiT is clamped by the host
-  if (!(fT >= p.f_loT) || !(fT + b <= p.f_hiT)) return;
-  tr.active = true;
-  tr.x = (float)(fT - kcd);
-  tr.kc = (int)kcd;
+  const double kr = yy + RND_MAGIC;                // f_hiT is clamped by the host: active => |yy| < 2^30
+  const double pr = ph + RND_MAGIC;
+  tr.active = (tau > p.T) && (fT >= p.f_loT) && (fT + b <= p.f_hiT);
+  tr.kc = __double2loint(kr);
+  tr.x = (float)(fT - (kr - RND_MAGIC));
   tr.b = (float)b;
-  tr.frac = (float)(ph - rint(ph));
-  const float q2f = (float)q2;
+  tr.frac = (float)(ph - (pr - RND_MAGIC));
+  // amplitude (f_a/F0)^(2/3) = q^2 (1 + cf q^2)^(2/3): the seed is good enough (1e-6 relative)
+  const float q2f = y0 * y0;
   float a = q2f;
-  if (pn1) a *= ex2_approx((2.0f / 3.0f) * lg2_approx(fmaf(tm.cf32, q2f, 1.0f)));
+  if (pn1) {
+    const float z = tm.cf32 * q2f;     // binomial series of (1+z)^(2/3): |error| < 0.014 z^6 (9e-7 at z = 0.2)
+    float g = fmaf(z, 14.0f / 729.0f, -7.0f / 243.0f);
+    g = fmaf(g, z, 4.0f / 81.0f);
+    g = fmaf(g, z, -1.0f / 9.0f);
+    g = fmaf(g, z, 2.0f / 3.0f);
+    g = fmaf(g, z, 1.0f);
+    if (z > 0.2f) g = ex2_approx((2.0f / 3.0f) * lg2_approx(1.0f + z));
+    a *= g;
+  }
   tr.amp = a;
 }
 
@@ -366,23 +379,23 @@ __device__ __forceinline__ constexpr float tay_c(int n, int pp) {
   return (float)(6.283185307179586 * s / (f * (double)(2 * n + 2 * pp + 1) * four));
 }
 
+template <int N>
+__device__ __forceinline__ float tay_poly(float z) {      // scalar FFMAs with immediate coefficients
+  float r = tay_c(N, 6);
+#pragma unroll
+  for (int pp = 5; pp >= 0; --pp) r = fmaf(r, z, tay_c(N, pp));
+  return r;
+}
+
 template <int ORD>
 __device__ __forceinline__ void series_central(const SeriesK<ORD> &k, float a, float &Jr, float &Ji) {
   const float t = PI_F * a;
-  const float2 z = bc(t * t);
-  float2 lo = make_float2(tay_c(0, 6), tay_c(1, 6));
-#pragma unroll
-  for (int pp = 5; pp >= 0; --pp) lo = __ffma2_rn(lo, z, make_float2(tay_c(0, pp), tay_c(1, pp)));
-  Jr = lo.x;                 // r^_0
-  Ji = k.pbs * lo.y;         // pi b r^_2
-  if (ORD == 0) Ji = 0.f;
-  if (ORD >= 2) {
-    float2 hi = make_float2(tay_c(2, 6), tay_c(3, 6));
-#pragma unroll
-    for (int pp = 5; pp >= 0; --pp) hi = __ffma2_rn(hi, z, make_float2(tay_c(2, pp), tay_c(3, pp)));
-    Jr = fmaf(-0.5f * k.pbs * k.pbs, hi.x, Jr);
-    if (ORD >= 3) Ji = fmaf(-(1.0f / 6.0f) * k.pbs * k.pbs * k.pbs, hi.y, Ji);
-  }
+  const float z = t * t;
+  Jr = tay_poly<0>(z);                    // r^_0
+  Ji = 0.f;
+  if (ORD >= 1) Ji = k.pbs * tay_poly<1>(z);             // pi b r^_2
+  if (ORD >= 2) Jr = fmaf(-0.5f * k.pbs * k.pbs, tay_poly<2>(z), Jr);
+  if (ORD >= 3) Ji = fmaf(-(1.0f / 6.0f) * k.pbs * k.pbs * k.pbs, tay_poly<3>(z), Ji);
 }
 
 // Closed Fresnel form (Eq.(29)-(30) P:219-226) rewritten with the auxiliary functions so that the
@@ -422,14 +435,31 @@ struct Acc {
   float2 A, B, I, W;
 };
 
+// Where the window of one (template, SFT) sits in the pair-planar store.  j0 = padded index of bin
+// m = -K; copy (j0 & 1) holds the pairs starting at even window offsets, the other copy those starting
+// at odd offsets; `row`/`urow` point at copy 0 of the SFT's row (channel 0).
+struct Win {
+  const float4 *dE, *dO;    // entry of window offset i: even i -> dE[i/2], odd i -> dO[(i-1)/2]
+  const float2 *uE, *uO;
+};
+__device__ __forceinline__ void win_init(const KParams &p, const float4 *row, int j0, Win &w) {
+  const unsigned cp = (unsigned)j0 & 1u, eE = (unsigned)j0 >> 1, eO = (unsigned)(j0 + 1) >> 1;
+  w.dE = row + (cp * p.cstrideD + eE);
+  w.dO = row + ((cp ^ 1u) * p.cstrideD + eO);
+  w.uE = p.ubp + (cp * p.cstrideU + eE);
+  w.uO = p.ubp + ((cp ^ 1u) * p.cstrideU + eO);
+}
+
+// pair of adjacent bins at window offsets (i, i+1)
 template <int CT>
-__device__ __forceinline__ void mac_pair(const KParams &p, const float4 *Drow, const float2 *urow, int q, float2 Jr,
-                                         float2 Ji, Acc (&acc)[CT]) {
+__device__ __forceinline__ void mac_pair(const KParams &p, const Win &w, int i, float2 Jr, float2 Ji, Acc (&acc)[CT]) {
+  const float4 *dp = (i & 1) ? w.dO + (i >> 1) : w.dE + (i >> 1);
+  const float2 *up = (i & 1) ? w.uO + (i >> 1) : w.uE + (i >> 1);
   const float2 mag = __ffma2_rn(Ji, Ji, __fmul2_rn(Jr, Jr));
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
-    const float4 d = __ldg(Drow + c * p.dstride + q);
-    const float2 u = __ldg(urow + c * p.npair + q);
+    const float4 d = __ldg(dp + c * p.dstride);
+    const float2 u = __ldg(up + c * p.npair);
     const float2 dre = make_float2(d.x, d.y), dim = make_float2(d.z, d.w);
     acc[c].A = __ffma2_rn(dre, Jr, acc[c].A);
     acc[c].B = __ffma2_rn(dim, Ji, acc[c].B);
@@ -439,48 +469,69 @@ __device__ __forceinline__ void mac_pair(const KParams &p, const float4 *Drow, c
   }
 }
 
-// Series path of one (template, SFT): all K+1 bin pairs.  Pair q holds m = -K+2q (lo) and -K+2q+1 (hi);
-// the hi lane of the last pair (m = K+1) is outside the band and gets J = 0.  The two pairs that are not
-// "two far bins" - the one holding the central bin m = 0 (with its neighbour m_p = +1 or -1) and the last
-// one (m = K) - share one packed far evaluation {m_p, K}.
-template <int ORD, int KT, int CT>
-__device__ __forceinline__ void series_pairs(const KParams &p, float xp, float b, const float4 *Drow, const float2 *urow,
-                                             Acc (&acc)[CT]) {
-  const int K = KT > 0 ? KT : p.K;
-  SeriesK<ORD> k;
-  series_setup<ORD>(xp, b, k);
-  const int qc = K >> 1;                 // pair holding m = 0 (lo lane if K even, hi lane if K odd)
-  const bool c_lo = (K & 1) == 0;
-  const float a0 = xp + (float)K;        // a' of m = -K
-  float2 Jc_r, Jc_i, Jl_r = make_float2(0.f, 0.f), Jl_i = make_float2(0.f, 0.f);
-  {
-    float c_r, c_i;
-    series_central<ORD>(k, xp, c_r, c_i);
-    float2 Fr = make_float2(0.f, 0.f), Fi = make_float2(0.f, 0.f);
-    if (K >= 1) series_far2<ORD>(k, rcp2(c_lo ? xp - 1.0f : xp + 1.0f, xp - (float)K), Fr, Fi);
-    Jc_r = c_lo ? make_float2(c_r, Fr.x) : make_float2(Fr.x, c_r);
-    Jc_i = c_lo ? make_float2(c_i, Fi.x) : make_float2(Fi.x, c_i);
-    if (K == 0) { Jc_r.y = 0.f; Jc_i.y = 0.f; }      // single pair: hi lane is m = 1 > K
-    Jl_r.x = Fr.y;
-    Jl_i.x = Fi.y;
-  }
+// one bin at window offset i (scalar; accumulates into the lo lanes)
+template <int CT>
+__device__ __forceinline__ void mac_single(const KParams &p, const Win &w, int i, float Jr, float Ji, Acc (&acc)[CT]) {
+  const float4 *dp = (i & 1) ? w.dO + (i >> 1) : w.dE + (i >> 1);
+  const float2 *up = (i & 1) ? w.uO + (i >> 1) : w.uE + (i >> 1);
+  const float mag = fmaf(Ji, Ji, Jr * Jr);
 #pragma unroll
-  for (int q = 0; q <= K; ++q) {
-    float2 Jr, Ji;
-    if (q == qc) { Jr = Jc_r; Ji = Jc_i; }
-    else if (q == K) { Jr = Jl_r; Ji = Jl_i; }
-    else {
-      const float a_lo = a0 - (float)(2 * q);
-      series_far2<ORD>(k, rcp2_adj(a_lo), Jr, Ji);
-    }
-    mac_pair<CT>(p, Drow, urow, q, Jr, Ji, acc);
+  for (int c = 0; c < CT; ++c) {
+    const float4 d = __ldg(dp + c * p.dstride);
+    const float2 u = __ldg(up + c * p.npair);
+    acc[c].A.x = fmaf(d.x, Jr, acc[c].A.x);
+    acc[c].B.x = fmaf(d.z, Ji, acc[c].B.x);
+    acc[c].I.x = fmaf(d.x, Ji, acc[c].I.x);
+    acc[c].I.x = fmaf(d.z, Jr, acc[c].I.x);
+    acc[c].W.x = fmaf(u.x, mag, acc[c].W.x);
   }
 }
 
-template <int KT, int CT>
-__device__ __forceinline__ void fresnel_pairs(const KParams &p, float x, float b, const float4 *Drow, const float2 *urow,
-                                              Acc (&acc)[CT], float &scale) {
+// Series path of one (template, SFT).  The 2K far bins are taken two adjacent bins at a time -
+// (-K,-K+1), ..., (-2,-1) on the low side, (1,2), ..., (K-1,K) on the high side (for odd K the bins
+// -1 and +1 are left over and evaluated as one non-adjacent pair) - and the central bin m = 0 alone.
+// `nxt` = track of the NEXT SFT: it does not depend on anything here and sits in this straight-line
+// code so that its fp64 dependency chain is issued between the fp32 work of the bin loop.
+template <int ORD, int KT, int CT, class CFG>
+__device__ __forceinline__ void series_pairs(const KParams &p, const Tmpl &tm, double dnext, Track &nxt, float xp, float b,
+                                             const Win &w, Acc (&acc)[CT]) {
   const int K = KT > 0 ? KT : p.K;
+  SeriesK<ORD> k;
+  series_setup<ORD>(xp, b, k);
+  track_eval<CFG>(p, tm, dnext, nxt);
+  const int odd = K & 1, half = K >> 1;
+  const float aN = xp + (float)K;              // a' of m = -K
+  const float aP = xp - (float)(1 + odd);      // a' of the first high-side pair's lo bin
+#pragma unroll
+  for (int q = 0; q < half; ++q) {
+    float2 Jr, Ji;
+    series_far2<ORD>(k, rcp2_adj(aN - (float)(2 * q)), Jr, Ji);
+    mac_pair<CT>(p, w, 2 * q, Jr, Ji, acc);
+  }
+  {
+    float c_r, c_i;
+    series_central<ORD>(k, xp, c_r, c_i);
+    mac_single<CT>(p, w, K, c_r, c_i, acc);
+  }
+  if (odd) {
+    float2 Jr, Ji;
+    series_far2<ORD>(k, rcp2(xp + 1.0f, xp - 1.0f), Jr, Ji);
+    mac_single<CT>(p, w, K - 1, Jr.x, Ji.x, acc);
+    mac_single<CT>(p, w, K + 1, Jr.y, Ji.y, acc);
+  }
+#pragma unroll
+  for (int q = 0; q < half; ++q) {
+    float2 Jr, Ji;
+    series_far2<ORD>(k, rcp2_adj(aP - (float)(2 * q)), Jr, Ji);
+    mac_pair<CT>(p, w, K + 1 + odd + 2 * q, Jr, Ji, acc);
+  }
+}
+
+template <int KT, int CT, class CFG>
+__device__ __forceinline__ void fresnel_pairs(const KParams &p, const Tmpl &tm, double dnext, Track &nxt, float x, float b,
+                                              const Win &w, Acc (&acc)[CT], float &scale) {
+  const int K = KT > 0 ? KT : p.K;
+  track_eval<CFG>(p, tm, dnext, nxt);
   FresK k;
   k.neg = b < 0.f;
   const float ab = fabsf(b);
@@ -498,7 +549,7 @@ __device__ __forceinline__ void fresnel_pairs(const KParams &p, float x, float b
     fresnel_bin(k, m_lo, Jr.x, Ji.x);
     if (m_lo + 1 > K) { Jr.y = 0.f; Ji.y = 0.f; }
     else fresnel_bin(k, m_lo + 1, Jr.y, Ji.y);
-    mac_pair<CT>(p, Drow, urow, q, Jr, Ji, acc);
+    mac_pair<CT>(p, w, 2 * q, Jr, Ji, acc);
   }
 }
 
@@ -511,26 +562,28 @@ __device__ __forceinline__ int path_of(float bmax) {
 }
 
 // Z_c = Re/Im of the per-(SFT, channel) complex term, H_c its <h,h> term (include/sft.h).
-// `bmax` is the warp-wide max |b| of the pairs being evaluated: it selects the series order for the
-// whole warp (a higher order than a lane needs is still correct for that lane).  `Drow0` points at the
-// padded row of SFT alpha, channel 0, copy 0.
+// Called by the whole warp as soon as one lane has an active pair (`go`); the other lanes run along on a
+// clamped window and their results are discarded, so the control flow stays warp-uniform.
+// `bmax` is the warp-wide max |b| of the active pairs: it selects the series order for the whole warp
+// (a higher order than a lane needs is still correct for that lane).  `Drow0` points at the padded row
+// of SFT alpha, channel 0, copy 0.  Also evaluates the track of the next SFT (see series_pairs).
 template <int KT, int CT, class CFG>
 __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, const float4 *Drow0, const float2 *rt,
-                                           const Track &tr, float bmax, const float (&us2)[CT], float &zr, float &zi,
-                                           float &hh) {
-  zr = 0.f; zi = 0.f; hh = 0.f;
+                                           const Track &tr, bool go, float bmax, const float (&us2)[CT], double dnext,
+                                           Track &nxt, float &zr, float &zi, float &hh) {
   // window start in the zero-padded row; windows that miss the stored band entirely contribute 0
-  const int j0 = tr.kc - p.kwin0;                       // kwin0 = k_lo + K - PAD
-  if ((unsigned)(j0 - 2) > (unsigned)p.jmax) return;    // 2 <= j0 <= nb - 1 + PAD  <=>  window overlaps the band
-  const unsigned e0 = (unsigned)(j0 >> 1), cp = (unsigned)(j0 & 1);
-  const float4 *Drow = Drow0 + (cp * p.cstrideD + e0);
-  const float2 *urow = p.ubp + (cp * p.cstrideU + e0);
-  // the same window of the next SFT will be wanted next: pull its lines into L1 now (rows are contiguous)
+  const int j0 = tr.kc - p.kwin0;                                  // kwin0 = k_lo + K - PAD
+  const bool ok = go && (unsigned)(j0 - 2) <= (unsigned)p.jmax;    // 2 <= j0 <= nb - 1 + PAD  <=>  window overlaps the band
+  Win w;
+  win_init(p, Drow0, ok ? j0 : 2, w);
+  // the same window of the next SFT will be wanted next: pull its lines (both parity copies) into L1 now
   {
-    const char *nx = (const char *)(Drow + p.npair);
+    const char *nE = (const char *)(w.dE + p.npair), *nO = (const char *)(w.dO + p.npair);
 #pragma unroll
-    for (int o = 0; o < (KT > 0 ? (KT + 1) * 16 + 127 : 128); o += 128)
-      asm volatile("prefetch.global.L1 [%0];" ::"l"(nx + o));
+    for (int o = 0; o < (KT > 0 ? (KT + 1) * 16 + 127 : 128); o += 128) {
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(nE + o));
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(nO + o));
+    }
   }
   Acc acc[CT];
 #pragma unroll
@@ -541,46 +594,51 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, con
   const float b = fres ? tr.b : 0.f;
   float scale = INV_2PI_F;     // the series evaluators return 2 pi J
   float t;                     // total phase / pi:  2 frac (= phi_a/pi) + prefactor phase / pi
-  if (bmax <= B_ORDER3 || fabsf(b) <= B_ORDER3) {
+  if (bmax <= B_ORDER3 || !(fabsf(b) > B_ORDER3)) {
     const float xp = fmaf(0.5f, b, tr.x);
-    if (bmax == 0.f) series_pairs<0, KT, CT>(p, xp, b, Drow, urow, acc);
-    else if (bmax <= B_ORDER1) series_pairs<1, KT, CT>(p, xp, b, Drow, urow, acc);
-    else if (bmax <= B_ORDER2) series_pairs<2, KT, CT>(p, xp, b, Drow, urow, acc);
-    else series_pairs<3, KT, CT>(p, xp, b, Drow, urow, acc);
+    if (bmax == 0.f) series_pairs<0, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
+    else if (bmax <= B_ORDER1) series_pairs<1, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
+    else if (bmax <= B_ORDER2) series_pairs<2, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
+    else series_pairs<3, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
     t = fmaf(2.0f, tr.frac, fmaf(0.25f, b, tr.x));         // prefactor e^{i pi (x + b/4)}
   } else {
-    fresnel_pairs<KT, CT>(p, tr.x, b, Drow, urow, acc, scale);
+    fresnel_pairs<KT, CT, CFG>(p, tm, dnext, nxt, tr.x, b, w, acc, scale);
     t = 2.0f * tr.frac;
   }
-  t = fmaf(-2.0f, rintf(0.5f * t), t);                       // into [-1, 1]
+  // |t| <= 1 + 1/2 + |b|/4: the MUFU sin/cos argument reduction (x/2pi rounded to fp32) stays below 3e-7 rad
   float sp, cp_;
   sincospi_fast(t, sp, cp_);
   const float as = scale * tr.amp;
   const float er = cp_ * as, ei = sp * as;
   const float a2 = as * as;
   const int resp = cfg_resp<CFG>(p);
+  float sr = 0.f, si = 0.f, sh = 0.f;
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
-    if (CT == 1 || us2[c] > 0.f) {
-      const float S1r = (acc[c].A.x + acc[c].A.y) - (acc[c].B.x + acc[c].B.y);
-      const float S1i = acc[c].I.x + acc[c].I.y;
-      const float S2 = acc[c].W.x + acc[c].W.y;
-      // response (Eq.(5)-(6) P:80-85 as Lambda z = Re[R z]; DESIGN C3/D4)
-      float2 R = tm.AE[c];
-      if (resp == 1) {
-        const float2 r = __ldg(rt + c * p.n_sft);
-        R = make_float2(tm.AE[c].x * r.x, tm.AE[c].x * r.y);      // AE is real here
-      } else if (resp == 2) {
-        const float2 cs = __ldg(rt + c * p.n_sft);
-        const float am = fmaf(p.depth, cs.x * tm.cl - cs.y * tm.sl, 1.0f);
-        R = make_float2(R.x * am, R.y * am);
-      }
-      const float gr = R.x * er - R.y * ei, gi = R.x * ei + R.y * er;   // p_c = R * A e^{i phi} pref
-      zr += gr * S1r - gi * S1i;
-      zi += gr * S1i + gi * S1r;
-      hh += (R.x * R.x + R.y * R.y) * a2 * us2[c] * S2;
+    const float S1r = (acc[c].A.x + acc[c].A.y) - (acc[c].B.x + acc[c].B.y);
+    const float S1i = acc[c].I.x + acc[c].I.y;
+    const float S2 = acc[c].W.x + acc[c].W.y;
+    // response (Eq.(5)-(6) P:80-85 as Lambda z = Re[R z]; DESIGN C3/D4)
+    float2 R = tm.AE[c];
+    if (resp == 1) {
+      const float2 r = __ldg(rt + c * p.n_sft);
+      R = make_float2(tm.AE[c].x * r.x, tm.AE[c].x * r.y);      // AE is real here
+    } else if (resp == 2) {
+      const float2 cs = __ldg(rt + c * p.n_sft);
+      const float am = fmaf(p.depth, cs.x * tm.cl - cs.y * tm.sl, 1.0f);
+      R = make_float2(R.x * am, R.y * am);
     }
+    const float gr = R.x * er - R.y * ei, gi = R.x * ei + R.y * er;   // p_c = R * A e^{i phi} pref
+    const float cr = gr * S1r - gi * S1i, ci = gr * S1i + gi * S1r;
+    const float chh = (R.x * R.x + R.y * R.y) * a2 * us2[c] * S2;
+    const bool present = CT == 1 || us2[c] > 0.f;      // gaps hold zeros in the store, but guard 0 * garbage
+    sr += present ? cr : 0.f;
+    si += present ? ci : 0.f;
+    sh += present ? chh : 0.f;
   }
+  zr = ok ? sr : 0.f;
+  zi = ok ? si : 0.f;
+  hh = ok ? sh : 0.f;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -619,25 +677,24 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
     const float4 *Drow0 = p.Dp + (size_t)a0 * p.npair;
     int *kcp = want_kc ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + a0 : nullptr;
     unsigned long long n_path[PATH_N] = {0, 0, 0, 0, 0};
+    Track tr;
+    track_eval<CFG>(p, tm, dalpha, tr);
 
     for (int g = a0; g < a1; g += GROUP) {
       const int ge = min(g + GROUP, a1);
       float fxh = 0.f, fhh = 0.f, fxi = 0.f;
-      for (int alpha = g; alpha < ge; ++alpha, dalpha += 1.0, ++usp, ++rt, Drow0 += p.npair) {
+      for (int alpha = g; alpha < ge; ++alpha, ++usp, ++rt, Drow0 += p.npair) {
         float us2[CT];
         bool any = false;
 #pragma unroll
         for (int c = 0; c < CT; ++c) {
           us2[c] = __ldg(usp + c * p.n_sft);
-          any |= us2[c] > 0.f;
+          any |= us2[c] > 0.f;                                   // warp-uniform
         }
-        Track tr;
-        tr.active = false;
-        tr.kc = -1;
-        tr.b = 0.f;
-        if (any || want_kc) track_eval<CFG>(p, tm, dalpha, tr);      // `any` is warp-uniform
+        dalpha += 1.0;
         const bool go = any && tr.active;
-        if (any) {
+        Track nxt;
+        if (__any_sync(0xffffffffu, go)) {
           const float ab = (go && cfg_kernel<CFG>(p) == 1) ? fabsf(tr.b) : 0.f;
           const float bmax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(ab)));
           if (CFG::KC && p.path_counts) {
@@ -646,18 +703,18 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
             for (int c = 0; c < CT; ++c) n_present += us2[c] > 0.f;
             n_path[path_of(bmax)] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * n_present);
           }
-          if (go) {
-            float zr, zi, hh;
-            pair_terms<KT, CT, CFG>(p, tm, Drow0, rt, tr, bmax, us2, zr, zi, hh);
-            if (MODE == 1) {
-              axh += (double)zr;
-              ahh += (double)hh;
-            } else {
-              fxh += zr;
-              fxi += zi;
-              fhh += hh;
-            }
+          float zr, zi, hh;
+          pair_terms<KT, CT, CFG>(p, tm, Drow0, rt, tr, go, bmax, us2, dalpha, nxt, zr, zi, hh);
+          if (MODE == 1) {
+            axh += (double)zr;
+            ahh += (double)hh;
+          } else {
+            fxh += zr;
+            fxi += zi;
+            fhh += hh;
           }
+        } else {
+          track_eval<CFG>(p, tm, dalpha, nxt);
         }
         if (CFG::KC && want_kc) {
           if (t < p.nT) {
@@ -666,6 +723,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
           }
           ++kcp;
         }
+        tr = nxt;
         if (MODE == 1) {
           txh[lane * 33 + (alpha - g)] = (float)axh;
           thh[lane * 33 + (alpha - g)] = (float)ahh;
