@@ -26,6 +26,9 @@ def _api():
 
 
 def _run_gpu(w, params=None, want_kc=True, **override):
+    """Runs the library twice: with the k_c output (run-time-flag kernel variant, which also fills the
+    evaluator-path counters) and without it (the compile-time-flag variant the benchmarks time, where
+    the plan has one).  Returns the k_c run; the other one is returned under "hot"."""
     api = _api()
     P = np.ascontiguousarray(w.params if params is None else params, dtype=np.float64)
     nT = P.shape[0]
@@ -33,7 +36,12 @@ def _run_gpu(w, params=None, want_kc=True, **override):
         xh, hh, xi = np.full(nT, np.nan), np.full(nT, np.nan), np.full(nT, np.nan)
         kc = np.full((nT, plan.n_channels, plan.n_sft), -7, dtype=np.int32) if want_kc else None
         plan.inner_products(P, xh, hh, xi, kc)
-    return dict(xh=xh, hh=hh, xh_im=xi, kc=kc)
+        paths = plan.path_counts() if want_kc else None
+        xh2, hh2, xi2 = np.full(nT, np.nan), np.full(nT, np.nan), np.full(nT, np.nan)
+        plan.inner_products(P, xh2, hh2, xi2, None)
+    if want_kc:
+        assert sum(paths.values()) == int((kc >= 0).sum()), (paths, int((kc >= 0).sum()))
+    return dict(xh=xh, hh=hh, xh_im=xi, kc=kc, paths=paths, hot=dict(xh=xh2, hh=hh2, xh_im=xi2, kc=None))
 
 
 def _check(w, g, o, xx, tol=TOL):
@@ -47,6 +55,8 @@ def _check(w, g, o, xx, tol=TOL):
     assert e_xi.max() <= tol, ("xh_im", e_xi.max(), int(e_xi.argmax()))
     assert e_hh.max() <= tol, ("hh", e_hh.max(), int(e_hh.argmax()))
     assert e_hh_rel[o["hh"] > 0].max(initial=0.0) <= tol, ("hh rel", e_hh_rel.max())
+    if g.get("hot") is not None:
+        _check(w, g["hot"], o, xx, tol)
     if g.get("kc") is not None:
         tie = (o["flags"] != 0)[:, None, :]
         bad = (g["kc"] != o["kc"]) & ~tie
@@ -233,3 +243,91 @@ def test_ended_and_degenerate_templates(et_small):
     tie = (o["flags"] != 0)[:, None, :]
     assert not ((g["kc"] != o["kc"]) & ~tie).any()
     assert g["hh"][2] == 0.0 and g["hh"][4] == 0.0
+
+
+# ------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times (default work-unit size,
+# hot kernel variants), on sampled templates the oracle computes one by one.
+def _sample_rows(n, k, seed):
+    rng = np.random.default_rng(seed)
+    return np.unique(np.concatenate([[0, 1, n - 1], rng.choice(n, size=k, replace=False)]))
+
+
+def test_config2_full_size_sampled():
+    """configs[1]: 4096 templates x 10,800 SFT slots, K = 8; 20 sampled templates against the oracle,
+    properties on all of them."""
+    api = _api()
+    w = wl.config2()
+    nT, N = w.n_templates, w.desc["n_sft"]
+    P = np.ascontiguousarray(w.params)
+    rows = _sample_rows(nT, 17, 21)
+    with api.plan_from_workload(w) as plan:
+        xh, hh, xi = np.empty(nT), np.empty(nT), np.empty(nT)
+        plan.inner_products(P, xh, hh, xi, None)
+        kc = np.empty((len(rows), 1, N), np.int32)
+        xs, hs, is_ = np.empty(len(rows)), np.empty(len(rows)), np.empty(len(rows))
+        plan.inner_products(np.ascontiguousarray(P[rows]), xs, hs, is_, kc)
+        paths = plan.path_counts()
+    o, xx, _, _ = _oracle(w, params=P[rows])
+    _check(w, dict(xh=xh[rows], hh=hh[rows], xh_im=xi[rows], kc=None), o, xx)
+    _check(w, dict(xh=xs, hh=hs, xh_im=is_, kc=kc), o, xx)
+    assert np.all(np.isfinite(xh)) and np.all(hh > 0)
+    assert xh[0] > 0.8 * hh[0] and abs(hh[0] - 900.0) < 0.1 * 900.0            # the injection: SNR 30
+    assert xh[0] > 0.9 * xh.max()                                               # and (nearly) the best match of the bank
+    assert sum(paths.values()) == int((kc >= 0).sum()) and paths["series1"] > paths["fresnel"] > 0
+
+
+def test_config3_full_size_sampled():
+    """configs[2]: cumulative SNR(t) for 16,384 templates x 10,800 SFTs (fp32 matrix), compared at 32
+    seeded SFT indices per template for sampled templates, plus properties that hold for every row."""
+    api = _api()
+    w = wl.config3()
+    nT, N = w.n_templates, w.desc["n_sft"]
+    P = np.ascontiguousarray(w.params)
+    import torch
+    with api.plan_from_workload(w) as plan:
+        Pd = torch.from_numpy(P).cuda()
+        snr = torch.empty((nT, N), dtype=torch.float32, device="cuda")
+        cx = torch.empty_like(snr)
+        ch = torch.empty_like(snr)
+        plan.cumulative_snr(Pd, snr, cx, ch)
+        xh = torch.empty(nT, dtype=torch.float64, device="cuda")
+        hh = torch.empty_like(xh)
+        plan.inner_products(Pd, xh, hh, None, None)
+        plan.sync()
+        # properties on the device, all rows
+        assert bool(torch.isfinite(snr).all())
+        assert bool((ch[:, 1:] >= ch[:, :-1] * (1.0 - 1e-6)).all())                   # <h,h> accumulates (fp32 store)
+        tot_err = (cx[:, -1].double() - xh).abs() / (xh.abs() + hh.sqrt())
+        assert float(tot_err.max()) < 1e-5                                            # last column = totals
+        assert float(((ch[:, -1].double() - hh).abs() / hh).max()) < 1e-5
+        rows = _sample_rows(nT, 9, 22)
+        idx = wl.config3_check_indices(nT, N)[rows]                                   # [rows][32] seeded indices
+        r = torch.from_numpy(rows).cuda()[:, None]
+        i = torch.from_numpy(idx).cuda()
+        g_snr, g_cx, g_ch = snr[r, i].cpu().numpy(), cx[r, i].cpu().numpy(), ch[r, i].cpu().numpy()
+    plan_o, store = to_oracle(w)
+    o = oin.cumulative_snr(plan_o, store, P[rows])
+    ref = oin.inner_products(plan_o, store, P[rows])
+    xx = oin.xx_band(plan_o, store)
+    norm = np.sqrt(xx * ref["hh"])[:, None]
+    take = lambda a: np.take_along_axis(a, idx, axis=1)
+    assert (np.abs(g_cx - take(o["cum_xh"])) / norm).max() <= TOL
+    assert (np.abs(g_ch - take(o["cum_hh"])) / norm).max() <= TOL
+    big = take(o["cum_hh"]) > 1e-3 * ref["hh"][:, None]
+    assert np.abs(g_snr - take(o["snr"]))[big].max() <= 1e-3 * max(1.0, np.abs(o["snr"]).max())
+
+
+def test_config4_full_size_sampled():
+    """configs[3]: 65,536 templates, 2 channels x 672 SFTs, annual response, K = 16."""
+    api = _api()
+    w = wl.config4()
+    nT = w.n_templates
+    P = np.ascontiguousarray(w.params)
+    rows = _sample_rows(nT, 29, 23)
+    with api.plan_from_workload(w) as plan:
+        xh, hh, xi = np.empty(nT), np.empty(nT), np.empty(nT)
+        plan.inner_products(P, xh, hh, xi, None)
+    o, xx, _, _ = _oracle(w, params=P[rows])
+    _check(w, dict(xh=xh[rows], hh=hh[rows], xh_im=xi[rows], kc=None), o, xx)
+    assert np.all(np.isfinite(xh)) and np.all(hh > 0)
