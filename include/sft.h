@@ -60,6 +60,9 @@ enum { SFT_RESP_NONE = 0,        /* R = 1                                       
        SFT_RESP_TABLE = 1,       /* R_{c,a} from sft_load_data's `response`             */
        SFT_RESP_ANNUAL = 2 };    /* R_{c,a} = [1 + depth cos(2 pi t_a/period + psi_c + lambda)]
                                     e^{i (chi_c + beta)}, (lambda, beta) per template    */
+enum { SFT_EVAL_AUTO = 0,        /* moment tables when they fit in device memory, else direct     */
+       SFT_EVAL_DIRECT = 1,      /* evaluate the 2K+1 kernel coefficients per (template, SFT)      */
+       SFT_EVAL_TABLE = 2 };     /* insist on the moment tables (SFT_ENOMEM if they do not fit)    */
 enum { SFT_MEM_HOST = 0, SFT_MEM_DEVICE = 1 };
 
 /* Analysis set-up.  Zero-initialise, then fill. */
@@ -81,6 +84,8 @@ typedef struct {
   double resp_depth;   /* SFT_RESP_ANNUAL: modulation depth                               */
   double resp_psi[SFT_MAX_CHANNELS]; /* SFT_RESP_ANNUAL: amplitude-modulation phase per channel */
   double resp_chi[SFT_MAX_CHANNELS]; /* SFT_RESP_ANNUAL: response phase per channel             */
+  int32_t evaluator;   /* SFT_EVAL_*: how sum_k conj(x~) F / S and sum_k |F|^2 / S are evaluated for
+                          |fdot| T^2 <= 0.12; results agree to ~1e-6 */
   int32_t device;      /* CUDA device ordinal                                             */
   void *stream;        /* cudaStream_t to order work on, or NULL for the legacy default stream */
 } sft_plan_desc;
@@ -142,9 +147,9 @@ double sft_plan_last_kernel_ms(sft_plan *plan);
 /* Diagnostic: how the coefficient evaluator (rows A4/A6 of the hot path) was used by the most recent
  * sft_inner_products call that had kc_out != NULL: the number of active (template, SFT, channel) pairs
  * evaluated with the series in b = fdot T^2 about the Dirichlet kernel at order 0, 1, 2, 3 (out[0..3])
- * and with the closed Fresnel form Eq.(29) P:219 (out[4]).  The order is chosen per warp of 32
- * templates from the largest |b| in the warp.  Blocks until that call finished.
- * Writes min(n_out, 5) values; host pointer. */
+ * with the closed Fresnel form Eq.(29) P:219 (out[4]) and through the moment tables (out[5]).  The
+ * path is chosen per warp of 32 templates from the largest |b| in the warp.
+ * Blocks until that call finished.  Writes min(n_out, 6) values; host pointer. */
 sft_status sft_plan_path_counts(sft_plan *plan, int64_t *out, int32_t n_out);
 
 /* Tuning knob: SFTs per work unit along the time axis (0 = automatic).  Results do not depend on it

@@ -18,7 +18,8 @@ KERNEL = {"dirichlet": 0, "fresnel": 1}
 RESPONSE = {"none": 0, "table": 1, "annual": 2}
 PHASE = {"fp64": 0, "split32": 1}
 MEM_HOST, MEM_DEVICE = 0, 1
-PATHS = ("series0", "series1", "series2", "series3", "fresnel")
+PATHS = ("series0", "series1", "series2", "series3", "fresnel", "table")
+EVALUATOR = {"auto": 0, "direct": 1, "table": 2}
 STATUS = {0: "SFT_OK", 1: "SFT_EINVAL", 2: "SFT_ESHAPE", 3: "SFT_ENODATA", 4: "SFT_EUNSUPPORTED",
           5: "SFT_ECUDA", 6: "SFT_ENOMEM"}
 
@@ -39,7 +40,7 @@ class PlanDesc(C.Structure):
                 ("f_lo", C.c_double), ("f_hi", C.c_double), ("f_ref", C.c_double),
                 ("resp_period", C.c_double), ("resp_depth", C.c_double),
                 ("resp_psi", C.c_double * MAX_CHANNELS), ("resp_chi", C.c_double * MAX_CHANNELS),
-                ("device", C.c_int32), ("stream", C.c_void_p)]
+                ("evaluator", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p)]
 
 
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
@@ -149,6 +150,8 @@ class Plan:
             pd.resp_psi[i] = float(v)
         for i, v in enumerate(d.get("resp_chi", ())):
             pd.resp_chi[i] = float(v)
+        ev = d.get("evaluator", "auto")
+        pd.evaluator = EVALUATOR[ev] if isinstance(ev, str) else int(ev)
         pd.device = int(device)
         pd.stream = C.c_void_p(int(stream)) if stream else None
         self.desc = pd
@@ -222,8 +225,8 @@ class Plan:
 
     def path_counts(self):
         """``sft_plan_path_counts``: dict path name -> active pairs of the last call that had kc_out."""
-        out = (C.c_int64 * 5)()
-        self._check(self.lib.sft_plan_path_counts(self._h, out, 5))
+        out = (C.c_int64 * 6)()
+        self._check(self.lib.sft_plan_path_counts(self._h, out, 6))
         return dict(zip(PATHS, [int(v) for v in out]))
 
 

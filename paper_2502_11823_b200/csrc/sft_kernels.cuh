@@ -24,6 +24,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "fresnel_aux_coeffs.h"
+#include "sft_table.cuh"
 
 namespace sftk {
 
@@ -63,6 +64,11 @@ struct KParams {
   int n_tgroups, n_items;  // work units: n_tgroups = ceil(nT/32) template groups x n_chunks
   int *counter;            // work-unit counter (zeroed before every launch)
   unsigned long long *path_counts;   // nullable [PATH_N]: active pairs per evaluator path (diagnostic)
+  // moment-table evaluator (sft_table.cuh); mtab == nullptr: direct evaluator only
+  const float4 *mtab;      // [C][n_sft][n_node][4]   8 complex64 moments per node, node = kcidx * TAB_R + cell
+  const float4 *htab;      // [C][n_kc * HTAB_R][4]   <h,h> polynomial per node
+  unsigned mrow, mchan;    // float4 entries per SFT row (n_node * 4) and per channel (n_sft * mrow), hchan likewise
+  unsigned hchan;
   double *part;            // [n_chunks][3][nT] chunk totals (xh, hh, xh_im)
   int *kc_out;             // [nT][C][n_sft] or null
   float *loc_xh, *loc_hh;  // cumulative mode: [nT][n_sft] chunk-local prefix sums
@@ -554,70 +560,153 @@ __device__ __forceinline__ void fresnel_pairs(const KParams &p, const Tmpl &tm, 
 }
 
 // Evaluator paths (warp-uniform): series order 0..3, closed Fresnel form.
-enum { PATH_ORD0 = 0, PATH_ORD1, PATH_ORD2, PATH_ORD3, PATH_FRESNEL, PATH_N };
+enum { PATH_ORD0 = 0, PATH_ORD1, PATH_ORD2, PATH_ORD3, PATH_FRESNEL, PATH_TABLE, PATH_N };
 
-__device__ __forceinline__ int path_of(float bmax) {
+__device__ __forceinline__ int path_of(float bmax, bool table) {
+  if (table && bmax <= B_TABLE) return PATH_TABLE;
   return bmax == 0.f ? PATH_ORD0 : bmax <= B_ORDER1 ? PATH_ORD1 : bmax <= B_ORDER2 ? PATH_ORD2 : bmax <= B_ORDER3 ? PATH_ORD3
                                                                                                                : PATH_FRESNEL;
+}
+
+// X + i s Y for complex X, Y held as (re, im) pairs; sp = (-s, s)
+__device__ __forceinline__ float2 cstep(float2 X, float2 sp, float2 Y) {
+  return __ffma2_rn(make_float2(Y.y, Y.x), sp, X);
+}
+
+// Moment-table evaluator of one (template, SFT): S1 = sum_m D J_m and S2 = sum_m u |J_m|^2 from the tables
+// of sft_table.cuh (true J, no 2 pi).  `kcidx` = k_c - (k_lo - K), already clamped to the table;
+// `Mrow` = row of SFT alpha, channel 0.  Also evaluates the track of the next SFT (see series_pairs).
+template <int CT, class CFG>
+__device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, double dnext, Track &nxt, float xp, float b,
+                                           int kcidx, const float4 *Mrow, float (&s1r)[CT], float (&s1i)[CT],
+                                           float (&s2)[CT]) {
+  const int cell = max(0, min(TAB_R - 1, (int)((xp + 0.5f) * (float)TAB_R)));
+  const int cellH = max(0, min(HTAB_R - 1, (int)((xp + 0.5f) * (float)HTAB_R)));
+  const float4 *mp = Mrow + (unsigned)(kcidx * TAB_R + cell) * 4u;
+  const float4 *hp = p.htab + (unsigned)(kcidx * HTAB_R + cellH) * 4u;
+  float4 Mq[CT][4], Hq[CT][3];
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) Mq[c][i] = __ldg(mp + c * p.mchan + i);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) Hq[c][i] = __ldg(hp + c * p.hchan + i);
+  }
+  track_eval<CFG>(p, tm, dnext, nxt);
+  const float a = (2.0f * PI_F) * (xp - (((float)cell + 0.5f) * (1.0f / TAB_R) - 0.5f));
+  const float aH = (2.0f * PI_F) * (xp - (((float)cellH + 0.5f) * (1.0f / HTAB_R) - 0.5f));
+  const float be = PI_F * b;
+  const float2 nb1 = make_float2(-be, be), nb2 = make_float2(-0.5f * be, 0.5f * be),
+               nb3 = make_float2(-(1.0f / 3.0f) * be, (1.0f / 3.0f) * be);
+  const float2 na1 = make_float2(-a, a), na2 = make_float2(-0.5f * a, 0.5f * a),
+               na3 = make_float2(-(1.0f / 3.0f) * a, (1.0f / 3.0f) * a), na4 = make_float2(-0.25f * a, 0.25f * a),
+               na5 = make_float2(-0.2f * a, 0.2f * a), na6 = make_float2(-(1.0f / 6.0f) * a, (1.0f / 6.0f) * a),
+               na7 = make_float2(-(1.0f / 7.0f) * a, (1.0f / 7.0f) * a);
+  const float be2 = be * be;
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+    const float2 M0 = make_float2(Mq[c][0].x, Mq[c][0].y), M1 = make_float2(Mq[c][0].z, Mq[c][0].w);
+    const float2 M2 = make_float2(Mq[c][1].x, Mq[c][1].y), M3 = make_float2(Mq[c][1].z, Mq[c][1].w);
+    const float2 M4 = make_float2(Mq[c][2].x, Mq[c][2].y), M5 = make_float2(Mq[c][2].z, Mq[c][2].w);
+    const float2 M6 = make_float2(Mq[c][3].x, Mq[c][3].y), M7 = make_float2(Mq[c][3].z, Mq[c][3].w);
+    // L_p = sum_n (i beta)^n / n! M_{p+2n}
+    const float2 L4 = cstep(M4, nb1, M6), L5 = cstep(M5, nb1, M7);
+    const float2 L2 = cstep(M2, nb1, cstep(M4, nb2, M6)), L3 = cstep(M3, nb1, cstep(M5, nb2, M7));
+    const float2 L0 = cstep(M0, nb1, cstep(M2, nb2, cstep(M4, nb3, M6)));
+    const float2 L1 = cstep(M1, nb1, cstep(M3, nb2, cstep(M5, nb3, M7)));
+    // S1 = sum_p (i a)^p / p! L_p
+    float2 S = cstep(M6, na7, M7);
+    S = cstep(L5, na6, S);
+    S = cstep(L4, na5, S);
+    S = cstep(L3, na4, S);
+    S = cstep(L2, na3, S);
+    S = cstep(L1, na2, S);
+    S = cstep(L0, na1, S);
+    s1r[c] = S.x;
+    s1i[c] = S.y;
+    // H = sum_P aH^P (h_{P,0} + beta^2 h_{P,2});  floats: h00 h10 h20 h30 | h40 h50 h02 h12 | h22 h32 h42 h52
+    float h = fmaf(be2, Hq[c][2].w, Hq[c][1].y);
+    h = fmaf(h, aH, fmaf(be2, Hq[c][2].z, Hq[c][1].x));
+    h = fmaf(h, aH, fmaf(be2, Hq[c][2].y, Hq[c][0].w));
+    h = fmaf(h, aH, fmaf(be2, Hq[c][2].x, Hq[c][0].z));
+    h = fmaf(h, aH, fmaf(be2, Hq[c][1].w, Hq[c][0].y));
+    h = fmaf(h, aH, fmaf(be2, Hq[c][1].z, Hq[c][0].x));
+    s2[c] = h;
+  }
 }
 
 // Z_c = Re/Im of the per-(SFT, channel) complex term, H_c its <h,h> term (include/sft.h).
 // Called by the whole warp as soon as one lane has an active pair (`go`); the other lanes run along on a
 // clamped window and their results are discarded, so the control flow stays warp-uniform.
-// `bmax` is the warp-wide max |b| of the active pairs: it selects the series order for the whole warp
-// (a higher order than a lane needs is still correct for that lane).  `Drow0` points at the padded row
-// of SFT alpha, channel 0, copy 0.  Also evaluates the track of the next SFT (see series_pairs).
+// `bmax` is the warp-wide max |b| of the active pairs: it selects the evaluator for the whole warp - the
+// moment tables up to B_TABLE (if the plan has them), else the series order (a higher order than a lane
+// needs is still correct for that lane) or the closed Fresnel form.  `Drow0` / `Mrow0` point at the row
+// of SFT alpha, channel 0, in the pair-planar store / the moment table.  Also evaluates the track of the
+// next SFT (see series_pairs).
 template <int KT, int CT, class CFG>
-__device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, const float4 *Drow0, const float2 *rt,
-                                           const Track &tr, bool go, float bmax, const float (&us2)[CT], double dnext,
-                                           Track &nxt, float &zr, float &zi, float &hh) {
+__device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, const float4 *Drow0, const float4 *Mrow0,
+                                           const float2 *rt, const Track &tr, bool go, float bmax, const float (&us2)[CT],
+                                           double dnext, Track &nxt, float &zr, float &zi, float &hh) {
   // window start in the zero-padded row; windows that miss the stored band entirely contribute 0
   const int j0 = tr.kc - p.kwin0;                                  // kwin0 = k_lo + K - PAD
   const bool ok = go && (unsigned)(j0 - 2) <= (unsigned)p.jmax;    // 2 <= j0 <= nb - 1 + PAD  <=>  window overlaps the band
-  Win w;
-  win_init(p, Drow0, ok ? j0 : 2, w);
-  // the same window of the next SFT will be wanted next: pull its lines (both parity copies) into L1 now
-  {
-    const char *nE = (const char *)(w.dE + p.npair), *nO = (const char *)(w.dO + p.npair);
-#pragma unroll
-    for (int o = 0; o < (KT > 0 ? (KT + 1) * 16 + 127 : 128); o += 128) {
-      asm volatile("prefetch.global.L1 [%0];" ::"l"(nE + o));
-      asm volatile("prefetch.global.L1 [%0];" ::"l"(nO + o));
-    }
-  }
-  Acc acc[CT];
-#pragma unroll
-  for (int c = 0; c < CT; ++c) {
-    acc[c].A = make_float2(0.f, 0.f); acc[c].B = acc[c].A; acc[c].I = acc[c].A; acc[c].W = acc[c].A;
-  }
+  const int j0c = ok ? j0 : 2;
   const bool fres = (cfg_kernel<CFG>(p) == 1);
   const float b = fres ? tr.b : 0.f;
-  float scale = INV_2PI_F;     // the series evaluators return 2 pi J
+  float s1r[CT], s1i[CT], s2[CT];
+  float scale;                 // the series evaluators return 2 pi J
   float t;                     // total phase / pi:  2 frac (= phi_a/pi) + prefactor phase / pi
-  if (bmax <= B_ORDER3 || !(fabsf(b) > B_ORDER3)) {
+  if (p.mtab != nullptr && bmax <= B_TABLE) {
     const float xp = fmaf(0.5f, b, tr.x);
-    if (bmax == 0.f) series_pairs<0, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
-    else if (bmax <= B_ORDER1) series_pairs<1, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
-    else if (bmax <= B_ORDER2) series_pairs<2, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
-    else series_pairs<3, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
-    t = fmaf(2.0f, tr.frac, fmaf(0.25f, b, tr.x));         // prefactor e^{i pi (x + b/4)}
+    table_eval<CT, CFG>(p, tm, dnext, nxt, xp, b, j0c - 2, Mrow0, s1r, s1i, s2);
+    scale = 1.0f;
+    t = fmaf(2.0f, tr.frac, fmaf(0.25f, b, tr.x));           // prefactor e^{i pi (x + b/4)}
   } else {
-    fresnel_pairs<KT, CT, CFG>(p, tm, dnext, nxt, tr.x, b, w, acc, scale);
-    t = 2.0f * tr.frac;
+    Win w;
+    win_init(p, Drow0, j0c, w);
+    // the same window of the next SFT will be wanted next: pull its lines (both parity copies) into L1 now
+    {
+      const char *nE = (const char *)(w.dE + p.npair), *nO = (const char *)(w.dO + p.npair);
+#pragma unroll
+      for (int o = 0; o < (KT > 0 ? (KT + 1) * 16 + 127 : 128); o += 128) {
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(nE + o));
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(nO + o));
+      }
+    }
+    Acc acc[CT];
+#pragma unroll
+    for (int c = 0; c < CT; ++c) {
+      acc[c].A = make_float2(0.f, 0.f); acc[c].B = acc[c].A; acc[c].I = acc[c].A; acc[c].W = acc[c].A;
+    }
+    scale = INV_2PI_F;
+    if (bmax <= B_ORDER3 || !(fabsf(b) > B_ORDER3)) {
+      const float xp = fmaf(0.5f, b, tr.x);
+      if (bmax == 0.f) series_pairs<0, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
+      else if (bmax <= B_ORDER1) series_pairs<1, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
+      else if (bmax <= B_ORDER2) series_pairs<2, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
+      else series_pairs<3, KT, CT, CFG>(p, tm, dnext, nxt, xp, b, w, acc);
+      t = fmaf(2.0f, tr.frac, fmaf(0.25f, b, tr.x));         // prefactor e^{i pi (x + b/4)}
+    } else {
+      fresnel_pairs<KT, CT, CFG>(p, tm, dnext, nxt, tr.x, b, w, acc, scale);
+      t = 2.0f * tr.frac;
+    }
+#pragma unroll
+    for (int c = 0; c < CT; ++c) {
+      s1r[c] = (acc[c].A.x + acc[c].A.y) - (acc[c].B.x + acc[c].B.y);
+      s1i[c] = acc[c].I.x + acc[c].I.y;
+      s2[c] = scale * (acc[c].W.x + acc[c].W.y);             // one of the two factors `scale` of |J|^2
+    }
   }
   // |t| <= 1 + 1/2 + |b|/4: the MUFU sin/cos argument reduction (x/2pi rounded to fp32) stays below 3e-7 rad
   float sp, cp_;
   sincospi_fast(t, sp, cp_);
   const float as = scale * tr.amp;
   const float er = cp_ * as, ei = sp * as;
-  const float a2 = as * as;
+  const float a2 = as * tr.amp;
   const int resp = cfg_resp<CFG>(p);
   float sr = 0.f, si = 0.f, sh = 0.f;
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
-    const float S1r = (acc[c].A.x + acc[c].A.y) - (acc[c].B.x + acc[c].B.y);
-    const float S1i = acc[c].I.x + acc[c].I.y;
-    const float S2 = acc[c].W.x + acc[c].W.y;
     // response (Eq.(5)-(6) P:80-85 as Lambda z = Re[R z]; DESIGN C3/D4)
     float2 R = tm.AE[c];
     if (resp == 1) {
@@ -628,9 +717,14 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, con
       const float am = fmaf(p.depth, cs.x * tm.cl - cs.y * tm.sl, 1.0f);
       R = make_float2(R.x * am, R.y * am);
     }
-    const float gr = R.x * er - R.y * ei, gi = R.x * ei + R.y * er;   // p_c = R * A e^{i phi} pref
-    const float cr = gr * S1r - gi * S1i, ci = gr * S1i + gi * S1r;
-    const float chh = (R.x * R.x + R.y * R.y) * a2 * us2[c] * S2;
+    float gr, gi, r2;
+    if (resp == 0) {                   // AE is real
+      gr = R.x * er; gi = R.x * ei; r2 = R.x * R.x;
+    } else {
+      gr = R.x * er - R.y * ei; gi = R.x * ei + R.y * er; r2 = R.x * R.x + R.y * R.y;   // p_c = R * A e^{i phi} pref
+    }
+    const float cr = gr * s1r[c] - gi * s1i[c], ci = gr * s1i[c] + gi * s1r[c];
+    const float chh = r2 * a2 * us2[c] * s2[c];
     const bool present = CT == 1 || us2[c] > 0.f;      // gaps hold zeros in the store, but guard 0 * garbage
     sr += present ? cr : 0.f;
     si += present ? ci : 0.f;
@@ -675,15 +769,16 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
     const float *usp = p.us2 + a0;
     const float2 *rt = p.rtab + a0;
     const float4 *Drow0 = p.Dp + (size_t)a0 * p.npair;
+    const float4 *Mrow0 = p.mtab ? p.mtab + (size_t)a0 * p.mrow : nullptr;
     int *kcp = want_kc ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + a0 : nullptr;
-    unsigned long long n_path[PATH_N] = {0, 0, 0, 0, 0};
+    unsigned long long n_path[PATH_N] = {0, 0, 0, 0, 0, 0};
     Track tr;
     track_eval<CFG>(p, tm, dalpha, tr);
 
     for (int g = a0; g < a1; g += GROUP) {
       const int ge = min(g + GROUP, a1);
       float fxh = 0.f, fhh = 0.f, fxi = 0.f;
-      for (int alpha = g; alpha < ge; ++alpha, ++usp, ++rt, Drow0 += p.npair) {
+      for (int alpha = g; alpha < ge; ++alpha, ++usp, ++rt, Drow0 += p.npair, Mrow0 += p.mrow) {
         float us2[CT];
         bool any = false;
 #pragma unroll
@@ -701,10 +796,10 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
             int n_present = 0;
 #pragma unroll
             for (int c = 0; c < CT; ++c) n_present += us2[c] > 0.f;
-            n_path[path_of(bmax)] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * n_present);
+            n_path[path_of(bmax, p.mtab != nullptr)] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * n_present);
           }
           float zr, zi, hh;
-          pair_terms<KT, CT, CFG>(p, tm, Drow0, rt, tr, go, bmax, us2, dalpha, nxt, zr, zi, hh);
+          pair_terms<KT, CT, CFG>(p, tm, Drow0, Mrow0, rt, tr, go, bmax, us2, dalpha, nxt, zr, zi, hh);
           if (MODE == 1) {
             axh += (double)zr;
             ahh += (double)hh;

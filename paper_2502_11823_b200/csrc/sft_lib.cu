@@ -36,6 +36,10 @@ struct sft_plan {
   float *loc = nullptr; size_t loc_bytes = 0;          // cumulative: chunk-local prefixes
   double *td = nullptr; size_t td_bytes = 0;           // per-template constants (sft_tmpl_kernel)
   float *tf = nullptr; size_t tf_bytes = 0;
+  float4 *mtab = nullptr;                              // [C][n_sft][n_node][4] data-moment table (sft_table.cuh), or null
+  float4 *htab = nullptr;                              // [C][n_kc * HTAB_R][4] <h,h> table
+  float2 *ptab = nullptr;                              // [(2K+1)][TAB_R][TAB_Q+1] kernel moments at the nodes
+  int n_kc = 0, n_node = 0;
   int *counter = nullptr;                              // work-unit counter of the persistent main kernel
   unsigned long long *path_counts = nullptr;           // [PATH_N] diagnostic counters
   int n_sm = 0;
@@ -98,6 +102,7 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   if (!(d.f_ref > 0.0)) return fail(nullptr, SFT_EINVAL, "f_ref must be > 0");
   if (!(d.f_hi >= d.f_lo)) return fail(nullptr, SFT_EINVAL, "need f_lo <= f_hi");
   if (d.response == SFT_RESP_ANNUAL && !(d.resp_period > 0.0)) return fail(nullptr, SFT_EINVAL, "resp_period must be > 0");
+  if (d.evaluator < SFT_EVAL_AUTO || d.evaluator > SFT_EVAL_TABLE) return fail(nullptr, SFT_EINVAL, "unknown evaluator %d", d.evaluator);
   int ndev = 0;
   cudaError_t e = cudaGetDeviceCount(&ndev);
   if (e != cudaSuccess) return fail(nullptr, SFT_ECUDA, "cudaGetDeviceCount: %s", cudaGetErrorString(e));
@@ -130,6 +135,30 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   alloc((void **)&p->ubp, 2 * C * npair * sizeof(float2));
   alloc((void **)&p->us2, C * N * sizeof(float));
   alloc((void **)&p->rtab, C * N * sizeof(float2));
+  // moment tables (sft_table.cuh): 64 bytes per node, TAB_R nodes per window position and SFT.  AUTO takes
+  // them when they fit in a quarter of the free device memory, TABLE insists, DIRECT never builds them.
+  p->n_kc = p->nb + 2 * d.K;
+  p->n_node = p->n_kc * sftk::TAB_R;
+  if (st == SFT_OK && d.evaluator != SFT_EVAL_DIRECT) {
+    const double m_bytes = (double)C * (double)N * p->n_node * 64.0;
+    size_t free_b = 0, total_b = 0;
+    cudaMemGetInfo(&free_b, &total_b);
+    const bool fits = m_bytes <= 0.25 * (double)free_b && (double)C * (double)N * p->n_node * 4.0 < 4.0e9;
+    if (!fits && d.evaluator == SFT_EVAL_TABLE)
+      st = fail(nullptr, SFT_ENOMEM, "moment tables of %.3g bytes do not fit (free %.3g)", m_bytes, (double)free_b);
+    if (fits) {
+      alloc((void **)&p->mtab, (size_t)m_bytes);
+      alloc((void **)&p->htab, C * (size_t)p->n_kc * sftk::HTAB_R * sftk::HTAB_W * sizeof(float));
+      alloc((void **)&p->ptab, (size_t)(2 * d.K + 1) * sftk::TAB_R * (sftk::TAB_Q + 1) * sizeof(float2));
+      if (st == SFT_OK) {
+        const int n = (2 * d.K + 1) * sftk::TAB_R;
+        sftk::sft_ptab_kernel<<<(n + 63) / 64, 64, 0, p->stream>>>(d.K, p->ptab);
+        p->launches++;
+        cudaError_t e2 = cudaGetLastError();
+        if (e2 != cudaSuccess) st = fail(nullptr, SFT_ECUDA, "kernel-moment table launch: %s", cudaGetErrorString(e2));
+      }
+    }
+  }
   alloc((void **)&p->counter, sizeof(int));
   alloc((void **)&p->path_counts, sftk::PATH_N * sizeof(unsigned long long));
   if (st == SFT_OK) {
@@ -169,6 +198,7 @@ SFT_API sft_status sft_plan_destroy(sft_plan *p) {
   cudaFree(p->Dp); cudaFree(p->ubp); cudaFree(p->us2); cudaFree(p->rtab);
   cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->loc);
   cudaFree(p->td); cudaFree(p->tf); cudaFree(p->counter); cudaFree(p->path_counts);
+  cudaFree(p->mtab); cudaFree(p->htab); cudaFree(p->ptab);
   if (p->ev0) cudaEventDestroy(p->ev0);
   if (p->ev1) cudaEventDestroy(p->ev1);
   delete p;
@@ -273,6 +303,17 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
       d_shape, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi, p->PAD, p->npair, S_ref, p->ubp + (size_t)channel * npair,
       p->ubp + (C + (size_t)channel) * npair);
   p->launches += 2;
+  if (p->mtab) {
+    const size_t per_chan = N * (size_t)p->n_node * 4;
+    const unsigned outs = (unsigned)p->n_node * (sftk::TAB_Q + 1);
+    const unsigned bpr = (outs + 255) / 256;
+    if ((double)bpr * (double)N > 2.0e9) return fail(p, SFT_EUNSUPPORTED, "moment-table build grid too large");
+    sftk::sft_mtab_kernel<<<(unsigned)(bpr * N), 256, 0, p->stream>>>(
+        p->Dp + (size_t)channel * N * npair, p->npair, p->n_node, p->d.K, p->ptab, bpr, (float2 *)(p->mtab + (size_t)channel * per_chan));
+    sftk::sft_htab_kernel<<<(unsigned)(p->n_kc * sftk::HTAB_R), 64, 0, p->stream>>>(
+        p->ubp + (size_t)channel * npair, p->d.K, (float *)(p->htab + (size_t)channel * p->n_kc * sftk::HTAB_R * 4));
+    p->launches += 2;
+  }
   cudaError_t e = cudaGetLastError();
   cudaError_t e2 = cudaStreamSynchronize(p->stream);
   if (tmp) cudaFree(tmp);
@@ -313,6 +354,11 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
     k.chi[c] = p->d.resp_chi[c];
   }
   k.depth = (float)p->d.resp_depth;
+  k.mtab = p->mtab;
+  k.htab = p->htab;
+  k.mrow = p->mtab ? (unsigned)p->n_node * 4u : 0u;
+  k.mchan = p->mtab ? (unsigned)(p->d.n_sft * p->n_node * 4) : 0u;
+  k.hchan = (unsigned)(p->n_kc * sftk::HTAB_R * 4);
   k.Dp = p->Dp;
   k.ubp = p->ubp;
   k.us2 = p->us2;

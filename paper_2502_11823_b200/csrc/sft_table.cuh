@@ -1,0 +1,163 @@
+// sft_table.cuh - the moment-table evaluator of libsft_b200.so: load-time kernels (sm_100a).
+//
+// Idea ("moment tables").  For one (channel, SFT) the contraction of rows A4+A6,
+//
+//   S1(xp, b) = sum_{m=-K..K} D_{kc+m} J_m(xp, b),
+//   J_m(xp, b) = (-1)^m int_{-1/2}^{1/2} exp(i (2 pi (xp - m) v + pi b v^2)) dv        (Eq.(28) P:215 about the SFT mid-point)
+//
+// is a smooth (entire) function of the template's fractional bin offset xp = f_a T + b/2 - k_c and of
+// b = fdot T^2: with E(v) = sum_m D_{kc+m} (-1)^m e^{-2 pi i m v} it is int e^{i(2 pi xp v + pi b v^2)} E(v) dv.
+// Expanding about a node xj (xp = xj + delta) and b = 0,
+//
+//   S1 = sum_{p,n} (i a)^p/p! (i beta)^n/n! M_{p+2n}(kc, xj),   a = 2 pi delta, beta = pi b,
+//   M_q(kc, xj) = sum_m D_{kc+m} (-1)^m rho_q(xj - m),   rho_q(a') = int_{-1/2}^{1/2} v^q e^{2 pi i a' v} dv,
+//
+// with |v| <= 1/2 the terms fall like (pi delta)^p/p! (pi b/4)^n/n!.  The moments M_q do not depend on
+// the template: they are computed ONCE per data set (as the SFTs themselves are) for
+// every window position kc and TAB_R nodes per bin, q = 0..TAB_Q, and kept in HBM; a template then
+// needs 64 bytes and ~20 packed FMAs per (SFT, channel) instead of evaluating 2K+1 kernel coefficients.
+// Truncation error at TAB_R = 4, TAB_Q = 7: <= 1e-6 sqrt(sum |D|^2) for |b| <= B_TABLE = 0.12 (measured
+// 4e-7 at b = 0.12, 3e-8 at b = 0.056); larger |b| takes the direct evaluator of sft_kernels.cuh.
+//
+// The <h,h> sum H(kc, xp, b) = sum_m u_{kc+m} |J_m|^2 (u = S_ref/S_k) does not depend on the data at
+// all; it is even in b and tabulated per window position on HTAB_R nodes per bin as
+//   H = sum_{P<=5} a^P (h_{P,0} + beta^2 h_{P,2})      (relative error < 3e-7 for |b| <= 0.12).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sftk {
+
+constexpr int TAB_R = 4;      // nodes per bin of the data-moment table
+constexpr int TAB_Q = 7;      // highest moment kept (TAB_Q + 1 complex64 = 64 bytes per node)
+constexpr int HTAB_R = 16;    // nodes per bin of the <h,h> table
+constexpr int HTAB_P = 5;     // highest power of a kept
+constexpr int HTAB_W = 16;    // floats per node: h_{0..5,0}, h_{0..5,2}, 4 x pad
+constexpr float B_TABLE = 0.12f;
+
+// sigma_q(a') with rho_q = sigma_q (q even), i sigma_q (q odd):  sigma_q = int v^q cos(w v) dv (q even), int v^q sin(w v) dv (q odd),
+// w = 2 pi a', over [-1/2, 1/2].  |a'| >= 1.5: integration by parts upwards in q (each step multiplies
+// the error by q/w < 1); below: power series in w (|w|/2 < 4.8: 40 terms leave < 1e-17).
+template <int NQ>
+__device__ void sigma_moments(double ap, double (&sig)[NQ]) {
+  const double w = 6.283185307179586 * ap;
+  if (fabs(ap) >= 1.5) {
+    double s, c;
+    sincospi(ap, &s, &c);              // sin(w/2), cos(w/2)
+    const double iw = 1.0 / w;
+    double hq = 1.0;                   // (1/2)^q
+    sig[0] = 2.0 * s * iw;
+#pragma unroll
+    for (int q = 1; q < NQ; ++q) {
+      hq *= 0.5;
+      sig[q] = (q & 1) ? (-2.0 * hq * c + q * sig[q - 1]) * iw : (2.0 * hq * s - q * sig[q - 1]) * iw;
+    }
+  } else {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) sig[q] = 0.0;
+    double term = 1.0;                 // w^k / k!
+    for (int k = 0; k < 44; ++k) {
+      const double sgn = ((k >> 1) & 1) ? -1.0 : 1.0;        // (-1)^floor(k/2)
+      double hp = ldexp(1.0, -(k + 1));                      // (1/2)^(q+k+1), q = 0
+#pragma unroll
+      for (int q = 0; q < NQ; ++q) {
+        if (((q + k) & 1) == 0) sig[q] += sgn * term * 2.0 * hp / (double)(q + k + 1);
+        hp *= 0.5;
+      }
+      term *= w / (double)(k + 1);
+    }
+  }
+}
+
+// P-table: ptab[mi][cell][q] = (-1)^m rho_q(xj_cell - m) as complex64, m = mi - K.
+__global__ void sft_ptab_kernel(int K, float2 *ptab) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (2 * K + 1) * TAB_R) return;
+  const int mi = idx / TAB_R, cell = idx - mi * TAB_R, m = mi - K;
+  const double xj = ((double)cell + 0.5) / TAB_R - 0.5;
+  double sig[TAB_Q + 1];
+  sigma_moments<TAB_Q + 1>(xj - (double)m, sig);
+  const double sg = (m & 1) ? -1.0 : 1.0;
+#pragma unroll
+  for (int q = 0; q <= TAB_Q; ++q) {
+    const double v = sg * sig[q];
+    ptab[(size_t)idx * (TAB_Q + 1) + q] = (q & 1) ? make_float2(0.f, (float)v) : make_float2((float)v, 0.f);
+  }
+}
+
+// Data-moment table of one channel: mtab[a][node][q], node = kcidx * TAB_R + cell, kcidx = kc - (k_lo - K).
+// 1-D grid of n_sft * bpr blocks (bpr = ceil(n_node * 8 / 256) blocks per SFT row); the padded whitened row of SFT a is read from copy 0 of the
+// pair-planar store (neighbouring threads share a window: L1 broadcast), ptab through L1 (consecutive
+// threads read consecutive entries).
+__global__ void __launch_bounds__(256) sft_mtab_kernel(const float4 *Dp0, int npair, int n_node, int K, const float2 *ptab,
+                                                       unsigned bpr, float2 *mtab) {
+  const unsigned a = blockIdx.x / bpr, bx = blockIdx.x - a * bpr;
+  const float4 *src = Dp0 + (size_t)a * npair;
+  constexpr int nq = TAB_Q + 1, per_bin = TAB_R * nq;
+  const int o = bx * blockDim.x + threadIdx.x;                // (node, q) flattened
+  if (o >= n_node * nq) return;
+  const int kcidx = o / per_bin, cq = o - kcidx * per_bin;     // cq = cell * nq + q
+  const float2 *pp = ptab + cq;
+  float re = 0.f, im = 0.f;
+  const int nb = 2 * K + 1;
+  for (int mi = 0; mi < nb; ++mi) {
+    const int j = kcidx + 2 + mi;                              // window start j0 = kcidx + 2
+    const float4 d4 = __ldg(src + (j >> 1));
+    const float dx = (j & 1) ? d4.y : d4.x, dy = (j & 1) ? d4.w : d4.z;
+    const float2 pv = __ldg(pp + (size_t)mi * per_bin);
+    re = fmaf(dx, pv.x, re); re = fmaf(-dy, pv.y, re);
+    im = fmaf(dx, pv.y, im); im = fmaf(dy, pv.x, im);
+  }
+  mtab[((size_t)a * n_node) * nq + o] = make_float2(re, im);
+}
+
+// <h,h> table of one channel: htab[nodeH][HTAB_W], nodeH = kcidx * HTAB_R + cell.  One block per node,
+// threads over the 2K+1 bins; fp64.  With c_{p,n} = (-1)^m i^(p+n) rho_{p+2n} / (p! n!) the polynomial of
+// |J_m|^2 in (a, beta) has the coefficients  h_{P,N} = sum_{p+p'=P, n+n'=N} Re[c_{p,n} conj(c_{p',n'})].
+__global__ void __launch_bounds__(64) sft_htab_kernel(const float2 *ub0, int K, float *htab) {
+  constexpr int NQ = HTAB_P + 5;        // rho_0 .. rho_{P+4}  (p <= 5, n <= 2)
+  __shared__ double red[2 * (HTAB_P + 1)];
+  const int node = blockIdx.x, kcidx = node / HTAB_R, cell = node - kcidx * HTAB_R;
+  if (threadIdx.x < 2 * (HTAB_P + 1)) red[threadIdx.x] = 0.0;
+  __syncthreads();
+  const double xj = ((double)cell + 0.5) / HTAB_R - 0.5;
+  const double fact[6] = {1.0, 1.0, 2.0, 6.0, 24.0, 120.0};
+  for (int mi = threadIdx.x; mi <= 2 * K; mi += blockDim.x) {
+    const int j = kcidx + 2 + mi;
+    const float2 u2 = __ldg(ub0 + (j >> 1));
+    const double u = (j & 1) ? (double)u2.y : (double)u2.x;
+    if (u == 0.0) continue;
+    double sig[NQ];
+    sigma_moments<NQ>(xj - (double)(mi - K), sig);
+    // rho_q = sigma_q (q even), i sigma_q (q odd), and p + 2n has the parity of p:
+    // c_{p,n} = e_p i^n sigma_{p+2n} / (p! n!) with the real sign e_p = i^p (p odd ? i : 1) = (-1)^ceil(p/2).
+    double h0[HTAB_P + 1], h2[HTAB_P + 1];
+#pragma unroll
+    for (int P = 0; P <= HTAB_P; ++P) {
+      double s0 = 0.0, s2 = 0.0;
+#pragma unroll
+      for (int p = 0; p <= P; ++p) {
+        const int pp = P - p;
+        const double sgn = ((((p + 1) >> 1) + ((pp + 1) >> 1)) & 1) ? -1.0 : 1.0;      // e_p e_p'
+        const double c00 = sig[p] / fact[p], d00 = sig[pp] / fact[pp];             // n = n' = 0
+        s0 += sgn * c00 * d00;
+        // N = 2: (n,n') = (1,1): i conj(i) = +1;  (2,0) and (0,2): i^2 = -1 each
+        const double c1 = sig[p + 2] / fact[p], d1 = sig[pp + 2] / fact[pp];
+        const double c2 = sig[p + 4] / (fact[p] * 2.0), d2 = sig[pp + 4] / (fact[pp] * 2.0);
+        s2 += sgn * (c1 * d1 - c2 * d00 - c00 * d2);
+      }
+      h0[P] = s0;
+      h2[P] = s2;
+    }
+#pragma unroll
+    for (int P = 0; P <= HTAB_P; ++P) {
+      atomicAdd(&red[P], u * h0[P]);
+      atomicAdd(&red[HTAB_P + 1 + P], u * h2[P]);
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < HTAB_W)
+    htab[(size_t)node * HTAB_W + threadIdx.x] = threadIdx.x < 2 * (HTAB_P + 1) ? (float)red[threadIdx.x] : 0.f;
+}
+
+}  // namespace sftk

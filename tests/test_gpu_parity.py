@@ -41,7 +41,14 @@ def _run_gpu(w, params=None, want_kc=True, **override):
         plan.inner_products(P, xh2, hh2, xi2, None)
     if want_kc:
         assert sum(paths.values()) == int((kc >= 0).sum()), (paths, int((kc >= 0).sum()))
-    return dict(xh=xh, hh=hh, xh_im=xi, kc=kc, paths=paths, hot=dict(xh=xh2, hh=hh2, xh_im=xi2, kc=None))
+    out = dict(xh=xh, hh=hh, xh_im=xi, kc=kc, paths=paths, hot=dict(xh=xh2, hh=hh2, xh_im=xi2, kc=None))
+    if "evaluator" not in override:
+        # the default evaluator is the moment tables (|b| <= 0.12); run the direct evaluator as well
+        with api.plan_from_workload(w, evaluator="direct", **override) as plan:
+            xh3, hh3, xi3 = np.full(nT, np.nan), np.full(nT, np.nan), np.full(nT, np.nan)
+            plan.inner_products(P, xh3, hh3, xi3, None)
+        out["hot_direct"] = dict(xh=xh3, hh=hh3, xh_im=xi3, kc=None)
+    return out
 
 
 def _check(w, g, o, xx, tol=TOL):
@@ -55,8 +62,9 @@ def _check(w, g, o, xx, tol=TOL):
     assert e_xi.max() <= tol, ("xh_im", e_xi.max(), int(e_xi.argmax()))
     assert e_hh.max() <= tol, ("hh", e_hh.max(), int(e_hh.argmax()))
     assert e_hh_rel[o["hh"] > 0].max(initial=0.0) <= tol, ("hh rel", e_hh_rel.max())
-    if g.get("hot") is not None:
-        _check(w, g["hot"], o, xx, tol)
+    for alt in ("hot", "hot_direct"):
+        if g.get(alt) is not None:
+            _check(w, g[alt], o, xx, tol)
     if g.get("kc") is not None:
         tie = (o["flags"] != 0)[:, None, :]
         bad = (g["kc"] != o["kc"]) & ~tie
@@ -274,7 +282,7 @@ def test_config2_full_size_sampled():
     assert np.all(np.isfinite(xh)) and np.all(hh > 0)
     assert xh[0] > 0.8 * hh[0] and abs(hh[0] - 900.0) < 0.1 * 900.0            # the injection: SNR 30
     assert xh[0] > 0.9 * xh.max()                                               # and (nearly) the best match of the bank
-    assert sum(paths.values()) == int((kc >= 0).sum()) and paths["series1"] > paths["fresnel"] > 0
+    assert sum(paths.values()) == int((kc >= 0).sum()) and paths["table"] > paths["fresnel"] > 0
 
 
 def test_config3_full_size_sampled():
