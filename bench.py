@@ -187,7 +187,7 @@ def run_ours(args, rank, world, local_rank):
         dist.barrier()
     w = make_workload(args.workload, rank, args.templates, args.n_sft, args.K)
     stream = torch.cuda.current_stream()
-    plan = api.plan_from_workload(w, device=local_rank, stream=stream.cuda_stream)
+    plan = api.plan_from_workload(w, device=local_rank, stream=stream.cuda_stream, evaluator=args.evaluator)
     if args.chunk:
         plan.set_chunk(args.chunk)
     nT = w.n_templates
@@ -204,14 +204,29 @@ def run_ours(args, rank, world, local_rank):
     plan.inner_products(P_dev, xh, hh, xi, kc)
     plan.sync()
     pairs = int((kc >= 0).sum().item())
+    paths = plan.path_counts()
     del kc
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
+    cumulative = args.workload == "config3"        # BASELINE.json configs[2]: the SNR(t) matrix is the output
+    d2h_bytes = 3 * nT * 8
+    if cumulative:
+        snr_dev = torch.empty((nT, plan.n_sft), dtype=torch.float32, device=dev)
+        snr_host = torch.empty((nT, plan.n_sft), dtype=torch.float32).pin_memory()
+        snr_np = snr_host.numpy()
+        d2h_bytes = int(snr_np.nbytes)
+
     def step_device():
-        plan.inner_products(P_dev, xh, hh, xi, None)
+        if cumulative:
+            plan.cumulative_snr(P_dev, snr_dev, None, None)
+        else:
+            plan.inner_products(P_dev, xh, hh, xi, None)
 
     def step_host():
-        plan.inner_products(P_np, out_np[0], out_np[1], out_np[2], None)
+        if cumulative:
+            plan.cumulative_snr(P_np, snr_np, None, None)
+        else:
+            plan.inner_products(P_np, out_np[0], out_np[1], out_np[2], None)
 
     def timed(fn, steps, warmup, record_kernel=False):
         for _ in range(warmup):
@@ -242,7 +257,7 @@ def run_ours(args, rank, world, local_rank):
     sampler.start()
     ms_dev, launches, kms = timed(step_device, args.steps, args.warmup, record_kernel=True)
     clocks = sampler.stop()
-    e2e_steps = max(3, min(args.steps, 50))
+    e2e_steps = max(3, min(args.steps, 5 if cumulative else 50))
     ms_host, _, _ = timed(step_host, e2e_steps, 3)
     ok = bool(torch.isfinite(xh).all().item() and (hh >= 0).all().item())
     t = torch.tensor([ms_dev, ms_host / e2e_steps, float(pairs)], dtype=torch.float64, device=dev)
@@ -262,7 +277,7 @@ def run_ours(args, rank, world, local_rank):
     value = pairs_all / (ms_step * 1e-3)
     e2e = pairs_all / (ms_host_step * 1e-3)
     k_ms = float(np.mean(kms)) if kms else None
-    roof = roofline(w, pairs, k_ms)
+    roof = roofline(w, pairs, k_ms, paths)
     cpu_val, cpu_n, cpu_dt, cpu_pairs = time_oracle(w, budget_s=args.cpu_budget)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -270,10 +285,11 @@ def run_ours(args, rank, world, local_rank):
         "dtype": "f32 (fp64 phase track + fp64 accumulators)", "data": "synthetic",
         "config": {"workload": w.name, "templates_per_gpu": nT, "n_sft_slots": int(w.desc["n_sft"]),
                    "n_channels": int(w.desc["n_channels"]), "K": int(w.desc["K"]), "kernel": w.desc["kernel"],
-                   "pn1": int(w.desc["pn1"]), "active_pairs_per_gpu": pairs, "bin_terms_per_gpu": pairs * (2 * w.desc["K"] + 1),
+                   "pn1": int(w.desc["pn1"]), "evaluator": args.evaluator,
+                   "call": "sft_cumulative_snr" if cumulative else "sft_inner_products", "active_pairs_per_gpu": pairs, "bin_terms_per_gpu": pairs * (2 * w.desc["K"] + 1),
                    "parallelism": "templates sharded over %d GPU(s), data store replicated, no collective" % world,
                    "cache": "l2_flush_between_steps (256 MiB memset, outside the per-step events)"},
-        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(P_np.nbytes), "d2h_bytes_per_step": int(3 * nT * 8),
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(P_np.nbytes), "d2h_bytes_per_step": int(d2h_bytes),
                 "ms_per_step": ms_host_step, "steps": e2e_steps},
         "gpu_launches": int(launches), "kernel_ms": k_ms, "results_finite": ok,
         "clocks": clocks, "roofline": roof,
@@ -290,34 +306,112 @@ def run_ours(args, rank, world, local_rank):
 
 # Algorithmic work per active pair and the ALU peak: DESIGN.md §7.
 SM_COUNT, SM_MAX_GHZ = 148, 1.965
+S_ORDER = {"series0": 1, "series1": 4, "series2": 11, "series3": 16}     # packed-lane ops of the far-bin recurrence
 
 
-def roofline(w, pairs, kernel_ms):
-    """ALU roofline of the fused main kernel: the path is bound by plain ALU
-    arithmetic (the 13 MB data store is L2 resident and shared by every template).  Unit: FP32-pipe
-    lane-operations (FFMA/FMUL/FADD = 1 op); peak = 148 SMs x 128 FP32 lanes x 1.965 GHz."""
-    K = int(w.desc["K"])
-    C = int(w.desc["n_channels"])
-    ops_pair = alg_fp32_ops_per_pair(K, C, w.desc["kernel"])
-    peak = SM_COUNT * 128 * SM_MAX_GHZ          # Gop/s
-    if not kernel_ms:
+def alg_instr_per_pair(path, K, C):
+    """Warp instructions the formulation needs per active (template, SFT) pair on evaluator path
+    ``path`` (a packed FFMA2/FMUL2 counts as ONE instruction, as it takes one issue slot):
+    fixed part = fp64 track 50 + SFT loop 13 + phase/prefactor/response/accumulation 23 (+12 per extra
+    channel); table: 21 shared + 38 per channel; series order n: per far bin 2.5 (reciprocal pair) +
+    s_n/2 + 1 (|J|^2) + 3.5 C (load + MACs), central bin 7(n+1) + 2 + 7 C; closed Fresnel form: 64 + 3.5 C
+    per bin."""
+    fixed = 86 + 12 * (C - 1)
+    if path == "table":
+        return fixed + 21 + 38 * C
+    if path == "fresnel":
+        return fixed + (2 * K + 1) * (64 + 3.5 * C)
+    n = int(path[-1])
+    return fixed + 2 * K * (2.5 + S_ORDER[path] / 2.0 + 1 + 3.5 * C) + 7 * (n + 1) + 2 + 7 * C
+
+
+def roofline(w, pairs, kernel_ms, paths):
+    """Issue-slot roofline of the fused main kernel.  The data are L2/L1 resident, so the
+    path is bound by plain ALU work; with the moment tables no single pipe dominates (ncu: FMA 38 %,
+    XU 34 %, ALU 26 %, FP64 23 %) and the binding resource is the warp schedulers' issue rate:
+    peak = 148 SMs x 4 schedulers x 1 warp instruction/clock x 32 lanes x 1.965 GHz (numerically equal
+    to the FP32 lane peak).  achieved = algorithmic instructions of the measured path mix x 32 lanes x
+    warp-pairs / kernel time."""
+    if not kernel_ms or not paths:
         return None
-    achieved = ops_pair * pairs / (kernel_ms * 1e-3) / 1e9
-    return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Gop/s (FP32-pipe lane ops)",
+    K, C = int(w.desc["K"]), int(w.desc["n_channels"])
+    tot = float(sum(paths.values()))
+    mix = {k: v / tot for k, v in paths.items() if v}
+    ops_pair = sum(f * alg_instr_per_pair(k, K, C) for k, f in mix.items())
+    peak = SM_COUNT * 4 * 32 * SM_MAX_GHZ          # G lane-instructions/s
+    achieved = ops_pair * (pairs / C) / (kernel_ms * 1e-3) / 1e9       # pairs counts channels; tracks do not
+    return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "G lane-instructions/s (issue slots)",
             "frac": achieved / peak, "traffic": None, "kernel": "sft_main_kernel", "kernel_ms": kernel_ms,
-            "alg_ops_per_pair": ops_pair,
-            "peak_source": "derived: 148 SM x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md unit counts/clocks), DESIGN.md §7"}
+            "alg_instr_per_pair": ops_pair, "path_mix": mix,
+            "peak_source": "derived: 148 SM x 4 schedulers x 32 lanes x 1.965 GHz (B200_PROFILING.md unit counts/clocks), DESIGN.md §7"}
 
 
-def alg_fp32_ops_per_pair(K, C, kernel):
-    """FP32-pipe-equivalent lane operations the method needs per active (template, SFT) pair
-    (DESIGN.md §7): per bin and channel 4 FMA (complex x complex MAC) + 2 (|F|^2 weight MAC) and the
-    coefficient evaluation (Dirichlet: 3, Fresnel series order 3: 14); per pair the fixed part
-    (phase/prefactor/response, ~40) plus the fp64 track counted at its 2:1 pipe-rate ratio
-    (~30 DFMA-class ops -> 60)."""
-    nb = 2 * K + 1
-    coeff = 3 if kernel == "dirichlet" else 14
-    return nb * (coeff + 6 * C) + 40 + 60
+def run_sweep(args):
+    """--sweep: BASELINE.json configs[4], one axis at a time around the config-2 point (templates,
+    SFTs, band half-width K, evaluator).  One JSON line per point: throughput, main-kernel time,
+    issue-slot roofline fraction and the normalised error against the oracle on 3 sampled templates.
+    The split-fp32 phase path is not built (SFT_EUNSUPPORTED): B200's FP64 pipe runs at
+    half the FP32 rate, a double-float track needs >= 10 FP32 operations per FP64 one."""
+    import torch
+    from paper_2502_11823_b200 import api, build, workloads as wl
+    from oracle import inner as oin
+    build.build()
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    points = []
+    for nt in [4 ** i for i in range(0, 11)]:
+        points.append(dict(axis="templates", n_templates=nt, n_sft=10800, K=8, evaluator="auto"))
+    for ns in (1024, 2700, 10800, 43200):
+        points.append(dict(axis="n_sft", n_templates=4096, n_sft=ns, K=8, evaluator="auto"))
+    for K in (2, 4, 8, 16, 32, 64):
+        for ev in ("auto", "direct"):
+            points.append(dict(axis="K", n_templates=4096, n_sft=10800, K=K, evaluator=ev))
+    cache = {}
+    for pt in points:
+        key = (pt["n_sft"], pt["K"])
+        if key not in cache:
+            cache.clear()
+            cache[key] = wl.et_bns(n_templates=4096, n_sft=pt["n_sft"], K=pt["K"], name="config5")
+        w0 = cache[key]
+        nT = pt["n_templates"]
+        w = wl.et_bns_bank(w0, nT) if nT != 4096 else w0
+        plan = api.plan_from_workload(w, device=0, stream=stream.cuda_stream, evaluator=pt["evaluator"])
+        P = torch.from_numpy(np.ascontiguousarray(w.params)).to(dev)
+        xh = torch.empty(nT, dtype=torch.float64, device=dev)
+        hh, xi = torch.empty_like(xh), torch.empty_like(xh)
+        ns = min(nT, 64)                                        # active pairs and path mix from a sample
+        kc = torch.empty((ns, 1, plan.n_sft), dtype=torch.int32, device=dev)
+        plan.inner_products(P[:ns].contiguous(), xh[:ns], hh[:ns], xi[:ns], kc)
+        plan.sync()
+        pairs = int((kc >= 0).sum().item()) * nT // ns
+        paths = plan.path_counts()
+        steps = 20 if nT <= 65536 else 5
+        kms, ms = [], 0.0
+        for i in range(3 + steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            plan.inner_products(P, xh, hh, xi, None)
+            b.record(stream)
+            torch.cuda.synchronize()
+            if i >= 3:
+                ms += a.elapsed_time(b)
+                kms.append(plan.last_kernel_ms())
+        rows = np.unique([0, nT // 2, nT - 1])
+        op, st = oracle_objects(w)[1:]
+        o = oin.inner_products(op, st, w.params[rows])
+        norm = np.sqrt(oin.xx_band(op, st) * o["hh"])
+        g_xh, g_hh = xh.cpu().numpy()[rows], hh.cpu().numpy()[rows]
+        err = float(max(np.max(np.abs(g_xh - o["xh"]) / norm), np.max(np.abs(g_hh - o["hh"]) / norm)))
+        roof = roofline(w, pairs, float(np.mean(kms)), paths)
+        print(json.dumps(dict(pt, workload="config5", active_pairs=pairs, ms_per_step=ms / steps,
+                              kernel_ms=float(np.mean(kms)), pairs_per_s=pairs / (ms / steps * 1e-3),
+                              roofline_frac=roof["frac"], alg_instr_per_pair=roof["alg_instr_per_pair"],
+                              path_mix=roof["path_mix"], oracle_err=err, phase_path="fp64")), flush=True)
+        plan.close()
+        del P, xh, hh, xi, kc
 
 
 def main():
@@ -331,12 +425,17 @@ def main():
     ap.add_argument("--n-sft", type=int, default=None, dest="n_sft")
     ap.add_argument("--K", type=int, default=None)
     ap.add_argument("--chunk", type=int, default=0)
+    ap.add_argument("--evaluator", default="auto", choices=["auto", "direct", "table"])
+    ap.add_argument("--sweep", action="store_true", help="config-5 scaling sweep (one JSON line per point)")
     ap.add_argument("--cpu-budget", type=float, default=12.0, dest="cpu_budget")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_ours(args, rank, world, local_rank)

@@ -69,6 +69,7 @@ struct KParams {
   const float4 *htab;      // [C][n_kc * HTAB_R][4]   <h,h> polynomial per node
   unsigned mrow, mchan;    // float4 entries per SFT row (n_node * 4) and per channel (n_sft * mrow), hchan likewise
   unsigned hchan;
+  float b_table;           // B_TABLE if the plan has the tables, else -1 (no |b| qualifies)
   double *part;            // [n_chunks][3][nT] chunk totals (xh, hh, xh_im)
   int *kc_out;             // [nT][C][n_sft] or null
   float *loc_xh, *loc_hh;  // cumulative mode: [nT][n_sft] chunk-local prefix sums
@@ -160,6 +161,7 @@ struct Tmpl {
 // One thread per template, once per call.
 __global__ void sft_tmpl_kernel(const KParams p, double *td, float *tf) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t == 0) *p.counter = 0;            // work-unit counter of the main kernel that follows on the stream
   if (t >= p.nT) return;
   const double *row = p.params + t * 8;
   const double mc = row[0], eta = row[1], tc = row[2], phic = row[3], amp = row[4];
@@ -563,14 +565,14 @@ __device__ __forceinline__ void fresnel_pairs(const KParams &p, const Tmpl &tm, 
 enum { PATH_ORD0 = 0, PATH_ORD1, PATH_ORD2, PATH_ORD3, PATH_FRESNEL, PATH_TABLE, PATH_N };
 
 __device__ __forceinline__ int path_of(float bmax, bool table) {
-  if (table && bmax <= B_TABLE) return PATH_TABLE;
+  if (table && bmax <= B_TABLE) return PATH_TABLE;   // same test as pair_terms
   return bmax == 0.f ? PATH_ORD0 : bmax <= B_ORDER1 ? PATH_ORD1 : bmax <= B_ORDER2 ? PATH_ORD2 : bmax <= B_ORDER3 ? PATH_ORD3
                                                                                                                : PATH_FRESNEL;
 }
 
-// X + i s Y for complex X, Y held as (re, im) pairs; sp = (-s, s)
-__device__ __forceinline__ float2 cstep(float2 X, float2 sp, float2 Y) {
-  return __ffma2_rn(make_float2(Y.y, Y.x), sp, X);
+// X + i s Y for complex X, Y held as (re, im) pairs: one packed FMA (swapped, lane-negated operand)
+__device__ __forceinline__ float2 cstep(float2 X, float s, float2 Y) {
+  return __ffma2_rn(make_float2(-Y.y, Y.x), make_float2(s, s), X);
 }
 
 // Moment-table evaluator of one (template, SFT): S1 = sum_m D J_m and S2 = sum_m u |J_m|^2 from the tables
@@ -596,12 +598,9 @@ __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, dou
   const float a = (2.0f * PI_F) * (xp - (((float)cell + 0.5f) * (1.0f / TAB_R) - 0.5f));
   const float aH = (2.0f * PI_F) * (xp - (((float)cellH + 0.5f) * (1.0f / HTAB_R) - 0.5f));
   const float be = PI_F * b;
-  const float2 nb1 = make_float2(-be, be), nb2 = make_float2(-0.5f * be, 0.5f * be),
-               nb3 = make_float2(-(1.0f / 3.0f) * be, (1.0f / 3.0f) * be);
-  const float2 na1 = make_float2(-a, a), na2 = make_float2(-0.5f * a, 0.5f * a),
-               na3 = make_float2(-(1.0f / 3.0f) * a, (1.0f / 3.0f) * a), na4 = make_float2(-0.25f * a, 0.25f * a),
-               na5 = make_float2(-0.2f * a, 0.2f * a), na6 = make_float2(-(1.0f / 6.0f) * a, (1.0f / 6.0f) * a),
-               na7 = make_float2(-(1.0f / 7.0f) * a, (1.0f / 7.0f) * a);
+  const float nb1 = be, nb2 = 0.5f * be, nb3 = (1.0f / 3.0f) * be;
+  const float na1 = a, na2 = 0.5f * a, na3 = (1.0f / 3.0f) * a, na4 = 0.25f * a, na5 = 0.2f * a, na6 = (1.0f / 6.0f) * a,
+              na7 = (1.0f / 7.0f) * a;
   const float be2 = be * be;
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
@@ -656,7 +655,7 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, con
   float s1r[CT], s1i[CT], s2[CT];
   float scale;                 // the series evaluators return 2 pi J
   float t;                     // total phase / pi:  2 frac (= phi_a/pi) + prefactor phase / pi
-  if (p.mtab != nullptr && bmax <= B_TABLE) {
+  if (bmax <= p.b_table) {
     const float xp = fmaf(0.5f, b, tr.x);
     table_eval<CT, CFG>(p, tm, dnext, nxt, xp, b, j0c - 2, Mrow0, s1r, s1i, s2);
     scale = 1.0f;
@@ -725,10 +724,14 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, con
     }
     const float cr = gr * s1r[c] - gi * s1i[c], ci = gr * s1i[c] + gi * s1r[c];
     const float chh = r2 * a2 * us2[c] * s2[c];
-    const bool present = CT == 1 || us2[c] > 0.f;      // gaps hold zeros in the store, but guard 0 * garbage
-    sr += present ? cr : 0.f;
-    si += present ? ci : 0.f;
-    sh += present ? chh : 0.f;
+    if (CT == 1) {
+      sr = cr; si = ci; sh = chh;
+    } else {
+      const bool present = us2[c] > 0.f;               // gaps hold zeros in the store, but guard 0 * garbage
+      sr += present ? cr : 0.f;
+      si += present ? ci : 0.f;
+      sh += present ? chh : 0.f;
+    }
   }
   zr = ok ? sr : 0.f;
   zi = ok ? si : 0.f;
@@ -853,24 +856,35 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
   }
 }
 
-// Sum of the chunk totals in fp64, fixed order (deterministic).  grid = (ceil(nT/64), 3 quantities).
-__global__ void __launch_bounds__(64) sft_reduce_kernel(const double *part, long long nT, int n_chunks, double *xh,
-                                                        double *hh, double *xi) {
-  const long long t = (long long)blockIdx.x * 64 + threadIdx.x;
+// Sum of the chunk totals in fp64, fixed order (deterministic).  grid = (ceil(nT/32), 3 quantities),
+// block = 32 templates x RED_SLICES chunk slices; slice s sums the chunks c = s (mod RED_SLICES).
+constexpr int RED_SLICES = 16;
+__global__ void __launch_bounds__(32 * RED_SLICES) sft_reduce_kernel(const double *part, long long nT, int n_chunks,
+                                                                     double *xh, double *hh, double *xi) {
+  __shared__ double sm[RED_SLICES][33];
+  const int tx = threadIdx.x & 31, sl = threadIdx.x >> 5;
+  const long long t = (long long)blockIdx.x * 32 + tx;
   double *out = blockIdx.y == 0 ? xh : blockIdx.y == 1 ? hh : xi;
-  if (t >= nT || !out) return;
-  const double *q = part + (size_t)blockIdx.y * nT + t;
+  if (!out) return;
   const size_t stride = (size_t)3 * nT;
-  double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-  int c = 0;
-  for (; c + 4 <= n_chunks; c += 4) {
-    s0 += q[(size_t)c * stride];
-    s1 += q[(size_t)(c + 1) * stride];
-    s2 += q[(size_t)(c + 2) * stride];
-    s3 += q[(size_t)(c + 3) * stride];
+  double s0 = 0.0, s1 = 0.0;
+  if (t < nT) {
+    const double *q = part + (size_t)blockIdx.y * nT + t;
+    int c = sl;
+    for (; c + RED_SLICES < n_chunks; c += 2 * RED_SLICES) {
+      s0 += q[(size_t)c * stride];
+      s1 += q[(size_t)(c + RED_SLICES) * stride];
+    }
+    if (c < n_chunks) s0 += q[(size_t)c * stride];
   }
-  for (; c < n_chunks; ++c) s0 += q[(size_t)c * stride];
-  out[t] = (s0 + s1) + (s2 + s3);
+  sm[sl][tx] = s0 + s1;
+  __syncthreads();
+  if (sl == 0 && t < nT) {
+    double s = sm[0][tx];
+#pragma unroll
+    for (int j = 1; j < RED_SLICES; ++j) s += sm[j][tx];
+    out[t] = s;
+  }
 }
 
 // Exclusive scan of the chunk totals along the chunk axis, in place, fp64 (the carries).

@@ -359,6 +359,7 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.mrow = p->mtab ? (unsigned)p->n_node * 4u : 0u;
   k.mchan = p->mtab ? (unsigned)(p->d.n_sft * p->n_node * 4) : 0u;
   k.hchan = (unsigned)(p->n_kc * sftk::HTAB_R * 4);
+  k.b_table = p->mtab ? sftk::B_TABLE : -1.0f;
   k.Dp = p->Dp;
   k.ubp = p->ubp;
   k.us2 = p->us2;
@@ -392,8 +393,7 @@ static void launch_variant(sft_plan *p, const KParams &k) {
 
 template <int MODE>
 static cudaError_t launch_main(sft_plan *p, const KParams &k) {
-  cudaMemsetAsync(p->counter, 0, sizeof(int), p->stream);
-  cudaEventRecord(p->ev0, p->stream);
+  cudaEventRecord(p->ev0, p->stream);             // (the work-unit counter was zeroed by sft_tmpl_kernel)
   const int C = k.C, K = k.K;
   const bool diag = k.kc_out != nullptr || k.path_counts != nullptr;
   const bool bns = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 0;
@@ -493,7 +493,8 @@ SFT_API sft_status sft_inner_products(sft_plan *p, int64_t nT, const double *par
   if (d_kc) CU(p, cudaMemsetAsync(p->path_counts, 0, sftk::PATH_N * sizeof(unsigned long long), p->stream));
   cudaError_t e = launch_main<0>(p, k);
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
-  sftk::sft_reduce_kernel<<<dim3((unsigned)((nT + 63) / 64), 3), 64, 0, p->stream>>>(p->part, nT, k.n_chunks, d_xh, d_hh, d_xi);
+  sftk::sft_reduce_kernel<<<dim3((unsigned)((nT + 31) / 32), 3), 32 * sftk::RED_SLICES, 0, p->stream>>>(p->part, nT, k.n_chunks, d_xh,
+                                                                                                        d_hh, d_xi);
   p->launches++;
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "reduce kernel launch: %s", cudaGetErrorString(e));

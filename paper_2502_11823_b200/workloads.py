@@ -214,6 +214,23 @@ def et_bns(n_templates=4096, n_sft=10800, K=8, fs=2048.0, T=8.0, tau_end=129.0, 
                     params=P, injection=inj, notes=dict(n_gaps=int(len(gaps)), f_start=float(f0), f_end=float(f1)))
 
 
+def et_bns_bank(w, n_templates, bank_seed=55):
+    """The data of ``w`` (an ``et_bns`` workload) with a different bank size (config 5's template axis)."""
+    import copy
+    rng = np.random.default_rng(bank_seed)
+    P = _rows(n_templates)
+    P[:] = w.injection
+    u = rng.uniform(-1e-3, 1e-3, (n_templates, 4))
+    P[:, 0] *= 1.0 + u[:, 0]
+    P[:, 1] = np.minimum(P[:, 1] * (1.0 + u[:, 1]), 0.25)
+    P[:, 2] += u[:, 2]
+    P[:, 3] += u[:, 3]
+    P[0] = w.injection
+    w2 = copy.copy(w)
+    w2.params = P
+    return w2
+
+
 def config2(**kw):
     return et_bns(**kw)
 
