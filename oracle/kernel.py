@@ -38,8 +38,13 @@ def fre_quadrature(a, b, nodes=None):
         span = float(np.max(np.abs(a)) + np.max(np.abs(b))) if a.size else 0.0
         nodes = 64 + 4 * int(np.ceil(span))
     s, w = _gauss_legendre_01(int(nodes))
-    ph = np.pi * (2.0 * a[..., None] * s + b[..., None] * s * s)
-    return np.sum(w * np.exp(1j * ph), axis=-1)
+    af, bf = a.reshape(-1), b.reshape(-1)
+    out = np.empty(af.shape, dtype=np.complex128)
+    step = max(1, (1 << 22) // int(nodes))          # same sums, evaluated in blocks of elements (memory only)
+    for i in range(0, af.size, step):
+        ph = np.pi * (2.0 * af[i:i + step, None] * s + bf[i:i + step, None] * s * s)
+        out[i:i + step] = np.sum(w * np.exp(1j * ph), axis=-1)
+    return out.reshape(a.shape)
 
 
 def dirichlet(a):

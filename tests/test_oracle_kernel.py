@@ -69,10 +69,10 @@ def test_discrete_minus_continuum_is_euler_maclaurin_end_term():
 
 def test_unit_total_power():
     """sum over ALL bins of |F(x-m, b)|^2 = int_0^1 |e^{..}|^2 ds = 1 (Parseval for one SFT)."""
-    m = np.arange(-20000, 20001)
+    m = np.arange(-5000, 5001)     # (|a| <= 5000 keeps pi a^2/b below fre_closed's phase guard: closed form throughout)
     for x, b in ((0.37, 0.0), (-0.2, 0.8), (0.1, 3.0)):
         tot = np.sum(np.abs(kern.fre_closed(x - m, b)) ** 2)
-        assert abs(tot - 1.0) < 2.5e-5          # tail beyond +-20000 bins ~ 2/(pi^2 20000)
+        assert 0.0 < 1.0 - tot < 6e-5           # tail beyond +-5000 bins ~ 2/(pi^2 5000) = 4.05e-5
 
 
 def test_P8_dirichlet_truncation_loss():
