@@ -171,6 +171,21 @@ def run_reference(args, rank, world):
         "gpu_launches": 0}), flush=True)
 
 
+def aggregate_over_ranks(ms_dev, ms_host_step, pairs, device, world):
+    """Whole-job numbers from per-rank ones: time = MAX over ranks (the slowest rank ends the step),
+    work = SUM over ranks (each rank has its own template shard; no data-path collective)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_dev, ms_host_step, float(pairs)], dtype=torch.float64, device=device)
+    if world > 1:
+        tmax = t.clone()
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone()
+        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        return float(tmax[0]), float(tmax[1]), float(tsum[2])
+    return float(t[0]), float(t[1]), float(t[2])
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -260,15 +275,7 @@ def run_ours(args, rank, world, local_rank):
     e2e_steps = max(3, min(args.steps, 5 if cumulative else 50))
     ms_host, _, _ = timed(step_host, e2e_steps, 3)
     ok = bool(torch.isfinite(xh).all().item() and (hh >= 0).all().item())
-    t = torch.tensor([ms_dev, ms_host / e2e_steps, float(pairs)], dtype=torch.float64, device=dev)
-    if world > 1:
-        tmax = t.clone()
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone()
-        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms_dev, ms_host_step, pairs_all = float(tmax[0]), float(tmax[1]), float(tsum[2])
-    else:
-        ms_host_step, pairs_all = float(t[1]), float(pairs)
+    ms_dev, ms_host_step, pairs_all = aggregate_over_ranks(ms_dev, ms_host / e2e_steps, pairs, dev, world)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
