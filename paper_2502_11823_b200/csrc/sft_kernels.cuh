@@ -277,16 +277,7 @@ __device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, dou
   // amplitude (f_a/F0)^(2/3) = q^2 (1 + cf q^2)^(2/3): the seed is good enough (1e-6 relative)
   const float q2f = y0 * y0;
   float a = q2f;
-  if (pn1) {
-    const float z = tm.cf32 * q2f;     // binomial series of (1+z)^(2/3): |error| < 0.014 z^6 (9e-7 at z = 0.2)
-    float g = fmaf(z, 14.0f / 729.0f, -7.0f / 243.0f);
-    g = fmaf(g, z, 4.0f / 81.0f);
-    g = fmaf(g, z, -1.0f / 9.0f);
-    g = fmaf(g, z, 2.0f / 3.0f);
-    g = fmaf(g, z, 1.0f);
-    if (z > 0.2f) g = ex2_approx((2.0f / 3.0f) * lg2_approx(1.0f + z));
-    a *= g;
-  }
+  if (pn1) a *= ex2_approx((2.0f / 3.0f) * lg2_approx(fmaf(tm.cf32, q2f, 1.0f)));
   tr.amp = a;
 }
 
@@ -582,8 +573,15 @@ template <int CT, class CFG>
 __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, double dnext, Track &nxt, float xp, float b,
                                            int kcidx, const float4 *Mrow, float (&s1r)[CT], float (&s1i)[CT],
                                            float (&s2)[CT]) {
-  const int cell = max(0, min(TAB_R - 1, (int)((xp + 0.5f) * (float)TAB_R)));
-  const int cellH = max(0, min(HTAB_R - 1, (int)((xp + 0.5f) * (float)HTAB_R)));
+  // node of the <h,h> table: cellH = floor((xp + 1/2) HTAB_R) by the 1.5 * 2^23 rounding trick, clamped (xp = 1/2
+  // exactly, NaN lanes); the data-moment node is cellH / 4 (HTAB_R = 4 TAB_R)
+  static_assert(HTAB_R == 4 * TAB_R, "node grids");
+  constexpr float RM = 12582912.0f;
+  float cm = fmaf(xp, (float)HTAB_R, 0.5f * HTAB_R - 0.5f + RM);
+  cm = fminf(fmaxf(cm, RM), RM + (float)(HTAB_R - 1));
+  const int cellH = __float_as_int(cm) & (HTAB_R - 1);
+  const int cell = cellH >> 2;
+  const float cHf = cm - RM;                                   // (float)cellH
   const float4 *mp = Mrow + (unsigned)(kcidx * TAB_R + cell) * 4u;
   const float4 *hp = p.htab + (unsigned)(kcidx * HTAB_R + cellH) * 4u;
   float4 Mq[CT][4], Hq[CT][3];
@@ -595,8 +593,9 @@ __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, dou
     for (int i = 0; i < 3; ++i) Hq[c][i] = __ldg(hp + c * p.hchan + i);
   }
   track_eval<CFG>(p, tm, dnext, nxt);
-  const float a = (2.0f * PI_F) * (xp - (((float)cell + 0.5f) * (1.0f / TAB_R) - 0.5f));
-  const float aH = (2.0f * PI_F) * (xp - (((float)cellH + 0.5f) * (1.0f / HTAB_R) - 0.5f));
+  // a = 2 pi (xp - node centre):  centre_H = (cellH + 1/2)/HTAB_R - 1/2,  centre_M = (cell + 1/2)/TAB_R - 1/2
+  const float aH = fmaf(cHf, -(2.0f * PI_F) / HTAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / HTAB_R)));
+  const float a = fmaf((float)cell, -(2.0f * PI_F) / TAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / TAB_R)));
   const float be = PI_F * b;
   const float nb1 = be, nb2 = 0.5f * be, nb3 = (1.0f / 3.0f) * be;
   const float na1 = a, na2 = 0.5f * a, na3 = (1.0f / 3.0f) * a, na4 = 0.25f * a, na5 = 0.2f * a, na6 = (1.0f / 6.0f) * a,
