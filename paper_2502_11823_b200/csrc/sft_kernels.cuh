@@ -902,19 +902,26 @@ __global__ void sft_scan_chunks_kernel(double *part, long long nT, int n_chunks)
 }
 
 // cum = carry (fp64) + chunk-local prefix (fp32);  snr = cum_xh / sqrt(cum_hh)  (0 where cum_hh == 0).
-__global__ void sft_fixup_kernel(const double *part, long long nT, int n_sft, int chunk, const float *loc_xh,
-                                 const float *loc_hh, float *snr, float *cum_xh, float *cum_hh) {
-  for (long long t = blockIdx.y; t < nT; t += gridDim.y) {
-    const double *carry = part + t;
-    for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < n_sft; a += gridDim.x * blockDim.x) {
-      const int ch = a / chunk;
-      const size_t i = (size_t)t * n_sft + a;
-      const double cx = carry[(size_t)ch * 3 * nT] + (double)loc_xh[i];
-      const double chh = carry[(size_t)ch * 3 * nT + nT] + (double)loc_hh[i];
-      if (snr) snr[i] = chh > 0.0 ? (float)(cx * rsqrt(chh)) : 0.f;
-      if (cum_xh) cum_xh[i] = (float)cx;
-      if (cum_hh) cum_hh[i] = (float)chh;
-    }
+// One warp per (template, chunk): the carry is split once into hi + lo floats, so that the per-element
+// work is two fp32 adds (error <= 1 ulp of the fp32 output) and the kernel runs at memory speed.
+// grid = (n_chunks, ceil(nT / 8)), block = 8 warps.
+__global__ void __launch_bounds__(256) sft_fixup_kernel(const double *part, long long nT, int n_sft, int chunk,
+                                                        const float *loc_xh, const float *loc_hh, float *snr,
+                                                        float *cum_xh, float *cum_hh) {
+  const int lane = threadIdx.x & 31, ch = blockIdx.x;
+  const long long t = (long long)blockIdx.y * 8 + (threadIdx.x >> 5);
+  if (t >= nT) return;
+  const double cx = part[(size_t)ch * 3 * nT + t], chh = part[(size_t)ch * 3 * nT + nT + t];
+  const float xh_hi = (float)cx, xh_lo = (float)(cx - (double)xh_hi);
+  const float hh_hi = (float)chh, hh_lo = (float)(chh - (double)hh_hi);
+  const int a0 = ch * chunk, a1 = min(a0 + chunk, n_sft);
+  const size_t row = (size_t)t * n_sft;
+  for (int a = a0 + lane; a < a1; a += 32) {
+    const float x = xh_hi + (xh_lo + __ldcs(loc_xh + row + a));
+    const float h = hh_hi + (hh_lo + __ldcs(loc_hh + row + a));
+    if (snr) __stcs(snr + row + a, h > 0.f ? x * rsqrt_approx(h) : 0.f);
+    if (cum_xh) __stcs(cum_xh + row + a, x);
+    if (cum_hh) __stcs(cum_hh + row + a, h);
   }
 }
 

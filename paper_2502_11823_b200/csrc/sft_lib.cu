@@ -548,7 +548,8 @@ SFT_API sft_status sft_cumulative_snr(sft_plan *p, int64_t nT, const double *par
   cudaError_t e = launch_main<1>(p, k);
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
   sftk::sft_scan_chunks_kernel<<<(unsigned)((nT + 255) / 256), 256, 0, p->stream>>>(p->part, nT, k.n_chunks);
-  dim3 fgrid((unsigned)((N + 255) / 256 < 64 ? (N + 255) / 256 : 64), (unsigned)(nT < 65535 ? nT : 65535));
+  if ((nT + 7) / 8 > 65535) return fail(p, SFT_EUNSUPPORTED, "cumulative call: more than 524,280 templates per call");
+  dim3 fgrid((unsigned)k.n_chunks, (unsigned)((nT + 7) / 8));
   sftk::sft_fixup_kernel<<<fgrid, 256, 0, p->stream>>>(p->part, nT, (int)N, k.chunk, k.loc_xh, k.loc_hh, d_snr, d_cx, d_ch);
   p->launches += 2;
   e = cudaGetLastError();
