@@ -284,7 +284,7 @@ def run_ours(args, rank, world, local_rank):
     value = pairs_all / (ms_step * 1e-3)
     e2e = pairs_all / (ms_host_step * 1e-3)
     k_ms = float(np.mean(kms)) if kms else None
-    roof = roofline(w, pairs, k_ms, paths)
+    roof = roofline(w, pairs, k_ms, paths, args.evaluator)
     cpu_val, cpu_n, cpu_dt, cpu_pairs = time_oracle(w, budget_s=args.cpu_budget)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -311,6 +311,11 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+# DRAM bytes (read + write) of one main-kernel launch from the ncu --set full captures in
+# profiles/r01d_kernel_v7_tables.md (config2-F; dram__bytes_read.sum + dram__bytes_write.sum).
+NCU_TRAFFIC = {("config2-F", "auto"): 1.865216e6 + 11.264e3, ("config2-F", "table"): 1.865216e6 + 11.264e3,
+               ("config2-F", "direct"): 8.213504e6 + 10.752e3}
+
 # Algorithmic work per active pair and the ALU peak: DESIGN.md §7.
 SM_COUNT, SM_MAX_GHZ = 148, 1.965
 S_ORDER = {"series0": 1, "series1": 4, "series2": 11, "series3": 16}     # packed-lane ops of the far-bin recurrence
@@ -332,7 +337,7 @@ def alg_instr_per_pair(path, K, C):
     return fixed + 2 * K * (2.5 + S_ORDER[path] / 2.0 + 1 + 3.5 * C) + 7 * (n + 1) + 2 + 7 * C
 
 
-def roofline(w, pairs, kernel_ms, paths):
+def roofline(w, pairs, kernel_ms, paths, evaluator="auto"):
     """Issue-slot roofline of the fused main kernel.  The data are L2/L1 resident, so the
     path is bound by plain ALU work; with the moment tables no single pipe dominates (ncu: FMA 38 %,
     XU 34 %, ALU 26 %, FP64 23 %) and the binding resource is the warp schedulers' issue rate:
@@ -348,7 +353,8 @@ def roofline(w, pairs, kernel_ms, paths):
     peak = SM_COUNT * 4 * 32 * SM_MAX_GHZ          # G lane-instructions/s
     achieved = ops_pair * (pairs / C) / (kernel_ms * 1e-3) / 1e9       # pairs counts channels; tracks do not
     return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "G lane-instructions/s (issue slots)",
-            "frac": achieved / peak, "traffic": None, "kernel": "sft_main_kernel", "kernel_ms": kernel_ms,
+            "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((w.name, evaluator)), "kernel": "sft_main_kernel",
+            "kernel_ms": kernel_ms,
             "alg_instr_per_pair": ops_pair, "path_mix": mix,
             "peak_source": "derived: 148 SM x 4 schedulers x 32 lanes x 1.965 GHz (B200_PROFILING.md unit counts/clocks), DESIGN.md §7"}
 
