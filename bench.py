@@ -363,8 +363,8 @@ def run_sweep(args):
     """--sweep: BASELINE.json configs[4], one axis at a time around the config-2 point (templates,
     SFTs, band half-width K, evaluator).  One JSON line per point: throughput, main-kernel time,
     issue-slot roofline fraction and the normalised error against the oracle on 3 sampled templates.
-    The split-fp32 phase path is not built (SFT_EUNSUPPORTED): B200's FP64 pipe runs at
-    half the FP32 rate, a double-float track needs >= 10 FP32 operations per FP64 one."""
+    The phase-path axis (fp64 vs split-fp32 = double-float track) is run at the config-2 point for both
+    evaluators."""
     import torch
     from paper_2502_11823_b200 import api, build, workloads as wl
     from oracle import inner as oin
@@ -381,6 +381,9 @@ def run_sweep(args):
     for K in (2, 4, 8, 16, 32, 64):
         for ev in ("auto", "direct"):
             points.append(dict(axis="K", n_templates=4096, n_sft=10800, K=K, evaluator=ev))
+    for ph in ("fp64", "split32"):
+        for ev in ("auto", "direct"):
+            points.append(dict(axis="phase_path", n_templates=4096, n_sft=10800, K=8, evaluator=ev, phase_path=ph))
     cache = {}
     for pt in points:
         key = (pt["n_sft"], pt["K"])
@@ -390,7 +393,8 @@ def run_sweep(args):
         w0 = cache[key]
         nT = pt["n_templates"]
         w = wl.et_bns_bank(w0, nT) if nT != 4096 else w0
-        plan = api.plan_from_workload(w, device=0, stream=stream.cuda_stream, evaluator=pt["evaluator"])
+        plan = api.plan_from_workload(w, device=0, stream=stream.cuda_stream, evaluator=pt["evaluator"],
+                                      phase_path=pt.get("phase_path", "fp64"))
         P = torch.from_numpy(np.ascontiguousarray(w.params)).to(dev)
         xh = torch.empty(nT, dtype=torch.float64, device=dev)
         hh, xi = torch.empty_like(xh), torch.empty_like(xh)
@@ -422,7 +426,7 @@ def run_sweep(args):
         print(json.dumps(dict(pt, workload="config5", active_pairs=pairs, ms_per_step=ms / steps,
                               kernel_ms=float(np.mean(kms)), pairs_per_s=pairs / (ms / steps * 1e-3),
                               roofline_frac=roof["frac"], alg_instr_per_pair=roof["alg_instr_per_pair"],
-                              path_mix=roof["path_mix"], oracle_err=err, phase_path="fp64")), flush=True)
+                              path_mix=roof["path_mix"], oracle_err=err, phase_path=pt.get("phase_path", "fp64"))), flush=True)
         plan.close()
         del P, xh, hh, xi, kc
 

@@ -55,7 +55,8 @@ enum { SFT_KERNEL_DIRICHLET = 0, /* F(a,0) = e^{i pi a} sinc(a), Eq.(B2)  
 enum { SFT_WF_PN0 = 0,           /* Newtonian restricted TaylorT3 inspiral              */
        SFT_WF_PN1 = 1 };         /* + 1PN phase and frequency terms                     */
 enum { SFT_PHASE_FP64 = 0,       /* phase/frequency track evaluated in fp64             */
-       SFT_PHASE_SPLIT32 = 1 };  /* track evaluated in double-float (2 x fp32) arithmetic */
+       SFT_PHASE_SPLIT32 = 1 };  /* track evaluated in double-float (2 x fp32) arithmetic: same bins,
+                                    phases to ~1e-7 rad; slower on B200       */
 enum { SFT_RESP_NONE = 0,        /* R = 1                                               */
        SFT_RESP_TABLE = 1,       /* R_{c,a} from sft_load_data's `response`             */
        SFT_RESP_ANNUAL = 2 };    /* R_{c,a} = [1 + depth cos(2 pi t_a/period + psi_c + lambda)]

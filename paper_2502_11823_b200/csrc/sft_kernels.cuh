@@ -46,7 +46,7 @@ struct KParams {
   int C, n_sft, nb, k_lo, kv_lo, kv_hi, K, PAD, npair;
   int kwin0, jmax;         // window start j0 = k_c - kwin0 in the padded row; in band iff 2 <= j0 <= jmax + 2
   unsigned dstride, cstrideD, cstrideU;   // entries: per channel (n_sft*npair), per copy (C*n_sft*npair), (C*npair)
-  int kernel, pn1, response;
+  int kernel, pn1, response, phase_path;
   double T, t0, f_loT, f_hiT, inv_fref;
   double sigma[MAXC];      // sqrt(T / S_ref,c)
   double chi[MAXC];        // SFT_RESP_ANNUAL response phase per channel
@@ -138,10 +138,11 @@ __device__ __forceinline__ void fresnel_w(float t, float &g, float &f) {
 }
 
 // Compile-time plan flags of a kernel variant; -1 = read the flag from KParams at run time.
-template <int KERNEL_, int PN1_, int RESP_, int KC_>
+template <int KERNEL_, int PN1_, int RESP_, int KC_, int PHASE_ = 0>
 struct Cfg {
-  static constexpr int KERNEL = KERNEL_, PN1 = PN1_, RESP = RESP_, KC = KC_;
+  static constexpr int KERNEL = KERNEL_, PN1 = PN1_, RESP = RESP_, KC = KC_, PHASE = PHASE_;
 };
+template <class CFG> __device__ __forceinline__ int cfg_phase(const KParams &p) { return CFG::PHASE >= 0 ? CFG::PHASE : p.phase_path; }
 template <class CFG> __device__ __forceinline__ int cfg_kernel(const KParams &p) { return CFG::KERNEL >= 0 ? CFG::KERNEL : p.kernel; }
 template <class CFG> __device__ __forceinline__ int cfg_pn1(const KParams &p) { return CFG::PN1 >= 0 ? CFG::PN1 : p.pn1; }
 template <class CFG> __device__ __forceinline__ int cfg_resp(const KParams &p) { return CFG::RESP >= 0 ? CFG::RESP : p.response; }
@@ -152,10 +153,53 @@ template <class CFG> __device__ __forceinline__ int cfg_resp(const KParams &p) {
 enum { TD_TAU0 = 0, TD_CTHETA, TD_PHIC, TD_CPHASE, TD_CPHI, TD_CF, TD_F0T, TD_BSCALE, TD_N };
 enum { TF_CF = 0, TF_CL, TF_SL, TF_AE, TF_N = TF_AE + 2 * MAXC };
 
+// Double-float ("split fp32") arithmetic for SFT_PHASE_SPLIT32: a value is the unevaluated sum h + l of two
+// floats, |l| <= ulp(h)/2 (48-bit significand).  Error-free transformations with explicit rounding intrinsics
+// (no contraction).
+struct df32 {
+  float h, l;
+};
+__device__ __forceinline__ df32 df_quick(float a, float b) {       // |a| >= |b|
+  const float s = __fadd_rn(a, b);
+  return {s, __fsub_rn(b, __fsub_rn(s, a))};
+}
+__device__ __forceinline__ df32 df_two_sum(float a, float b) {
+  const float s = __fadd_rn(a, b), bb = __fsub_rn(s, a);
+  return {s, __fadd_rn(__fsub_rn(a, __fsub_rn(s, bb)), __fsub_rn(b, bb))};
+}
+__device__ __forceinline__ df32 df_add(df32 x, df32 y) {
+  const df32 s = df_two_sum(x.h, y.h);
+  return df_quick(s.h, __fadd_rn(s.l, __fadd_rn(x.l, y.l)));
+}
+__device__ __forceinline__ df32 df_neg(df32 x) { return {-x.h, -x.l}; }
+__device__ __forceinline__ df32 df_mul(df32 x, df32 y) {
+  const float ph = __fmul_rn(x.h, y.h);
+  float pl = __fmaf_rn(x.h, y.h, -ph);
+  pl = __fmaf_rn(x.h, y.l, pl);
+  pl = __fmaf_rn(x.l, y.h, pl);
+  return df_quick(ph, pl);
+}
+__device__ __forceinline__ df32 df_mul_f(df32 x, float c) {
+  const float ph = __fmul_rn(x.h, c);
+  return df_quick(ph, __fmaf_rn(x.l, c, __fmaf_rn(x.h, c, -ph)));
+}
+__device__ __forceinline__ df32 df_from(double d) {
+  const float h = (float)d;
+  return {h, (float)(d - (double)h)};
+}
+// x > y ?
+__device__ __forceinline__ bool df_gt(df32 x, df32 y) { return x.h > y.h || (x.h == y.h && x.l > y.l); }
+__device__ __forceinline__ bool df_ge(df32 x, df32 y) { return x.h > y.h || (x.h == y.h && x.l >= y.l); }
+
+struct TmplS {           // the fp64 members of Tmpl as double-floats (SFT_PHASE_SPLIT32 only)
+  df32 tau0, cTheta, phic_cyc, cphase, cphi, cf, F0T, bscale, T, f_loT, f_hiT;
+};
+
 struct Tmpl {
   double tau0, cTheta, phic_cyc, cphase, cphi, cf, F0T, bscale;   // tau0 = t_c - t0
   float cf32, cl, sl;
   float2 AE[MAXC];   // amp (F0/f_ref)^(2/3) sigma_c e^{i(chi_c+beta)}
+  TmplS s;
 };
 
 // One thread per template, once per call.
@@ -221,6 +265,12 @@ __device__ __forceinline__ void tmpl_load(const KParams &p, long long t, Tmpl &t
 #pragma unroll
   for (int c = 0; c < CT; ++c)
     tm.AE[c] = make_float2(__ldg(f + (TF_AE + 2 * c) * n), __ldg(f + (TF_AE + 2 * c + 1) * n));
+  if (p.phase_path == 1) {           // once per work unit: the per-SFT arithmetic then stays off the FP64 pipe
+    tm.s.tau0 = df_from(tm.tau0); tm.s.cTheta = df_from(tm.cTheta); tm.s.phic_cyc = df_from(tm.phic_cyc);
+    tm.s.cphase = df_from(tm.cphase); tm.s.cphi = df_from(tm.cphi); tm.s.cf = df_from(tm.cf);
+    tm.s.F0T = df_from(tm.F0T); tm.s.bscale = df_from(tm.bscale); tm.s.T = df_from(p.T);
+    tm.s.f_loT = df_from(p.f_loT); tm.s.f_hiT = df_from(p.f_hiT);
+  }
 }
 
 // The four numbers of P:164 at t_a, reduced for fp32 consumption.
@@ -244,8 +294,66 @@ struct Track {
 // for y exactly half-way between two bins, which DESIGN A5 flags as a tie anyway.
 constexpr double RND_MAGIC = 6755399441055744.0;   // 1.5 * 2^52
 
+// The same track in double-float arithmetic (SFT_PHASE_SPLIT32): no FP64 instruction per SFT.  Relative
+// accuracy ~1e-14 (2^-48 per operation): 1e-8 rad at 1e6 rad of phase, 1e-11 bins.
+template <class CFG>
+__device__ __forceinline__ void track_eval_split32(const KParams &p, const Tmpl &tm, double dalpha, Track &tr) {
+  const TmplS &c = tm.s;
+  const float al = (float)dalpha;                                   // SFT index: exact in fp32 (< 2^24)
+  const df32 tau = df_add(c.tau0, df_neg(df_mul_f(c.T, al)));
+  const df32 theta = df_mul(c.cTheta, tau);
+  const float y0 = ex2_approx(-0.125f * lg2_approx(theta.h));
+  const df32 y = {y0, 0.f};
+  const df32 y2 = df_mul(y, y), y4 = df_mul(y2, y2), y8 = df_mul(y4, y4);
+  const df32 one = {1.f, 0.f};
+  const df32 r = df_add(one, df_neg(df_mul(theta, y8)));            // ~8e: fp32 accuracy would do, kept in df for the sum
+  const float sr = fmaf(r.h, 9.0f / 128.0f, 0.125f) * r.h;          // s = r/8 + 9 r^2/128, |s| ~ 1e-6: fp32 suffices
+  const df32 q = df_add(y, df_mul_f(y, sr));                        // Theta^(-1/8), error ~ y * 6e-8 * |s| ~ 1e-13
+  const df32 q2 = df_mul(q, q), q3 = df_mul(q2, q), q4 = df_mul(q2, q2), q8 = df_mul(q4, q4), q11 = df_mul(q8, q3);
+  const bool pn1 = cfg_pn1<CFG>(p) != 0;
+  df32 ph, fT, b;
+  const df32 thq3 = df_mul(theta, q3);
+  if (pn1) {
+    ph = df_add(c.phic_cyc, df_neg(df_mul(df_mul(c.cphase, thq3), df_add(one, df_mul(c.cphi, q2)))));
+    fT = df_mul(df_mul(c.F0T, q3), df_add(one, df_mul(c.cf, q2)));
+    const df32 k375 = {0.375f, 0.f};
+    b = df_mul(df_mul(c.bscale, q11), df_add(k375, df_mul_f(df_mul(c.cf, q2), 0.625f)));
+  } else {
+    ph = df_add(c.phic_cyc, df_neg(df_mul(c.cphase, thq3)));
+    fT = df_mul(c.F0T, q3);
+    b = df_mul_f(df_mul(c.bscale, q11), 0.375f);
+  }
+  const df32 yy = (cfg_kernel<CFG>(p) == 1) ? df_add(fT, df_mul_f(b, 0.5f)) : fT;
+  // k_c = rint(yy): round the high part, fix up with the rest (|rest| can exceed 1/2 by the low part only)
+  float kf = rintf(yy.h);
+  float rest = __fadd_rn(__fsub_rn(yy.h, kf), yy.l);
+  if (rest > 0.5f) { kf += 1.0f; rest -= 1.0f; }
+  if (rest < -0.5f) { kf -= 1.0f; rest += 1.0f; }
+  tr.active = df_gt(tau, c.T) && df_ge(fT, c.f_loT) && df_ge(c.f_hiT, df_add(fT, b));
+  tr.kc = (int)kf;
+  const df32 xd = df_add(fT, {-kf, 0.f});
+  tr.x = xd.h;
+  tr.b = b.h;
+  const float pk = rintf(ph.h);
+  float fr = __fadd_rn(__fsub_rn(ph.h, pk), ph.l);
+  tr.frac = fr - rintf(fr);
+  const float q2f = y0 * y0;
+  float a = q2f;
+  if (pn1) a *= ex2_approx((2.0f / 3.0f) * lg2_approx(fmaf(tm.cf32, q2f, 1.0f)));
+  tr.amp = a;
+}
+
+template <class CFG>
+__device__ __forceinline__ void track_eval_fp64(const KParams &p, const Tmpl &tm, double dalpha, Track &tr);
+
 template <class CFG>
 __device__ __forceinline__ void track_eval(const KParams &p, const Tmpl &tm, double dalpha, Track &tr) {
+  if (cfg_phase<CFG>(p) == 1) track_eval_split32<CFG>(p, tm, dalpha, tr);
+  else track_eval_fp64<CFG>(p, tm, dalpha, tr);
+}
+
+template <class CFG>
+__device__ __forceinline__ void track_eval_fp64(const KParams &p, const Tmpl &tm, double dalpha, Track &tr) {
   const double tau = fma(-dalpha, p.T, tm.tau0);
   const double theta = tm.cTheta * tau;
   const float y0 = ex2_approx(-0.125f * lg2_approx((float)theta));

@@ -97,7 +97,6 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   if (d.kernel != SFT_KERNEL_DIRICHLET && d.kernel != SFT_KERNEL_FRESNEL) return fail(nullptr, SFT_EINVAL, "unknown kernel %d", d.kernel);
   if (d.waveform != SFT_WF_PN0 && d.waveform != SFT_WF_PN1) return fail(nullptr, SFT_EINVAL, "unknown waveform %d", d.waveform);
   if (d.phase_path != SFT_PHASE_FP64 && d.phase_path != SFT_PHASE_SPLIT32) return fail(nullptr, SFT_EINVAL, "unknown phase_path %d", d.phase_path);
-  if (d.phase_path == SFT_PHASE_SPLIT32) return fail(nullptr, SFT_EUNSUPPORTED, "SFT_PHASE_SPLIT32 is not implemented in this build");
   if (d.response < SFT_RESP_NONE || d.response > SFT_RESP_ANNUAL) return fail(nullptr, SFT_EINVAL, "unknown response %d", d.response);
   if (!(d.f_ref > 0.0)) return fail(nullptr, SFT_EINVAL, "f_ref must be > 0");
   if (!(d.f_hi >= d.f_lo)) return fail(nullptr, SFT_EINVAL, "need f_lo <= f_hi");
@@ -147,7 +146,7 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
     if (!fits && d.evaluator == SFT_EVAL_TABLE)
       st = fail(nullptr, SFT_ENOMEM, "moment tables of %.3g bytes do not fit (free %.3g)", m_bytes, (double)free_b);
     if (fits) {
-      alloc((void **)&p->mtab, (size_t)m_bytes);
+      alloc((void **)&p->mtab, (size_t)m_bytes + (size_t)p->n_node * 64);   // + one row: nodes are prefetched one SFT ahead
       alloc((void **)&p->htab, C * (size_t)p->n_kc * sftk::HTAB_R * sftk::HTAB_W * sizeof(float));
       alloc((void **)&p->ptab, (size_t)(2 * d.K + 1) * sftk::TAB_R * (sftk::TAB_Q + 1) * sizeof(float2));
       if (st == SFT_OK) {
@@ -344,6 +343,7 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.kernel = p->d.kernel;
   k.pn1 = p->d.waveform == SFT_WF_PN1;
   k.response = p->d.response;
+  k.phase_path = p->d.phase_path;
   k.T = p->d.t_sft;
   k.t0 = p->d.t0;
   k.f_loT = p->d.f_lo * p->d.t_sft;
@@ -374,11 +374,12 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
 //   CfgBNS  = Fresnel kernel, 0PN+1PN, no response      (configs 2, 3, 5)
 //   CfgNewt = Fresnel kernel, 0PN, no response          (config 1)
 //   CfgLISA = Fresnel kernel, 0PN+1PN, annual response  (config 4)
-//   CfgAny  = run-time flags, optional k_c output and path counters
+//   CfgAny  = run-time flags (incl. the phase path), optional k_c output and path counters
 using CfgBNS = sftk::Cfg<1, 1, 0, 0>;
 using CfgNewt = sftk::Cfg<1, 0, 0, 0>;
 using CfgLISA = sftk::Cfg<1, 1, 2, 0>;
-using CfgAny = sftk::Cfg<-1, -1, -1, 1>;
+using CfgAny = sftk::Cfg<-1, -1, -1, 1, -1>;
+using CfgBNS32 = sftk::Cfg<1, 1, 0, 0, 1>;    // CfgBNS with the split-fp32 (double-float) phase track (config 5)
 
 template <int KT, int CT, int MODE, class CFG>
 static void launch_variant(sft_plan *p, const KParams &k) {
@@ -395,11 +396,14 @@ template <int MODE>
 static cudaError_t launch_main(sft_plan *p, const KParams &k) {
   cudaEventRecord(p->ev0, p->stream);             // (the work-unit counter was zeroed by sft_tmpl_kernel)
   const int C = k.C, K = k.K;
-  const bool diag = k.kc_out != nullptr || k.path_counts != nullptr;
+  const bool diag = k.kc_out != nullptr || k.path_counts != nullptr || k.phase_path != 0;
+  const bool bns32 = k.kc_out == nullptr && k.path_counts == nullptr && k.phase_path == 1 && k.kernel == 1 && k.pn1 == 1 &&
+                     k.response == 0 && C == 1 && K == 8;
   const bool bns = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 0;
   const bool newt = !diag && k.kernel == 1 && k.pn1 == 0 && k.response == 0;
   const bool lisa = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 2;
-  if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS>(p, k);
+  if (bns32) launch_variant<8, 1, MODE, CfgBNS32>(p, k);
+  else if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS>(p, k);
   else if (bns && C == 1 && K == 16) launch_variant<16, 1, MODE, CfgBNS>(p, k);
   else if (bns && C == 1) launch_variant<0, 1, MODE, CfgBNS>(p, k);
   else if (newt && C == 1 && K == 4) launch_variant<4, 1, MODE, CfgNewt>(p, k);

@@ -151,6 +151,21 @@ def test_chunking_is_invisible(et_small, chunk):
     _check(w, dict(xh=xh, hh=hh, xh_im=xi, kc=None), o, xx)
 
 
+def test_split_fp32_phase_path(et_small):
+    """SFT_PHASE_SPLIT32 (config 5's phase-path axis): the track in double-float arithmetic gives the same
+    results and the same bins as the fp64 track, for both kernel variants (run-time flags / CfgBNS32)."""
+    w = et_small
+    o, xx, _, _ = _oracle(w)
+    g = _run_gpu(w, phase_path="split32")
+    _check(w, g, o, xx)
+    w1 = wl.config1()
+    o1, xx1, _, _ = _oracle(w1)
+    _check(w1, _run_gpu(w1, phase_path="split32"), o1, xx1)
+    w4 = wl.config4(n_templates=64)
+    o4, xx4, _, _ = _oracle(w4)
+    _check(w4, _run_gpu(w4, phase_path="split32"), o4, xx4)
+
+
 def test_config4_small():
     """BASELINE.json configs[3] recipe with 300 templates: 2 channels, annual response, K = 16
     clipping at k < 1, 0PN+1PN."""
