@@ -285,6 +285,12 @@ def run_ours(args, rank, world, local_rank):
     e2e = pairs_all / (ms_host_step * 1e-3)
     k_ms = float(np.mean(kms)) if kms else None
     roof = roofline(w, pairs, k_ms, paths, args.evaluator)
+    if roof:
+        # pipe rates of this GPU (Gop/s) and the schedulers' sustained rate on the table kernel's instruction mix
+        # with every stall removed (instructions/clock/scheduler): the ceiling for that mix, beside the nominal peak
+        pk = api.measure_alu_peaks(local_rank)
+        roof["measured_alu"] = pk
+        roof["frac_of_mix_ceiling"] = roof["frac"] / pk["table_mix_ipc"] if pk.get("table_mix_ipc") else None
     cpu_val, cpu_n, cpu_dt, cpu_pairs = time_oracle(w, budget_s=args.cpu_budget)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

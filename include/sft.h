@@ -159,9 +159,11 @@ sft_status sft_plan_set_chunk(sft_plan *plan, int32_t sfts_per_unit);
 
 /* Diagnostic: measures the plain-ALU pipe rates of `device` that bound this path (the
  * data store is L2 resident, so FP32 / FP64 / XU issue rates, not HBM, are the roofline).  Writes up
- * to 5 doubles, in 1e9 lane-operations per second (one FMA = one operation):
+ * to 6 doubles, in 1e9 lane-operations per second (one FMA = one operation):
  *   out[0] fma.rn.f32, out[1] fma.rn.f32x2 (2 lanes per instruction), out[2] fma.rn.f64,
- *   out[3] rcp.approx.f32 (XU/MUFU), out[4] a 4:1 FFMA:MUFU mix (all its operations counted).
+ *   out[3] rcp.approx.f32 (XU/MUFU), out[4] a 4:1 FFMA:MUFU mix (all its operations counted);
+ *   out[5] (not Gop/s) warp instructions per clock and scheduler sustained on the instruction mix of the
+ *   moment-table kernel with all dependencies and memory stalls removed: the ceiling for that mix.
  * Runs a few ms of synthetic kernels on the device's default stream; touches no plan.  Errors are
  * reported through sft_last_error(NULL). */
 sft_status sft_measure_alu_peaks(int32_t device, double *out_gops, int32_t n_out);

@@ -246,11 +246,11 @@ def plan_from_workload(w, device=0, stream=None, **override):
 def measure_alu_peaks(device=0):
     """``sft_measure_alu_peaks``: dict of measured pipe rates in Gop/s (lane operations)."""
     lib = load_library()
-    out = (C.c_double * 5)()
-    st = lib.sft_measure_alu_peaks(int(device), out, 5)
+    out = (C.c_double * 6)()
+    st = lib.sft_measure_alu_peaks(int(device), out, 6)
     if st != 0:
         raise SftError(st, lib.sft_last_error(None).decode())
-    return dict(zip(("ffma", "ffma2", "dfma", "mufu_rcp", "ffma_mufu_mix"), [float(v) for v in out]))
+    return dict(zip(("ffma", "ffma2", "dfma", "mufu_rcp", "ffma_mufu_mix", "table_mix_ipc"), [float(v) for v in out]))
 
 
 def version():
