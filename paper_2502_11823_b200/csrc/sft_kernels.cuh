@@ -1024,6 +1024,21 @@ __global__ void __launch_bounds__(256) sft_fixup_kernel(const double *part, long
   const float hh_hi = (float)chh, hh_lo = (float)(chh - (double)hh_hi);
   const int a0 = ch * chunk, a1 = min(a0 + chunk, n_sft);
   const size_t row = (size_t)t * n_sft;
+  const size_t al = (size_t)loc_xh | (size_t)loc_hh | (size_t)snr | (size_t)cum_xh | (size_t)cum_hh;   // (null = aligned)
+  if (((n_sft | chunk) & 3) == 0 && (al & 15) == 0) {   // rows and chunk starts 16-byte aligned: 4 SFTs per lane
+    for (int a = a0 + 4 * lane; a < a1; a += 128) {
+      const float4 lx = __ldcs((const float4 *)(loc_xh + row + a)), lh = __ldcs((const float4 *)(loc_hh + row + a));
+      float4 x, h, q;
+      x.x = xh_hi + (xh_lo + lx.x); x.y = xh_hi + (xh_lo + lx.y); x.z = xh_hi + (xh_lo + lx.z); x.w = xh_hi + (xh_lo + lx.w);
+      h.x = hh_hi + (hh_lo + lh.x); h.y = hh_hi + (hh_lo + lh.y); h.z = hh_hi + (hh_lo + lh.z); h.w = hh_hi + (hh_lo + lh.w);
+      q.x = h.x > 0.f ? x.x * rsqrt_approx(h.x) : 0.f; q.y = h.y > 0.f ? x.y * rsqrt_approx(h.y) : 0.f;
+      q.z = h.z > 0.f ? x.z * rsqrt_approx(h.z) : 0.f; q.w = h.w > 0.f ? x.w * rsqrt_approx(h.w) : 0.f;
+      if (snr) __stcs((float4 *)(snr + row + a), q);
+      if (cum_xh) __stcs((float4 *)(cum_xh + row + a), x);
+      if (cum_hh) __stcs((float4 *)(cum_hh + row + a), h);
+    }
+    return;
+  }
   for (int a = a0 + lane; a < a1; a += 32) {
     const float x = xh_hi + (xh_lo + __ldcs(loc_xh + row + a));
     const float h = hh_hi + (hh_lo + __ldcs(loc_hh + row + a));
