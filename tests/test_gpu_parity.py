@@ -176,6 +176,43 @@ def test_config4_small():
     assert g["xh"][0] > 0.5 * g["hh"][0]
 
 
+@pytest.mark.parametrize("C", [3, 4])
+def test_three_and_four_channels(C):
+    """SFT_MAX_CHANNELS = 4: the run-time-flag kernel variants with 3 and 4 channels (extra channels = scaled,
+    gap-punched copies of the LISA pair with their own response phases), annual response and cumulative call."""
+    import copy
+    w0 = wl.config4(n_templates=70)
+    w = copy.copy(w0)
+    rng = np.random.default_rng(90 + C)
+    n_sft = w0.desc["n_sft"]
+    extra = C - 2
+    bins = [w0.bins[0], w0.bins[1]] + [(0.5 + 0.25 * i) * w0.bins[i % 2] for i in range(extra)]
+    scale = [w0.psd_scale[0], w0.psd_scale[1]]
+    for i in range(extra):
+        s = w0.psd_scale[i % 2] * (1.0 + 0.5 * i)
+        s = s.copy()
+        s[rng.choice(n_sft, size=n_sft // 7, replace=False)] = 0.0         # gaps of their own
+        scale.append(s)
+    shape = [w0.psd_shape[0], w0.psd_shape[1]] + [w0.psd_shape[i % 2] * (2.0 + i) for i in range(extra)]
+    w.bins = np.ascontiguousarray(np.stack(bins)).astype(np.complex64)
+    w.bins[2:][np.stack(scale[2:]) <= 0.0] = 0.0
+    w.psd_scale = np.stack(scale)
+    w.psd_shape = np.stack(shape)
+    w.desc = dict(w0.desc, n_channels=C, resp_psi=tuple(0.4 * c for c in range(C)), resp_chi=tuple(0.7 * c - 0.3 for c in range(C)))
+    o, xx, plan_o, store = _oracle(w)
+    g = _run_gpu(w)
+    _check(w, g, o, xx)
+    assert np.any(g["kc"][:, 2, :] != g["kc"][:, 0, :])                    # the extra channel's own gaps show up
+    api = _api()
+    oc = oin.cumulative_snr(plan_o, store, w.params[:33])
+    with api.plan_from_workload(w) as plan:
+        cx = np.empty((33, n_sft), np.float32)
+        ch = np.empty((33, n_sft), np.float32)
+        plan.cumulative_snr(np.ascontiguousarray(w.params[:33]), None, cx, ch)
+    norm = np.sqrt(xx * o["hh"][:33])[:, None]
+    assert (np.abs(cx - oc["cum_xh"]) / norm).max() <= TOL and (np.abs(ch - oc["cum_hh"]) / norm).max() <= TOL
+
+
 def test_response_table():
     """SFT_RESP_TABLE: an arbitrary complex per-(channel, SFT) response."""
     w = wl.config4(n_templates=40)
