@@ -33,6 +33,7 @@ struct sft_plan {
   double *part = nullptr; size_t part_bytes = 0;
   double *d_params = nullptr; size_t params_bytes = 0;
   void *d_out = nullptr; size_t out_bytes = 0;         // staging for host outputs
+  void *h_pin = nullptr; size_t pin_bytes = 0;         // pinned host staging (params in, result vectors out)
   float *loc = nullptr; size_t loc_bytes = 0;          // cumulative: chunk-local prefixes
   double *td = nullptr; size_t td_bytes = 0;           // per-template constants (sft_tmpl_kernel)
   float *tf = nullptr; size_t tf_bytes = 0;
@@ -68,6 +69,15 @@ static sft_status fail(sft_plan *p, sft_status st, const char *fmt, ...) {
       return fail(p, e_ == cudaErrorMemoryAllocation ? SFT_ENOMEM : SFT_ECUDA, "%s: %s", #call, \
                   cudaGetErrorString(e_));                                                  \
   } while (0)
+
+static sft_status grow_pinned(sft_plan *p, size_t need) {
+  if (p->pin_bytes >= need) return SFT_OK;
+  if (p->h_pin) { cudaFreeHost(p->h_pin); p->h_pin = nullptr; p->pin_bytes = 0; }
+  cudaError_t e = cudaMallocHost(&p->h_pin, need);
+  if (e != cudaSuccess) return fail(p, SFT_ENOMEM, "cudaMallocHost(%zu): %s", need, cudaGetErrorString(e));
+  p->pin_bytes = need;
+  return SFT_OK;
+}
 
 static sft_status grow(sft_plan *p, void **ptr, size_t *have, size_t need) {
   if (*have >= need) return SFT_OK;
@@ -196,6 +206,7 @@ SFT_API sft_status sft_plan_destroy(sft_plan *p) {
   cudaStreamSynchronize(p->stream);
   cudaFree(p->Dp); cudaFree(p->ubp); cudaFree(p->us2); cudaFree(p->rtab);
   cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->loc);
+  if (p->h_pin) cudaFreeHost(p->h_pin);
   cudaFree(p->td); cudaFree(p->tf); cudaFree(p->counter); cudaFree(p->path_counts);
   cudaFree(p->mtab); cudaFree(p->htab); cudaFree(p->ptab);
   if (p->ev0) cudaEventDestroy(p->ev0);
@@ -504,12 +515,14 @@ SFT_API sft_status sft_inner_products(sft_plan *p, int64_t nT, const double *par
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "reduce kernel launch: %s", cudaGetErrorString(e));
   if (mem == SFT_MEM_HOST) {
     // results go to caller memory only after the stream finished without error
-    std::vector<double> h(3 * (size_t)nT);
-    CU(p, cudaMemcpyAsync(h.data(), d_xh, 3 * (size_t)nT * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    st = grow_pinned(p, 3 * (size_t)nT * sizeof(double));
+    if (st != SFT_OK) return st;
+    double *h = (double *)p->h_pin;
+    CU(p, cudaMemcpyAsync(h, d_xh, 3 * (size_t)nT * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
     CU(p, cudaStreamSynchronize(p->stream));
-    memcpy(xh, h.data(), (size_t)nT * sizeof(double));
-    memcpy(hh, h.data() + nT, (size_t)nT * sizeof(double));
-    if (xh_im) memcpy(xh_im, h.data() + 2 * nT, (size_t)nT * sizeof(double));
+    memcpy(xh, h, (size_t)nT * sizeof(double));
+    memcpy(hh, h + nT, (size_t)nT * sizeof(double));
+    if (xh_im) memcpy(xh_im, h + 2 * nT, (size_t)nT * sizeof(double));
     if (kc_out) {
       CU(p, cudaMemcpyAsync(kc_out, d_kc, (size_t)nT * C * N * sizeof(int), cudaMemcpyDeviceToHost, p->stream));
       CU(p, cudaStreamSynchronize(p->stream));
