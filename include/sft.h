@@ -111,6 +111,22 @@ sft_status sft_load_data(sft_plan *plan, int32_t channel, const float *sft_bins,
                          const double *psd_scale, const double *psd_shape,
                          const float *response, int32_t mem);
 
+/* Data SFTs from a time series (Eq.(26), section V.A): for each of n_sft disjoint segments of n
+ * samples (a trailing partial segment is ignored, DESIGN A13)
+ *     bins[a][k - k_lo] = dt sum_{j<n} x[a n + j] exp(-2 pi i j k / n),   k_lo <= k < k_hi,
+ * as complex64 interleaved [n_sft][k_hi-k_lo].  x holds n_sft*n doubles (16-byte aligned if on the device).
+ * n = 64 .. 16384 a power of two: one shared-memory FFT per segment, the series is read once; other n: direct
+ * summation over the band.  No plan needed; `stream` is a cudaStream_t or NULL; blocks until done. */
+sft_status sft_compute_sfts(int32_t device, void *stream, const double *x, int64_t n_sft, int32_t n,
+                            double dt, int32_t k_lo, int32_t k_hi, float *bins, int32_t mem);
+
+/* sft_compute_sfts + sft_load_data in one call: channel `channel` of the plan from its strain time series
+ * x[n_samples] (n_samples >= n_sft * t_sft * fs; sample j of SFT a is x[a n + j], t = t0 + (a n + j)/fs).
+ * The SFT bins never leave the device.  Noise description and `mem` as in sft_load_data. */
+sft_status sft_ingest_timeseries(sft_plan *plan, int32_t channel, const double *x, int64_t n_samples,
+                                 const double *psd_scale, const double *psd_shape,
+                                 const float *response, int32_t mem);
+
 /* ([x,h]) and ([h,h]) for n_templates templates (Eq.(35) P:259 with ONE df, DESIGN A1).
  *   params  [n_templates][SFT_NPARAM] doubles, row-major:
  *           m_chirp [Msun], eta, t_c [s], phi_c [rad], amp, lambda [rad], beta [rad], reserved(0)

@@ -45,7 +45,8 @@ class PlanDesc(C.Structure):
 
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
-           "sft_plan_set_chunk", "sft_plan_path_counts", "sft_last_error", "sft_version",
+           "sft_plan_set_chunk", "sft_plan_path_counts", "sft_compute_sfts", "sft_ingest_timeseries",
+           "sft_last_error", "sft_version",
            "sft_measure_alu_peaks"]
 
 _lib = None
@@ -73,13 +74,16 @@ def load_library(path=None):
     lib.sft_plan_last_kernel_ms.restype = dbl
     lib.sft_plan_set_chunk.argtypes = [vp, i32]
     lib.sft_plan_path_counts.argtypes = [vp, C.POINTER(i64), i32]
+    lib.sft_compute_sfts.argtypes = [i32, vp, vp, i64, i32, dbl, i32, i32, vp, i32]
+    lib.sft_ingest_timeseries.argtypes = [vp, i32, vp, i64, vp, vp, vp, i32]
     lib.sft_measure_alu_peaks.argtypes = [i32, C.POINTER(dbl), i32]
     lib.sft_measure_alu_peaks.restype = i32
     lib.sft_last_error.argtypes = [vp]
     lib.sft_last_error.restype = C.c_char_p
     lib.sft_version.restype = C.c_char_p
     for f in ("sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
-              "sft_cumulative_snr", "sft_plan_sync", "sft_plan_set_chunk", "sft_plan_path_counts"):
+              "sft_cumulative_snr", "sft_plan_sync", "sft_plan_set_chunk", "sft_plan_path_counts",
+              "sft_compute_sfts", "sft_ingest_timeseries"):
         getattr(lib, f).restype = i32
     _lib = lib
     return lib
@@ -191,6 +195,16 @@ class Plan:
             _ptr(psd_shape, np.float64, (self.nb,), "psd_shape"),
             _ptr(response, np.complex64, (self.n_sft,), "response"), mem))
 
+    def ingest_timeseries(self, channel, x, psd_scale, psd_shape=None, response=None):
+        """``sft_ingest_timeseries``: float64 strain series [>= n_sft * n] instead of precomputed SFT bins."""
+        mem = _where([x, psd_scale, psd_shape, response])
+        ns = int(x.shape[0])
+        self._check(self.lib.sft_ingest_timeseries(
+            self._h, int(channel), _ptr(x, np.float64, (ns,), "x"), ns,
+            _ptr(psd_scale, np.float64, (self.n_sft,), "psd_scale"),
+            _ptr(psd_shape, np.float64, (self.nb,), "psd_shape"),
+            _ptr(response, np.complex64, (self.n_sft,), "response"), mem))
+
     def inner_products(self, params, xh, hh, xh_im=None, kc_out=None):
         """``sft_inner_products`` into caller-allocated outputs."""
         nT = int(params.shape[0])
@@ -241,6 +255,17 @@ def plan_from_workload(w, device=0, stream=None, **override):
                        np.ascontiguousarray(w.psd_scale[c], dtype=np.float64),
                        np.ascontiguousarray(w.psd_shape[c], dtype=np.float64), resp)
     return plan
+
+
+def compute_sfts(x, n_sft, n, dt, k_lo, k_hi, bins, device=0, stream=None):
+    """``sft_compute_sfts``: band-limited data SFTs of a float64 series into complex64 ``bins`` [n_sft][k_hi-k_lo]."""
+    lib = load_library()
+    mem = _where([x, bins])
+    st = lib.sft_compute_sfts(int(device), C.c_void_p(int(stream)) if stream else None,
+                              _ptr(x, np.float64, None, "x"), int(n_sft), int(n), float(dt), int(k_lo), int(k_hi),
+                              _ptr(bins, np.complex64, (int(n_sft), int(k_hi) - int(k_lo)), "bins"), mem)
+    if st != 0:
+        raise SftError(st, lib.sft_last_error(None).decode())
 
 
 def measure_alu_peaks(device=0):

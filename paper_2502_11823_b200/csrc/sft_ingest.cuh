@@ -1,0 +1,109 @@
+// sft_ingest.cuh - data SFTs from the time series on the GPU (section V.A:
+// "SFTs can be computed online as data arrives", O(N0 log n_SFT)).  Computes Eq.(26) P:205,
+//
+//   x~_a[k] = dt sum_{j<n} x[a n + j] exp(-2 pi i j k / n),      k_lo <= k < k_hi,
+//
+// for every disjoint segment a of n = T_SFT fs samples (a trailing partial segment is dropped,
+// DESIGN A13) and keeps ONLY the stored band: the time series is read from HBM exactly once (8 bytes per
+// sample: this kernel's roofline) and (k_hi - k_lo) complex64 bins per SFT are written.
+//
+// n a power of two, 64 <= n <= 16384: one block per segment does a real-input FFT entirely in shared memory
+// (227 KB per SM on B200: a 16384-sample segment packs into 8192 complex fp32 = 64 KB, three blocks per SM so
+// that loads of one segment overlap the butterflies of another): z[j] = x[2j] + i x[2j+1], in-place radix-2
+// decimation in frequency (output bit-reversed, read back through brev), twiddles from an fp64-evaluated table,
+// then the split  X[k] = 1/2 [(Z[k] + conj Z[m-k]) - i w^k (Z[k] - conj Z[m-k])],  w = e^{-2 pi i / n}, for the band only.
+// Any other n: direct summation over the band with exact integer phase reduction (j k mod n), fp64 accumulators.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sftk {
+
+constexpr int FFT_MAX_N = 16384;
+
+// twiddle table W[t] = exp(-2 pi i t / n), t < n/2 (fp64-evaluated, stored as complex64)
+__global__ void sft_twiddle_kernel(int n, float2 *W) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n / 2) return;
+  double s, c;
+  sincospi(2.0 * (double)t / (double)n, &s, &c);
+  W[t] = make_float2((float)c, (float)-s);
+}
+
+// One block per segment.  Dynamic shared memory: (n/2) float2.
+__global__ void __launch_bounds__(512) sft_rfft_band_kernel(const double *x, int n, int log2m, double dt, int k_lo, int nb,
+                                                            const float2 *W, float2 *bins) {
+  extern __shared__ float2 z[];
+  const int m = n >> 1;
+  const double *seg = x + (size_t)blockIdx.x * n;
+  // load + pack: z[j] = x[2j] + i x[2j+1]  (16-byte loads of two doubles)
+  for (int j = threadIdx.x; j < m; j += blockDim.x) {
+    const double2 v = __ldcs((const double2 *)seg + j);
+    z[j] = make_float2((float)v.x, (float)v.y);
+  }
+  __syncthreads();
+  // in-place radix-2 DIF over m points: twiddle of the m-point transform = W_n^(2t)
+  for (int h = m >> 1, tw = 2; h >= 1; h >>= 1, tw <<= 1) {
+    for (int i = threadIdx.x; i < (m >> 1); i += blockDim.x) {
+      const int pos = i & (h - 1);                   // index inside the half-block
+      const int a = ((i - pos) << 1) + pos;          // first element of the butterfly
+      const float2 u = z[a], v = z[a + h];
+      const float2 d = make_float2(u.x - v.x, u.y - v.y);
+      const float2 w = __ldg(W + pos * tw);          // exp(-2 pi i pos / (2h)) = W_n^(pos * n/(2h)) ; n/(2h) = tw
+      z[a] = make_float2(u.x + v.x, u.y + v.y);
+      z[a + h] = make_float2(d.x * w.x - d.y * w.y, d.x * w.y + d.y * w.x);
+    }
+    __syncthreads();
+  }
+  // band bins from the bit-reversed m-point spectrum
+  float2 *out = bins + (size_t)blockIdx.x * nb;
+  const float fdt = (float)dt;
+  for (int q = threadIdx.x; q < nb; q += blockDim.x) {
+    const int k = k_lo + q;
+    float2 X = make_float2(0.f, 0.f);
+    if (k >= 0 && k <= m) {
+      const int k1 = k & (m - 1), k2 = (m - k) & (m - 1);       // Z[m] = Z[0]
+      const float2 A = z[__brev((unsigned)k1) >> (32 - log2m)];
+      const float2 Bc = z[__brev((unsigned)k2) >> (32 - log2m)];
+      const float2 B = make_float2(Bc.x, -Bc.y);                 // conj Z[m-k]
+      const float2 S = make_float2(A.x + B.x, A.y + B.y), D = make_float2(A.x - B.x, A.y - B.y);
+      float2 w;                                                  // w^k, k <= m = n/2
+      if (k < m) w = __ldg(W + k); else w = make_float2(-1.f, 0.f);
+      // -i w D = -i (wr + i wi)(Dr + i Di) = (wr Di + wi Dr) - i (wr Dr - wi Di)
+      const float tr = w.x * D.y + w.y * D.x, ti = -(w.x * D.x - w.y * D.y);
+      X = make_float2(0.5f * fdt * (S.x + tr), 0.5f * fdt * (S.y + ti));
+    }
+    out[q] = X;
+  }
+}
+
+// Direct band DFT for any n: block per segment, one thread per bin, samples staged through shared memory.
+__global__ void __launch_bounds__(256) sft_dft_band_kernel(const double *x, int n, double dt, int k_lo, int nb, float2 *bins) {
+  __shared__ double xs[1024];
+  const double *seg = x + (size_t)blockIdx.x * n;
+  for (int q0 = 0; q0 < nb; q0 += blockDim.x) {
+    const int q = q0 + threadIdx.x, k = k_lo + q;
+    double re = 0.0, im = 0.0;
+    long long ph = 0;                                 // (j k) mod n, exact
+    const long long kk = ((long long)k % n + n) % n;
+    for (int j0 = 0; j0 < n; j0 += 1024) {
+      __syncthreads();
+      for (int j = threadIdx.x; j < 1024 && j0 + j < n; j += blockDim.x) xs[j] = seg[j0 + j];
+      __syncthreads();
+      const int je = min(1024, n - j0);
+      if (q < nb) {
+        for (int j = 0; j < je; ++j) {
+          double s, c;
+          sincospi(2.0 * (double)ph / (double)n, &s, &c);
+          re = fma(xs[j], c, re);
+          im = fma(xs[j], -s, im);
+          ph += kk;
+          if (ph >= n) ph -= n;
+        }
+      }
+    }
+    if (q < nb) bins[(size_t)blockIdx.x * nb + q] = make_float2((float)(dt * re), (float)(dt * im));
+  }
+}
+
+}  // namespace sftk

@@ -11,6 +11,7 @@
 #include "../../include/sft.h"
 #include "sft_kernels.cuh"
 #include "alu_peaks.cuh"
+#include "sft_ingest.cuh"
 
 #define SFT_API extern "C" __attribute__((visibility("default")))
 
@@ -332,6 +333,109 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
   p->sigma[channel] = sqrt(p->d.t_sft / S_ref);
   p->loaded[channel] = true;
   return SFT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Data SFTs from the time series (sft_ingest.cuh).  `x` and `bins` are DEVICE pointers here.
+static cudaError_t compute_sfts_device(cudaStream_t stream, const double *x, int64_t n_sft, int n, double dt, int k_lo,
+                                       int k_hi, float2 *bins, long long *launches) {
+  const int nb = k_hi - k_lo;
+  const bool pow2 = n >= 64 && n <= sftk::FFT_MAX_N && (n & (n - 1)) == 0 && (((size_t)x & 15) == 0);
+  if (pow2) {
+    float2 *W = nullptr;
+    cudaError_t e = cudaMalloc((void **)&W, (size_t)(n / 2) * sizeof(float2));
+    if (e != cudaSuccess) return e;
+    sftk::sft_twiddle_kernel<<<(n / 2 + 255) / 256, 256, 0, stream>>>(n, W);
+    int log2m = 0;
+    while ((1 << log2m) < n / 2) ++log2m;
+    const size_t smem = (size_t)(n / 2) * sizeof(float2);
+    cudaFuncSetAttribute(sftk::sft_rfft_band_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    sftk::sft_rfft_band_kernel<<<(unsigned)n_sft, 512, smem, stream>>>(x, n, log2m, dt, k_lo, nb, W, bins);
+    if (launches) *launches += 2;
+    e = cudaGetLastError();
+    cudaError_t e2 = cudaStreamSynchronize(stream);
+    cudaFree(W);
+    return e != cudaSuccess ? e : e2;
+  }
+  sftk::sft_dft_band_kernel<<<(unsigned)n_sft, 256, 0, stream>>>(x, n, dt, k_lo, nb, bins);
+  if (launches) *launches += 1;
+  return cudaGetLastError();
+}
+
+SFT_API sft_status sft_compute_sfts(int32_t device, void *stream, const double *x, int64_t n_sft, int32_t n, double dt,
+                                    int32_t k_lo, int32_t k_hi, float *bins, int32_t mem) {
+  g_create_err[0] = 0;
+  if (!x || !bins) return fail(nullptr, SFT_EINVAL, "sft_compute_sfts: x and bins are required");
+  if (n_sft < 1 || n_sft > (1ll << 30) || n < 2 || !(dt > 0.0) || k_lo < 0 || k_hi <= k_lo)
+    return fail(nullptr, SFT_EINVAL, "sft_compute_sfts: need n_sft >= 1, n >= 2, dt > 0, 0 <= k_lo < k_hi");
+  if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(nullptr, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
+  CU(nullptr, cudaSetDevice(device));
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t nb = (size_t)(k_hi - k_lo), b_x = (size_t)n_sft * n * sizeof(double), b_out = (size_t)n_sft * nb * sizeof(float2);
+  const double *d_x = x;
+  float2 *d_out = (float2 *)bins;
+  void *tmp = nullptr;
+  if (mem == SFT_MEM_HOST) {
+    cudaError_t e = cudaMalloc(&tmp, b_x + b_out + 256);
+    if (e != cudaSuccess) return fail(nullptr, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(e));
+    cudaMemcpyAsync(tmp, x, b_x, cudaMemcpyHostToDevice, st);
+    d_x = (const double *)tmp;
+    d_out = (float2 *)((char *)tmp + ((b_x + 255) & ~size_t(255)));
+  }
+  cudaError_t e = compute_sfts_device(st, d_x, n_sft, n, dt, k_lo, k_hi, d_out, nullptr);
+  if (e == cudaSuccess && mem == SFT_MEM_HOST) {
+    e = cudaMemcpyAsync(bins, d_out, b_out, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  }
+  if (tmp) { cudaStreamSynchronize(st); cudaFree(tmp); }
+  if (e != cudaSuccess) return fail(nullptr, SFT_ECUDA, "sft_compute_sfts: %s", cudaGetErrorString(e));
+  return SFT_OK;
+}
+
+SFT_API sft_status sft_ingest_timeseries(sft_plan *p, int32_t channel, const double *x, int64_t n_samples,
+                                         const double *psd_scale, const double *psd_shape, const float *response, int32_t mem) {
+  if (!p) return SFT_EINVAL;
+  p->err[0] = 0;
+  if (!x || !psd_scale) return fail(p, SFT_EINVAL, "x and psd_scale are required");
+  if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(p, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
+  const size_t N = p->d.n_sft, n = p->n_samp, nb = p->nb;
+  if (n_samples < (int64_t)(N * n)) return fail(p, SFT_ESHAPE, "%lld samples < n_sft * n = %zu", (long long)n_samples, N * n);
+  CU(p, cudaSetDevice(p->d.device));
+  const size_t b_x = N * n * sizeof(double), b_bins = N * nb * sizeof(float2);
+  void *tmp = nullptr;
+  cudaError_t e = cudaMalloc(&tmp, (mem == SFT_MEM_HOST ? b_x : 0) + b_bins + 512);
+  if (e != cudaSuccess) return fail(p, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(e));
+  float2 *d_bins = (float2 *)tmp;
+  const double *d_x = x;
+  if (mem == SFT_MEM_HOST) {
+    double *dx = (double *)((char *)tmp + ((b_bins + 255) & ~size_t(255)));
+    cudaMemcpyAsync(dx, x, b_x, cudaMemcpyHostToDevice, p->stream);
+    d_x = dx;
+  }
+  e = compute_sfts_device(p->stream, d_x, (int64_t)N, (int)n, 1.0 / p->d.fs, p->d.k_lo, p->d.k_hi, d_bins, &p->launches);
+  if (e != cudaSuccess) { cudaStreamSynchronize(p->stream); cudaFree(tmp); return fail(p, SFT_ECUDA, "SFT kernel: %s", cudaGetErrorString(e)); }
+  // the noise description may live on either side: bring it to the device, then the common whitening path
+  sft_status st = SFT_OK;
+  void *tmp2 = nullptr;
+  const double *d_scale = psd_scale, *d_shape = psd_shape;
+  const float *d_resp = response;
+  if (mem == SFT_MEM_HOST) {
+    const size_t b_scale = N * sizeof(double), b_shape = psd_shape ? nb * sizeof(double) : 0;
+    const size_t b_resp = (response && p->d.response == SFT_RESP_TABLE) ? N * sizeof(float2) : 0;
+    e = cudaMalloc(&tmp2, b_scale + b_shape + b_resp + 768);
+    if (e != cudaSuccess) { cudaStreamSynchronize(p->stream); cudaFree(tmp); return fail(p, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(e)); }
+    char *q = (char *)tmp2;
+    cudaMemcpyAsync(q, psd_scale, b_scale, cudaMemcpyHostToDevice, p->stream);
+    d_scale = (const double *)q;
+    q += (b_scale + 255) & ~size_t(255);
+    if (psd_shape) { cudaMemcpyAsync(q, psd_shape, b_shape, cudaMemcpyHostToDevice, p->stream); d_shape = (const double *)q; q += (b_shape + 255) & ~size_t(255); }
+    if (b_resp) { cudaMemcpyAsync(q, response, b_resp, cudaMemcpyHostToDevice, p->stream); d_resp = (const float *)q; }
+  }
+  st = sft_load_data(p, channel, (const float *)d_bins, d_scale, d_shape, d_resp, SFT_MEM_DEVICE);
+  cudaStreamSynchronize(p->stream);
+  cudaFree(tmp);
+  if (tmp2) cudaFree(tmp2);
+  return st;
 }
 
 // ---------------------------------------------------------------------------------------------
