@@ -437,6 +437,49 @@ def run_sweep(args):
         del P, xh, hh, xi, kc
 
 
+def run_ingest(args):
+    """--ingest: SURVEY section 8(f) NEXT-1 - sft_compute_sfts on a series shaped like config 2 (10,800 segments of
+    16,384 float64 samples, 1.42 GB, device resident; band bins 5..186).  HBM-bound: the series is read once.
+    One JSON line: samples/s and achieved GB/s against the measured copy bandwidth (MEASURED_PEAKS.json)."""
+    import torch
+    from paper_2502_11823_b200 import api, build
+    build.build()
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    n_sft, n, k_lo, k_hi, dt = 10800, 16384, 5, 187, 1.0 / 2048.0
+    g = torch.Generator(device=dev)
+    g.manual_seed(11)
+    x = torch.randn(n_sft * n, dtype=torch.float64, device=dev, generator=g) * 1e-23
+    bins = torch.empty((n_sft, k_hi - k_lo), dtype=torch.complex64, device=dev)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ms = 0.0
+    for i in range(args.warmup + args.steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        api.compute_sfts(x, n_sft, n, dt, k_lo, k_hi, bins, device=0, stream=stream.cuda_stream)
+        b.record(stream)
+        torch.cuda.synchronize()
+        if i >= args.warmup:
+            ms += a.elapsed_time(b)
+    ms /= args.steps
+    nbytes = x.numel() * 8 + bins.numel() * 8
+    peak, src = 6650.0, "fallback (B200_PROFILING.md)"
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            peak, src = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        pass
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "data-SFT generation (sft_compute_sfts)", "value": x.numel() / (ms * 1e-3), "unit": "samples/s",
+                      "ms_per_step": ms, "steps": args.steps, "warmup": args.warmup, "dtype": "f32 (f64 input)", "data": "synthetic",
+                      "config": {"workload": "config2-shaped series", "n_sft": n_sft, "n": n, "band": [k_lo, k_hi],
+                                 "cache": "l2_flush_between_steps; includes the twiddle-table kernel and the end-of-call sync"},
+                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                                   "traffic": None, "peak_source": src, "alg_bytes": nbytes}}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -450,14 +493,15 @@ def main():
     ap.add_argument("--chunk", type=int, default=0)
     ap.add_argument("--evaluator", default="auto", choices=["auto", "direct", "table"])
     ap.add_argument("--sweep", action="store_true", help="config-5 scaling sweep (one JSON line per point)")
+    ap.add_argument("--ingest", action="store_true", help="time the GPU data-SFT generation (NEXT-1)")
     ap.add_argument("--cpu-budget", type=float, default=12.0, dest="cpu_budget")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.sweep:
+    if args.sweep or args.ingest:
         if rank == 0:
-            run_sweep(args)
+            run_sweep(args) if args.sweep else run_ingest(args)
     elif args.impl == "reference":
         run_reference(args, rank, world)
     else:

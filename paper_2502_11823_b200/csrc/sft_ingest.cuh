@@ -30,6 +30,39 @@ __global__ void sft_twiddle_kernel(int n, float2 *W) {
   W[t] = make_float2((float)c, (float)-s);
 }
 
+// R consecutive radix-2 DIF stages (half-blocks h, h/2, .., h >> (R-1)) on groups of 2^R points held in registers:
+// the group of `base` is {base + j hl}, hl = h >> (R-1), j < 2^R; stage s couples j and j + 2^(R-1-s).
+template <int R>
+__device__ __forceinline__ void dif_pass(float2 *z, const float2 *W, int m, int n, int h, int tid, int nthr) {
+  constexpr int G = 1 << R;
+  const int hl = h >> (R - 1);
+  for (int g = tid; g < (m >> R); g += nthr) {
+    const int pos = g & (hl - 1);
+    const int base = ((g - pos) << R) + pos;          // groups tile blocks of 2h = hl * 2^R points
+    float2 v[G];
+#pragma unroll
+    for (int j = 0; j < G; ++j) v[j] = z[base + j * hl];
+#pragma unroll
+    for (int s = 0; s < R; ++s) {
+      const int hj = G >> (s + 1);                    // partner distance in j
+      const int hs = h >> s;                          // half-block of this stage
+      const int tw = n / (2 * hs);
+#pragma unroll
+      for (int j = 0; j < G; ++j) {
+        if ((j / hj) & 1) continue;
+        const float2 u = v[j], w2 = v[j + hj];
+        const int p = (base + j * hl) & (hs - 1);
+        const float2 w = __ldg(W + p * tw);
+        const float2 d = make_float2(u.x - w2.x, u.y - w2.y);
+        v[j] = make_float2(u.x + w2.x, u.y + w2.y);
+        v[j + hj] = make_float2(d.x * w.x - d.y * w.y, d.x * w.y + d.y * w.x);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < G; ++j) z[base + j * hl] = v[j];
+  }
+}
+
 // One block per segment.  Dynamic shared memory: (n/2) float2.
 __global__ void __launch_bounds__(512) sft_rfft_band_kernel(const double *x, int n, int log2m, double dt, int k_lo, int nb,
                                                             const float2 *W, float2 *bins) {
@@ -42,19 +75,16 @@ __global__ void __launch_bounds__(512) sft_rfft_band_kernel(const double *x, int
     z[j] = make_float2((float)v.x, (float)v.y);
   }
   __syncthreads();
-  // in-place radix-2 DIF over m points: twiddle of the m-point transform = W_n^(2t)
-  for (int h = m >> 1, tw = 2; h >= 1; h >>= 1, tw <<= 1) {
-    for (int i = threadIdx.x; i < (m >> 1); i += blockDim.x) {
-      const int pos = i & (h - 1);                   // index inside the half-block
-      const int a = ((i - pos) << 1) + pos;          // first element of the butterfly
-      const float2 u = z[a], v = z[a + h];
-      const float2 d = make_float2(u.x - v.x, u.y - v.y);
-      const float2 w = __ldg(W + pos * tw);          // exp(-2 pi i pos / (2h)) = W_n^(pos * n/(2h)) ; n/(2h) = tw
-      z[a] = make_float2(u.x + v.x, u.y + v.y);
-      z[a + h] = make_float2(d.x * w.x - d.y * w.y, d.x * w.y + d.y * w.x);
-    }
+  // in-place radix-2 DIF network over m points (twiddle of a stage with half-block h: exp(-2 pi i pos / 2h) =
+  // W[pos * n / 2h]), three consecutive stages at a time in registers (8 points per thread and pass), then the rest
+  int h = m >> 1;                                    // half-block of the next stage
+  while (h >= 4) {
+    dif_pass<3>(z, W, m, n, h, threadIdx.x, blockDim.x);
+    h >>= 3;
     __syncthreads();
   }
+  if (h == 2) { dif_pass<2>(z, W, m, n, h, threadIdx.x, blockDim.x); __syncthreads(); }
+  else if (h == 1) { dif_pass<1>(z, W, m, n, h, threadIdx.x, blockDim.x); __syncthreads(); }
   // band bins from the bit-reversed m-point spectrum
   float2 *out = bins + (size_t)blockIdx.x * nb;
   const float fdt = (float)dt;

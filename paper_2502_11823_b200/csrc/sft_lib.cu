@@ -7,6 +7,8 @@
 #include <string.h>
 #include <new>
 #include <vector>
+#include <mutex>
+#include <utility>
 
 #include "../../include/sft.h"
 #include "sft_kernels.cuh"
@@ -342,20 +344,33 @@ static cudaError_t compute_sfts_device(cudaStream_t stream, const double *x, int
   const int nb = k_hi - k_lo;
   const bool pow2 = n >= 64 && n <= sftk::FFT_MAX_N && (n & (n - 1)) == 0 && (((size_t)x & 15) == 0);
   if (pow2) {
+    // twiddle tables are kept per (device, n) for the life of the process (<= 64 KB each)
+    static std::mutex mu;
+    static std::vector<std::pair<std::pair<int, int>, float2 *>> cache;
+    int dev = 0;
+    cudaGetDevice(&dev);
     float2 *W = nullptr;
-    cudaError_t e = cudaMalloc((void **)&W, (size_t)(n / 2) * sizeof(float2));
-    if (e != cudaSuccess) return e;
-    sftk::sft_twiddle_kernel<<<(n / 2 + 255) / 256, 256, 0, stream>>>(n, W);
+    {
+      std::lock_guard<std::mutex> lk(mu);
+      for (auto &c : cache)
+        if (c.first.first == dev && c.first.second == n) W = c.second;
+      if (!W) {
+        cudaError_t e = cudaMalloc((void **)&W, (size_t)(n / 2) * sizeof(float2));
+        if (e != cudaSuccess) return e;
+        sftk::sft_twiddle_kernel<<<(n / 2 + 255) / 256, 256, 0, stream>>>(n, W);
+        e = cudaStreamSynchronize(stream);
+        if (e != cudaSuccess) { cudaFree(W); return e; }
+        cache.push_back({{dev, n}, W});
+        if (launches) *launches += 1;
+      }
+    }
     int log2m = 0;
     while ((1 << log2m) < n / 2) ++log2m;
     const size_t smem = (size_t)(n / 2) * sizeof(float2);
     cudaFuncSetAttribute(sftk::sft_rfft_band_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     sftk::sft_rfft_band_kernel<<<(unsigned)n_sft, 512, smem, stream>>>(x, n, log2m, dt, k_lo, nb, W, bins);
-    if (launches) *launches += 2;
-    e = cudaGetLastError();
-    cudaError_t e2 = cudaStreamSynchronize(stream);
-    cudaFree(W);
-    return e != cudaSuccess ? e : e2;
+    if (launches) *launches += 1;
+    return cudaGetLastError();
   }
   sftk::sft_dft_band_kernel<<<(unsigned)n_sft, 256, 0, stream>>>(x, n, dt, k_lo, nb, bins);
   if (launches) *launches += 1;
@@ -383,10 +398,8 @@ SFT_API sft_status sft_compute_sfts(int32_t device, void *stream, const double *
     d_out = (float2 *)((char *)tmp + ((b_x + 255) & ~size_t(255)));
   }
   cudaError_t e = compute_sfts_device(st, d_x, n_sft, n, dt, k_lo, k_hi, d_out, nullptr);
-  if (e == cudaSuccess && mem == SFT_MEM_HOST) {
-    e = cudaMemcpyAsync(bins, d_out, b_out, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  }
+  if (e == cudaSuccess && mem == SFT_MEM_HOST) e = cudaMemcpyAsync(bins, d_out, b_out, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   if (tmp) { cudaStreamSynchronize(st); cudaFree(tmp); }
   if (e != cudaSuccess) return fail(nullptr, SFT_ECUDA, "sft_compute_sfts: %s", cudaGetErrorString(e));
   return SFT_OK;
