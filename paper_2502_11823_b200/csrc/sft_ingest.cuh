@@ -30,41 +30,58 @@ __global__ void sft_twiddle_kernel(int n, float2 *W) {
   W[t] = make_float2((float)c, (float)-s);
 }
 
+// Shared-memory index with one float2 of padding per 16: keeps every pass of the FFT bank-conflict free.
+__device__ __forceinline__ int padi(int i) { return i + (i >> 4); }
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+// v * exp(-2 pi i q / 8), q = 0..3 (compile-time after unrolling)
+__device__ __forceinline__ float2 rot8(float2 v, int q) {
+  const float c = 0.70710678118654752f;
+  switch (q & 3) {
+    case 0: return v;
+    case 1: return make_float2(c * (v.x + v.y), c * (v.y - v.x));
+    case 2: return make_float2(v.y, -v.x);
+    default: return make_float2(c * (v.y - v.x), -c * (v.x + v.y));
+  }
+}
+
 // R consecutive radix-2 DIF stages (half-blocks h, h/2, .., h >> (R-1)) on groups of 2^R points held in registers:
-// the group of `base` is {base + j hl}, hl = h >> (R-1), j < 2^R; stage s couples j and j + 2^(R-1-s).
+// the group of `base` is {base + j hl}, hl = h >> (R-1), j < 2^R; stage s couples j and j + 2^(R-1-s).  The twiddle of
+// element j in stage s is exp(-2 pi i ((pos + j hl) mod hs) / 2 hs), hs = h >> s, i.e. w0^(2^s) times a multiple of an
+// eighth of a turn, with w0 = exp(-2 pi i pos / 2h) the only table look-up of the group.
 template <int R>
 __device__ __forceinline__ void dif_pass(float2 *z, const float2 *W, int m, int n, int h, int tid, int nthr) {
   constexpr int G = 1 << R;
   const int hl = h >> (R - 1);
+  const int tw = n / (2 * h);
   for (int g = tid; g < (m >> R); g += nthr) {
     const int pos = g & (hl - 1);
     const int base = ((g - pos) << R) + pos;          // groups tile blocks of 2h = hl * 2^R points
     float2 v[G];
 #pragma unroll
-    for (int j = 0; j < G; ++j) v[j] = z[base + j * hl];
+    for (int j = 0; j < G; ++j) v[j] = z[padi(base + j * hl)];
+    float2 wp = __ldg(W + pos * tw);                  // w0^(2^s)
 #pragma unroll
     for (int s = 0; s < R; ++s) {
-      const int hj = G >> (s + 1);                    // partner distance in j
-      const int hs = h >> s;                          // half-block of this stage
-      const int tw = n / (2 * hs);
+      const int hj = G >> (s + 1);                    // partner distance in j = points per half-block in units of hl
 #pragma unroll
       for (int j = 0; j < G; ++j) {
         if ((j / hj) & 1) continue;
         const float2 u = v[j], w2 = v[j + hj];
-        const int p = (base + j * hl) & (hs - 1);
-        const float2 w = __ldg(W + p * tw);
         const float2 d = make_float2(u.x - w2.x, u.y - w2.y);
         v[j] = make_float2(u.x + w2.x, u.y + w2.y);
-        v[j + hj] = make_float2(d.x * w.x - d.y * w.y, d.x * w.y + d.y * w.x);
+        // ((j hl) mod hs) / (2 hs) = (j mod hj) / (2 hj) of a turn = (j mod hj) * (4 / hj) eighths
+        v[j + hj] = rot8(cmul(d, wp), (j % hj) * (4 / hj));
       }
+      if (s + 1 < R) wp = cmul(wp, wp);
     }
 #pragma unroll
-    for (int j = 0; j < G; ++j) z[base + j * hl] = v[j];
+    for (int j = 0; j < G; ++j) z[padi(base + j * hl)] = v[j];
   }
 }
 
-// One block per segment.  Dynamic shared memory: (n/2) float2.
-__global__ void __launch_bounds__(512) sft_rfft_band_kernel(const double *x, int n, int log2m, double dt, int k_lo, int nb,
+// One block per segment.  Dynamic shared memory: (n/2 + n/32) float2.
+__global__ void __launch_bounds__(256) sft_rfft_band_kernel(const double *x, int n, int log2m, double dt, int k_lo, int nb,
                                                             const float2 *W, float2 *bins) {
   extern __shared__ float2 z[];
   const int m = n >> 1;
@@ -72,11 +89,11 @@ __global__ void __launch_bounds__(512) sft_rfft_band_kernel(const double *x, int
   // load + pack: z[j] = x[2j] + i x[2j+1]  (16-byte loads of two doubles)
   for (int j = threadIdx.x; j < m; j += blockDim.x) {
     const double2 v = __ldcs((const double2 *)seg + j);
-    z[j] = make_float2((float)v.x, (float)v.y);
+    z[padi(j)] = make_float2((float)v.x, (float)v.y);
   }
   __syncthreads();
-  // in-place radix-2 DIF network over m points (twiddle of a stage with half-block h: exp(-2 pi i pos / 2h) =
-  // W[pos * n / 2h]), three consecutive stages at a time in registers (8 points per thread and pass), then the rest
+  // in-place radix-2 DIF network over m points, three consecutive stages at a time in registers (8 points per
+  // thread and pass), then the rest
   int h = m >> 1;                                    // half-block of the next stage
   while (h >= 4) {
     dif_pass<3>(z, W, m, n, h, threadIdx.x, blockDim.x);
@@ -93,8 +110,8 @@ __global__ void __launch_bounds__(512) sft_rfft_band_kernel(const double *x, int
     float2 X = make_float2(0.f, 0.f);
     if (k >= 0 && k <= m) {
       const int k1 = k & (m - 1), k2 = (m - k) & (m - 1);       // Z[m] = Z[0]
-      const float2 A = z[__brev((unsigned)k1) >> (32 - log2m)];
-      const float2 Bc = z[__brev((unsigned)k2) >> (32 - log2m)];
+      const float2 A = z[padi((int)(__brev((unsigned)k1) >> (32 - log2m)))];
+      const float2 Bc = z[padi((int)(__brev((unsigned)k2) >> (32 - log2m)))];
       const float2 B = make_float2(Bc.x, -Bc.y);                 // conj Z[m-k]
       const float2 S = make_float2(A.x + B.x, A.y + B.y), D = make_float2(A.x - B.x, A.y - B.y);
       float2 w;                                                  // w^k, k <= m = n/2

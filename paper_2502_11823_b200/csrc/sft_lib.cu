@@ -366,9 +366,9 @@ static cudaError_t compute_sfts_device(cudaStream_t stream, const double *x, int
     }
     int log2m = 0;
     while ((1 << log2m) < n / 2) ++log2m;
-    const size_t smem = (size_t)(n / 2) * sizeof(float2);
+    const size_t smem = (size_t)(n / 2 + n / 32 + 1) * sizeof(float2);
     cudaFuncSetAttribute(sftk::sft_rfft_band_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    sftk::sft_rfft_band_kernel<<<(unsigned)n_sft, 512, smem, stream>>>(x, n, log2m, dt, k_lo, nb, W, bins);
+    sftk::sft_rfft_band_kernel<<<(unsigned)n_sft, 256, smem, stream>>>(x, n, log2m, dt, k_lo, nb, W, bins);
     if (launches) *launches += 1;
     return cudaGetLastError();
   }
