@@ -331,12 +331,14 @@ def alg_instr_per_pair(path, K, C):
     """Warp instructions the formulation needs per active (template, SFT) pair on evaluator path
     ``path`` (a packed FFMA2/FMUL2 counts as ONE instruction, as it takes one issue slot):
     fixed part = fp64 track 50 + SFT loop 13 + phase/prefactor/response/accumulation 23 (+12 per extra
-    channel); table: 21 shared + 38 per channel; series order n: per far bin 2.5 (reciprocal pair) +
+    channel); table tier 1: 21 shared + 38 per channel, tier 2: 21 + 134 per channel; series order n: per far bin 2.5 (reciprocal pair) +
     s_n/2 + 1 (|J|^2) + 3.5 C (load + MACs), central bin 7(n+1) + 2 + 7 C; closed Fresnel form: 64 + 3.5 C
     per bin."""
     fixed = 86 + 12 * (C - 1)
     if path == "table":
         return fixed + 21 + 38 * C
+    if path == "table2":                 # 14 loads, 71 packed FMAs + 22 scalings for S1, 24 + 3 for H
+        return fixed + 21 + 134 * C
     if path == "fresnel":
         return fixed + (2 * K + 1) * (64 + 3.5 * C)
     n = int(path[-1])

@@ -86,7 +86,7 @@ typedef struct {
   double resp_psi[SFT_MAX_CHANNELS]; /* SFT_RESP_ANNUAL: amplitude-modulation phase per channel */
   double resp_chi[SFT_MAX_CHANNELS]; /* SFT_RESP_ANNUAL: response phase per channel             */
   int32_t evaluator;   /* SFT_EVAL_*: how sum_k conj(x~) F / S and sum_k |F|^2 / S are evaluated for
-                          |fdot| T^2 <= 0.12; results agree to ~1e-6 */
+                          |fdot| T^2 <= 1; results agree to ~1e-6 */
   int32_t device;      /* CUDA device ordinal                                             */
   void *stream;        /* cudaStream_t to order work on, or NULL for the legacy default stream */
 } sft_plan_desc;
@@ -164,9 +164,10 @@ double sft_plan_last_kernel_ms(sft_plan *plan);
 /* Diagnostic: how the coefficient evaluator (rows A4/A6 of the hot path) was used by the most recent
  * sft_inner_products call that had kc_out != NULL: the number of active (template, SFT, channel) pairs
  * evaluated with the series in b = fdot T^2 about the Dirichlet kernel at order 0, 1, 2, 3 (out[0..3])
- * with the closed Fresnel form Eq.(29) P:219 (out[4]) and through the moment tables (out[5]).  The
- * path is chosen per warp of 32 templates from the largest |b| in the warp.
- * Blocks until that call finished.  Writes min(n_out, 6) values; host pointer. */
+ * with the closed Fresnel form Eq.(29) P:219 (out[4]) and through the moment tables (out[5]: tier 1,
+ * |b| <= 0.12; out[6]: tier 2, |b| <= 1).  The path is chosen per warp of 32 templates from the largest
+ * |b| in the warp.  Blocks until that call finished.  Writes min(n_out, 7) values;
+ * host pointer. */
 sft_status sft_plan_path_counts(sft_plan *plan, int64_t *out, int32_t n_out);
 
 /* Tuning knob: SFTs per work unit along the time axis (0 = automatic).  Results do not depend on it

@@ -18,7 +18,7 @@ KERNEL = {"dirichlet": 0, "fresnel": 1}
 RESPONSE = {"none": 0, "table": 1, "annual": 2}
 PHASE = {"fp64": 0, "split32": 1}
 MEM_HOST, MEM_DEVICE = 0, 1
-PATHS = ("series0", "series1", "series2", "series3", "fresnel", "table")
+PATHS = ("series0", "series1", "series2", "series3", "fresnel", "table", "table2")
 EVALUATOR = {"auto": 0, "direct": 1, "table": 2}
 STATUS = {0: "SFT_OK", 1: "SFT_EINVAL", 2: "SFT_ESHAPE", 3: "SFT_ENODATA", 4: "SFT_EUNSUPPORTED",
           5: "SFT_ECUDA", 6: "SFT_ENOMEM"}
@@ -239,8 +239,8 @@ class Plan:
 
     def path_counts(self):
         """``sft_plan_path_counts``: dict path name -> active pairs of the last call that had kc_out."""
-        out = (C.c_int64 * 6)()
-        self._check(self.lib.sft_plan_path_counts(self._h, out, 6))
+        out = (C.c_int64 * 7)()
+        self._check(self.lib.sft_plan_path_counts(self._h, out, 7))
         return dict(zip(PATHS, [int(v) for v in out]))
 
 

@@ -69,7 +69,7 @@ struct KParams {
   const float4 *htab;      // [C][n_kc * HTAB_R][4]   <h,h> polynomial per node
   unsigned mrow, mchan;    // float4 entries per SFT row (n_node * 4) and per channel (n_sft * mrow), hchan likewise
   unsigned hchan;
-  float b_table;           // B_TABLE if the plan has the tables, else -1 (no |b| qualifies)
+  float b_table, b_table2; // B_TABLE, B_TABLE2 if the plan has the tables, else -1 (no |b| qualifies)
   double *part;            // [n_chunks][3][nT] chunk totals (xh, hh, xh_im)
   int *kc_out;             // [nT][C][n_sft] or null
   float *loc_xh, *loc_hh;  // cumulative mode: [nT][n_sft] chunk-local prefix sums
@@ -661,10 +661,11 @@ __device__ __forceinline__ void fresnel_pairs(const KParams &p, const Tmpl &tm, 
 }
 
 // Evaluator paths (warp-uniform): series order 0..3, closed Fresnel form.
-enum { PATH_ORD0 = 0, PATH_ORD1, PATH_ORD2, PATH_ORD3, PATH_FRESNEL, PATH_TABLE, PATH_N };
+enum { PATH_ORD0 = 0, PATH_ORD1, PATH_ORD2, PATH_ORD3, PATH_FRESNEL, PATH_TABLE, PATH_TABLE2, PATH_N };
 
 __device__ __forceinline__ int path_of(float bmax, bool table) {
-  if (table && bmax <= B_TABLE) return PATH_TABLE;   // same test as pair_terms
+  if (table && bmax <= B_TABLE) return PATH_TABLE;   // same tests as pair_terms
+  if (table && bmax <= B_TABLE2) return PATH_TABLE2;
   return bmax == 0.f ? PATH_ORD0 : bmax <= B_ORDER1 ? PATH_ORD1 : bmax <= B_ORDER2 ? PATH_ORD2 : bmax <= B_ORDER3 ? PATH_ORD3
                                                                                                                : PATH_FRESNEL;
 }
@@ -676,11 +677,16 @@ __device__ __forceinline__ float2 cstep(float2 X, float s, float2 Y) {
 
 // Moment-table evaluator of one (template, SFT): S1 = sum_m D J_m and S2 = sum_m u |J_m|^2 from the tables
 // of sft_table.cuh (true J, no 2 pi).  `kcidx` = k_c - (k_lo - K), already clamped to the table;
-// `Mrow` = row of SFT alpha, channel 0.  Also evaluates the track of the next SFT (see series_pairs).
-template <int CT, class CFG>
+// `Mrow` = row of SFT alpha, channel 0.  TIER 1: moments q <= 7, H to beta^2 (|b| <= B_TABLE); TIER 2: q <= 15,
+// H to beta^6 (|b| <= B_TABLE2).  Also evaluates the track of the next SFT (see series_pairs).
+template <int CT, class CFG, int TIER>
 __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, double dnext, Track &nxt, float xp, float b,
                                            int kcidx, const float4 *Mrow, float (&s1r)[CT], float (&s1i)[CT],
                                            float (&s2)[CT]) {
+  constexpr int Q = TIER == 1 ? TAB_Q1 : TAB_Q;          // highest moment
+  constexpr int NL = (Q + 1) / 2;                         // float4 loads of moments per channel
+  constexpr int NHB = TIER == 1 ? 2 : HTAB_NB;            // powers of beta^2 in H
+  constexpr int NHL = (NHB * (HTAB_P + 1) + 3) / 4;       // float4 loads of H coefficients
   // node of the <h,h> table: cellH = floor((xp + 1/2) HTAB_R) by the 1.5 * 2^23 rounding trick, clamped (xp = 1/2
   // exactly, NaN lanes); the data-moment node is cellH / 4 (HTAB_R = 4 TAB_R)
   static_assert(HTAB_R == 4 * TAB_R, "node grids");
@@ -690,53 +696,55 @@ __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, dou
   const int cellH = __float_as_int(cm) & (HTAB_R - 1);
   const int cell = cellH >> 2;
   const float cHf = cm - RM;                                   // (float)cellH
-  const float4 *mp = Mrow + (unsigned)(kcidx * TAB_R + cell) * 4u;
-  const float4 *hp = p.htab + (unsigned)(kcidx * HTAB_R + cellH) * 4u;
-  float4 Mq[CT][4], Hq[CT][3];
+  const float4 *mp = Mrow + (unsigned)(kcidx * TAB_R + cell) * (unsigned)((TAB_Q + 1) / 2);
+  const float4 *hp = p.htab + (unsigned)(kcidx * HTAB_R + cellH) * (unsigned)(HTAB_W / 4);
+  float4 Mq[CT][NL], Hq[CT][NHL];
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) Mq[c][i] = __ldg(mp + c * p.mchan + i);
+    for (int i = 0; i < NL; ++i) Mq[c][i] = __ldg(mp + c * p.mchan + i);
 #pragma unroll
-    for (int i = 0; i < 3; ++i) Hq[c][i] = __ldg(hp + c * p.hchan + i);
+    for (int i = 0; i < NHL; ++i) Hq[c][i] = __ldg(hp + c * p.hchan + i);
   }
   track_eval<CFG>(p, tm, dnext, nxt);
   // a = 2 pi (xp - node centre):  centre_H = (cellH + 1/2)/HTAB_R - 1/2,  centre_M = (cell + 1/2)/TAB_R - 1/2
   const float aH = fmaf(cHf, -(2.0f * PI_F) / HTAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / HTAB_R)));
   const float a = fmaf((float)cell, -(2.0f * PI_F) / TAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / TAB_R)));
   const float be = PI_F * b;
-  const float nb1 = be, nb2 = 0.5f * be, nb3 = (1.0f / 3.0f) * be;
-  const float na1 = a, na2 = 0.5f * a, na3 = (1.0f / 3.0f) * a, na4 = 0.25f * a, na5 = 0.2f * a, na6 = (1.0f / 6.0f) * a,
-              na7 = (1.0f / 7.0f) * a;
+  float nb_[Q / 2 + 1], na_[Q + 1];                       // beta / k, a / k
+#pragma unroll
+  for (int k = 1; k <= Q / 2; ++k) nb_[k] = be * (1.0f / (float)k);
+#pragma unroll
+  for (int k = 1; k <= Q; ++k) na_[k] = a * (1.0f / (float)k);
   const float be2 = be * be;
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
-    const float2 M0 = make_float2(Mq[c][0].x, Mq[c][0].y), M1 = make_float2(Mq[c][0].z, Mq[c][0].w);
-    const float2 M2 = make_float2(Mq[c][1].x, Mq[c][1].y), M3 = make_float2(Mq[c][1].z, Mq[c][1].w);
-    const float2 M4 = make_float2(Mq[c][2].x, Mq[c][2].y), M5 = make_float2(Mq[c][2].z, Mq[c][2].w);
-    const float2 M6 = make_float2(Mq[c][3].x, Mq[c][3].y), M7 = make_float2(Mq[c][3].z, Mq[c][3].w);
-    // L_p = sum_n (i beta)^n / n! M_{p+2n}
-    const float2 L4 = cstep(M4, nb1, M6), L5 = cstep(M5, nb1, M7);
-    const float2 L2 = cstep(M2, nb1, cstep(M4, nb2, M6)), L3 = cstep(M3, nb1, cstep(M5, nb2, M7));
-    const float2 L0 = cstep(M0, nb1, cstep(M2, nb2, cstep(M4, nb3, M6)));
-    const float2 L1 = cstep(M1, nb1, cstep(M3, nb2, cstep(M5, nb3, M7)));
-    // S1 = sum_p (i a)^p / p! L_p
-    float2 S = cstep(M6, na7, M7);
-    S = cstep(L5, na6, S);
-    S = cstep(L4, na5, S);
-    S = cstep(L3, na4, S);
-    S = cstep(L2, na3, S);
-    S = cstep(L1, na2, S);
-    S = cstep(L0, na1, S);
+    float2 M[Q + 1];
+#pragma unroll
+    for (int q = 0; q <= Q; ++q)
+      M[q] = (q & 1) ? make_float2(Mq[c][q >> 1].z, Mq[c][q >> 1].w) : make_float2(Mq[c][q >> 1].x, Mq[c][q >> 1].y);
+    // S1 = sum_p (i a)^p / p! L_p,  L_p = sum_n (i beta)^n / n! M_{p+2n}: both by Horner, one packed FMA per step
+    float2 S = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int pq = Q; pq >= 0; --pq) {
+      const int nmax = (Q - pq) / 2;
+      float2 L = M[pq + 2 * nmax];
+#pragma unroll
+      for (int n = nmax; n >= 1; --n) L = cstep(M[pq + 2 * (n - 1)], nb_[n], L);
+      S = pq == Q ? L : cstep(L, na_[pq + 1], S);
+    }
     s1r[c] = S.x;
     s1i[c] = S.y;
-    // H = sum_P aH^P (h_{P,0} + beta^2 h_{P,2});  floats: h00 h10 h20 h30 | h40 h50 h02 h12 | h22 h32 h42 h52
-    float h = fmaf(be2, Hq[c][2].w, Hq[c][1].y);
-    h = fmaf(h, aH, fmaf(be2, Hq[c][2].z, Hq[c][1].x));
-    h = fmaf(h, aH, fmaf(be2, Hq[c][2].y, Hq[c][0].w));
-    h = fmaf(h, aH, fmaf(be2, Hq[c][2].x, Hq[c][0].z));
-    h = fmaf(h, aH, fmaf(be2, Hq[c][1].w, Hq[c][0].y));
-    h = fmaf(h, aH, fmaf(be2, Hq[c][1].z, Hq[c][0].x));
+    // H = sum_P aH^P sum_N beta^(2N) h_{P,2N};  floats: [N][P], P fastest
+    const float *hf = (const float *)&Hq[c][0];
+    float h = 0.f;
+#pragma unroll
+    for (int P = HTAB_P; P >= 0; --P) {
+      float g = hf[(NHB - 1) * (HTAB_P + 1) + P];
+#pragma unroll
+      for (int N = NHB - 2; N >= 0; --N) g = fmaf(g, be2, hf[N * (HTAB_P + 1) + P]);
+      h = P == HTAB_P ? g : fmaf(h, aH, g);
+    }
     s2[c] = h;
   }
 }
@@ -762,9 +770,10 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, con
   float s1r[CT], s1i[CT], s2[CT];
   float scale;                 // the series evaluators return 2 pi J
   float t;                     // total phase / pi:  2 frac (= phi_a/pi) + prefactor phase / pi
-  if (bmax <= p.b_table) {
+  if (bmax <= p.b_table2) {
     const float xp = fmaf(0.5f, b, tr.x);
-    table_eval<CT, CFG>(p, tm, dnext, nxt, xp, b, j0c - 2, Mrow0, s1r, s1i, s2);
+    if (bmax <= p.b_table) table_eval<CT, CFG, 1>(p, tm, dnext, nxt, xp, b, j0c - 2, Mrow0, s1r, s1i, s2);
+    else table_eval<CT, CFG, 2>(p, tm, dnext, nxt, xp, b, j0c - 2, Mrow0, s1r, s1i, s2);
     scale = 1.0f;
     t = fmaf(2.0f, tr.frac, fmaf(0.25f, b, tr.x));           // prefactor e^{i pi (x + b/4)}
   } else {
@@ -881,7 +890,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
     const float4 *Drow0 = p.Dp + (size_t)a0 * p.npair;
     const float4 *Mrow0 = p.mtab ? p.mtab + (size_t)a0 * p.mrow : nullptr;
     int *kcp = want_kc ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + a0 : nullptr;
-    unsigned long long n_path[PATH_N] = {0, 0, 0, 0, 0, 0};
+    unsigned long long n_path[PATH_N] = {0, 0, 0, 0, 0, 0, 0};
     Track tr;
     track_eval<CFG>(p, tm, dalpha, tr);
 

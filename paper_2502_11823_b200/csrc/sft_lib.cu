@@ -152,14 +152,14 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   p->n_kc = p->nb + 2 * d.K;
   p->n_node = p->n_kc * sftk::TAB_R;
   if (st == SFT_OK && d.evaluator != SFT_EVAL_DIRECT) {
-    const double m_bytes = (double)C * (double)N * p->n_node * 64.0;
+    const double m_bytes = (double)C * (double)N * p->n_node * (8.0 * (sftk::TAB_Q + 1));
     size_t free_b = 0, total_b = 0;
     cudaMemGetInfo(&free_b, &total_b);
-    const bool fits = m_bytes <= 0.25 * (double)free_b && (double)C * (double)N * p->n_node * 4.0 < 4.0e9;
+    const bool fits = m_bytes <= 0.25 * (double)free_b && (double)C * (double)N * p->n_node * ((sftk::TAB_Q + 1) / 2) < 4.0e9;
     if (!fits && d.evaluator == SFT_EVAL_TABLE)
       st = fail(nullptr, SFT_ENOMEM, "moment tables of %.3g bytes do not fit (free %.3g)", m_bytes, (double)free_b);
     if (fits) {
-      alloc((void **)&p->mtab, (size_t)m_bytes + (size_t)p->n_node * 64);   // + one row: nodes are prefetched one SFT ahead
+      alloc((void **)&p->mtab, (size_t)m_bytes + (size_t)p->n_node * 8 * (sftk::TAB_Q + 1));   // (+ one spare row)
       alloc((void **)&p->htab, C * (size_t)p->n_kc * sftk::HTAB_R * sftk::HTAB_W * sizeof(float));
       alloc((void **)&p->ptab, (size_t)(2 * d.K + 1) * sftk::TAB_R * (sftk::TAB_Q + 1) * sizeof(float2));
       if (st == SFT_OK) {
@@ -317,14 +317,14 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
       p->ubp + (C + (size_t)channel) * npair);
   p->launches += 2;
   if (p->mtab) {
-    const size_t per_chan = N * (size_t)p->n_node * 4;
+    const size_t per_chan = N * (size_t)p->n_node * ((sftk::TAB_Q + 1) / 2);
     const unsigned outs = (unsigned)p->n_node * (sftk::TAB_Q + 1);
     const unsigned bpr = (outs + 255) / 256;
     if ((double)bpr * (double)N > 2.0e9) return fail(p, SFT_EUNSUPPORTED, "moment-table build grid too large");
     sftk::sft_mtab_kernel<<<(unsigned)(bpr * N), 256, 0, p->stream>>>(
         p->Dp + (size_t)channel * N * npair, p->npair, p->n_node, p->d.K, p->ptab, bpr, (float2 *)(p->mtab + (size_t)channel * per_chan));
     sftk::sft_htab_kernel<<<(unsigned)(p->n_kc * sftk::HTAB_R), 64, 0, p->stream>>>(
-        p->ubp + (size_t)channel * npair, p->d.K, (float *)(p->htab + (size_t)channel * p->n_kc * sftk::HTAB_R * 4));
+        p->ubp + (size_t)channel * npair, p->d.K, (float *)(p->htab + (size_t)channel * p->n_kc * sftk::HTAB_R * (sftk::HTAB_W / 4)));
     p->launches += 2;
   }
   cudaError_t e = cudaGetLastError();
@@ -484,10 +484,11 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.depth = (float)p->d.resp_depth;
   k.mtab = p->mtab;
   k.htab = p->htab;
-  k.mrow = p->mtab ? (unsigned)p->n_node * 4u : 0u;
-  k.mchan = p->mtab ? (unsigned)(p->d.n_sft * p->n_node * 4) : 0u;
-  k.hchan = (unsigned)(p->n_kc * sftk::HTAB_R * 4);
+  k.mrow = p->mtab ? (unsigned)p->n_node * (unsigned)((sftk::TAB_Q + 1) / 2) : 0u;
+  k.mchan = p->mtab ? (unsigned)(p->d.n_sft * p->n_node * ((sftk::TAB_Q + 1) / 2)) : 0u;
+  k.hchan = (unsigned)(p->n_kc * sftk::HTAB_R * (sftk::HTAB_W / 4));
   k.b_table = p->mtab ? sftk::B_TABLE : -1.0f;
+  k.b_table2 = p->mtab ? sftk::B_TABLE2 : -1.0f;
   k.Dp = p->Dp;
   k.ubp = p->ubp;
   k.us2 = p->us2;

@@ -16,12 +16,13 @@
 // the template: they are computed ONCE per data set (as the SFTs themselves are) for
 // every window position kc and TAB_R nodes per bin, q = 0..TAB_Q, and kept in HBM; a template then
 // needs 64 bytes and ~20 packed FMAs per (SFT, channel) instead of evaluating 2K+1 kernel coefficients.
-// Truncation error at TAB_R = 4, TAB_Q = 7: <= 1e-6 sqrt(sum |D|^2) for |b| <= B_TABLE = 0.12 (measured
-// 4e-7 at b = 0.12, 3e-8 at b = 0.056); larger |b| takes the direct evaluator of sft_kernels.cuh.
+// Truncation error at TAB_R = 4 (measured against fp64 quadrature, moments stored as complex64), relative to
+// sqrt(sum |D|^2):  tier 1, q <= 7:  4e-7 at |b| = 0.12 (3e-8 at 0.056);  tier 2, q <= 15:  2e-8 up to |b| = 0.5,
+// 2.4e-7 at |b| = 1.0 (7e-6 at 1.5).  |b| > B_TABLE2 = 1 takes the direct evaluator of sft_kernels.cuh.
 //
 // The <h,h> sum H(kc, xp, b) = sum_m u_{kc+m} |J_m|^2 (u = S_ref/S_k) does not depend on the data at
 // all; it is even in b and tabulated per window position on HTAB_R nodes per bin as
-//   H = sum_{P<=5} a^P (h_{P,0} + beta^2 h_{P,2})      (relative error < 3e-7 for |b| <= 0.12).
+//   H = sum_{P<=5} a^P sum_N beta^(2N) h_{P,2N}:  N <= 1: relative error < 3e-7 for |b| <= 0.12;  N <= 3: 9e-8 at |b| = 1.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -29,11 +30,14 @@
 namespace sftk {
 
 constexpr int TAB_R = 4;      // nodes per bin of the data-moment table
-constexpr int TAB_Q = 7;      // highest moment kept (TAB_Q + 1 complex64 = 64 bytes per node)
+constexpr int TAB_Q = 15;     // highest moment kept (TAB_Q + 1 complex64 = 128 bytes per node)
+constexpr int TAB_Q1 = 7;     // highest moment used by tier 1 (the first 64 bytes of a node)
 constexpr int HTAB_R = 16;    // nodes per bin of the <h,h> table
 constexpr int HTAB_P = 5;     // highest power of a kept
-constexpr int HTAB_W = 16;    // floats per node: h_{0..5,0}, h_{0..5,2}, 4 x pad
-constexpr float B_TABLE = 0.12f;
+constexpr int HTAB_NB = 4;    // powers of beta^2 kept: beta^0, beta^2, beta^4, beta^6 (tier 1 uses the first two)
+constexpr int HTAB_W = 32;    // floats per node: h_{0..5,0}, h_{0..5,2}, h_{0..5,4}, h_{0..5,6}, 8 x pad
+constexpr float B_TABLE = 0.12f;    // tier 1: moments q <= 7, H to beta^2
+constexpr float B_TABLE2 = 1.0f;    // tier 2: moments q <= 15, H to beta^6
 
 // sigma_q(a') with rho_q = sigma_q (q even), i sigma_q (q odd):  sigma_q = int v^q cos(w v) dv (q even), int v^q sin(w v) dv (q odd),
 // w = 2 pi a', over [-1/2, 1/2].  |a'| >= 1.5: integration by parts upwards in q (each step multiplies
@@ -112,16 +116,21 @@ __global__ void __launch_bounds__(256) sft_mtab_kernel(const float4 *Dp0, int np
 }
 
 // <h,h> table of one channel: htab[nodeH][HTAB_W], nodeH = kcidx * HTAB_R + cell.  One block per node,
-// threads over the 2K+1 bins; fp64.  With c_{p,n} = (-1)^m i^(p+n) rho_{p+2n} / (p! n!) the polynomial of
-// |J_m|^2 in (a, beta) has the coefficients  h_{P,N} = sum_{p+p'=P, n+n'=N} Re[c_{p,n} conj(c_{p',n'})].
+// threads over the 2K+1 bins; fp64.  rho_q = sigma_q (q even), i sigma_q (q odd), and p + 2n has the parity of
+// p, so the coefficient of a^p beta^n in J_m is  c_{p,n} = (-1)^m e_p i^n sigma_{p+2n} / (p! n!)  with the real
+// sign e_p = i^p (p odd ? i : 1) = (-1)^ceil(p/2); the polynomial of |J_m|^2 has the coefficients
+//   h_{P,2N} = sum_{p+p'=P} sum_{n+n'=2N} e_p e_p' (-1)^((n-n')/2) sigma_{p+2n} sigma_{p'+2n'} / (p! p'! n! n'!)
+// (odd powers of beta cancel: |J|^2 is even in b).
 __global__ void __launch_bounds__(64) sft_htab_kernel(const float2 *ub0, int K, float *htab) {
-  constexpr int NQ = HTAB_P + 5;        // rho_0 .. rho_{P+4}  (p <= 5, n <= 2)
-  __shared__ double red[2 * (HTAB_P + 1)];
+  constexpr int NMAX = 2 * (HTAB_NB - 1);         // highest single power of beta: 6
+  constexpr int NQ = HTAB_P + 2 * NMAX + 1;       // sigma_0 .. sigma_{P + 2 NMAX}
+  constexpr int NH = HTAB_NB * (HTAB_P + 1);
+  __shared__ double red[NH];
   const int node = blockIdx.x, kcidx = node / HTAB_R, cell = node - kcidx * HTAB_R;
-  if (threadIdx.x < 2 * (HTAB_P + 1)) red[threadIdx.x] = 0.0;
+  if (threadIdx.x < NH) red[threadIdx.x] = 0.0;
   __syncthreads();
   const double xj = ((double)cell + 0.5) / HTAB_R - 0.5;
-  const double fact[6] = {1.0, 1.0, 2.0, 6.0, 24.0, 120.0};
+  const double fact[7] = {1.0, 1.0, 2.0, 6.0, 24.0, 120.0, 720.0};
   for (int mi = threadIdx.x; mi <= 2 * K; mi += blockDim.x) {
     const int j = kcidx + 2 + mi;
     const float2 u2 = __ldg(ub0 + (j >> 1));
@@ -129,35 +138,26 @@ __global__ void __launch_bounds__(64) sft_htab_kernel(const float2 *ub0, int K, 
     if (u == 0.0) continue;
     double sig[NQ];
     sigma_moments<NQ>(xj - (double)(mi - K), sig);
-    // rho_q = sigma_q (q even), i sigma_q (q odd), and p + 2n has the parity of p:
-    // c_{p,n} = e_p i^n sigma_{p+2n} / (p! n!) with the real sign e_p = i^p (p odd ? i : 1) = (-1)^ceil(p/2).
-    double h0[HTAB_P + 1], h2[HTAB_P + 1];
-#pragma unroll
     for (int P = 0; P <= HTAB_P; ++P) {
-      double s0 = 0.0, s2 = 0.0;
-#pragma unroll
-      for (int p = 0; p <= P; ++p) {
-        const int pp = P - p;
-        const double sgn = ((((p + 1) >> 1) + ((pp + 1) >> 1)) & 1) ? -1.0 : 1.0;      // e_p e_p'
-        const double c00 = sig[p] / fact[p], d00 = sig[pp] / fact[pp];             // n = n' = 0
-        s0 += sgn * c00 * d00;
-        // N = 2: (n,n') = (1,1): i conj(i) = +1;  (2,0) and (0,2): i^2 = -1 each
-        const double c1 = sig[p + 2] / fact[p], d1 = sig[pp + 2] / fact[pp];
-        const double c2 = sig[p + 4] / (fact[p] * 2.0), d2 = sig[pp + 4] / (fact[pp] * 2.0);
-        s2 += sgn * (c1 * d1 - c2 * d00 - c00 * d2);
+      for (int N2 = 0; N2 < HTAB_NB; ++N2) {
+        double acc = 0.0;
+        for (int p = 0; p <= P; ++p) {
+          const int pp = P - p;
+          const double sgn_p = ((((p + 1) >> 1) + ((pp + 1) >> 1)) & 1) ? -1.0 : 1.0;      // e_p e_p'
+          for (int n = 0; n <= 2 * N2; ++n) {
+            const int nn = 2 * N2 - n;
+            if (n > NMAX || nn > NMAX) continue;
+            const int hd = n - nn;                                                        // even
+            const double sgn_n = ((hd / 2) & 1) ? -1.0 : 1.0;                             // (-1)^((n-n')/2)
+            acc += sgn_p * sgn_n * sig[p + 2 * n] * sig[pp + 2 * nn] / (fact[p] * fact[pp] * fact[n] * fact[nn]);
+          }
+        }
+        atomicAdd(&red[N2 * (HTAB_P + 1) + P], u * acc);
       }
-      h0[P] = s0;
-      h2[P] = s2;
-    }
-#pragma unroll
-    for (int P = 0; P <= HTAB_P; ++P) {
-      atomicAdd(&red[P], u * h0[P]);
-      atomicAdd(&red[HTAB_P + 1 + P], u * h2[P]);
     }
   }
   __syncthreads();
-  if (threadIdx.x < HTAB_W)
-    htab[(size_t)node * HTAB_W + threadIdx.x] = threadIdx.x < 2 * (HTAB_P + 1) ? (float)red[threadIdx.x] : 0.f;
+  if (threadIdx.x < HTAB_W) htab[(size_t)node * HTAB_W + threadIdx.x] = threadIdx.x < NH ? (float)red[threadIdx.x] : 0.f;
 }
 
 }  // namespace sftk

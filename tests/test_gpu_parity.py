@@ -334,7 +334,7 @@ def test_config2_full_size_sampled():
     assert np.all(np.isfinite(xh)) and np.all(hh > 0)
     assert xh[0] > 0.8 * hh[0] and abs(hh[0] - 900.0) < 0.1 * 900.0            # the injection: SNR 30
     assert xh[0] > 0.9 * xh.max()                                               # and (nearly) the best match of the bank
-    assert sum(paths.values()) == int((kc >= 0).sum()) and paths["table"] > paths["fresnel"] > 0
+    assert sum(paths.values()) == int((kc >= 0).sum()) and paths["table"] > paths["table2"] > paths["fresnel"] > 0 and paths["series3"] == 0
 
 
 def test_config3_full_size_sampled():
