@@ -13,7 +13,11 @@
 // (largest b, most expensive) first, so that no SM idles behind a tail of equal-sized blocks.  The
 // per-template constants are computed once per call by sft_tmpl_kernel.
 //
-// Inner loop.  The 2K+1 bins of a pair are processed two adjacent bins at a time with the packed
+// Evaluators.  For |b| = |fdot| T^2 <= 1 a template reads pre-contracted data moments from the tables of
+// sft_table.cuh (64 or 128 bytes and 19 or 71 packed FMAs per (SFT, channel)); otherwise, or when the plan
+// has no tables, the 2K+1 kernel coefficients are evaluated and contracted directly:
+//
+// Direct inner loop.  The 2K+1 bins of a pair are processed two adjacent bins at a time with the packed
 // fp32x2 instructions of sm_100 (FADD2/FMUL2/FFMA2: one issue slot, two lanes).  The store keeps
 // the whitened data "pair-planar", {re_j, re_j+1, im_j, im_j+1} per 16 bytes, in two copies (pairs
 // starting at even / odd bins), so that ONE aligned 128-bit load delivers both packed operands of a

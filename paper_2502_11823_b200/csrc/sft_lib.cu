@@ -739,29 +739,27 @@ SFT_API sft_status sft_measure_alu_peaks(int32_t device, double *out, int32_t n_
     const double mult = which == 1 ? 2.0 : (which == 4 ? 1.25 : 1.0);   // packed: 2 lanes; mix: 8 FFMA + 2 MUFU per 8
     res[which] = lane_ops * mult / (best * 1e-3) / 1e9;
   }
-  cudaEvent_t e0x = e0, e1x = e1;
-  float *d2 = d;
   // out[5]: instructions per clock and scheduler sustained on the moment-table kernel's instruction mix
   double mix_ipc = 0.0;
   {
     const int mblocks = prop.multiProcessorCount * 5;
     float best = 1e30f;
     for (int rep = 0; rep < 4; ++rep) {
-      cudaEventRecord(e0x, 0);
-      sftk::peak_mix_table_kernel<<<mblocks, 128>>>(d2, 1.0000001f, 1e-9f);
-      cudaEventRecord(e1x, 0);
-      if (cudaEventSynchronize(e1x) != cudaSuccess) break;
+      cudaEventRecord(e0, 0);
+      sftk::peak_mix_table_kernel<<<mblocks, 128>>>(d, 1.0000001f, 1e-9f);
+      cudaEventRecord(e1, 0);
+      if (cudaEventSynchronize(e1) != cudaSuccess) break;
       float ms = 0.f;
-      cudaEventElapsedTime(&ms, e0x, e1x);
+      cudaEventElapsedTime(&ms, e0, e1);
       if (rep > 0 && ms < best) best = ms;
     }
     const double warp_instr = (double)mblocks * 4 * sftk::MIXT_ITERS * sftk::MIXT_INSTR;
     const double sched_clocks = best * 1e-3 * (double)prop.clockRate * 1e3 * prop.multiProcessorCount * 4;
     mix_ipc = warp_instr / sched_clocks;
   }
-  cudaEventDestroy(e0x);
-  cudaEventDestroy(e1x);
-  cudaFree(d2);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d);
   for (int i = 0; i < n_out && i < 5; ++i) out[i] = res[i];
   if (n_out > 5) out[5] = mix_ipc;
   return SFT_OK;
