@@ -287,6 +287,20 @@ def test_errors_on_device(et_small):
     plan.close()
 
 
+def test_evaluator_selection_by_memory():
+    """SFT_EVAL_AUTO falls back to the direct evaluator when the moment tables would not fit in a quarter of the
+    free device memory; SFT_EVAL_TABLE reports SFT_ENOMEM instead."""
+    api = _api()
+    desc = dict(n_channels=1, n_sft=200000, t_sft=8.0, fs=2048.0, t0=0.0, k_lo=10, k_hi=4010, K=8, kernel="fresnel",
+                pn1=1, response="none", f_lo=0.0, f_hi=1e9, f_ref=10.0)           # tables: 411 GB
+    with pytest.raises(api.SftError) as ei:
+        api.Plan(dict(desc, evaluator="table"))
+    assert "SFT_ENOMEM" in str(ei.value)
+    api.Plan(dict(desc, evaluator="auto")).close()                                 # 12.9 GB store only: fine
+    with pytest.raises(api.SftError):
+        api.Plan(dict(desc, evaluator=7))
+
+
 def test_ended_and_degenerate_templates(et_small):
     """Templates whose t_c lies inside / before the data (inactive from some SFT on; all inactive)."""
     w = et_small
