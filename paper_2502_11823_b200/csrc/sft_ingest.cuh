@@ -34,23 +34,28 @@ __global__ void sft_twiddle_kernel(int n, float2 *W) {
 __device__ __forceinline__ int padi(int i) { return i + (i >> 4); }
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-// v * exp(-2 pi i q / 8), q = 0..3 (compile-time after unrolling)
-__device__ __forceinline__ float2 rot8(float2 v, int q) {
-  const float c = 0.70710678118654752f;
-  switch (q & 3) {
+// v * exp(-2 pi i q / 16), q = 0..7 (compile-time after unrolling)
+__device__ __forceinline__ float2 rot16(float2 v, int q) {
+  const float c2 = 0.70710678118654752f, c1 = 0.92387953251128674f, s1 = 0.38268343236508977f;
+  switch (q & 7) {
     case 0: return v;
-    case 1: return make_float2(c * (v.x + v.y), c * (v.y - v.x));
-    case 2: return make_float2(v.y, -v.x);
-    default: return make_float2(c * (v.y - v.x), -c * (v.x + v.y));
+    case 1: return make_float2(c1 * v.x + s1 * v.y, c1 * v.y - s1 * v.x);
+    case 2: return make_float2(c2 * (v.x + v.y), c2 * (v.y - v.x));
+    case 3: return make_float2(s1 * v.x + c1 * v.y, s1 * v.y - c1 * v.x);
+    case 4: return make_float2(v.y, -v.x);
+    case 5: return make_float2(c1 * v.y - s1 * v.x, -s1 * v.y - c1 * v.x);
+    case 6: return make_float2(c2 * (v.y - v.x), -c2 * (v.x + v.y));
+    default: return make_float2(s1 * v.y - c1 * v.x, -c1 * v.y - s1 * v.x);
   }
 }
 
 // R consecutive radix-2 DIF stages (half-blocks h, h/2, .., h >> (R-1)) on groups of 2^R points held in registers:
 // the group of `base` is {base + j hl}, hl = h >> (R-1), j < 2^R; stage s couples j and j + 2^(R-1-s).  The twiddle of
-// element j in stage s is exp(-2 pi i ((pos + j hl) mod hs) / 2 hs), hs = h >> s, i.e. w0^(2^s) times a multiple of an
-// eighth of a turn, with w0 = exp(-2 pi i pos / 2h) the only table look-up of the group.
-template <int R>
-__device__ __forceinline__ void dif_pass(float2 *z, const float2 *W, int m, int n, int h, int tid, int nthr) {
+// element j in stage s is exp(-2 pi i ((pos + j hl) mod hs) / 2 hs), hs = h >> s, i.e. w0^(2^s) times a multiple of a
+// sixteenth of a turn, with w0 = exp(-2 pi i pos / 2h) the only table look-up of the group.  GLOBAL: the points come
+// straight from the time series (z[j] = x[2j] + i x[2j+1], 16-byte loads) instead of shared memory (first pass).
+template <int R, bool GLOBAL>
+__device__ __forceinline__ void dif_pass(float2 *z, const double *seg, const float2 *W, int m, int n, int h, int tid, int nthr) {
   constexpr int G = 1 << R;
   const int hl = h >> (R - 1);
   const int tw = n / (2 * h);
@@ -59,7 +64,14 @@ __device__ __forceinline__ void dif_pass(float2 *z, const float2 *W, int m, int 
     const int base = ((g - pos) << R) + pos;          // groups tile blocks of 2h = hl * 2^R points
     float2 v[G];
 #pragma unroll
-    for (int j = 0; j < G; ++j) v[j] = z[padi(base + j * hl)];
+    for (int j = 0; j < G; ++j) {
+      if (GLOBAL) {
+        const double2 d = __ldcs((const double2 *)seg + (base + j * hl));
+        v[j] = make_float2((float)d.x, (float)d.y);
+      } else {
+        v[j] = z[padi(base + j * hl)];
+      }
+    }
     float2 wp = __ldg(W + pos * tw);                  // w0^(2^s)
 #pragma unroll
     for (int s = 0; s < R; ++s) {
@@ -70,8 +82,8 @@ __device__ __forceinline__ void dif_pass(float2 *z, const float2 *W, int m, int 
         const float2 u = v[j], w2 = v[j + hj];
         const float2 d = make_float2(u.x - w2.x, u.y - w2.y);
         v[j] = make_float2(u.x + w2.x, u.y + w2.y);
-        // ((j hl) mod hs) / (2 hs) = (j mod hj) / (2 hj) of a turn = (j mod hj) * (4 / hj) eighths
-        v[j + hj] = rot8(cmul(d, wp), (j % hj) * (4 / hj));
+        // ((j hl) mod hs) / (2 hs) = (j mod hj) / (2 hj) of a turn = (j mod hj) * (8 / hj) sixteenths
+        v[j + hj] = rot16(cmul(d, wp), (j % hj) * (8 / hj));
       }
       if (s + 1 < R) wp = cmul(wp, wp);
     }
@@ -86,22 +98,20 @@ __global__ void __launch_bounds__(256) sft_rfft_band_kernel(const double *x, int
   extern __shared__ float2 z[];
   const int m = n >> 1;
   const double *seg = x + (size_t)blockIdx.x * n;
-  // load + pack: z[j] = x[2j] + i x[2j+1]  (16-byte loads of two doubles)
-  for (int j = threadIdx.x; j < m; j += blockDim.x) {
-    const double2 v = __ldcs((const double2 *)seg + j);
-    z[padi(j)] = make_float2((float)v.x, (float)v.y);
-  }
-  __syncthreads();
-  // in-place radix-2 DIF network over m points, three consecutive stages at a time in registers (8 points per
-  // thread and pass), then the rest
+  // in-place radix-2 DIF network over m points, up to four consecutive stages at a time in registers.  The first pass
+  // reads the series from global memory (the only HBM traffic of the kernel) and leaves its output in shared memory.
   int h = m >> 1;                                    // half-block of the next stage
-  while (h >= 4) {
-    dif_pass<3>(z, W, m, n, h, threadIdx.x, blockDim.x);
-    h >>= 3;
+  int r = log2m;                                     // stages left
+  dif_pass<4, true>(z, seg, W, m, n, h, threadIdx.x, blockDim.x);       // log2m >= 5
+  h >>= 4; r -= 4;
+  __syncthreads();
+  while (r > 0) {
+    if (r == 4 || (r > 4 && r % 3 == 1)) { dif_pass<4, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 4; r -= 4; }
+    else if (r >= 3) { dif_pass<3, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 3; r -= 3; }
+    else if (r == 2) { dif_pass<2, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 2; r -= 2; }
+    else { dif_pass<1, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 1; r -= 1; }
     __syncthreads();
   }
-  if (h == 2) { dif_pass<2>(z, W, m, n, h, threadIdx.x, blockDim.x); __syncthreads(); }
-  else if (h == 1) { dif_pass<1>(z, W, m, n, h, threadIdx.x, blockDim.x); __syncthreads(); }
   // band bins from the bit-reversed m-point spectrum
   float2 *out = bins + (size_t)blockIdx.x * nb;
   const float fdt = (float)dt;
