@@ -295,10 +295,11 @@ def run_ours(args, rank, world, local_rank):
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32 (fp64 phase track + fp64 accumulators)", "data": "synthetic",
+        "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name, "templates_per_gpu": nT, "n_sft_slots": int(w.desc["n_sft"]),
                    "n_channels": int(w.desc["n_channels"]), "K": int(w.desc["K"]), "kernel": w.desc["kernel"],
                    "pn1": int(w.desc["pn1"]), "evaluator": args.evaluator,
+                   "arithmetic": "fp32 evaluators and contraction, fp64 phase/frequency track, fp64 accumulators",
                    "call": "sft_cumulative_snr" if cumulative else "sft_inner_products", "active_pairs_per_gpu": pairs, "bin_terms_per_gpu": pairs * (2 * w.desc["K"] + 1),
                    "parallelism": "templates sharded over %d GPU(s), data store replicated, no collective" % world,
                    "cache": "l2_flush_between_steps (256 MiB memset, outside the per-step events)"},

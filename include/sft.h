@@ -170,6 +170,13 @@ double sft_plan_last_kernel_ms(sft_plan *plan);
  * host pointer. */
 sft_status sft_plan_path_counts(sft_plan *plan, int64_t *out, int32_t n_out);
 
+/* SFT-length rule Eq.(33)-(34) P:244-248: the longest T_SFT for which the quadratic per-SFT phase model Eq.(17) is off by
+ * at most ~delta radians, T_SFT(delta) = (2 delta / max fddot)^(1/3), for this library's inspiral waveform (DESIGN W1) up to
+ * GW frequency f_max [Hz], where fddot = d^2 f/dt^2 is largest.  Host arithmetic only (no device needed).  *fddot_max
+ * (nullable) receives max fddot [Hz/s^2].  Paper's Table I (1.4+1.4 Msun to 10 Hz): delta = 1 -> 73 s. */
+sft_status sft_tsft_rule(double m_chirp, double eta, int32_t waveform, double f_max, double delta,
+                         double *t_sft, double *fddot_max);
+
 /* Tuning knob: SFTs per work unit along the time axis (0 = automatic).  Results do not depend on it
  * beyond fp64 summation order. */
 sft_status sft_plan_set_chunk(sft_plan *plan, int32_t sfts_per_unit);

@@ -46,7 +46,7 @@ class PlanDesc(C.Structure):
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
            "sft_plan_set_chunk", "sft_plan_path_counts", "sft_compute_sfts", "sft_ingest_timeseries",
-           "sft_last_error", "sft_version",
+           "sft_tsft_rule", "sft_last_error", "sft_version",
            "sft_measure_alu_peaks"]
 
 _lib = None
@@ -74,6 +74,8 @@ def load_library(path=None):
     lib.sft_plan_last_kernel_ms.restype = dbl
     lib.sft_plan_set_chunk.argtypes = [vp, i32]
     lib.sft_plan_path_counts.argtypes = [vp, C.POINTER(i64), i32]
+    lib.sft_tsft_rule.argtypes = [dbl, dbl, i32, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
+    lib.sft_tsft_rule.restype = i32
     lib.sft_compute_sfts.argtypes = [i32, vp, vp, i64, i32, dbl, i32, i32, vp, i32]
     lib.sft_ingest_timeseries.argtypes = [vp, i32, vp, i64, vp, vp, vp, i32]
     lib.sft_measure_alu_peaks.argtypes = [i32, C.POINTER(dbl), i32]
@@ -255,6 +257,16 @@ def plan_from_workload(w, device=0, stream=None, **override):
                        np.ascontiguousarray(w.psd_scale[c], dtype=np.float64),
                        np.ascontiguousarray(w.psd_shape[c], dtype=np.float64), resp)
     return plan
+
+
+def tsft_rule(m_chirp, eta, f_max, delta, pn1=1):
+    """``sft_tsft_rule``: (T_SFT [s], max fddot [Hz/s^2]) of Eq.(34) for this library's waveform.  No GPU needed."""
+    lib = load_library()
+    t, fdd = C.c_double(), C.c_double()
+    st = lib.sft_tsft_rule(float(m_chirp), float(eta), int(pn1), float(f_max), float(delta), C.byref(t), C.byref(fdd))
+    if st != 0:
+        raise SftError(st, lib.sft_last_error(None).decode())
+    return t.value, fdd.value
 
 
 def compute_sfts(x, n_sft, n, dt, k_lo, k_hi, bins, device=0, stream=None):

@@ -247,6 +247,38 @@ SFT_API sft_status sft_plan_path_counts(sft_plan *p, int64_t *out, int32_t n_out
   return SFT_OK;
 }
 
+// SFT-length rule, Eq.(33)-(34) P:244-248 (host arithmetic only).
+SFT_API sft_status sft_tsft_rule(double m_chirp, double eta, int32_t waveform, double f_max, double delta, double *t_sft,
+                                 double *fddot_max) {
+  g_create_err[0] = 0;
+  if (!t_sft) return fail(nullptr, SFT_EINVAL, "sft_tsft_rule: t_sft is NULL");
+  if (!(m_chirp > 0.0) || !(eta > 0.0) || !(eta <= 0.25) || !(f_max > 0.0) || !(delta > 0.0))
+    return fail(nullptr, SFT_EINVAL, "sft_tsft_rule: need m_chirp, f_max, delta > 0 and 0 < eta <= 1/4");
+  if (waveform != SFT_WF_PN0 && waveform != SFT_WF_PN1) return fail(nullptr, SFT_EINVAL, "unknown waveform %d", waveform);
+  const double PI = 3.141592653589793;
+  const double M = m_chirp * pow(eta, -0.6) * sftk::GMSUN_S;
+  const double cf = waveform == SFT_WF_PN1 ? 743.0 / 2688.0 + 11.0 / 32.0 * eta : 0.0;
+  // Theta at which f(Theta) = Theta^(-3/8) (1 + cf Theta^(-1/4)) / (8 pi M) reaches f_max: f falls monotonically with Theta;
+  // start from the 0PN root (where the 1PN f is higher, i.e. the root lies at larger Theta) and use Newton's method in
+  // u = Theta^(-1/8):  g(u) = u^3 (1 + cf u^2) - 8 pi M f_max
+  const double target = 8.0 * PI * M * f_max;
+  double u = cbrt(target);
+  for (int it = 0; it < 60; ++it) {
+    const double g = u * u * u * (1.0 + cf * u * u) - target, dg = 3.0 * u * u + 5.0 * cf * u * u * u * u;
+    const double un = u - g / dg;
+    if (fabs(un - u) <= 1e-15 * fabs(u)) { u = un; break; }
+    u = un;
+  }
+  if (!(u > 0.0) || !isfinite(u)) return fail(nullptr, SFT_EINVAL, "sft_tsft_rule: no root for f_max = %g", f_max);
+  // d^2 f / dt^2 = k^2/(8 pi M) [ (3/8)(11/8) Theta^(-19/8) + (5/8)(13/8) cf Theta^(-21/8) ],  k = eta/(5M), Theta^(-1/8) = u
+  const double k = eta / (5.0 * M);
+  const double u19 = pow(u, 19.0), u21 = u19 * u * u;
+  const double fdd = k * k / (8.0 * PI * M) * (0.375 * 1.375 * u19 + 0.625 * 1.625 * cf * u21);
+  if (fddot_max) *fddot_max = fdd;
+  *t_sft = cbrt(2.0 * delta / fdd);
+  return SFT_OK;
+}
+
 SFT_API sft_status sft_plan_set_chunk(sft_plan *p, int32_t c) {
   if (!p) return SFT_EINVAL;
   if (c < 0) return fail(p, SFT_EINVAL, "sfts_per_block must be >= 0");

@@ -101,3 +101,27 @@ def test_binding_rejects_wrong_dtypes(lib):
         api._ptr(np.zeros(4, np.float64), np.float64, (5,), "x")
     with pytest.raises(TypeError):
         api._ptr(np.zeros((4, 4), np.float64)[:, ::2], np.float64, None, "x")
+
+
+def test_tsft_rule_against_the_papers_tables():
+    """sft_tsft_rule (host arithmetic, no device): Eq.(34) P:248 reproduces the paper's printed Table I within 2 % with this
+    library's PN waveform (the paper uses IMRPhenomT), max fddot ~ 5e-6 Hz/s^2, the delta^(1/3) law of Table II
+    exactly, and Table II itself within 6 % at 0PN (the 1PN expansion is poor that close to MECO)."""
+    import json
+    import os
+    from paper_2502_11823_b200 import api
+    g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.json")))
+    eta, mc = 0.25, 2.8 * 0.25 ** 0.6
+    for pn1 in (0, 1):
+        for d, T in zip(g["table1"]["delta"], g["table1"]["t_sft"]):
+            t, fdd = api.tsft_rule(mc, eta, 10.0, d, pn1)
+            assert abs(t - T) <= 0.02 * T, (pn1, d, t, T)
+            assert abs(fdd - g["bns"]["max_fddot_printed"]) <= 0.05 * g["bns"]["max_fddot_printed"]
+    mc2 = 2e6 * 0.25 ** 0.6
+    ts = [api.tsft_rule(mc2, eta, 1.9e-3, d, 0)[0] for d in g["table2"]["delta"]]
+    for d, t, T in zip(g["table2"]["delta"], ts, g["table2"]["t_sft"]):
+        assert abs(t - T) <= 0.06 * T, (d, t, T)
+        assert abs(t / ts[0] - (d / g["table2"]["delta"][0]) ** (1.0 / 3.0)) < 1e-12
+    import pytest
+    with pytest.raises(api.SftError):
+        api.tsft_rule(mc, 0.3, 10.0, 1.0)
