@@ -150,6 +150,13 @@ sft_status sft_inner_products(sft_plan *plan, int64_t n_templates, const double 
 sft_status sft_cumulative_snr(sft_plan *plan, int64_t n_templates, const double *params,
                               float *snr, float *cum_xh, float *cum_hh, int32_t mem);
 
+/* Statistics on top of sft_inner_products' outputs (all arrays [n_templates] doubles, `mem` as above):
+ *   loglike         L = <x,h> - <h,h>/2                                   (Eq.(2)), nullable
+ *   rho2_phase_max  (<x,h_c>^2 + <x,h_s>^2) / <h_c,h_c> = (xh^2 + xh_im^2) / hh, the detection statistic maximised
+ *                   over distance and initial phase (Eq.(7)-(9) P:97-101; 0 where hh == 0), nullable */
+sft_status sft_statistics(sft_plan *plan, int64_t n_templates, const double *xh, const double *xh_im,
+                          const double *hh, double *loglike, double *rho2_phase_max, int32_t mem);
+
 /* Blocks until all work enqueued on the plan's stream has finished. */
 sft_status sft_plan_sync(sft_plan *plan);
 

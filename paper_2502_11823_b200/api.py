@@ -46,7 +46,7 @@ class PlanDesc(C.Structure):
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
            "sft_plan_set_chunk", "sft_plan_path_counts", "sft_compute_sfts", "sft_ingest_timeseries",
-           "sft_tsft_rule", "sft_last_error", "sft_version",
+           "sft_tsft_rule", "sft_statistics", "sft_last_error", "sft_version",
            "sft_measure_alu_peaks"]
 
 _lib = None
@@ -74,6 +74,8 @@ def load_library(path=None):
     lib.sft_plan_last_kernel_ms.restype = dbl
     lib.sft_plan_set_chunk.argtypes = [vp, i32]
     lib.sft_plan_path_counts.argtypes = [vp, C.POINTER(i64), i32]
+    lib.sft_statistics.argtypes = [vp, i64, vp, vp, vp, vp, vp, i32]
+    lib.sft_statistics.restype = i32
     lib.sft_tsft_rule.argtypes = [dbl, dbl, i32, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
     lib.sft_tsft_rule.restype = i32
     lib.sft_compute_sfts.argtypes = [i32, vp, vp, i64, i32, dbl, i32, i32, vp, i32]
@@ -226,6 +228,15 @@ class Plan:
             self._h, nT, _ptr(params, np.float64, (nT, NPARAM), "params"),
             _ptr(snr, np.float32, shp, "snr"), _ptr(cum_xh, np.float32, shp, "cum_xh"),
             _ptr(cum_hh, np.float32, shp, "cum_hh"), mem))
+
+    def statistics(self, xh, xh_im, hh, loglike=None, rho2_phase_max=None):
+        """``sft_statistics``: log-likelihood and phase-maximised statistic from the inner products."""
+        nT = int(xh.shape[0])
+        mem = _where([xh, xh_im, hh, loglike, rho2_phase_max])
+        self._check(self.lib.sft_statistics(
+            self._h, nT, _ptr(xh, np.float64, (nT,), "xh"), _ptr(xh_im, np.float64, (nT,), "xh_im"),
+            _ptr(hh, np.float64, (nT,), "hh"), _ptr(loglike, np.float64, (nT,), "loglike"),
+            _ptr(rho2_phase_max, np.float64, (nT,), "rho2_phase_max"), mem))
 
     def sync(self):
         self._check(self.lib.sft_plan_sync(self._h))

@@ -1007,6 +1007,18 @@ __global__ void __launch_bounds__(32 * RED_SLICES) sft_reduce_kernel(const doubl
   }
 }
 
+// Statistics on top of the inner products: log-likelihood L = <x,h> - <h,h>/2 (Eq.(2)) and the
+// statistic maximised over distance and initial phase, (<x,h_c>^2 + <x,h_s>^2) / <h_c,h_c> (Eq.(7)-(9) P:97-101): shifting
+// phi_c by pi/2 turns the complex sum Z into iZ, so <x,h_c> = Re Z = xh, <x,h_s> = -Im Z, and <h_c,h_c> = <h_s,h_s> = hh.
+__global__ void sft_statistics_kernel(long long n, const double *xh, const double *xi, const double *hh, double *loglike,
+                                      double *rho2max) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const double a = xh[t], b = xi[t], h = hh[t];
+  if (loglike) loglike[t] = a - 0.5 * h;
+  if (rho2max) rho2max[t] = h > 0.0 ? (a * a + b * b) / h : 0.0;
+}
+
 // Exclusive scan of the chunk totals along the chunk axis, in place, fp64 (the carries).
 __global__ void sft_scan_chunks_kernel(double *part, long long nT, int n_chunks) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;

@@ -681,6 +681,43 @@ SFT_API sft_status sft_inner_products(sft_plan *p, int64_t nT, const double *par
   return SFT_OK;
 }
 
+SFT_API sft_status sft_statistics(sft_plan *p, int64_t nT, const double *xh, const double *xh_im, const double *hh,
+                                  double *loglike, double *rho2_phase_max, int32_t mem) {
+  if (!p) return SFT_EINVAL;
+  p->err[0] = 0;
+  if (nT < 0) return fail(p, SFT_EINVAL, "n_templates < 0");
+  if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(p, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
+  if (nT == 0) return SFT_OK;
+  if (!xh || !xh_im || !hh) return fail(p, SFT_EINVAL, "xh, xh_im and hh are required");
+  if (!loglike && !rho2_phase_max) return fail(p, SFT_EINVAL, "at least one of loglike, rho2_phase_max must be non-NULL");
+  CU(p, cudaSetDevice(p->d.device));
+  const size_t b = (size_t)nT * sizeof(double);
+  const double *d_xh = xh, *d_xi = xh_im, *d_hh = hh;
+  double *d_l = loglike, *d_r = rho2_phase_max;
+  if (mem == SFT_MEM_HOST) {
+    sft_status st = grow(p, &p->d_out, &p->out_bytes, 5 * b);
+    if (st != SFT_OK) return st;
+    double *q = (double *)p->d_out;
+    CU(p, cudaMemcpyAsync(q, xh, b, cudaMemcpyHostToDevice, p->stream));
+    CU(p, cudaMemcpyAsync(q + nT, xh_im, b, cudaMemcpyHostToDevice, p->stream));
+    CU(p, cudaMemcpyAsync(q + 2 * nT, hh, b, cudaMemcpyHostToDevice, p->stream));
+    d_xh = q; d_xi = q + nT; d_hh = q + 2 * nT;
+    d_l = loglike ? q + 3 * nT : nullptr;
+    d_r = rho2_phase_max ? q + 4 * nT : nullptr;
+  }
+  sftk::sft_statistics_kernel<<<(unsigned)((nT + 255) / 256), 256, 0, p->stream>>>(nT, d_xh, d_xi, d_hh, d_l, d_r);
+  p->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "statistics kernel launch: %s", cudaGetErrorString(e));
+  if (mem == SFT_MEM_HOST) {
+    CU(p, cudaStreamSynchronize(p->stream));
+    if (loglike) CU(p, cudaMemcpyAsync(loglike, d_l, b, cudaMemcpyDeviceToHost, p->stream));
+    if (rho2_phase_max) CU(p, cudaMemcpyAsync(rho2_phase_max, d_r, b, cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
+  }
+  return SFT_OK;
+}
+
 SFT_API sft_status sft_cumulative_snr(sft_plan *p, int64_t nT, const double *params, float *snr, float *cum_xh,
                                          float *cum_hh, int32_t mem) {
   if (!p) return SFT_EINVAL;

@@ -213,6 +213,28 @@ def test_three_and_four_channels(C):
     assert (np.abs(cx - oc["cum_xh"]) / norm).max() <= TOL and (np.abs(ch - oc["cum_hh"]) / norm).max() <= TOL
 
 
+def test_statistics_phase_maximised(et_small):
+    """sft_statistics (NEXT-3): L = <x,h> - <h,h>/2 (Eq.(2)) and the phase-maximised statistic of Eq.(7) P:97,
+    checked against the oracle's inner products of the two quadratures h_c (phi_c) and h_s (phi_c + pi/2)."""
+    api = _api()
+    w = et_small
+    P = np.ascontiguousarray(w.params[:48])
+    Ps = P.copy()
+    Ps[:, 3] += 0.5 * np.pi
+    oc, xx, _, _ = _oracle(w, params=P)
+    os_, _, _, _ = _oracle(w, params=Ps)
+    stat_o = (oc["xh"] ** 2 + os_["xh"] ** 2) / oc["hh"]
+    with api.plan_from_workload(w) as plan:
+        xh, hh, xi = np.empty(48), np.empty(48), np.empty(48)
+        plan.inner_products(P, xh, hh, xi, None)
+        L, stat = np.empty(48), np.empty(48)
+        plan.statistics(xh, xi, hh, L, stat)
+    assert np.allclose(L, xh - 0.5 * hh, rtol=0, atol=1e-12 * np.abs(xh).max())
+    tol = 2.0 * 1e-4 * np.sqrt(xx * oc["hh"]) * np.sqrt(oc["xh"] ** 2 + os_["xh"] ** 2) / oc["hh"] + 1e-4 * stat_o
+    assert np.all(np.abs(stat - stat_o) <= tol), np.abs(stat - stat_o).max()
+    assert np.abs(stat - stat_o).max() <= 1e-3 * stat_o.max()
+
+
 def test_response_table():
     """SFT_RESP_TABLE: an arbitrary complex per-(channel, SFT) response."""
     w = wl.config4(n_templates=40)
