@@ -683,14 +683,20 @@ __device__ __forceinline__ float2 cstep(float2 X, float s, float2 Y) {
 // of sft_table.cuh (true J, no 2 pi).  `kcidx` = k_c - (k_lo - K), already clamped to the table;
 // `Mrow` = row of SFT alpha, channel 0.  TIER 1: moments q <= 7, H to beta^2 (|b| <= B_TABLE); TIER 2: q <= 15,
 // H to beta^6 (|b| <= B_TABLE2).  Also evaluates the track of the next SFT (see series_pairs).
-template <int CT, class CFG, int TIER>
-__device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, double dnext, Track &nxt, float xp, float b,
-                                           int kcidx, const float4 *Mrow, float (&s1r)[CT], float (&s1i)[CT],
-                                           float (&s2)[CT]) {
-  constexpr int Q = TIER == 1 ? TAB_Q1 : TAB_Q;          // highest moment
-  constexpr int NL = (Q + 1) / 2;                         // float4 loads of moments per channel
-  constexpr int NHB = TIER == 1 ? 2 : HTAB_NB;            // powers of beta^2 in H
-  constexpr int NHL = (NHB * (HTAB_P + 1) + 3) / 4;       // float4 loads of H coefficients
+template <int CT, int TIER>
+struct TableData {
+  static constexpr int Q = TIER == 1 ? TAB_Q1 : TAB_Q;          // highest moment
+  static constexpr int NL = (Q + 1) / 2;                         // float4 loads of moments per channel
+  static constexpr int NHB = TIER == 1 ? 2 : HTAB_NB;            // powers of beta^2 in H
+  static constexpr int NHL = (NHB * (HTAB_P + 1) + 3) / 4;       // float4 loads of H coefficients
+  float4 Mq[CT][NL], Hq[CT][NHL];
+  float a, aH, be;
+};
+
+// node look-up and loads
+template <int CT, int TIER>
+__device__ __forceinline__ void table_load(const KParams &p, float xp, float b, int kcidx, const float4 *Mrow,
+                                           TableData<CT, TIER> &d) {
   // node of the <h,h> table: cellH = floor((xp + 1/2) HTAB_R) by the 1.5 * 2^23 rounding trick, clamped (xp = 1/2
   // exactly, NaN lanes); the data-moment node is cellH / 4 (HTAB_R = 4 TAB_R)
   static_assert(HTAB_R == 4 * TAB_R, "node grids");
@@ -702,19 +708,24 @@ __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, dou
   const float cHf = cm - RM;                                   // (float)cellH
   const float4 *mp = Mrow + (unsigned)(kcidx * TAB_R + cell) * (unsigned)((TAB_Q + 1) / 2);
   const float4 *hp = p.htab + (unsigned)(kcidx * HTAB_R + cellH) * (unsigned)(HTAB_W / 4);
-  float4 Mq[CT][NL], Hq[CT][NHL];
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
 #pragma unroll
-    for (int i = 0; i < NL; ++i) Mq[c][i] = __ldg(mp + c * p.mchan + i);
+    for (int i = 0; i < TableData<CT, TIER>::NL; ++i) d.Mq[c][i] = __ldg(mp + c * p.mchan + i);
 #pragma unroll
-    for (int i = 0; i < NHL; ++i) Hq[c][i] = __ldg(hp + c * p.hchan + i);
+    for (int i = 0; i < TableData<CT, TIER>::NHL; ++i) d.Hq[c][i] = __ldg(hp + c * p.hchan + i);
   }
-  track_eval<CFG>(p, tm, dnext, nxt);
   // a = 2 pi (xp - node centre):  centre_H = (cellH + 1/2)/HTAB_R - 1/2,  centre_M = (cell + 1/2)/TAB_R - 1/2
-  const float aH = fmaf(cHf, -(2.0f * PI_F) / HTAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / HTAB_R)));
-  const float a = fmaf((float)cell, -(2.0f * PI_F) / TAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / TAB_R)));
-  const float be = PI_F * b;
+  d.aH = fmaf(cHf, -(2.0f * PI_F) / HTAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / HTAB_R)));
+  d.a = fmaf((float)cell, -(2.0f * PI_F) / TAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / TAB_R)));
+  d.be = PI_F * b;
+}
+
+// the two Horner evaluations
+template <int CT, int TIER>
+__device__ __forceinline__ void table_math(const TableData<CT, TIER> &d, float (&s1r)[CT], float (&s1i)[CT], float (&s2)[CT]) {
+  constexpr int Q = TableData<CT, TIER>::Q, NHB = TableData<CT, TIER>::NHB;
+  const float a = d.a, aH = d.aH, be = d.be;
   float nb_[Q / 2 + 1], na_[Q + 1];                       // beta / k, a / k
 #pragma unroll
   for (int k = 1; k <= Q / 2; ++k) nb_[k] = be * (1.0f / (float)k);
@@ -726,7 +737,7 @@ __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, dou
     float2 M[Q + 1];
 #pragma unroll
     for (int q = 0; q <= Q; ++q)
-      M[q] = (q & 1) ? make_float2(Mq[c][q >> 1].z, Mq[c][q >> 1].w) : make_float2(Mq[c][q >> 1].x, Mq[c][q >> 1].y);
+      M[q] = (q & 1) ? make_float2(d.Mq[c][q >> 1].z, d.Mq[c][q >> 1].w) : make_float2(d.Mq[c][q >> 1].x, d.Mq[c][q >> 1].y);
     // S1 = sum_p (i a)^p / p! L_p,  L_p = sum_n (i beta)^n / n! M_{p+2n}: both by Horner, one packed FMA per step
     float2 S = make_float2(0.f, 0.f);
 #pragma unroll
@@ -740,7 +751,7 @@ __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, dou
     s1r[c] = S.x;
     s1i[c] = S.y;
     // H = sum_P aH^P sum_N beta^(2N) h_{P,2N};  floats: [N][P], P fastest
-    const float *hf = (const float *)&Hq[c][0];
+    const float *hf = (const float *)&d.Hq[c][0];
     float h = 0.f;
 #pragma unroll
     for (int P = HTAB_P; P >= 0; --P) {
@@ -751,6 +762,87 @@ __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, dou
     }
     s2[c] = h;
   }
+}
+
+template <int CT, class CFG, int TIER>
+__device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, double dnext, Track &nxt, float xp, float b,
+                                           int kcidx, const float4 *Mrow, float (&s1r)[CT], float (&s1i)[CT],
+                                           float (&s2)[CT]) {
+  TableData<CT, TIER> d;
+  table_load<CT, TIER>(p, xp, b, kcidx, Mrow, d);
+  track_eval<CFG>(p, tm, dnext, nxt);
+  table_math<CT, TIER>(d, s1r, s1i, s2);
+}
+
+// Phase, amplitude, response and noise weight applied to the contracted sums of one (template, SFT).
+template <int CT, class CFG>
+__device__ __forceinline__ void finish_terms(const KParams &p, const Tmpl &tm, const float2 *rt, const Track &tr, bool ok,
+                                             float scale, float t, const float (&s1r)[CT], const float (&s1i)[CT],
+                                             const float (&s2)[CT], const float (&us2)[CT], float &zr, float &zi, float &hh) {
+  // |t| <= 1 + 1/2 + |b|/4: the MUFU sin/cos argument reduction (x/2pi rounded to fp32) stays below 3e-7 rad
+  float sp, cp_;
+  sincospi_fast(t, sp, cp_);
+  const float as = scale * tr.amp;
+  const float er = cp_ * as, ei = sp * as;
+  const float a2 = as * tr.amp;
+  const int resp = cfg_resp<CFG>(p);
+  float sr = 0.f, si = 0.f, sh = 0.f;
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+    // response (Eq.(5)-(6) P:80-85 as Lambda z = Re[R z]; DESIGN C3/D4)
+    float2 R = tm.AE[c];
+    if (resp == 1) {
+      const float2 r = __ldg(rt + c * p.n_sft);
+      R = make_float2(tm.AE[c].x * r.x, tm.AE[c].x * r.y);      // AE is real here
+    } else if (resp == 2) {
+      const float2 cs = __ldg(rt + c * p.n_sft);
+      const float am = fmaf(p.depth, cs.x * tm.cl - cs.y * tm.sl, 1.0f);
+      R = make_float2(R.x * am, R.y * am);
+    }
+    float gr, gi, r2;
+    if (resp == 0) {                   // AE is real
+      gr = R.x * er; gi = R.x * ei; r2 = R.x * R.x;
+    } else {
+      gr = R.x * er - R.y * ei; gi = R.x * ei + R.y * er; r2 = R.x * R.x + R.y * R.y;   // p_c = R * A e^{i phi} pref
+    }
+    const float cr = gr * s1r[c] - gi * s1i[c], ci = gr * s1i[c] + gi * s1r[c];
+    const float chh = r2 * a2 * us2[c] * s2[c];
+    if (CT == 1) {
+      sr = cr; si = ci; sh = chh;
+    } else {
+      const bool present = us2[c] > 0.f;               // gaps hold zeros in the store, but guard 0 * garbage
+      sr += present ? cr : 0.f;
+      si += present ? ci : 0.f;
+      sh += present ? chh : 0.f;
+    }
+  }
+  zr = ok ? sr : 0.f;
+  zi = ok ? si : 0.f;
+  hh = ok ? sh : 0.f;
+}
+
+// Two consecutive SFTs (A = alpha, B = alpha + 1) of one template through the tier-1 moment tables at once: twice the
+// independent work in one straight-line block (the fp64 tracks of alpha + 2 and alpha + 3 included), so that the
+// fixed-latency dependency chains of one fill the issue gaps of the other.
+template <int CT, class CFG>
+__device__ __forceinline__ void duo_terms(const KParams &p, const Tmpl &tm, const float4 *Mrow0, const float2 *rt,
+                                          const Track &trA, const Track &trB, bool goA, bool goB, const float (&usA)[CT],
+                                          const float (&usB)[CT], double dnext, Track &nA, Track &nB, float &zrA, float &ziA,
+                                          float &hhA, float &zrB, float &ziB, float &hhB) {
+  const int j0A = trA.kc - p.kwin0, j0B = trB.kc - p.kwin0;
+  const bool okA = goA && (unsigned)(j0A - 2) <= (unsigned)p.jmax, okB = goB && (unsigned)(j0B - 2) <= (unsigned)p.jmax;
+  const bool fres = (cfg_kernel<CFG>(p) == 1);
+  const float bA = fres ? trA.b : 0.f, bB = fres ? trB.b : 0.f;
+  TableData<CT, 1> dA, dB;
+  table_load<CT, 1>(p, fmaf(0.5f, bA, trA.x), bA, okA ? j0A - 2 : 0, Mrow0, dA);
+  table_load<CT, 1>(p, fmaf(0.5f, bB, trB.x), bB, okB ? j0B - 2 : 0, Mrow0 + p.mrow, dB);
+  track_eval<CFG>(p, tm, dnext, nA);
+  track_eval<CFG>(p, tm, dnext + 1.0, nB);
+  float s1rA[CT], s1iA[CT], s2A[CT], s1rB[CT], s1iB[CT], s2B[CT];
+  table_math<CT, 1>(dA, s1rA, s1iA, s2A);
+  table_math<CT, 1>(dB, s1rB, s1iB, s2B);
+  finish_terms<CT, CFG>(p, tm, rt, trA, okA, 1.0f, fmaf(2.0f, trA.frac, fmaf(0.25f, bA, trA.x)), s1rA, s1iA, s2A, usA, zrA, ziA, hhA);
+  finish_terms<CT, CFG>(p, tm, rt + 1, trB, okB, 1.0f, fmaf(2.0f, trB.frac, fmaf(0.25f, bB, trB.x)), s1rB, s1iB, s2B, usB, zrB, ziB, hhB);
 }
 
 // Z_c = Re/Im of the per-(SFT, channel) complex term, H_c its <h,h> term (include/sft.h).
@@ -816,46 +908,7 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, con
       s2[c] = scale * (acc[c].W.x + acc[c].W.y);             // one of the two factors `scale` of |J|^2
     }
   }
-  // |t| <= 1 + 1/2 + |b|/4: the MUFU sin/cos argument reduction (x/2pi rounded to fp32) stays below 3e-7 rad
-  float sp, cp_;
-  sincospi_fast(t, sp, cp_);
-  const float as = scale * tr.amp;
-  const float er = cp_ * as, ei = sp * as;
-  const float a2 = as * tr.amp;
-  const int resp = cfg_resp<CFG>(p);
-  float sr = 0.f, si = 0.f, sh = 0.f;
-#pragma unroll
-  for (int c = 0; c < CT; ++c) {
-    // response (Eq.(5)-(6) P:80-85 as Lambda z = Re[R z]; DESIGN C3/D4)
-    float2 R = tm.AE[c];
-    if (resp == 1) {
-      const float2 r = __ldg(rt + c * p.n_sft);
-      R = make_float2(tm.AE[c].x * r.x, tm.AE[c].x * r.y);      // AE is real here
-    } else if (resp == 2) {
-      const float2 cs = __ldg(rt + c * p.n_sft);
-      const float am = fmaf(p.depth, cs.x * tm.cl - cs.y * tm.sl, 1.0f);
-      R = make_float2(R.x * am, R.y * am);
-    }
-    float gr, gi, r2;
-    if (resp == 0) {                   // AE is real
-      gr = R.x * er; gi = R.x * ei; r2 = R.x * R.x;
-    } else {
-      gr = R.x * er - R.y * ei; gi = R.x * ei + R.y * er; r2 = R.x * R.x + R.y * R.y;   // p_c = R * A e^{i phi} pref
-    }
-    const float cr = gr * s1r[c] - gi * s1i[c], ci = gr * s1i[c] + gi * s1r[c];
-    const float chh = r2 * a2 * us2[c] * s2[c];
-    if (CT == 1) {
-      sr = cr; si = ci; sh = chh;
-    } else {
-      const bool present = us2[c] > 0.f;               // gaps hold zeros in the store, but guard 0 * garbage
-      sr += present ? cr : 0.f;
-      si += present ? ci : 0.f;
-      sh += present ? chh : 0.f;
-    }
-  }
-  zr = ok ? sr : 0.f;
-  zi = ok ? si : 0.f;
-  hh = ok ? sh : 0.f;
+  finish_terms<CT, CFG>(p, tm, rt, tr, ok, scale, t, s1r, s1i, s2, us2, zr, zi, hh);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -866,7 +919,7 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, con
 // The SFT loop runs in groups of GROUP: fp32 partial sums flushed into fp64 per group (MODE 0),
 // one transposed store per group (MODE 1).
 // ---------------------------------------------------------------------------------------------
-template <int KT, int CT, int MODE, class CFG, int MINB>
+template <int KT, int CT, int MODE, class CFG, int MINB, bool DUO>
 __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
   constexpr int GROUP = MODE == 1 ? 32 : FLUSH;
   __shared__ float tile_s[MODE == 1 ? (TILE / 32) * 2 * 32 * 33 : 1];
@@ -895,25 +948,75 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
     const float4 *Mrow0 = p.mtab ? p.mtab + (size_t)a0 * p.mrow : nullptr;
     int *kcp = want_kc ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + a0 : nullptr;
     unsigned long long n_path[PATH_N] = {0, 0, 0, 0, 0, 0, 0};
-    Track tr;
+    Track tr, tr2;                                   // tracks of SFT alpha and alpha + 1
     track_eval<CFG>(p, tm, dalpha, tr);
+    track_eval<CFG>(p, tm, dalpha + 1.0, tr2);
 
     for (int g = a0; g < a1; g += GROUP) {
       const int ge = min(g + GROUP, a1);
       float fxh = 0.f, fhh = 0.f, fxi = 0.f;
-      for (int alpha = g; alpha < ge; ++alpha, ++usp, ++rt, Drow0 += p.npair, Mrow0 += p.mrow) {
-        float us2[CT];
-        bool any = false;
+      int alpha = g;
+      while (alpha < ge) {
+        float us2[CT], us2b[CT];
+        bool any = false, anyb = false;
 #pragma unroll
         for (int c = 0; c < CT; ++c) {
           us2[c] = __ldg(usp + c * p.n_sft);
           any |= us2[c] > 0.f;                                   // warp-uniform
         }
-        dalpha += 1.0;
         const bool go = any && tr.active;
-        Track nxt;
+        const float ab = (go && cfg_kernel<CFG>(p) == 1) ? fabsf(tr.b) : 0.f;
+        // two SFTs at once when both are present and both go through the tier-1 tables
+        bool duo = false, gob = false;
+        if (DUO && alpha + 1 < ge) {
+#pragma unroll
+          for (int c = 0; c < CT; ++c) {
+            us2b[c] = __ldg(usp + c * p.n_sft + 1);
+            anyb |= us2b[c] > 0.f;
+          }
+          gob = anyb && tr2.active;
+          const float abb = (gob && cfg_kernel<CFG>(p) == 1) ? fabsf(tr2.b) : 0.f;
+          const float bm2 = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(ab, abb))));
+          duo = bm2 <= p.b_table && __any_sync(0xffffffffu, go) && __any_sync(0xffffffffu, gob);
+        }
+        if (duo) {
+          Track nA, nB;
+          float zrA, ziA, hhA, zrB, ziB, hhB;
+          duo_terms<CT, CFG>(p, tm, Mrow0, rt, tr, tr2, go, gob, us2, us2b, dalpha + 2.0, nA, nB, zrA, ziA, hhA, zrB, ziB, hhB);
+          if (CFG::KC && p.path_counts) {
+            int npa = 0, npb = 0;
+#pragma unroll
+            for (int c = 0; c < CT; ++c) { npa += us2[c] > 0.f; npb += us2b[c] > 0.f; }
+            n_path[PATH_TABLE] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * npa + __popc(__ballot_sync(0xffffffffu, gob)) * npb);
+          }
+          if (CFG::KC && want_kc) {
+            if (t < p.nT) {
+#pragma unroll
+              for (int c = 0; c < CT; ++c) {
+                kcp[(size_t)c * p.n_sft] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
+                kcp[(size_t)c * p.n_sft + 1] = (tr2.active && us2b[c] > 0.f) ? tr2.kc : -1;
+              }
+            }
+            kcp += 2;
+          }
+          if (MODE == 1) {
+            axh += (double)zrA; ahh += (double)hhA;
+            txh[lane * 33 + (alpha - g)] = (float)axh;
+            thh[lane * 33 + (alpha - g)] = (float)ahh;
+            axh += (double)zrB; ahh += (double)hhB;
+            txh[lane * 33 + (alpha + 1 - g)] = (float)axh;
+            thh[lane * 33 + (alpha + 1 - g)] = (float)ahh;
+          } else {
+            fxh += zrA + zrB;
+            fxi += ziA + ziB;
+            fhh += hhA + hhB;
+          }
+          tr = nA; tr2 = nB;
+          alpha += 2; dalpha += 2.0; usp += 2; rt += 2; Drow0 += 2 * p.npair; Mrow0 += 2 * p.mrow;
+          continue;
+        }
+        Track nxt;                                               // track of SFT alpha + 2
         if (__any_sync(0xffffffffu, go)) {
-          const float ab = (go && cfg_kernel<CFG>(p) == 1) ? fabsf(tr.b) : 0.f;
           const float bmax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(ab)));
           if (CFG::KC && p.path_counts) {
             int n_present = 0;
@@ -922,7 +1025,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
             n_path[path_of(bmax, p.mtab != nullptr)] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * n_present);
           }
           float zr, zi, hh;
-          pair_terms<KT, CT, CFG>(p, tm, Drow0, Mrow0, rt, tr, go, bmax, us2, dalpha, nxt, zr, zi, hh);
+          pair_terms<KT, CT, CFG>(p, tm, Drow0, Mrow0, rt, tr, go, bmax, us2, dalpha + 2.0, nxt, zr, zi, hh);
           if (MODE == 1) {
             axh += (double)zr;
             ahh += (double)hh;
@@ -932,7 +1035,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
             fhh += hh;
           }
         } else {
-          track_eval<CFG>(p, tm, dalpha, nxt);
+          track_eval<CFG>(p, tm, dalpha + 2.0, nxt);
         }
         if (CFG::KC && want_kc) {
           if (t < p.nT) {
@@ -941,11 +1044,13 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
           }
           ++kcp;
         }
-        tr = nxt;
+        tr = tr2;
+        tr2 = nxt;
         if (MODE == 1) {
           txh[lane * 33 + (alpha - g)] = (float)axh;
           thh[lane * 33 + (alpha - g)] = (float)ahh;
         }
+        ++alpha; dalpha += 1.0; ++usp; ++rt; Drow0 += p.npair; Mrow0 += p.mrow;
       }
       if (MODE == 0) {
         axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;

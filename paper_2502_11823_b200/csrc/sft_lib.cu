@@ -527,6 +527,9 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.rtab = p->rtab;
 }
 
+#ifndef SFT_DUO
+#define SFT_DUO true        // two consecutive SFTs per step through the tier-1 tables (sft_kernels.cuh :: duo_terms)
+#endif
 #ifndef SFT_MINB
 #define SFT_MINB 5          // resident 128-thread blocks per SM the main kernel is compiled for
 #endif
@@ -544,7 +547,7 @@ using CfgBNS32 = sftk::Cfg<1, 1, 0, 0, 1>;    // CfgBNS with the split-fp32 (dou
 
 template <int KT, int CT, int MODE, class CFG>
 static void launch_variant(sft_plan *p, const KParams &k) {
-  auto kern = sftk::sft_main_kernel<KT, CT, MODE, CFG, SFT_MINB>;
+  auto kern = sftk::sft_main_kernel<KT, CT, MODE, CFG, SFT_MINB, SFT_DUO>;
   int per_sm = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, sftk::TILE, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
   long long blocks = (long long)p->n_sm * per_sm;
