@@ -764,6 +764,60 @@ __device__ __forceinline__ void table_math(const TableData<CT, TIER> &d, float (
   }
 }
 
+// table_math for two independent (template, SFT) streams with every Horner step issued for both in turn, so that the
+// dependent chains of one fill the latency of the other without relying on the scheduler's window.
+template <int CT, int TIER>
+__device__ __forceinline__ void table_math2(const TableData<CT, TIER> &dA, const TableData<CT, TIER> &dB, float (&s1rA)[CT],
+                                            float (&s1iA)[CT], float (&s2A)[CT], float (&s1rB)[CT], float (&s1iB)[CT],
+                                            float (&s2B)[CT]) {
+  constexpr int Q = TableData<CT, TIER>::Q, NHB = TableData<CT, TIER>::NHB;
+  float nbA[Q / 2 + 1], naA[Q + 1], nbB[Q / 2 + 1], naB[Q + 1];
+#pragma unroll
+  for (int k = 1; k <= Q / 2; ++k) { nbA[k] = dA.be * (1.0f / (float)k); nbB[k] = dB.be * (1.0f / (float)k); }
+#pragma unroll
+  for (int k = 1; k <= Q; ++k) { naA[k] = dA.a * (1.0f / (float)k); naB[k] = dB.a * (1.0f / (float)k); }
+  const float be2A = dA.be * dA.be, be2B = dB.be * dB.be;
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+    float2 MA[Q + 1], MB[Q + 1];
+#pragma unroll
+    for (int q = 0; q <= Q; ++q) {
+      MA[q] = (q & 1) ? make_float2(dA.Mq[c][q >> 1].z, dA.Mq[c][q >> 1].w) : make_float2(dA.Mq[c][q >> 1].x, dA.Mq[c][q >> 1].y);
+      MB[q] = (q & 1) ? make_float2(dB.Mq[c][q >> 1].z, dB.Mq[c][q >> 1].w) : make_float2(dB.Mq[c][q >> 1].x, dB.Mq[c][q >> 1].y);
+    }
+    float2 SA = make_float2(0.f, 0.f), SB = SA;
+#pragma unroll
+    for (int pq = Q; pq >= 0; --pq) {
+      const int nmax = (Q - pq) / 2;
+      float2 LA = MA[pq + 2 * nmax], LB = MB[pq + 2 * nmax];
+#pragma unroll
+      for (int n = nmax; n >= 1; --n) {
+        LA = cstep(MA[pq + 2 * (n - 1)], nbA[n], LA);
+        LB = cstep(MB[pq + 2 * (n - 1)], nbB[n], LB);
+      }
+      SA = pq == Q ? LA : cstep(LA, naA[pq + 1], SA);
+      SB = pq == Q ? LB : cstep(LB, naB[pq + 1], SB);
+    }
+    s1rA[c] = SA.x; s1iA[c] = SA.y;
+    s1rB[c] = SB.x; s1iB[c] = SB.y;
+    const float *hA = (const float *)&dA.Hq[c][0], *hB = (const float *)&dB.Hq[c][0];
+    float ha = 0.f, hb = 0.f;
+#pragma unroll
+    for (int P = HTAB_P; P >= 0; --P) {
+      float gA = hA[(NHB - 1) * (HTAB_P + 1) + P], gB = hB[(NHB - 1) * (HTAB_P + 1) + P];
+#pragma unroll
+      for (int N = NHB - 2; N >= 0; --N) {
+        gA = fmaf(gA, be2A, hA[N * (HTAB_P + 1) + P]);
+        gB = fmaf(gB, be2B, hB[N * (HTAB_P + 1) + P]);
+      }
+      ha = P == HTAB_P ? gA : fmaf(ha, dA.aH, gA);
+      hb = P == HTAB_P ? gB : fmaf(hb, dB.aH, gB);
+    }
+    s2A[c] = ha;
+    s2B[c] = hb;
+  }
+}
+
 template <int CT, class CFG, int TIER>
 __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, double dnext, Track &nxt, float xp, float b,
                                            int kcidx, const float4 *Mrow, float (&s1r)[CT], float (&s1i)[CT],
@@ -839,8 +893,7 @@ __device__ __forceinline__ void duo_terms(const KParams &p, const Tmpl &tm, cons
   track_eval<CFG>(p, tm, dnext, nA);
   track_eval<CFG>(p, tm, dnext + 1.0, nB);
   float s1rA[CT], s1iA[CT], s2A[CT], s1rB[CT], s1iB[CT], s2B[CT];
-  table_math<CT, 1>(dA, s1rA, s1iA, s2A);
-  table_math<CT, 1>(dB, s1rB, s1iB, s2B);
+  table_math2<CT, 1>(dA, dB, s1rA, s1iA, s2A, s1rB, s1iB, s2B);
   finish_terms<CT, CFG>(p, tm, rt, trA, okA, 1.0f, fmaf(2.0f, trA.frac, fmaf(0.25f, bA, trA.x)), s1rA, s1iA, s2A, usA, zrA, ziA, hhA);
   finish_terms<CT, CFG>(p, tm, rt + 1, trB, okB, 1.0f, fmaf(2.0f, trB.frac, fmaf(0.25f, bB, trB.x)), s1rB, s1iB, s2B, usB, zrB, ziB, hhB);
 }
