@@ -93,7 +93,9 @@ typedef struct {
 
 /* Creates a plan: validates `desc`, selects the device, allocates the (empty) data-SFT store
  * [n_channels][n_sft][k_hi-k_lo] complex64 + weight tables in device memory (SFTs are
- * "computed once ... reused").  *out is set only on SFT_OK. */
+ * "computed once ... reused") and, unless SFT_EVAL_DIRECT, the moment tables of the
+ * table evaluator (128 bytes per SFT, window position k_c and quarter bin).
+ * *out is set only on SFT_OK. */
 sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out);
 
 /* Frees the plan and all device memory it owns.  NULL is accepted. */
@@ -106,7 +108,8 @@ sft_status sft_plan_destroy(sft_plan *plan);
  *   psd_shape  [k_hi-k_lo] S_c(f_k) > 0 (one-sided PSD); NULL => 1
  *   response   complex64 interleaved [n_sft] R_{c,a}; required iff plan response == SFT_RESP_TABLE, else ignored/NULL
  *   mem        SFT_MEM_HOST or SFT_MEM_DEVICE: where ALL the non-NULL pointers of this call live
- * May be called again for the same channel to replace its data. */
+ * Also (re)builds the channel's moment tables.  May be called again for the same channel to replace
+ * its data. */
 sft_status sft_load_data(sft_plan *plan, int32_t channel, const float *sft_bins,
                          const double *psd_scale, const double *psd_shape,
                          const float *response, int32_t mem);
