@@ -127,7 +127,7 @@ def test_et_small_masked_and_dirichlet(et_small):
         assert 0 < (o["kc"] >= 0).sum() <= o["kc"].size
 
 
-@pytest.mark.parametrize("K", [0, 1, 2, 5, 16, 32, 64])
+@pytest.mark.parametrize("K", [0, 1, 2, 5, 16, 32, 64, 128])
 def test_band_half_widths(et_small, K):
     """Config 5's K axis: specialised (4, 8, 16) and generic code paths, including K = 0."""
     w = et_small
@@ -135,6 +135,31 @@ def test_band_half_widths(et_small, K):
     o, xx, _, _ = _oracle(w, params=P, K=K)
     g = _run_gpu(w, params=P, K=K)
     _check(w, g, o, xx)
+
+
+@pytest.mark.parametrize("n_sft", [1, 2, 3, 9, 33])
+def test_tiny_sft_counts(n_sft):
+    """Degenerate time axes: 1, 2, 3, 9 and 33 SFT slots (the kernels take two SFTs per step and keep tracks two SFTs
+    ahead; work units of at most 32 SFTs), inner products and the cumulative call, with and without gaps."""
+    api = _api()
+    for gap_fraction in (0.0, 0.34):
+        w = wl.et_bns(n_templates=37, n_sft=n_sft, K=8, gap_fraction=gap_fraction, name="et-tiny", tau_end=129.0 + 8.0 * (1200 - n_sft))
+        o, xx, plan_o, store = _oracle(w)
+        g = _run_gpu(w)
+        if (o["kc"] >= 0).any():
+            _check(w, g, o, xx)
+        else:
+            assert np.all(g["xh"] == 0.0) and np.all(g["hh"] == 0.0)
+        oc = oin.cumulative_snr(plan_o, store, w.params)
+        with api.plan_from_workload(w) as plan:
+            cx = np.full((37, n_sft), np.nan, np.float32)
+            ch = np.full((37, n_sft), np.nan, np.float32)
+            snr = np.full((37, n_sft), np.nan, np.float32)
+            plan.cumulative_snr(np.ascontiguousarray(w.params), snr, cx, ch)
+        norm = np.sqrt(max(xx, 1e-300) * np.maximum(o["hh"], 1e-300))[:, None]
+        assert np.all(np.isfinite(snr))
+        assert (np.abs(cx - oc["cum_xh"]) / norm).max() <= TOL * 1.0001 or np.abs(cx - oc["cum_xh"]).max() == 0.0
+        assert (np.abs(ch - oc["cum_hh"]) / norm).max() <= TOL * 1.0001 or np.abs(ch - oc["cum_hh"]).max() == 0.0
 
 
 @pytest.mark.parametrize("chunk", [1, 7, 32, 64, 5000])
