@@ -105,13 +105,21 @@ __global__ void __launch_bounds__(256) sft_rfft_band_kernel(const double *x, int
   dif_pass<4, true>(z, seg, W, m, n, h, threadIdx.x, blockDim.x);       // log2m >= 5
   h >>= 4; r -= 4;
   __syncthreads();
-  while (r > 0) {
-    if (r == 4 || (r > 4 && r % 3 == 1)) { dif_pass<4, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 4; r -= 4; }
-    else if (r >= 3) { dif_pass<3, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 3; r -= 3; }
-    else if (r == 2) { dif_pass<2, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 2; r -= 2; }
-    else { dif_pass<1, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 1; r -= 1; }
+  while (r >= 2) {
+    if (r >= 4) { dif_pass<4, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 4; r -= 4; }
+    else if (r == 3) { dif_pass<3, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 3; r -= 3; }
+    else { dif_pass<2, false>(z, seg, W, m, n, h, threadIdx.x, blockDim.x); h >>= 2; r -= 2; }
     __syncthreads();
   }
+  // r == 1: the last stage (pairs (2i, 2i+1), twiddle 1) is not run over the array: the few outputs needed below take
+  // their butterfly themselves,  Z(pos) = z[pos] + z[pos+1] (pos even),  z[pos-1] - z[pos] (pos odd)
+  const bool fold = r == 1;
+  auto zout = [&](int pos) {
+    const float2 v = z[padi(pos)];
+    if (!fold) return v;
+    const float2 w2 = z[padi(pos ^ 1)];
+    return (pos & 1) ? make_float2(w2.x - v.x, w2.y - v.y) : make_float2(v.x + w2.x, v.y + w2.y);
+  };
   // band bins from the bit-reversed m-point spectrum
   float2 *out = bins + (size_t)blockIdx.x * nb;
   const float fdt = (float)dt;
@@ -120,8 +128,8 @@ __global__ void __launch_bounds__(256) sft_rfft_band_kernel(const double *x, int
     float2 X = make_float2(0.f, 0.f);
     if (k >= 0 && k <= m) {
       const int k1 = k & (m - 1), k2 = (m - k) & (m - 1);       // Z[m] = Z[0]
-      const float2 A = z[padi((int)(__brev((unsigned)k1) >> (32 - log2m)))];
-      const float2 Bc = z[padi((int)(__brev((unsigned)k2) >> (32 - log2m)))];
+      const float2 A = zout((int)(__brev((unsigned)k1) >> (32 - log2m)));
+      const float2 Bc = zout((int)(__brev((unsigned)k2) >> (32 - log2m)));
       const float2 B = make_float2(Bc.x, -Bc.y);                 // conj Z[m-k]
       const float2 S = make_float2(A.x + B.x, A.y + B.y), D = make_float2(A.x - B.x, A.y - B.y);
       float2 w;                                                  // w^k, k <= m = n/2
