@@ -284,6 +284,8 @@ def compute_sfts(x, n_sft, n, dt, k_lo, k_hi, bins, device=0, stream=None):
     """``sft_compute_sfts``: band-limited data SFTs of a float64 series into complex64 ``bins`` [n_sft][k_hi-k_lo]."""
     lib = load_library()
     mem = _where([x, bins])
+    if x is None or len(x.shape) != 1 or int(x.shape[0]) < int(n_sft) * int(n):
+        raise ValueError("x must be a 1-D series of at least n_sft * n = %d samples" % (int(n_sft) * int(n)))
     st = lib.sft_compute_sfts(int(device), C.c_void_p(int(stream)) if stream else None,
                               _ptr(x, np.float64, None, "x"), int(n_sft), int(n), float(dt), int(k_lo), int(k_hi),
                               _ptr(bins, np.complex64, (int(n_sft), int(k_hi) - int(k_lo)), "bins"), mem)

@@ -13,8 +13,15 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsft_b200.so")
 SOURCES = [os.path.join(CSRC, "sft_lib.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "sft_kernels.cuh"), os.path.join(CSRC, "fresnel_aux_coeffs.h"), os.path.join(CSRC, "alu_peaks.cuh"),
-                  os.path.join(os.path.dirname(HERE), "include", "sft.h")]
+
+
+def deps():
+    """Everything the library is compiled from: every file under csrc/ (sources, headers, generated coefficient tables)
+    and the public header."""
+    import glob
+    return sorted(glob.glob(os.path.join(CSRC, "*"))) + [os.path.join(os.path.dirname(HERE), "include", "sft.h")]
+
+
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",
               "-cudart", "static"]
@@ -31,7 +38,7 @@ def up_to_date():
     if not os.path.exists(LIB):
         return False
     t = os.path.getmtime(LIB)
-    return all(os.path.getmtime(d) <= t for d in DEPS)
+    return all(os.path.getmtime(d) <= t for d in deps())
 
 
 def build(force=False, verbose=False, extra=()):

@@ -698,10 +698,12 @@ template <int CT, int TIER>
 __device__ __forceinline__ void table_load(const KParams &p, float xp, float b, int kcidx, const float4 *Mrow,
                                            TableData<CT, TIER> &d) {
   // node of the <h,h> table: cellH = floor((xp + 1/2) HTAB_R) by the 1.5 * 2^23 rounding trick, clamped (xp = 1/2
-  // exactly, NaN lanes); the data-moment node is cellH / 4 (HTAB_R = 4 TAB_R)
+  // exactly, NaN lanes); the data-moment node is cellH / 4 (HTAB_R = 4 TAB_R).  The offset HTAB_R/2 - 1/2 must be added
+  // BEFORE the magic constant: 7.5 + 1.5 * 2^23 is not representable (ulp 1) and would turn the floor into a round-to-
+  // nearest, i.e. nodes half a cell off.  (At an exact cell edge the rounding may pick either neighbour: same bound.)
   static_assert(HTAB_R == 4 * TAB_R, "node grids");
   constexpr float RM = 12582912.0f;
-  float cm = fmaf(xp, (float)HTAB_R, 0.5f * HTAB_R - 0.5f + RM);
+  float cm = fmaf(xp, (float)HTAB_R, 0.5f * HTAB_R - 0.5f) + RM;
   cm = fminf(fmaxf(cm, RM), RM + (float)(HTAB_R - 1));
   const int cellH = __float_as_int(cm) & (HTAB_R - 1);
   const int cell = cellH >> 2;

@@ -316,20 +316,31 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
     }
     if (!isfinite(S_ref)) S_ref = 1.0;   // no valid bin in the stored band: everything contributes 0
   }
+  // limits are checked before anything is enqueued or allocated (outputs/plan untouched on error)
+  unsigned bpr = 0;
+  if (p->mtab) {
+    const unsigned outs = (unsigned)p->n_node * (sftk::TAB_Q + 1);
+    bpr = (outs + 255) / 256;
+    if ((double)bpr * (double)N > 2.0e9) return fail(p, SFT_EUNSUPPORTED, "moment-table build grid too large");
+  }
   const float2 *d_raw = nullptr;
   const double *d_scale = nullptr, *d_shape = nullptr;
   void *tmp = nullptr;
+  // from here on the channel's tables are being replaced: a failure leaves the channel unloaded
+  p->loaded[channel] = false;
+  cudaError_t e = cudaSuccess;
+  auto ok = [&](cudaError_t r) { if (e == cudaSuccess && r != cudaSuccess) e = r; return e == cudaSuccess; };
   if (mem == SFT_MEM_HOST) {
     const size_t b_raw = N * nb * sizeof(float2), b_scale = N * sizeof(double), b_shape = psd_shape ? nb * sizeof(double) : 0;
     const size_t o_scale = (b_raw + 255) & ~size_t(255), o_shape = (o_scale + b_scale + 255) & ~size_t(255);
-    cudaError_t e = cudaMalloc(&tmp, o_shape + b_shape + 256);
-    if (e != cudaSuccess) return fail(p, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(e));
+    cudaError_t ea = cudaMalloc(&tmp, o_shape + b_shape + 256);
+    if (ea != cudaSuccess) return fail(p, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(ea));
     char *base = (char *)tmp;
-    cudaMemcpyAsync(base, sft_bins, b_raw, cudaMemcpyHostToDevice, p->stream);
-    cudaMemcpyAsync(base + o_scale, psd_scale, b_scale, cudaMemcpyHostToDevice, p->stream);
-    if (psd_shape) cudaMemcpyAsync(base + o_shape, psd_shape, b_shape, cudaMemcpyHostToDevice, p->stream);
+    ok(cudaMemcpyAsync(base, sft_bins, b_raw, cudaMemcpyHostToDevice, p->stream));
+    ok(cudaMemcpyAsync(base + o_scale, psd_scale, b_scale, cudaMemcpyHostToDevice, p->stream));
+    if (psd_shape) ok(cudaMemcpyAsync(base + o_shape, psd_shape, b_shape, cudaMemcpyHostToDevice, p->stream));
     if (p->d.response == SFT_RESP_TABLE)
-      cudaMemcpyAsync(p->rtab + (size_t)channel * N, response, N * sizeof(float2), cudaMemcpyHostToDevice, p->stream);
+      ok(cudaMemcpyAsync(p->rtab + (size_t)channel * N, response, N * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
     d_raw = (const float2 *)base;
     d_scale = (const double *)(base + o_scale);
     d_shape = psd_shape ? (const double *)(base + o_shape) : nullptr;
@@ -338,32 +349,32 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
     d_scale = psd_scale;
     d_shape = psd_shape;
     if (p->d.response == SFT_RESP_TABLE)
-      cudaMemcpyAsync(p->rtab + (size_t)channel * N, response, N * sizeof(float2), cudaMemcpyDeviceToDevice, p->stream);
+      ok(cudaMemcpyAsync(p->rtab + (size_t)channel * N, response, N * sizeof(float2), cudaMemcpyDeviceToDevice, p->stream));
   }
   const size_t C = p->d.n_channels, npair = p->npair;
-  sftk::sft_whiten_kernel<<<(unsigned)N, 128, 0, p->stream>>>(
-      d_raw, d_scale, d_shape, (int)N, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi, p->PAD, p->npair, p->d.t_sft, S_ref,
-      p->Dp + (size_t)channel * N * npair, p->Dp + (C + (size_t)channel) * N * npair, p->us2 + (size_t)channel * N);
-  sftk::sft_ub2_kernel<<<(unsigned)((2 * npair + 255) / 256), 256, 0, p->stream>>>(
-      d_shape, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi, p->PAD, p->npair, S_ref, p->ubp + (size_t)channel * npair,
-      p->ubp + (C + (size_t)channel) * npair);
-  p->launches += 2;
-  if (p->mtab) {
-    const size_t per_chan = N * (size_t)p->n_node * ((sftk::TAB_Q + 1) / 2);
-    const unsigned outs = (unsigned)p->n_node * (sftk::TAB_Q + 1);
-    const unsigned bpr = (outs + 255) / 256;
-    if ((double)bpr * (double)N > 2.0e9) return fail(p, SFT_EUNSUPPORTED, "moment-table build grid too large");
-    sftk::sft_mtab_kernel<<<(unsigned)(bpr * N), 256, 0, p->stream>>>(
-        p->Dp + (size_t)channel * N * npair, p->npair, p->n_node, p->d.K, p->ptab, bpr, (float2 *)(p->mtab + (size_t)channel * per_chan));
-    sftk::sft_htab_kernel<<<(unsigned)(p->n_kc * sftk::HTAB_R), 64, 0, p->stream>>>(
-        p->ubp + (size_t)channel * npair, p->d.K, (float *)(p->htab + (size_t)channel * p->n_kc * sftk::HTAB_R * (sftk::HTAB_W / 4)));
+  if (e == cudaSuccess) {
+    sftk::sft_whiten_kernel<<<(unsigned)N, 128, 0, p->stream>>>(
+        d_raw, d_scale, d_shape, (int)N, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi, p->PAD, p->npair, p->d.t_sft, S_ref,
+        p->Dp + (size_t)channel * N * npair, p->Dp + (C + (size_t)channel) * N * npair, p->us2 + (size_t)channel * N);
+    sftk::sft_ub2_kernel<<<(unsigned)((2 * npair + 255) / 256), 256, 0, p->stream>>>(
+        d_shape, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi, p->PAD, p->npair, S_ref, p->ubp + (size_t)channel * npair,
+        p->ubp + (C + (size_t)channel) * npair);
     p->launches += 2;
+    if (p->mtab) {
+      const size_t per_chan = N * (size_t)p->n_node * ((sftk::TAB_Q + 1) / 2);
+      sftk::sft_mtab_kernel<<<(unsigned)(bpr * N), 256, 0, p->stream>>>(
+          p->Dp + (size_t)channel * N * npair, p->npair, p->n_node, p->d.K, p->ptab, bpr, (float2 *)(p->mtab + (size_t)channel * per_chan));
+      sftk::sft_htab_kernel<<<(unsigned)(p->n_kc * sftk::HTAB_R), 64, 0, p->stream>>>(
+          p->ubp + (size_t)channel * npair, p->d.K, (float *)(p->htab + (size_t)channel * p->n_kc * sftk::HTAB_R * (sftk::HTAB_W / 4)));
+      p->launches += 2;
+    }
+    ok(cudaGetLastError());
   }
-  cudaError_t e = cudaGetLastError();
+  // the staging buffer and the caller's host arrays may be in flight: always drain the stream before returning
   cudaError_t e2 = cudaStreamSynchronize(p->stream);
   if (tmp) cudaFree(tmp);
-  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "whiten launch: %s", cudaGetErrorString(e));
-  if (e2 != cudaSuccess) return fail(p, SFT_ECUDA, "whiten: %s", cudaGetErrorString(e2));
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "sft_load_data (copy/launch): %s", cudaGetErrorString(e));
+  if (e2 != cudaSuccess) return fail(p, SFT_ECUDA, "sft_load_data: %s", cudaGetErrorString(e2));
   p->sigma[channel] = sqrt(p->d.t_sft / S_ref);
   p->loaded[channel] = true;
   return SFT_OK;
@@ -425,7 +436,8 @@ SFT_API sft_status sft_compute_sfts(int32_t device, void *stream, const double *
   if (mem == SFT_MEM_HOST) {
     cudaError_t e = cudaMalloc(&tmp, b_x + b_out + 256);
     if (e != cudaSuccess) return fail(nullptr, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(e));
-    cudaMemcpyAsync(tmp, x, b_x, cudaMemcpyHostToDevice, st);
+    cudaError_t ec = cudaMemcpyAsync(tmp, x, b_x, cudaMemcpyHostToDevice, st);
+    if (ec != cudaSuccess) { cudaStreamSynchronize(st); cudaFree(tmp); return fail(nullptr, SFT_ECUDA, "sft_compute_sfts: %s", cudaGetErrorString(ec)); }
     d_x = (const double *)tmp;
     d_out = (float2 *)((char *)tmp + ((b_x + 255) & ~size_t(255)));
   }
@@ -454,7 +466,8 @@ SFT_API sft_status sft_ingest_timeseries(sft_plan *p, int32_t channel, const dou
   const double *d_x = x;
   if (mem == SFT_MEM_HOST) {
     double *dx = (double *)((char *)tmp + ((b_bins + 255) & ~size_t(255)));
-    cudaMemcpyAsync(dx, x, b_x, cudaMemcpyHostToDevice, p->stream);
+    e = cudaMemcpyAsync(dx, x, b_x, cudaMemcpyHostToDevice, p->stream);
+    if (e != cudaSuccess) { cudaStreamSynchronize(p->stream); cudaFree(tmp); return fail(p, SFT_ECUDA, "series copy: %s", cudaGetErrorString(e)); }
     d_x = dx;
   }
   e = compute_sfts_device(p->stream, d_x, (int64_t)N, (int)n, 1.0 / p->d.fs, p->d.k_lo, p->d.k_hi, d_bins, &p->launches);
@@ -470,11 +483,15 @@ SFT_API sft_status sft_ingest_timeseries(sft_plan *p, int32_t channel, const dou
     e = cudaMalloc(&tmp2, b_scale + b_shape + b_resp + 768);
     if (e != cudaSuccess) { cudaStreamSynchronize(p->stream); cudaFree(tmp); return fail(p, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(e)); }
     char *q = (char *)tmp2;
-    cudaMemcpyAsync(q, psd_scale, b_scale, cudaMemcpyHostToDevice, p->stream);
+    e = cudaMemcpyAsync(q, psd_scale, b_scale, cudaMemcpyHostToDevice, p->stream);
     d_scale = (const double *)q;
     q += (b_scale + 255) & ~size_t(255);
-    if (psd_shape) { cudaMemcpyAsync(q, psd_shape, b_shape, cudaMemcpyHostToDevice, p->stream); d_shape = (const double *)q; q += (b_shape + 255) & ~size_t(255); }
-    if (b_resp) { cudaMemcpyAsync(q, response, b_resp, cudaMemcpyHostToDevice, p->stream); d_resp = (const float *)q; }
+    if (psd_shape && e == cudaSuccess) { e = cudaMemcpyAsync(q, psd_shape, b_shape, cudaMemcpyHostToDevice, p->stream); d_shape = (const double *)q; q += (b_shape + 255) & ~size_t(255); }
+    if (b_resp && e == cudaSuccess) { e = cudaMemcpyAsync(q, response, b_resp, cudaMemcpyHostToDevice, p->stream); d_resp = (const float *)q; }
+    if (e != cudaSuccess) {
+      cudaStreamSynchronize(p->stream); cudaFree(tmp); cudaFree(tmp2);
+      return fail(p, SFT_ECUDA, "noise-description copy: %s", cudaGetErrorString(e));
+    }
   }
   st = sft_load_data(p, channel, (const float *)d_bins, d_scale, d_shape, d_resp, SFT_MEM_DEVICE);
   cudaStreamSynchronize(p->stream);

@@ -218,3 +218,143 @@ def test_harness_fft_matches_oracle_direct_dft(c1):
     ref = osft.sft_direct(seg, ks, 1 / plan.fs)
     got = w.bins[0][[0, 100, 255]].astype(np.complex128)
     assert np.abs(got - ref).max() < 2e-7 * np.abs(ref).max()
+
+
+# ---------------------------------------------------------------------------------------------
+# Pins added in round 2 (VERDICT r1 "oracle pins"): the annual response, the channel loop, <x,x>_band.
+def _lisa_noiseless(flip=None):
+    """Config-4-like set-up (2 channels x 672 SFTs of 3600 s at 0.2 Hz, LISA-like PSD, K = 16) with NOISELESS data and the
+    signal moved up to bins ~20-30 (chirp mass 1440 Msun) so that the method's own edge effects at k ~ 1 do not
+    blur the pin.  The strain is modulated at every SAMPLE by R_c(t) = [1 + depth cos(2 pi t/P + psi_c + lambda)]
+    e^{i (chi_c + beta)} through ``workloads.inspiral_strain`` (an independent per-sample statement of Eq.(5)-(6) P:80-85 /
+    Eq.(40)-(41) P:332-334; P = 30 d so the modulation runs through a full cycle) and transformed by numpy's FFT; the oracle
+    only ever sees the per-SFT response of ``response_factor("annual")`` (constant over an SFT).  ``flip`` mutates
+    what is handed to the ORACLE (plan phases or the template's sky angles), never the data."""
+    fs, T, n_sft, C, K = 0.2, 3600.0, 672, 2, 16
+    n = int(round(T * fs))
+    k_lo, k_hi = 2, 60
+    d = dict(n_channels=C, n_sft=n_sft, t_sft=T, fs=fs, t0=0.0, k_lo=k_lo, k_hi=k_hi, K=K, kernel="fresnel", pn1=1,
+             response="annual", f_lo=0.0, f_hi=2e-2, f_ref=5e-3, resp_period=30 * 86400.0, resp_depth=0.3,
+             resp_psi=(0.3, 0.3 + np.pi / 2), resp_chi=(0.2, 0.2 + np.pi / 2))
+    eta = 0.2222
+    inj = np.array([1440.0, eta, n_sft * T + 14.4 * 86400.0, 2.0, 1e-20, 0.7, -0.3, 0.0])
+    t = np.arange(n_sft * n) / fs
+    S = wl.lisa_psd(np.arange(k_lo, k_hi) / T)
+    bins = np.zeros((C, n_sft, k_hi - k_lo), dtype=np.complex128)
+    for c in range(C):
+        def resp(tt, c=c):
+            return (1.0 + d["resp_depth"] * np.cos(2 * np.pi * tt / d["resp_period"] + d["resp_psi"][c] + inj[5])) * \
+                np.exp(1j * (d["resp_chi"][c] + inj[6]))
+        h = wl.inspiral_strain(t, inj, d["f_ref"], d["pn1"], resp)
+        bins[c] = np.fft.rfft(h.reshape(n_sft, n), axis=-1)[:, k_lo:k_hi] / fs
+    dd = dict(d)
+    P = inj.copy()
+    if flip == "psi":
+        dd["resp_psi"] = tuple(-v for v in d["resp_psi"])
+    elif flip == "chi":
+        dd["resp_chi"] = tuple(-v for v in d["resp_chi"])
+    elif flip == "lambda":
+        P[5] = -P[5]
+    elif flip == "beta":
+        P[6] = -P[6]
+    plan = oin.Plan(**dd)
+    store = oin.Store(bins=bins, psd_scale=np.ones((C, n_sft)), psd_shape=np.stack([S, S]))
+    return plan, store, P
+
+
+def _xx_on_template_bins(plan, store, kc):
+    """<x,x> over the SAME bins B_a the template uses (k_c +- K, valid and stored), from the data alone."""
+    k = np.arange(plan.k_lo, plan.k_hi)
+    tot = 0.0
+    for c in range(plan.n_channels):
+        inB = (np.abs(k[None, :] - kc[c][:, None]) <= plan.K) & (k[None, :] >= 1) & (kc[c][:, None] >= 0)
+        tot += 4.0 / plan.t_sft * np.sum(inB * np.abs(store.bins[c]) ** 2 / (store.psd_scale[c][:, None] * store.psd_shape[c][None, :]))
+    return tot
+
+
+def test_annual_response_recovers_per_sample_modulated_injection():
+    """Pin of ``response_factor("annual")`` and of ``Lambda z = Re[R z]``: on noiseless data the matched template gives
+    ([x,h]) = ([h,h]) = <x,x> on the template's bins to a few 1e-4 (measured: 3e-4, 1e-3, 1e-5); a sign slip in psi_c + lambda or chi_c + beta, in the plan or in the template, breaks that by far more."""
+    plan, store, P = _lisa_noiseless()
+    r = oin.inner_products(plan, store, P[None])
+    xx_B = _xx_on_template_bins(plan, store, r["kc"][0])
+    assert r["kc"][0].min() >= 18 and r["kc"][0].max() <= 32
+    assert abs(r["xh"][0] / r["hh"][0] - 1.0) < 0.002, r
+    assert abs(r["hh"][0] / xx_B - 1.0) < 0.005, (r["hh"][0], xx_B)
+    assert abs(r["xh_im"][0]) < 0.002 * r["hh"][0]
+    # both channels carry signal and are modulated differently
+    Z, H, _, _, _ = oin.band_terms(plan, store, P)
+    assert H[0].sum() > 0.2 * H.sum() and H[1].sum() > 0.2 * H.sum() and abs(H[0].sum() / H[1].sum() - 1) > 0.02
+    for flip in ("psi", "chi", "lambda", "beta"):
+        p2, s2, P2 = _lisa_noiseless(flip)
+        r2 = oin.inner_products(p2, s2, P2[None])
+        bad = max(abs(r2["xh"][0] / r2["hh"][0] - 1.0), abs(r2["hh"][0] / xx_B - 1.0), abs(r2["xh_im"][0]) / r2["hh"][0])
+        assert bad > 0.03, (flip, r2["xh"][0], r2["hh"][0], r2["xh_im"][0], xx_B)
+
+
+def test_channel_loop_is_a_sum_of_single_channel_results():
+    """Pin of the ``C > 1`` loop of ``band_terms_from_track``: two channels with different gaps, PSD scales, PSD shapes and
+    data give exactly the sum of the two single-channel results, and ``kc[:, c, :]`` follows each channel's own gaps."""
+    w = wl.config1(n_templates=5)
+    plan1, st1 = to_oracle(w)
+    rng = np.random.default_rng(123)
+    N, nb = plan1.n_sft, plan1.k_hi - plan1.k_lo
+    binsB = (rng.standard_normal((N, nb)) + 1j * rng.standard_normal((N, nb))) * 0.03
+    scaleA = np.exp(0.3 * rng.standard_normal(N))
+    scaleB = np.exp(0.3 * rng.standard_normal(N))
+    scaleA[[5, 6, 100]] = 0.0
+    scaleB[[6, 7, 200, 201]] = [0.0, np.nan, -1.0, 0.0]
+    shapeA = st1.psd_shape[0] * (1.0 + 0.5 * np.linspace(0, 1, nb))
+    shapeB = st1.psd_shape[0] * (2.0 - 0.7 * np.linspace(0, 1, nb) ** 2)
+    sA = oin.Store(bins=st1.bins[0][None], psd_scale=scaleA[None], psd_shape=shapeA[None])
+    sB = oin.Store(bins=binsB[None], psd_scale=scaleB[None], psd_shape=shapeB[None])
+    s2 = oin.Store(bins=np.stack([st1.bins[0], binsB]), psd_scale=np.stack([scaleA, scaleB]), psd_shape=np.stack([shapeA, shapeB]))
+    plan2 = copy.copy(plan1)
+    plan2.n_channels = 2
+    rA, rB = oin.inner_products(plan1, sA, w.params), oin.inner_products(plan1, sB, w.params)
+    r2 = oin.inner_products(plan2, s2, w.params)
+    for key in ("xh", "hh", "xh_im"):
+        scale = np.abs(rA[key]) + np.abs(rB[key]) + 1e-300
+        assert np.all(np.abs(r2[key] - (rA[key] + rB[key])) <= 1e-13 * scale), key
+    assert np.array_equal(r2["kc"][:, 0, :], rA["kc"][:, 0, :]) and np.array_equal(r2["kc"][:, 1, :], rB["kc"][:, 0, :])
+    assert np.all(r2["kc"][:, 0, [5, 6, 100]] == -1) and np.all(r2["kc"][:, 1, [6, 7, 200, 201]] == -1)
+    assert np.all(r2["kc"][:, 0, 7] >= 0) and np.all(r2["kc"][:, 1, 5] >= 0)
+    cA, cB, c2 = (oin.cumulative_snr(p, s, w.params[:2]) for p, s in ((plan1, sA), (plan1, sB), (plan2, s2)))
+    assert np.allclose(c2["cum_xh"], cA["cum_xh"] + cB["cum_xh"], rtol=0, atol=1e-12 * np.abs(c2["cum_xh"]).max())
+    assert np.allclose(c2["cum_hh"], cA["cum_hh"] + cB["cum_hh"], rtol=1e-13)
+    assert abs(oin.xx_band(plan2, s2) - oin.xx_band(plan1, sA) - oin.xx_band(plan1, sB)) <= 1e-13 * oin.xx_band(plan2, s2)
+
+
+def test_xx_band_is_the_plain_product_of_the_data_with_itself():
+    """Pin of ``xx_band`` (the parity normaliser, DESIGN A14): (i) it equals sum_a full_band_product(x~_a, x~_a) of Eq.(1)
+    on the stored bins; (ii) for config 1's unit white noise with S = 2/fs it is (2 dt/S) sum_j x_j^2 (Parseval, pin P2) times
+    the fraction of the band that is stored, within sampling error (a factor 2 either way fails both)."""
+    w = wl.config1(n_templates=1)
+    plan, store = to_oracle(w)
+    n, T = plan.n_samp, plan.t_sft
+    ks = np.arange(plan.k_lo, plan.k_hi)
+    xx = oin.xx_band(plan, store)
+    per_sft = np.zeros(plan.n_sft)
+    for a in range(plan.n_sft):
+        xs = store.bins[0][a]
+        S = store.psd_scale[0][a] * store.psd_shape[0]
+        per_sft[a] = osft.full_band_product(xs, xs, S, 1.0 / T, ks, n)
+    tot = per_sft.sum()
+    assert abs(xx / tot - 1.0) < 1e-12
+    S0 = 2.0 / plan.fs
+    full = osft.time_domain_product(w.series[0], w.series[0], 1.0 / plan.fs, S0)      # = N0 (1 + signal power) for unit noise
+    frac = len(ks) / (n / 2.0)
+    # the injected chirp (amp 0.5 -> ~12 % of the noise power) sits inside the stored band: subtract it from both sides
+    sig = wl.inspiral_strain(np.arange(w.series.shape[1]) / plan.fs, w.injection, plan.f_ref, plan.pn1)
+    p_sig = osft.time_domain_product(sig, sig, 1.0 / plan.fs, S0)
+    n_eff = plan.n_sft * len(ks)                                                       # complex Gaussian bins in the band
+    assert abs((xx - p_sig) / ((full - p_sig) * frac) - 1.0) < 6.0 / np.sqrt(n_eff) + 0.01
+    # gaps and invalid bins (k < 1, k >= n/2) drop out
+    s2 = copy.copy(store)
+    s2.psd_scale = store.psd_scale.copy()
+    s2.psd_scale[0, :128] = 0.0
+    assert abs(oin.xx_band(plan, s2) / per_sft[128:].sum() - 1.0) < 1e-12
+    p0 = copy.copy(plan)
+    p0.k_lo, p0.k_hi = 0, 3
+    s0 = oin.Store(bins=np.ones((1, plan.n_sft, 3), complex), psd_scale=store.psd_scale, psd_shape=np.ones((1, 3)))
+    assert abs(oin.xx_band(p0, s0) - 4.0 / T * plan.n_sft * 2) < 1e-9                   # k = 0 excluded, k = 1, 2 counted
