@@ -698,15 +698,14 @@ template <int CT, int TIER>
 __device__ __forceinline__ void table_load(const KParams &p, float xp, float b, int kcidx, const float4 *Mrow,
                                            TableData<CT, TIER> &d) {
   // node of the <h,h> table: cellH = floor((xp + 1/2) HTAB_R) by the 1.5 * 2^23 rounding trick, clamped (xp = 1/2
-  // exactly, NaN lanes); the data-moment node is cellH / 4 (HTAB_R = 4 TAB_R).  The offset HTAB_R/2 - 1/2 must be added
-  // BEFORE the magic constant: 7.5 + 1.5 * 2^23 is not representable (ulp 1) and would turn the floor into a round-to-
+  // exactly, NaN lanes); the data-moment node is cellH >> HTAB_SHIFT.  The offset HTAB_R/2 - 1/2 must be added
+  // BEFORE the magic constant: 31.5 + 1.5 * 2^23 is not representable (ulp 1) and would turn the floor into a round-to-
   // nearest, i.e. nodes half a cell off.  (At an exact cell edge the rounding may pick either neighbour: same bound.)
-  static_assert(HTAB_R == 4 * TAB_R, "node grids");
   constexpr float RM = 12582912.0f;
   float cm = fmaf(xp, (float)HTAB_R, 0.5f * HTAB_R - 0.5f) + RM;
   cm = fminf(fmaxf(cm, RM), RM + (float)(HTAB_R - 1));
   const int cellH = __float_as_int(cm) & (HTAB_R - 1);
-  const int cell = cellH >> 2;
+  const int cell = cellH >> HTAB_SHIFT;
   const float cHf = cm - RM;                                   // (float)cellH
   const float4 *mp = Mrow + (unsigned)(kcidx * TAB_R + cell) * (unsigned)((TAB_Q + 1) / 2);
   const float4 *hp = p.htab + (unsigned)(kcidx * HTAB_R + cellH) * (unsigned)(HTAB_W / 4);
@@ -967,17 +966,374 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, con
 }
 
 // ---------------------------------------------------------------------------------------------
+// Fast path for "clean" blocks.  A block = up to SUB = 32 consecutive SFT slots of one work unit.
+// It is clean when, for ALL 32 templates of the warp, every SFT of the block is active (DESIGN A12), its window lies
+// in the stored band and |b| <= B_TABLE (tier-1 moment tables).  For an inspiral f, fdot, k_c and b grow with time and
+// tau = t_c - t_a falls, so these conditions hold on the whole block iff they hold at its two end SFTs: they are
+// decided ONCE per block (two closed-form track evaluations and one warp vote) instead of once per SFT, and the loop
+// over the block's present SFTs then runs with no vote, no activity mask and no evaluator branch at all.
+//
+// Track inside a clean block.  With u = alpha - alpha_m (alpha_m = block start + 16) the closed forms of DESIGN W1 are
+// powers of Theta = Theta_m (1 - eps u), eps = T / tau_m, so phase [cycles], y = f T (+ b/2) [bins], b and the amplitude
+// are polynomials in u with geometrically falling coefficients:
+//     phi/2pi (u) = sum_k p_k u^k,   p_k = -c_phase (-eps)^k [binom(5/8,k) Theta_m^(5/8) + c_phi binom(3/8,k) Theta_m^(3/8)],
+//     f T   = d(phi/2pi)/du,    b = fdot T^2 = d(f T)/du        (exactly: dphi/dt = 2 pi f, t = alpha T),
+// evaluated at degree 6 (phase) and 5 (y) - the terms up to u^2 by fp64 Horner, the small tail from u^3 on in fp32:
+// 11 fp64 instructions per (template, SFT) instead of 33 - and by fp32 Horner at degree 2 / 3 for b / the amplitude.  The polynomial is used only where its first dropped term is
+// below 5e-11 bins in y (so that k_c stays bit-identical to the closed form evaluated in fp64: a different k_c would
+// need y within 5e-11 of a half-integer) and 1e-10 cycles in phase: |p_7| <= 5e-11 / (7 * 16^6); measured against
+// 40-digit arithmetic the bound overestimates the actual error by ~1.2 (tests/test_gpu_parity.py checks k_c bit-exact).
+// For config 2 that is tau_m >~ 9,000 s: 90 % of the SFTs.  Clean blocks closer to coalescence run the same loop with
+// the closed-form fp64 track.
+// ---------------------------------------------------------------------------------------------
+constexpr int SUB = 32;                       // SFT slots per block of the fast path
+// Validity of the polynomial track on a block (u in [-16, 15]); p_k = phase coefficients [cycles], y_k those of y [bins]:
+constexpr double POLY_P7_MAX = 5e-11 / (7.0 * 16777216.0);      // phase after u^6, y after u^5: first dropped term 7 |p_7| 16^6 <= 5e-11 bins
+constexpr double POLY_P5_MAX = 1e-7 / (20.0 * 4096.0);          // b after u^2: 20 |p_5| 16^3 <= 1e-7
+constexpr double POLY_P3_MAX = 0.05 / 4096.0;                   // the terms from u^3 on are summed in fp32: |phase tail| <~ 0.05 cycles
+constexpr double POLY_Y3_MAX = 5e-4 / 4096.0;                   //                                        |y tail| <~ 5e-4 bins
+constexpr double POLY_EPS_MAX = 0.03 / 16.0;                    // amplitude after u^3: quartic term 0.08 (16 eps)^4 <= 7e-8
+
+// u = j - 16 for slot j of a block: as double, and {u, u^3} as floats
+__constant__ double c_ud[SUB] = {-16., -15., -14., -13., -12., -11., -10., -9., -8., -7., -6., -5., -4., -3., -2., -1.,
+                                 0.,   1.,   2.,   3.,   4.,   5.,   6.,   7.,  8.,  9.,  10., 11., 12., 13., 14., 15.};
+__constant__ float2 c_uf[SUB] = {{-16.f, -4096.f}, {-15.f, -3375.f}, {-14.f, -2744.f}, {-13.f, -2197.f}, {-12.f, -1728.f}, {-11.f, -1331.f},
+                                 {-10.f, -1000.f}, {-9.f, -729.f},   {-8.f, -512.f},   {-7.f, -343.f},   {-6.f, -216.f},   {-5.f, -125.f},
+                                 {-4.f, -64.f},    {-3.f, -27.f},    {-2.f, -8.f},     {-1.f, -1.f},     {0.f, 0.f},       {1.f, 1.f},
+                                 {2.f, 8.f},       {3.f, 27.f},      {4.f, 64.f},      {5.f, 125.f},     {6.f, 216.f},     {7.f, 343.f},
+                                 {8.f, 512.f},     {9.f, 729.f},     {10.f, 1000.f},   {11.f, 1331.f},   {12.f, 1728.f},   {13.f, 2197.f},
+                                 {14.f, 2744.f},   {15.f, 3375.f}};
+
+// Polynomial track of one template on one block.  The terms up to u^2 are kept in fp64 (the phase reaches 1e5+ cycles, y
+// 1e2+ bins), the terms from u^3 on - below 0.05 cycles / 5e-4 bins by the validity test - are summed in fp32.
+struct FastCoef {
+  double p0, p1, p2;        // phase [cycles]
+  double y0, y1, y2;        // y = f T + (Fresnel kernel: b/2) [bins]
+  float pt[4];              // p_3 .. p_6
+  float yt[3];              // y_3 .. y_5
+  float bc[3];              // b = fdot T^2 (0 for the Dirichlet kernel)
+  float ac[4];              // amplitude (f/F0)^(2/3) (x the template's amplitude constant where that is real)
+};
+
+// What the table evaluator needs of one (template, SFT).
+struct FTrack {
+  int kc;
+  float xp;      // f T + b/2 - k_c  (b = 0 for the Dirichlet kernel)
+  float b, frac, amp;
+};
+
+// Coefficients about slot 16 of the block starting at SFT g.  Returns false where the polynomial must not be used.
+// `ascale` multiplies the amplitude polynomial.
+template <class CFG>
+__device__ __forceinline__ bool fast_coef(const KParams &p, const Tmpl &tm, int g, float ascale, FastCoef &fc) {
+  const bool pn1 = cfg_pn1<CFG>(p) != 0, fres = cfg_kernel<CFG>(p) == 1;
+  const double tau = fma(-(double)(g + 16), p.T, tm.tau0);
+  const double theta = tm.cTheta * tau;
+  const float y0 = ex2_approx(-0.125f * lg2_approx((float)theta));
+  const double y = (double)y0;
+  const double y2 = y * y, y4 = y2 * y2, y8 = y4 * y4;
+  const double r = fma(-theta, y8, 1.0);
+  const double q = fma(y, fma(r, 9.0 / 128.0, 0.125) * r, y);       // Theta^(-1/8) (see track_eval_fp64)
+  const double q2 = q * q, q3 = q2 * q, q4 = q2 * q2, q8 = q4 * q4;
+  const double eps = (tm.cTheta * p.T) * q8;                         // T / tau_m
+  const double me = -eps;
+  double A = theta * q3;                                             // Theta^(5/8)
+  double B = pn1 ? tm.cphi * (theta * (q3 * q2)) : 0.0;              // c_phi Theta^(3/8)
+  const double mc = -tm.cphase;
+  double pk[8];
+  pk[0] = fma(mc, A + B, tm.phic_cyc);
+#pragma unroll
+  for (int k = 1; k <= 7; ++k) {
+    A *= me * ((0.625 - (double)(k - 1)) / (double)k);               // binom(5/8, k) (-eps)^k Theta_m^(5/8)
+    if (pn1) B *= me * ((0.375 - (double)(k - 1)) / (double)k);
+    pk[k] = mc * (A + B);
+  }
+  double yk[6];
+#pragma unroll
+  for (int k = 0; k < 6; ++k) {
+    const double ft = (double)(k + 1) * pk[k + 1];
+    yk[k] = fres ? fma(0.5 * (double)((k + 1) * (k + 2)), pk[k + 2], ft) : ft;
+  }
+  fc.p0 = pk[0]; fc.p1 = pk[1]; fc.p2 = pk[2];
+  fc.y0 = yk[0]; fc.y1 = yk[1]; fc.y2 = yk[2];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) fc.pt[k] = (float)pk[3 + k];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) fc.yt[k] = (float)yk[3 + k];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) fc.bc[k] = fres ? (float)((double)((k + 1) * (k + 2)) * pk[k + 2]) : 0.f;
+  // amplitude q^2 (1 + cf q^2)^(2/3) = a_m (1 - eps u)^(-s1),  s1 = -dln a/dln Theta = (1 + 2 w/3)/4,  w = cf q^2/(1 + cf q^2)
+  double am = q2, s1 = 0.25;
+  if (pn1) {
+    const double gq = fma(tm.cf, q2, 1.0);
+    am = q2 * (double)cbrtf((float)(gq * gq));                       // (1 + cf q^2)^(2/3) ~ 1.0x: fp32 cube root, 1e-7 relative
+    s1 = 0.25 * fma(2.0 / 3.0, tm.cf * q2 / gq, 1.0);
+  }
+  am *= (double)ascale;
+  const double a1 = am * s1 * eps, a2 = a1 * (0.5 * (s1 + 1.0)) * eps, a3 = a2 * ((s1 + 2.0) * (1.0 / 3.0)) * eps;
+  fc.ac[0] = (float)am; fc.ac[1] = (float)a1; fc.ac[2] = (float)a2; fc.ac[3] = (float)a3;
+  return fabs(pk[7]) <= POLY_P7_MAX && fabs(pk[5]) <= POLY_P5_MAX && fabs(pk[3]) <= POLY_P3_MAX && fabs(yk[3]) <= POLY_Y3_MAX &&
+         eps <= POLY_EPS_MAX && eps > 0.0;
+}
+
+// The coefficients live in shared memory between the set-up of a block and its loop (26 registers per thread otherwise):
+// 7 x 16 bytes per thread, laid out [vector][thread] so that every LDS.128 / STS.128 of a warp is conflict free.
+constexpr int COEF_V = 7;
+__device__ __forceinline__ void coef_store(float4 *cs, const FastCoef &fc) {       // cs = slot of this thread
+  *reinterpret_cast<double2 *>(cs) = make_double2(fc.p0, fc.p1);
+  *reinterpret_cast<double2 *>(cs + TILE) = make_double2(fc.p2, fc.y0);
+  *reinterpret_cast<double2 *>(cs + 2 * TILE) = make_double2(fc.y1, fc.y2);
+  cs[3 * TILE] = make_float4(fc.pt[0], fc.pt[1], fc.pt[2], fc.pt[3]);
+  cs[4 * TILE] = make_float4(fc.yt[0], fc.yt[1], fc.yt[2], fc.bc[0]);
+  cs[5 * TILE] = make_float4(fc.bc[1], fc.bc[2], fc.ac[0], fc.ac[1]);
+  cs[6 * TILE] = make_float4(fc.ac[2], fc.ac[3], 0.f, 0.f);
+}
+
+__device__ __forceinline__ void ftrack_poly1(const double2 d0, const double2 d1, const double2 d2, const float4 f3, const float4 f4,
+                                             const float4 f5, const float2 f6, int j, FTrack &t) {
+  const double u = c_ud[j];
+  const float2 uu = c_uf[j];
+  const float uf = uu.x;
+  const float tp = uu.y * fmaf(fmaf(fmaf(f3.w, uf, f3.z), uf, f3.y), uf, f3.x);
+  const float ty = uu.y * fmaf(fmaf(f4.z, uf, f4.y), uf, f4.x);
+  const double ph = fma(fma(d1.x, u, d0.y), u, d0.x);
+  const double yy = fma(fma(d2.y, u, d2.x), u, d1.y) + (double)ty;
+  const double kr = yy + RND_MAGIC, pr = ph + RND_MAGIC;
+  t.kc = __double2loint(kr);
+  t.xp = (float)(yy - (kr - RND_MAGIC));
+  t.frac = (float)(ph - (pr - RND_MAGIC)) + tp;
+  t.b = fmaf(fmaf(f5.y, uf, f5.x), uf, f4.w);
+  t.amp = fmaf(fmaf(fmaf(f6.y, uf, f6.x), uf, f5.w), uf, f5.z);
+}
+
+// tracks of slots jA and jB from the thread's coefficient slot
+__device__ __forceinline__ void ftrack_poly2(const float4 *cs, int jA, int jB, FTrack &A, FTrack &B) {
+  const double2 d0 = *reinterpret_cast<const double2 *>(cs);
+  const double2 d1 = *reinterpret_cast<const double2 *>(cs + TILE);
+  const double2 d2 = *reinterpret_cast<const double2 *>(cs + 2 * TILE);
+  const float4 f3 = cs[3 * TILE], f4 = cs[4 * TILE], f5 = cs[5 * TILE];
+  const float2 f6 = *reinterpret_cast<const float2 *>(cs + 6 * TILE);
+  ftrack_poly1(d0, d1, d2, f3, f4, f5, f6, jA, A);
+  ftrack_poly1(d0, d1, d2, f3, f4, f5, f6, jB, B);
+}
+
+template <class CFG>
+__device__ __forceinline__ void ftrack_closed(const KParams &p, const Tmpl &tm, double dalpha, float ascale, FTrack &t) {
+  Track tr;
+  track_eval_fp64<CFG>(p, tm, dalpha, tr);
+  t.kc = tr.kc;
+  t.b = (cfg_kernel<CFG>(p) == 1) ? tr.b : 0.f;
+  t.xp = fmaf(0.5f, t.b, tr.x);
+  t.frac = tr.frac;
+  t.amp = tr.amp * ascale;
+}
+
+// Is the block [g, ge) clean for this warp (see above)?  Returns 0 = no (generic loop), 1 = clean, closed-form track,
+// 2 = clean, polynomial track (coefficients in the thread's shared-memory slot cs).  `mask` receives the block's presence bits (any channel), usv[c] the
+// weight 1/s of SFT g + lane.
+template <int CT, class CFG>
+__device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int g, int ge, int lane, float ascale, float4 *cs,
+                                          unsigned &mask, float (&usv)[CT]) {
+  bool pres = false;
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+    usv[c] = (g + lane < ge) ? __ldg(p.us2 + (size_t)c * p.n_sft + g + lane) : 0.f;
+    pres |= usv[c] > 0.f;
+  }
+  mask = __ballot_sync(0xffffffffu, pres);
+  if (mask == 0u || p.mtab == nullptr || cfg_phase<CFG>(p) != 0) return 0;
+  const bool fres = cfg_kernel<CFG>(p) == 1;
+  FastCoef fc;
+  const bool poly = __all_sync(0xffffffffu, fast_coef<CFG>(p, tm, g, ascale, fc));
+  if (poly) {
+    // the end SFTs from the polynomial itself (its error is far below the 1e-9 tie window of DESIGN A5/A12)
+    auto end = [&](int j, double &fT, float &b, int &kc) {
+      const double u = c_ud[j];
+      const float2 uu = c_uf[j];
+      const float ty = uu.y * fmaf(fmaf(fc.yt[2], uu.x, fc.yt[1]), uu.x, fc.yt[0]);
+      const double yy = fma(fma(fc.y2, u, fc.y1), u, fc.y0) + (double)ty;
+      b = fmaf(fmaf(fc.bc[2], uu.x, fc.bc[1]), uu.x, fc.bc[0]);
+      kc = __double2loint(yy + RND_MAGIC);
+      fT = fma(-0.5, (double)b, yy);                             // (b = 0 for the Dirichlet kernel: y = f T)
+    };
+    double fl, fh;
+    float bl, bh;
+    int kl, kh;
+    end(0, fl, bl, kl);
+    end(ge - 1 - g, fh, bh, kh);
+    const double tau_h = fma(-(double)(ge - 1), p.T, tm.tau0);
+    // Dirichlet kernel: the band edge test needs fdot T^2 although the evaluator does not (2 p_2 at the centre; +-1e-9 ties are flagged)
+    const double b_edge = fres ? (double)bh : 2.0 * fc.p2;
+    const bool ok = tau_h > p.T && fl >= p.f_loT && fh + b_edge <= p.f_hiT && (unsigned)(kl - p.kwin0 - 2) <= (unsigned)p.jmax &&
+                    (unsigned)(kh - p.kwin0 - 2) <= (unsigned)p.jmax && bl >= 0.f && bh >= bl && bh <= p.b_table && kh >= kl;
+    if (!__all_sync(0xffffffffu, ok)) return 0;
+    coef_store(cs, fc);
+    return 2;
+  }
+  Track lo, hi;
+  track_eval_fp64<CFG>(p, tm, (double)g, lo);
+  track_eval_fp64<CFG>(p, tm, (double)(ge - 1), hi);
+  const float bl = fres ? lo.b : 0.f, bh = fres ? hi.b : 0.f;
+  const int j0l = lo.kc - p.kwin0, j0h = hi.kc - p.kwin0;
+  const bool ok = lo.active && hi.active && (unsigned)(j0l - 2) <= (unsigned)p.jmax && (unsigned)(j0h - 2) <= (unsigned)p.jmax &&
+                  bl >= 0.f && bh >= bl && bh <= p.b_table && hi.kc >= lo.kc;
+  return __all_sync(0xffffffffu, ok) ? 1 : 0;
+}
+
+// table_load for a clean block: |xp| <= 1/2 (no clamp: the scale HTAB_R (1 - 2^-20) keeps xp = 1/2 inside the last cell), 32-bit
+// table indices, no integer-to-float conversion.  `row` = float4 index of the SFT's row in mtab (channel 0).
+template <int CT>
+__device__ __forceinline__ void table_load_fast(const KParams &p, float xp, float b, int kcidx, unsigned row, TableData<CT, 1> &d) {
+  constexpr float RM = 12582912.0f;
+  const float cm = fmaf(xp, (float)HTAB_R * (1.0f - 9.5367431640625e-7f), 0.5f * HTAB_R - 0.5f) + RM;
+  const unsigned cb = __float_as_uint(cm);
+  const unsigned cellH = cb & (unsigned)(HTAB_R - 1);
+  const float cHf = cm - RM;                                                      // (float)cellH
+  const float cSf = __uint_as_float(cb & ~(unsigned)((1 << HTAB_SHIFT) - 1)) - RM;   // cell << HTAB_SHIFT, cell = data-moment node
+  const float4 *mp = p.mtab + (row + ((unsigned)kcidx * TAB_R + (cellH >> HTAB_SHIFT)) * (unsigned)((TAB_Q + 1) / 2));
+  const float4 *hp = p.htab + ((unsigned)kcidx * HTAB_R + cellH) * (unsigned)(HTAB_W / 4);
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+#pragma unroll
+    for (int i = 0; i < TableData<CT, 1>::NL; ++i) d.Mq[c][i] = __ldg(mp + c * p.mchan + i);
+#pragma unroll
+    for (int i = 0; i < TableData<CT, 1>::NHL; ++i) d.Hq[c][i] = __ldg(hp + c * p.hchan + i);
+  }
+  d.aH = fmaf(cHf, -(2.0f * PI_F) / HTAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / HTAB_R)));
+  d.a = fmaf(cSf, -(2.0f * PI_F) / HTAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / TAB_R)));
+  d.be = PI_F * b;
+}
+
+// Phase, amplitude, response and noise weight for a clean block (every lane active and in band).  Where the template's
+// amplitude constant is real (no response) it is already inside `amp`.
+template <int CT, class CFG>
+__device__ __forceinline__ void finish_fast(const KParams &p, const Tmpl &tm, const float2 *rt, float amp, float t, const float (&s1r)[CT],
+                                            const float (&s1i)[CT], const float (&s2)[CT], const float (&us2)[CT], float &zr, float &zi,
+                                            float &hh) {
+  if (CFG::RESP == 0 && CT == 1) {
+    float sp, cp_;
+    sincospi_fast(t, sp, cp_);
+    const float er = cp_ * amp, ei = sp * amp;
+    zr = er * s1r[0] - ei * s1i[0];
+    zi = er * s1i[0] + ei * s1r[0];
+    hh = (amp * amp) * (us2[0] * s2[0]);
+  } else {
+    Track tr;
+    tr.amp = amp;
+    finish_terms<CT, CFG>(p, tm, rt, tr, true, 1.0f, t, s1r, s1i, s2, us2, zr, zi, hh);
+  }
+}
+
+// Transposed store of one tile of chunk-local prefix sums (MODE 1): rows = templates, 128-byte rows along the SFT axis.
+__device__ __forceinline__ void tile_store(const KParams &p, const float *txh, const float *thh, int tg, int g, int n, int lane) {
+  __syncwarp();
+  for (int r = 0; r < 32; ++r) {
+    const long long tt = (long long)tg * 32 + r;
+    if (tt < p.nT && lane < n) {
+      p.loc_xh[(size_t)tt * p.n_sft + g + lane] = txh[r * 33 + lane];
+      p.loc_hh[(size_t)tt * p.n_sft + g + lane] = thh[r * 33 + lane];
+    }
+  }
+  __syncwarp();
+}
+
+// The loop over the present SFTs of a clean block, two at a time.  Accumulates into axh / ahh / axi (fp64; fp32 partial
+// sums over the block).
+template <int CT, int MODE, class CFG, bool POLY>
+__device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, const float4 *cs, unsigned mask, const float (&usv)[CT],
+                                           float ascale, int g, int ge, int tg, int lane, long long t, bool want_kc, double &axh,
+                                           double &ahh, double &axi, float *txh, float *thh, unsigned long long *n_path) {
+  const int n = ge - g;
+  const unsigned row0 = (unsigned)g * p.mrow;
+  const float2 *rt = p.rtab + g;
+  int *kcp = (CFG::KC && want_kc) ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + g : nullptr;
+  if (MODE == 1) {                     // slots before the first present SFT keep the running sums
+    const int j0 = __ffs(mask) - 1;
+    for (int k = 0; k < j0; ++k) { txh[lane * 33 + k] = (float)axh; thh[lane * 33 + k] = (float)ahh; }
+  }
+  if (CFG::KC && kcp && t < p.nT) {
+    for (int k = 0; k < n; ++k)
+#pragma unroll
+      for (int c = 0; c < CT; ++c) kcp[(size_t)c * p.n_sft + k] = -1;
+  }
+  float fxh = 0.f, fhh = 0.f, fxi = 0.f;
+  while (mask) {
+    const int jA = __ffs(mask) - 1;
+    mask &= mask - 1;
+    const bool vB = mask != 0u;
+    const int jB = vB ? __ffs(mask) - 1 : jA;
+    mask &= mask - 1;                  // (0 stays 0)
+    FTrack A, B;
+    if (POLY) {
+      ftrack_poly2(cs, jA, jB, A, B);
+    } else {
+      ftrack_closed<CFG>(p, tm, (double)(g + jA), ascale, A);
+      ftrack_closed<CFG>(p, tm, (double)(g + jB), ascale, B);
+    }
+    float usA[CT], usB[CT];
+#pragma unroll
+    for (int c = 0; c < CT; ++c) {
+      usA[c] = __shfl_sync(0xffffffffu, usv[c], jA);
+      usB[c] = vB ? __shfl_sync(0xffffffffu, usv[c], jB) : 0.f;
+    }
+    TableData<CT, 1> dA, dB;
+    table_load_fast<CT>(p, A.xp, A.b, A.kc - p.kwin0 - 2, row0 + (unsigned)jA * p.mrow, dA);
+    table_load_fast<CT>(p, B.xp, B.b, B.kc - p.kwin0 - 2, row0 + (unsigned)jB * p.mrow, dB);
+    float s1rA[CT], s1iA[CT], s2A[CT], s1rB[CT], s1iB[CT], s2B[CT];
+    table_math2<CT, 1>(dA, dB, s1rA, s1iA, s2A, s1rB, s1iB, s2B);
+    float zrA, ziA, hhA, zrB, ziB, hhB;
+    // prefactor e^{i pi (x + b/4)},  x + b/4 = xp - b/4
+    finish_fast<CT, CFG>(p, tm, rt + jA, A.amp, fmaf(2.0f, A.frac, fmaf(-0.25f, A.b, A.xp)), s1rA, s1iA, s2A, usA, zrA, ziA, hhA);
+    finish_fast<CT, CFG>(p, tm, rt + jB, vB ? B.amp : 0.f, fmaf(2.0f, B.frac, fmaf(-0.25f, B.b, B.xp)), s1rB, s1iB, s2B, usB, zrB, ziB, hhB);
+    if (CFG::KC && p.path_counts) {
+      int np_ = 0;
+#pragma unroll
+      for (int c = 0; c < CT; ++c) np_ += (usA[c] > 0.f) + (vB && usB[c] > 0.f);
+      n_path[PATH_TABLE] += 32u * (unsigned)np_;
+    }
+    if (CFG::KC && kcp && t < p.nT) {
+#pragma unroll
+      for (int c = 0; c < CT; ++c) {
+        if (usA[c] > 0.f) kcp[(size_t)c * p.n_sft + jA] = A.kc;
+        if (vB && usB[c] > 0.f) kcp[(size_t)c * p.n_sft + jB] = B.kc;
+      }
+    }
+    if (MODE == 1) {
+      const int endA = vB ? jB : n, endB = mask ? __ffs(mask) - 1 : n;
+      axh += (double)zrA; ahh += (double)hhA;
+      for (int k = jA; k < endA; ++k) { txh[lane * 33 + k] = (float)axh; thh[lane * 33 + k] = (float)ahh; }
+      if (vB) {
+        axh += (double)zrB; ahh += (double)hhB;
+        for (int k = jB; k < endB; ++k) { txh[lane * 33 + k] = (float)axh; thh[lane * 33 + k] = (float)ahh; }
+      }
+    } else {
+      fxh += zrA + zrB;
+      fxi += ziA + ziB;
+      fhh += hhA + hhB;
+    }
+  }
+  if (MODE == 0) {
+    axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
+  } else {
+    tile_store(p, txh, thh, tg, g, n, lane);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Main fused kernel.  Persistent grid; every warp draws (32 templates) x (SFT chunk) work units from
 // p.counter.  CT == number of channels (exactly).
 // MODE 0: chunk totals only.  MODE 1 (cumulative): additionally writes chunk-local inclusive prefix
 // sums, transposed through shared memory so that global stores are 128-byte rows along the SFT axis.
-// The SFT loop runs in groups of GROUP: fp32 partial sums flushed into fp64 per group (MODE 0),
+// A work unit is walked in blocks of SUB = 32 SFT slots: clean blocks take the fast path above, all others the
+// generic loop below, which runs in groups of GROUP SFTs: fp32 partial sums flushed into fp64 per group (MODE 0),
 // one transposed store per group (MODE 1).
 // ---------------------------------------------------------------------------------------------
 template <int KT, int CT, int MODE, class CFG, int MINB, bool DUO>
 __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
   constexpr int GROUP = MODE == 1 ? 32 : FLUSH;
   __shared__ float tile_s[MODE == 1 ? (TILE / 32) * 2 * 32 * 33 : 1];
+  __shared__ float4 coef_s[COEF_V * TILE];             // polynomial-track coefficients of the current block, per thread
+  float4 *cs = coef_s + threadIdx.x;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float *txh = tile_s + (MODE == 1 ? warp * 2 * 32 * 33 : 0);
   float *thh = txh + (MODE == 1 ? 32 * 33 : 0);
@@ -993,133 +1349,144 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
     const long long t = (long long)tg * 32 + lane;
     const int a0 = ch * p.chunk;
     const int a1 = min(a0 + p.chunk, p.n_sft);
-    Tmpl tm;
-    tmpl_load<CT>(p, t, tm);
     double axh = 0.0, ahh = 0.0, axi = 0.0;
-    double dalpha = (double)a0;
-    const float *usp = p.us2 + a0;
-    const float2 *rt = p.rtab + a0;
-    const float4 *Drow0 = p.Dp + (size_t)a0 * p.npair;
-    const float4 *Mrow0 = p.mtab ? p.mtab + (size_t)a0 * p.mrow : nullptr;
-    int *kcp = want_kc ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + a0 : nullptr;
     unsigned long long n_path[PATH_N] = {0, 0, 0, 0, 0, 0, 0};
-    Track tr, tr2;                                   // tracks of SFT alpha and alpha + 1
-    track_eval<CFG>(p, tm, dalpha, tr);
-    track_eval<CFG>(p, tm, dalpha + 1.0, tr2);
 
-    for (int g = a0; g < a1; g += GROUP) {
-      const int ge = min(g + GROUP, a1);
-      float fxh = 0.f, fhh = 0.f, fxi = 0.f;
-      int alpha = g;
-      while (alpha < ge) {
-        float us2[CT], us2b[CT];
-        bool any = false, anyb = false;
-#pragma unroll
-        for (int c = 0; c < CT; ++c) {
-          us2[c] = __ldg(usp + c * p.n_sft);
-          any |= us2[c] > 0.f;                                   // warp-uniform
+    for (int gs = a0; gs < a1; gs += SUB) {
+      const int gend = min(gs + SUB, a1);
+      Tmpl tm;
+      tmpl_load<CT>(p, t, tm);
+      {
+        unsigned mask;
+        float usv[CT];
+        // where the template's amplitude constant is real (no response, one channel) it is folded into the amplitude
+        const float ascale = (CFG::RESP == 0 && CT == 1) ? tm.AE[0].x : 1.0f;
+        const int kind = fast_setup<CT, CFG>(p, tm, gs, gend, lane, ascale, cs, mask, usv);
+        if (kind == 2) {
+          fast_block<CT, MODE, CFG, true>(p, tm, cs, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
+          continue;
         }
-        const bool go = any && tr.active;
-        const float ab = (go && cfg_kernel<CFG>(p) == 1) ? fabsf(tr.b) : 0.f;
-        // two SFTs at once when both are present and both go through the tier-1 tables
-        bool duo = false, gob = false;
-        if (DUO && alpha + 1 < ge) {
+        if (kind == 1) {
+          fast_block<CT, MODE, CFG, false>(p, tm, cs, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
+          continue;
+        }
+      }
+      // ---- generic loop over [gs, gend) ----
+      double dalpha = (double)gs;
+      const float *usp = p.us2 + gs;
+      const float2 *rt = p.rtab + gs;
+      const float4 *Drow0 = p.Dp + (size_t)gs * p.npair;
+      const float4 *Mrow0 = p.mtab ? p.mtab + (size_t)gs * p.mrow : nullptr;
+      int *kcp = want_kc ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + gs : nullptr;
+      Track tr, tr2;                                   // tracks of SFT alpha and alpha + 1
+      track_eval<CFG>(p, tm, dalpha, tr);
+      track_eval<CFG>(p, tm, dalpha + 1.0, tr2);
+
+      for (int g = gs; g < gend; g += GROUP) {
+        const int ge = min(g + GROUP, gend);
+        float fxh = 0.f, fhh = 0.f, fxi = 0.f;
+        int alpha = g;
+        while (alpha < ge) {
+          float us2[CT], us2b[CT];
+          bool any = false, anyb = false;
 #pragma unroll
           for (int c = 0; c < CT; ++c) {
-            us2b[c] = __ldg(usp + c * p.n_sft + 1);
-            anyb |= us2b[c] > 0.f;
+            us2[c] = __ldg(usp + c * p.n_sft);
+            any |= us2[c] > 0.f;                                   // warp-uniform
           }
-          gob = anyb && tr2.active;
-          const float abb = (gob && cfg_kernel<CFG>(p) == 1) ? fabsf(tr2.b) : 0.f;
-          const float bm2 = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(ab, abb))));
-          duo = bm2 <= p.b_table && __any_sync(0xffffffffu, go) && __any_sync(0xffffffffu, gob);
-        }
-        if (duo) {
-          Track nA, nB;
-          float zrA, ziA, hhA, zrB, ziB, hhB;
-          duo_terms<CT, CFG>(p, tm, Mrow0, rt, tr, tr2, go, gob, us2, us2b, dalpha + 2.0, nA, nB, zrA, ziA, hhA, zrB, ziB, hhB);
-          if (CFG::KC && p.path_counts) {
-            int npa = 0, npb = 0;
+          const bool go = any && tr.active;
+          const float ab = (go && cfg_kernel<CFG>(p) == 1) ? fabsf(tr.b) : 0.f;
+          // two SFTs at once when both are present and both go through the tier-1 tables
+          bool duo = false, gob = false;
+          if (DUO && alpha + 1 < ge) {
 #pragma unroll
-            for (int c = 0; c < CT; ++c) { npa += us2[c] > 0.f; npb += us2b[c] > 0.f; }
-            n_path[PATH_TABLE] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * npa + __popc(__ballot_sync(0xffffffffu, gob)) * npb);
+            for (int c = 0; c < CT; ++c) {
+              us2b[c] = __ldg(usp + c * p.n_sft + 1);
+              anyb |= us2b[c] > 0.f;
+            }
+            gob = anyb && tr2.active;
+            const float abb = (gob && cfg_kernel<CFG>(p) == 1) ? fabsf(tr2.b) : 0.f;
+            const float bm2 = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(ab, abb))));
+            duo = bm2 <= p.b_table && __any_sync(0xffffffffu, go) && __any_sync(0xffffffffu, gob);
+          }
+          if (duo) {
+            Track nA, nB;
+            float zrA, ziA, hhA, zrB, ziB, hhB;
+            duo_terms<CT, CFG>(p, tm, Mrow0, rt, tr, tr2, go, gob, us2, us2b, dalpha + 2.0, nA, nB, zrA, ziA, hhA, zrB, ziB, hhB);
+            if (CFG::KC && p.path_counts) {
+              int npa = 0, npb = 0;
+#pragma unroll
+              for (int c = 0; c < CT; ++c) { npa += us2[c] > 0.f; npb += us2b[c] > 0.f; }
+              n_path[PATH_TABLE] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * npa + __popc(__ballot_sync(0xffffffffu, gob)) * npb);
+            }
+            if (CFG::KC && want_kc) {
+              if (t < p.nT) {
+#pragma unroll
+                for (int c = 0; c < CT; ++c) {
+                  kcp[(size_t)c * p.n_sft] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
+                  kcp[(size_t)c * p.n_sft + 1] = (tr2.active && us2b[c] > 0.f) ? tr2.kc : -1;
+                }
+              }
+              kcp += 2;
+            }
+            if (MODE == 1) {
+              axh += (double)zrA; ahh += (double)hhA;
+              txh[lane * 33 + (alpha - g)] = (float)axh;
+              thh[lane * 33 + (alpha - g)] = (float)ahh;
+              axh += (double)zrB; ahh += (double)hhB;
+              txh[lane * 33 + (alpha + 1 - g)] = (float)axh;
+              thh[lane * 33 + (alpha + 1 - g)] = (float)ahh;
+            } else {
+              fxh += zrA + zrB;
+              fxi += ziA + ziB;
+              fhh += hhA + hhB;
+            }
+            tr = nA; tr2 = nB;
+            alpha += 2; dalpha += 2.0; usp += 2; rt += 2; Drow0 += 2 * p.npair; Mrow0 += 2 * p.mrow;
+            continue;
+          }
+          Track nxt;                                               // track of SFT alpha + 2
+          if (__any_sync(0xffffffffu, go)) {
+            const float bmax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(ab)));
+            if (CFG::KC && p.path_counts) {
+              int n_present = 0;
+#pragma unroll
+              for (int c = 0; c < CT; ++c) n_present += us2[c] > 0.f;
+              n_path[path_of(bmax, p.mtab != nullptr)] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * n_present);
+            }
+            float zr, zi, hh;
+            pair_terms<KT, CT, CFG>(p, tm, Drow0, Mrow0, rt, tr, go, bmax, us2, dalpha + 2.0, nxt, zr, zi, hh);
+            if (MODE == 1) {
+              axh += (double)zr;
+              ahh += (double)hh;
+            } else {
+              fxh += zr;
+              fxi += zi;
+              fhh += hh;
+            }
+          } else {
+            track_eval<CFG>(p, tm, dalpha + 2.0, nxt);
           }
           if (CFG::KC && want_kc) {
             if (t < p.nT) {
 #pragma unroll
-              for (int c = 0; c < CT; ++c) {
-                kcp[(size_t)c * p.n_sft] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
-                kcp[(size_t)c * p.n_sft + 1] = (tr2.active && us2b[c] > 0.f) ? tr2.kc : -1;
-              }
+              for (int c = 0; c < CT; ++c) kcp[(size_t)c * p.n_sft] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
             }
-            kcp += 2;
+            ++kcp;
           }
+          tr = tr2;
+          tr2 = nxt;
           if (MODE == 1) {
-            axh += (double)zrA; ahh += (double)hhA;
             txh[lane * 33 + (alpha - g)] = (float)axh;
             thh[lane * 33 + (alpha - g)] = (float)ahh;
-            axh += (double)zrB; ahh += (double)hhB;
-            txh[lane * 33 + (alpha + 1 - g)] = (float)axh;
-            thh[lane * 33 + (alpha + 1 - g)] = (float)ahh;
-          } else {
-            fxh += zrA + zrB;
-            fxi += ziA + ziB;
-            fhh += hhA + hhB;
           }
-          tr = nA; tr2 = nB;
-          alpha += 2; dalpha += 2.0; usp += 2; rt += 2; Drow0 += 2 * p.npair; Mrow0 += 2 * p.mrow;
-          continue;
+          ++alpha; dalpha += 1.0; ++usp; ++rt; Drow0 += p.npair; Mrow0 += p.mrow;
         }
-        Track nxt;                                               // track of SFT alpha + 2
-        if (__any_sync(0xffffffffu, go)) {
-          const float bmax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(ab)));
-          if (CFG::KC && p.path_counts) {
-            int n_present = 0;
-#pragma unroll
-            for (int c = 0; c < CT; ++c) n_present += us2[c] > 0.f;
-            n_path[path_of(bmax, p.mtab != nullptr)] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * n_present);
-          }
-          float zr, zi, hh;
-          pair_terms<KT, CT, CFG>(p, tm, Drow0, Mrow0, rt, tr, go, bmax, us2, dalpha + 2.0, nxt, zr, zi, hh);
-          if (MODE == 1) {
-            axh += (double)zr;
-            ahh += (double)hh;
-          } else {
-            fxh += zr;
-            fxi += zi;
-            fhh += hh;
-          }
+        if (MODE == 0) {
+          axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
         } else {
-          track_eval<CFG>(p, tm, dalpha + 2.0, nxt);
+          tile_store(p, txh, thh, tg, g, ge - g, lane);
         }
-        if (CFG::KC && want_kc) {
-          if (t < p.nT) {
-#pragma unroll
-            for (int c = 0; c < CT; ++c) kcp[(size_t)c * p.n_sft] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
-          }
-          ++kcp;
-        }
-        tr = tr2;
-        tr2 = nxt;
-        if (MODE == 1) {
-          txh[lane * 33 + (alpha - g)] = (float)axh;
-          thh[lane * 33 + (alpha - g)] = (float)ahh;
-        }
-        ++alpha; dalpha += 1.0; ++usp; ++rt; Drow0 += p.npair; Mrow0 += p.mrow;
-      }
-      if (MODE == 0) {
-        axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
-      } else {
-        __syncwarp();
-        const int n = ge - g;
-        for (int r = 0; r < 32; ++r) {
-          const long long tt = (long long)tg * 32 + r;
-          if (tt < p.nT && lane < n) {
-            p.loc_xh[(size_t)tt * p.n_sft + g + lane] = txh[r * 33 + lane];
-            p.loc_hh[(size_t)tt * p.n_sft + g + lane] = thh[r * 33 + lane];
-          }
-        }
-        __syncwarp();
       }
     }
     if (t < p.nT) {

@@ -583,6 +583,11 @@ static cudaError_t launch_main(sft_plan *p, const KParams &k) {
   const bool bns = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 0;
   const bool newt = !diag && k.kernel == 1 && k.pn1 == 0 && k.response == 0;
   const bool lisa = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 2;
+#ifdef SFT_FEW_VARIANTS      // development builds: only the config-2 variant and the single-channel run-time-flag variant
+  (void)bns32; (void)newt; (void)lisa;
+  if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS>(p, k);
+  else launch_variant<0, 1, MODE, CfgAny>(p, k);
+#else
   if (bns32) launch_variant<8, 1, MODE, CfgBNS32>(p, k);
   else if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS>(p, k);
   else if (bns && C == 1 && K == 16) launch_variant<16, 1, MODE, CfgBNS>(p, k);
@@ -593,6 +598,7 @@ static cudaError_t launch_main(sft_plan *p, const KParams &k) {
   else if (C == 2) launch_variant<0, 2, MODE, CfgAny>(p, k);
   else if (C == 3) launch_variant<0, 3, MODE, CfgAny>(p, k);
   else launch_variant<0, 4, MODE, CfgAny>(p, k);
+#endif
   cudaEventRecord(p->ev1, p->stream);
   p->timed = true;
   p->launches++;

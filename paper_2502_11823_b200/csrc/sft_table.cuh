@@ -21,8 +21,9 @@
 // 2.4e-7 at |b| = 1.0 (7e-6 at 1.5).  |b| > B_TABLE2 = 1 takes the direct evaluator of sft_kernels.cuh.
 //
 // The <h,h> sum H(kc, xp, b) = sum_m u_{kc+m} |J_m|^2 (u = S_ref/S_k) does not depend on the data at
-// all; it is even in b and tabulated per window position on HTAB_R nodes per bin as
-//   H = sum_{P<=5} a^P sum_N beta^(2N) h_{P,2N}:  N <= 1: relative error < 3e-7 for |b| <= 0.12;  N <= 3: 9e-8 at |b| = 1.
+// all; it is even in b and tabulated per window position on HTAB_R = 64 nodes per bin as
+//   H = sum_{P<=3} a^P sum_N beta^(2N) h_{P,2N}:  N <= 1: relative error < 3e-7 for |b| <= 0.12;  N <= 3: 9e-8 at |b| = 1
+// (|a| <= 2 pi / 128 = 0.05 about a node: the cubic in a is exact to ~1e-8; 32 bytes and 7 FMAs per (template, SFT) in tier 1).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -32,10 +33,12 @@ namespace sftk {
 constexpr int TAB_R = 4;      // nodes per bin of the data-moment table
 constexpr int TAB_Q = 15;     // highest moment kept (TAB_Q + 1 complex64 = 128 bytes per node)
 constexpr int TAB_Q1 = 7;     // highest moment used by tier 1 (the first 64 bytes of a node)
-constexpr int HTAB_R = 16;    // nodes per bin of the <h,h> table
-constexpr int HTAB_P = 5;     // highest power of a kept
+constexpr int HTAB_R = 64;    // nodes per bin of the <h,h> table
+constexpr int HTAB_SHIFT = 4; // HTAB_R = TAB_R << HTAB_SHIFT: the data-moment node of an <h,h> node is cellH >> HTAB_SHIFT
+constexpr int HTAB_P = 3;     // highest power of a kept (|a| <= 2 pi / 128: the a^4 term is below 1e-7 of H)
 constexpr int HTAB_NB = 4;    // powers of beta^2 kept: beta^0, beta^2, beta^4, beta^6 (tier 1 uses the first two)
-constexpr int HTAB_W = 32;    // floats per node: h_{0..5,0}, h_{0..5,2}, h_{0..5,4}, h_{0..5,6}, 8 x pad
+constexpr int HTAB_W = 16;    // floats per node: h_{0..3,0}, h_{0..3,2}, h_{0..3,4}, h_{0..3,6} (tier 1 reads the first 32 bytes)
+static_assert(HTAB_R == (TAB_R << HTAB_SHIFT) && HTAB_W == HTAB_NB * (HTAB_P + 1) && HTAB_W % 4 == 0, "table geometry");
 constexpr float B_TABLE = 0.12f;    // tier 1: moments q <= 7, H to beta^2
 constexpr float B_TABLE2 = 1.0f;    // tier 2: moments q <= 15, H to beta^6
 
