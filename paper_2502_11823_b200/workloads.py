@@ -231,6 +231,26 @@ def et_bns_bank(w, n_templates, bank_seed=55):
     return w2
 
 
+def et_bns_wide_bank(w, n_templates, bank_seed=56):
+    """The data of ``w`` (an ``et_bns`` workload) with a WIDE, shuffled bank: chirp mass +-10 %, eta in [0.2, 0.25],
+    coalescence times from a third of the way through the data to 3000 s after its end, phases uniform.  Neighbouring
+    rows (the 32 templates a warp holds) then sit at different bins (tens of bins apart), at different drifts b = fdot T^2
+    (0.01 ... > 4), and some are ended, out of band or not yet in band at the same SFT.  Row 0 stays the injected signal."""
+    import copy
+    rng = np.random.default_rng(bank_seed)
+    T_obs = w.desc["n_sft"] * w.desc["t_sft"]
+    P = _rows(n_templates)
+    P[:] = w.injection
+    P[:, 0] *= 1.0 + rng.uniform(-0.1, 0.1, n_templates)
+    P[:, 1] = rng.uniform(0.2, 0.25, n_templates)
+    P[:, 2] = rng.uniform(T_obs / 3.0, T_obs + 3000.0, n_templates)
+    P[:, 3] = rng.uniform(0.0, 2.0 * np.pi, n_templates)
+    P[0] = w.injection
+    w2 = copy.copy(w)
+    w2.params = P
+    return w2
+
+
 def config2(**kw):
     return et_bns(**kw)
 
