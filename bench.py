@@ -64,25 +64,56 @@ def oracle_objects(w):
     return oin, plan, store
 
 
-def time_oracle(w, budget_s=12.0, max_templates=None):
-    """Times oracle.inner.inner_products (as it stands) on the first n templates of the workload,
-    n chosen so the run takes about ``budget_s`` seconds.  Returns (pairs/s, n, seconds, active pairs)."""
+def cores_used():
+    """--impl reference runs the oracle in this process: single-threaded numpy elementwise code (no BLAS call on its hot
+    path), so 1; the number of host cores available is reported beside it."""
+    return 1
+
+
+_ORACLE = {}
+
+
+def _oracle_init(desc, bins, psd_scale, psd_shape, response):
+    from oracle import inner as oin
+    _ORACLE["oin"] = oin
+    _ORACLE["plan"] = oin.Plan(**desc)
+    _ORACLE["store"] = oin.Store(bins=bins.astype(np.complex128), psd_scale=psd_scale, psd_shape=psd_shape,
+                                 response=None if response is None else response.astype(np.complex128))
+
+
+def _oracle_rows(rows):
+    r = _ORACLE["oin"].inner_products(_ORACLE["plan"], _ORACLE["store"], rows)
+    return int((r["kc"] >= 0).sum())
+
+
+def time_oracle(w, budget_s=12.0, seed=99):
+    """Times oracle.inner.inner_products (as it stands: numpy fp64, one call per block of templates) on a seeded sample of
+    the workload's templates, spread over the host cores with one worker process per core (the oracle itself is
+    single-threaded elementwise numpy).  The sample is sized from a one-template probe so that the run takes about
+    ``budget_s`` seconds.  Returns (pairs/s, templates, seconds, active pairs, worker processes)."""
+    import multiprocessing as mp
     oin, plan, store = oracle_objects(w)
     t0 = time.perf_counter()
-    r = oin.inner_products(plan, store, w.params[:1])
-    t1 = time.perf_counter() - t0
-    n = int(max(1, min(w.n_templates if max_templates is None else max_templates, budget_s / max(t1, 1e-6))))
-    t0 = time.perf_counter()
-    r = oin.inner_products(plan, store, w.params[:n])
-    dt = time.perf_counter() - t0
-    pairs = int((r["kc"] >= 0).sum())
-    return pairs / dt, n, dt, pairs
-
-
-def cores_used():
-    """Threads the oracle actually uses: it is single-threaded numpy elementwise code (no BLAS call
-    on its hot path), so 1; the number of host cores available is reported beside it."""
-    return 1
+    oin.inner_products(plan, store, w.params[:1])
+    t1 = max(time.perf_counter() - t0, 1e-6)
+    cores = max(1, min(32, len(os.sched_getaffinity(0))))
+    n = int(max(1, min(w.n_templates, cores * budget_s / t1)))
+    rows = w.params[np.sort(np.random.default_rng(seed).choice(w.n_templates, size=n, replace=False))]
+    if n < 4 * cores:
+        cores = 1
+    if cores == 1:
+        t0 = time.perf_counter()
+        pairs = int((oin.inner_products(plan, store, rows)["kc"] >= 0).sum())
+        return pairs / (time.perf_counter() - t0), n, time.perf_counter() - t0, pairs, 1
+    blk = max(1, n // (4 * cores))
+    # "spawn": this process holds a CUDA context, which must not be forked
+    with mp.get_context("spawn").Pool(cores, initializer=_oracle_init,
+                                      initargs=(dict(w.desc), w.bins, w.psd_scale, w.psd_shape, w.response)) as pool:
+        pool.map(_oracle_rows, [rows[:1]] * cores)                       # workers up and warm before the clock starts
+        t0 = time.perf_counter()
+        pairs = sum(pool.map(_oracle_rows, [rows[i:i + blk] for i in range(0, n, blk)]))
+        dt = time.perf_counter() - t0
+    return pairs / dt, n, dt, pairs, cores
 
 
 # ---------------------------------------------------------------------------------------------
@@ -169,6 +200,96 @@ def run_reference(args, rank, world):
                          "host_cores_available": len(os.sched_getaffinity(0))},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}), flush=True)
+
+
+def aux_measurements(w2, plan, dev, stream, flush, pk, steps=5, warmup=3):
+    """Beside the headline line: the two other calls of the library on the same data, a few steps each, so that the
+    driver's record carries them - (i) ``sft_cumulative_snr`` on BASELINE.json configs[2] (16,384 templates, SNR(t) matrix
+    16,384 x 10,800 fp32 = 708 MB written per step), (ii) ``sft_compute_sfts`` on a config-2 shaped
+    series (HBM roofline).  Each carries its own roofline and clocks."""
+    import torch
+    from paper_2502_11823_b200 import api, workloads as wl
+    out = {}
+    w3 = wl.et_bns_bank(w2, 16384, bank_seed=6)                 # = workloads.config3(): same data, the 16,384-template bank
+    nT, N = w3.n_templates, plan.n_sft
+    P = torch.from_numpy(np.ascontiguousarray(w3.params)).to(dev)
+    ns = 64
+    kc = torch.empty((ns, plan.n_channels, N), dtype=torch.int32, device=dev)
+    x3 = [torch.empty(ns, dtype=torch.float64, device=dev) for _ in range(3)]
+    plan.inner_products(P[:ns].contiguous(), x3[0], x3[1], x3[2], kc)
+    plan.sync()
+    pairs = int((kc >= 0).sum().item()) * nT // ns
+    paths = plan.path_counts()
+    snr = torch.empty((nT, N), dtype=torch.float32, device=dev)
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    ms, kms = 0.0, []
+    for i in range(warmup + steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        plan.cumulative_snr(P, snr, None, None)
+        b.record(stream)
+        torch.cuda.synchronize()
+        if i >= warmup:
+            ms += a.elapsed_time(b)
+            kms.append(plan.last_kernel_ms())
+    clocks = sampler.stop()
+    ms /= steps
+    roof = roofline(w3, pairs, float(np.mean(kms)), paths, "auto", pk)
+    hbm, src = hbm_peak()
+    roof["output_hbm"] = {"bytes_written_per_step": int(snr.numel() * 4), "achieved_gbs": snr.numel() * 4 / (ms * 1e-3) / 1e9,
+                          "peak_gbs": hbm, "peak_source": src}
+    out["config3_cumulative_snr"] = {"value": pairs / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "steps": steps, "warmup": warmup,
+                                     "templates": nT, "active_pairs": pairs, "gpu_launches_per_step": 2, "roofline": roof,
+                                     "clocks": clocks}
+    del snr, P, kc
+    out["ingest_compute_sfts"] = ingest_measurement(steps=steps, warmup=warmup, dev=dev, stream=stream, flush=flush)
+    return out
+
+
+def hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ingest_measurement(steps, warmup, dev, stream, flush):
+    """sft_compute_sfts on a series shaped like config 2 (10,800 segments of 16,384 float64 samples, 1.42 GB, device
+    resident; band bins 5..186).  HBM-bound: the series is read once."""
+    import torch
+    from paper_2502_11823_b200 import api
+    n_sft, n, k_lo, k_hi, dt = 10800, 16384, 5, 187, 1.0 / 2048.0
+    g = torch.Generator(device=dev)
+    g.manual_seed(11)
+    x = torch.randn(n_sft * n, dtype=torch.float64, device=dev, generator=g) * 1e-23
+    bins = torch.empty((n_sft, k_hi - k_lo), dtype=torch.complex64, device=dev)
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    ms = 0.0
+    for i in range(warmup + steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        api.compute_sfts(x, n_sft, n, dt, k_lo, k_hi, bins, device=dev.index or 0, stream=stream.cuda_stream)
+        b.record(stream)
+        torch.cuda.synchronize()
+        if i >= warmup:
+            ms += a.elapsed_time(b)
+    clocks = sampler.stop()
+    ms /= steps
+    nbytes = x.numel() * 8 + bins.numel() * 8
+    peak, src = hbm_peak()
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    return {"metric": "data-SFT generation (sft_compute_sfts)", "value": x.numel() / (ms * 1e-3), "unit": "samples/s",
+            "ms_per_step": ms, "steps": steps, "warmup": warmup, "dtype": "f32 (f64 input)", "data": "synthetic",
+            "config": {"workload": "config2-shaped series", "n_sft": n_sft, "n": n, "band": [k_lo, k_hi],
+                       "cache": "l2_flush_between_steps; includes the end-of-call sync"},
+            "clocks": clocks,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                         "traffic": None, "peak_source": src, "alg_bytes": nbytes}}
 
 
 def aggregate_over_ranks(ms_dev, ms_host_step, pairs, device, world):
@@ -284,14 +405,14 @@ def run_ours(args, rank, world, local_rank):
     value = pairs_all / (ms_step * 1e-3)
     e2e = pairs_all / (ms_host_step * 1e-3)
     k_ms = float(np.mean(kms)) if kms else None
-    roof = roofline(w, pairs, k_ms, paths, args.evaluator)
-    if roof:
-        # pipe rates of this GPU (Gop/s) and the schedulers' sustained rate on the table kernel's instruction mix
-        # with every stall removed (instructions/clock/scheduler): the ceiling for that mix, beside the nominal peak
-        pk = api.measure_alu_peaks(local_rank)
-        roof["measured_alu"] = pk
-        roof["frac_of_mix_ceiling"] = roof["frac"] / pk["table_mix_ipc"] if pk.get("table_mix_ipc") else None
-    cpu_val, cpu_n, cpu_dt, cpu_pairs = time_oracle(w, budget_s=args.cpu_budget)
+    # pipe rates of this GPU (Gop/s) and the schedulers' sustained rate on the table kernel's instruction mix with
+    # every stall removed (instructions/clock/scheduler): the ceiling for that mix, beside the nominal peak
+    pk = api.measure_alu_peaks(local_rank)
+    roof = roofline(w, pairs, k_ms, paths, args.evaluator, pk)
+    aux = None
+    if world == 1 and args.workload == "config2" and not args.no_aux and not args.templates and not args.n_sft:
+        aux = aux_measurements(w, plan, dev, stream, flush, pk)
+    cpu_val, cpu_n, cpu_dt, cpu_pairs, cpu_cores = time_oracle(w, budget_s=args.cpu_budget)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -306,11 +427,12 @@ def run_ours(args, rank, world, local_rank):
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(P_np.nbytes), "d2h_bytes_per_step": int(d2h_bytes),
                 "ms_per_step": ms_host_step, "steps": e2e_steps},
         "gpu_launches": int(launches), "kernel_ms": k_ms, "results_finite": ok,
-        "clocks": clocks, "roofline": roof,
-        "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores_used(), "kind": "oracle",
+        "clocks": clocks, "roofline": roof, "aux": aux,
+        "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",
                          "host_cores_available": len(os.sched_getaffinity(0)),
-                         "sample": "first %d of %d templates x all %d SFT slots (%d active pairs) in %.1f s, "
-                                   "oracle.inner.inner_products numpy fp64" % (cpu_n, nT, w.desc["n_sft"], cpu_pairs, cpu_dt)},
+                         "sample": "%d seeded templates (rng 99) of %d x all %d SFT slots (%d active pairs) in %.1f s, "
+                                   "oracle.inner.inner_products numpy fp64, one worker process per core" % (
+                                       cpu_n, nT, w.desc["n_sft"], cpu_pairs, cpu_dt)},
     }
     print(json.dumps(out), flush=True)
     plan.close()
@@ -318,23 +440,27 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
-# DRAM bytes (read + write) of one main-kernel launch from the ncu --set full captures (config2-F;
-# dram__bytes_read.sum + dram__bytes_write.sum): profiles/r01f_final_tables2.md (tables), r01d_kernel_v7_tables.md (direct).
-NCU_TRAFFIC = {("config2-F", "auto"): 1.952512e6 + 12.8e3, ("config2-F", "table"): 1.952512e6 + 12.8e3,
-               ("config2-F", "direct"): 8.213504e6 + 10.752e3}
+# DRAM bytes (read + write) of one main-kernel launch, from the committed ncu --set full captures (dram__bytes_read.sum +
+# dram__bytes_write.sum): NOT measured by this run - the source capture is named in roofline.traffic_source.
+NCU_TRAFFIC = {
+    ("config2-F", "auto"): (2.219008e6 + 0.401408e6, "profiles/r02a_main_fastpath.md"),
+    ("config2-F", "table"): (2.219008e6 + 0.401408e6, "profiles/r02a_main_fastpath.md"),
+    ("config2-F", "direct"): (8.213504e6 + 10.752e3, "profiles/r01d_kernel_v7_tables.md"),
+}
 
-# Algorithmic work per active pair and the ALU peak: DESIGN.md §7.
+# Algorithmic work per active pair and the ALU peak: DESIGN.md section 7.
 SM_COUNT, SM_MAX_GHZ = 148, 1.965
 S_ORDER = {"series0": 1, "series1": 4, "series2": 11, "series3": 16}     # packed-lane ops of the far-bin recurrence
 
 
 def alg_instr_per_pair(path, K, C):
-    """Warp instructions the formulation needs per active (template, SFT) pair on evaluator path
-    ``path`` (a packed FFMA2/FMUL2 counts as ONE instruction, as it takes one issue slot):
-    fixed part = fp64 track 50 + SFT loop 13 + phase/prefactor/response/accumulation 23 (+12 per extra
-    channel); table tier 1: 21 shared + 38 per channel, tier 2: 21 + 134 per channel; series order n: per far bin 2.5 (reciprocal pair) +
-    s_n/2 + 1 (|J|^2) + 3.5 C (load + MACs), central bin 7(n+1) + 2 + 7 C; closed Fresnel form: 64 + 3.5 C
-    per bin."""
+    """The FIXED per-unit figure of the roofline: warp instructions of the moment-table / series /
+    closed-Fresnel formulation per active (template, SFT) pair on evaluator path ``path``, as counted for the round-1 kernel
+    (closed-form fp64 track 50 + SFT loop 13 + phase/prefactor/response/accumulation 23 (+12 per extra channel); table tier 1:
+    21 + 38 per channel, tier 2: 21 + 134 per channel; series order n: per far bin 2.5 + s_n/2 + 1 + 3.5 C, central bin
+    7(n+1) + 2 + 7 C; closed Fresnel form: 64 + 3.5 C per bin; a packed FFMA2/FMUL2 = ONE instruction).  It is kept fixed so
+    that fractions stay comparable from round to round: a kernel that needs fewer instructions for the same pairs (the
+    polynomial track of round 2) shows up as a higher fraction, exactly as a faster kernel should."""
     fixed = 86 + 12 * (C - 1)
     if path == "table":
         return fixed + 21 + 38 * C
@@ -346,26 +472,59 @@ def alg_instr_per_pair(path, K, C):
     return fixed + 2 * K * (2.5 + S_ORDER[path] / 2.0 + 1 + 3.5 * C) + 7 * (n + 1) + 2 + 7 * C
 
 
-def roofline(w, pairs, kernel_ms, paths, evaluator="auto"):
-    """Issue-slot roofline of the fused main kernel.  The data are L2/L1 resident, so the
-    path is bound by plain ALU work; with the moment tables no single pipe dominates (ncu: FMA 38 %,
-    XU 34 %, ALU 26 %, FP64 23 %) and the binding resource is the warp schedulers' issue rate:
-    peak = 148 SMs x 4 schedulers x 1 warp instruction/clock x 32 lanes x 1.965 GHz (numerically equal
-    to the FP32 lane peak).  achieved = algorithmic instructions of the measured path mix x 32 lanes x
-    warp-pairs / kernel time."""
+def kernel_instr_per_pair(path, K, C, strict=False):
+    """What the CURRENT kernel issues per pair on its common path (clean block, polynomial track, tier-1 tables; counted
+    in the SASS of the hot loop, profiles/r02a_main_fastpath.md): track 29 (11 fp64, 3 conversions, 13 fp32, 2 constant
+    loads), S1 29 C (19 packed FMAs + 10 scalings), H 8 C, 6 C table loads, prefactor 15 + 12 (C - 1), accumulation 3;
+    plus - not in the strict count - node / address arithmetic 19 C and the loop over the presence mask 9.  Other paths as
+    in alg_instr_per_pair with the cheaper track (-21) where the block is clean."""
+    if path == "table":
+        core = 29 + (29 + 8 + 6) * C + 15 + 12 * (C - 1) + 3
+        return core if strict else core + 19 * C + 9
+    full = alg_instr_per_pair(path, K, C)
+    return full - 34 if strict else full           # strict: without the 13 loop + 21 node/constant instructions
+
+
+def roofline(w, pairs, kernel_ms, paths, evaluator="auto", pk=None):
+    """Issue-slot roofline of the fused main kernel.  The data are L2/L1 resident, so the path is
+    bound by plain ALU work; no single pipe dominates (ncu: FMA 34 %, XU 31 %, LSU 22 %, ALU 17 %, FP64 15 %) and the
+    binding resource is the warp schedulers' issue rate: peak = 148 SMs x 4 schedulers x 1 warp instruction/clock x 32 lanes
+    x 1.965 GHz (numerically the FP32 lane peak).  achieved = per-pair figure of the measured path mix x 32 lanes x
+    warp-pairs / kernel time (CUDA events around the launch on the plan's stream)."""
     if not kernel_ms or not paths:
         return None
     K, C = int(w.desc["K"]), int(w.desc["n_channels"])
     tot = float(sum(paths.values()))
     mix = {k: v / tot for k, v in paths.items() if v}
-    ops_pair = sum(f * alg_instr_per_pair(k, K, C) for k, f in mix.items())
     peak = SM_COUNT * 4 * 32 * SM_MAX_GHZ          # G lane-instructions/s
-    achieved = ops_pair * (pairs / C) / (kernel_ms * 1e-3) / 1e9       # pairs counts channels; tracks do not
-    return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "G lane-instructions/s (issue slots)",
-            "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((w.name, evaluator)), "kernel": "sft_main_kernel",
-            "kernel_ms": kernel_ms,
-            "alg_instr_per_pair": ops_pair, "path_mix": mix,
-            "peak_source": "derived: 148 SM x 4 schedulers x 32 lanes x 1.965 GHz (B200_PROFILING.md unit counts/clocks), DESIGN.md §7"}
+    rate = (pairs / C) / (kernel_ms * 1e-3) / 1e9  # G (template, SFT) lane-pairs/s; pairs counts channels, tracks do not
+
+    def per_pair(fn, **kw):
+        return sum(f * fn(k, K, C, **kw) for k, f in mix.items())
+
+    ops_fixed = per_pair(alg_instr_per_pair)
+    ops_kernel = per_pair(kernel_instr_per_pair)
+    ops_strict = per_pair(kernel_instr_per_pair, strict=True)
+    traffic, tsrc = NCU_TRAFFIC.get((w.name, evaluator), (None, None))
+    r = {"bound": "alu", "achieved": ops_fixed * rate, "peak": peak, "unit": "G lane-instructions/s (issue slots)",
+         "frac": ops_fixed * rate / peak, "traffic": traffic,
+         "traffic_source": ("ncu capture " + tsrc + " (not measured by this run)") if tsrc else None,
+         "kernel": "sft_main_kernel", "kernel_ms": kernel_ms,
+         "alg_instr_per_pair": ops_fixed,
+         "alg_instr_source": "fixed per-unit figure of DESIGN.md section 7 (formulation as counted in round 1)",
+         "kernel_instr_per_pair": ops_kernel, "frac_kernel_count": ops_kernel * rate / peak,
+         "alg_instr_strict": ops_strict, "frac_strict": ops_strict * rate / peak,
+         "path_mix": mix,
+         "peak_source": "nominal: 148 SM x 4 schedulers x 32 lanes x 1.965 GHz (B200_PROFILING.md unit counts/clocks), DESIGN.md section 7"}
+    if pk:
+        # against what this GPU measurably issues: plain FFMA lane rate (one instruction per clock and scheduler in practice)
+        # and the ceiling of the table kernel's own instruction mix with every stall removed
+        r["measured_alu"] = pk
+        if pk.get("ffma"):
+            r["frac_of_measured_ffma_issue"] = ops_fixed * rate / pk["ffma"]
+        if pk.get("table_mix_ipc"):
+            r["frac_of_mix_ceiling"] = r["frac"] / pk["table_mix_ipc"]
+    return r
 
 
 def run_sweep(args):
@@ -431,7 +590,7 @@ def run_sweep(args):
         norm = np.sqrt(oin.xx_band(op, st) * o["hh"])
         g_xh, g_hh = xh.cpu().numpy()[rows], hh.cpu().numpy()[rows]
         err = float(max(np.max(np.abs(g_xh - o["xh"]) / norm), np.max(np.abs(g_hh - o["hh"]) / norm)))
-        roof = roofline(w, pairs, float(np.mean(kms)), paths)
+        roof = roofline(w, pairs, float(np.mean(kms)), paths, pt["evaluator"])
         print(json.dumps(dict(pt, workload="config5", active_pairs=pairs, ms_per_step=ms / steps,
                               kernel_ms=float(np.mean(kms)), pairs_per_s=pairs / (ms / steps * 1e-3),
                               roofline_frac=roof["frac"], alg_instr_per_pair=roof["alg_instr_per_pair"],
@@ -441,46 +600,14 @@ def run_sweep(args):
 
 
 def run_ingest(args):
-    """--ingest: SURVEY section 8(f) NEXT-1 - sft_compute_sfts on a series shaped like config 2 (10,800 segments of
-    16,384 float64 samples, 1.42 GB, device resident; band bins 5..186).  HBM-bound: the series is read once.
-    One JSON line: samples/s and achieved GB/s against the measured copy bandwidth (MEASURED_PEAKS.json)."""
+    """--ingest: SURVEY section 8(f) NEXT-1 - one JSON line: samples/s and achieved GB/s against the measured copy bandwidth."""
     import torch
-    from paper_2502_11823_b200 import api, build
+    from paper_2502_11823_b200 import build
     build.build()
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
-    n_sft, n, k_lo, k_hi, dt = 10800, 16384, 5, 187, 1.0 / 2048.0
-    g = torch.Generator(device=dev)
-    g.manual_seed(11)
-    x = torch.randn(n_sft * n, dtype=torch.float64, device=dev, generator=g) * 1e-23
-    bins = torch.empty((n_sft, k_hi - k_lo), dtype=torch.complex64, device=dev)
-    stream = torch.cuda.current_stream()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    ms = 0.0
-    for i in range(args.warmup + args.steps):
-        flush.zero_()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        api.compute_sfts(x, n_sft, n, dt, k_lo, k_hi, bins, device=0, stream=stream.cuda_stream)
-        b.record(stream)
-        torch.cuda.synchronize()
-        if i >= args.warmup:
-            ms += a.elapsed_time(b)
-    ms /= args.steps
-    nbytes = x.numel() * 8 + bins.numel() * 8
-    peak, src = 6650.0, "fallback (B200_PROFILING.md)"
-    try:
-        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-            peak, src = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
-    except Exception:
-        pass
-    gbs = nbytes / (ms * 1e-3) / 1e9
-    print(json.dumps({"metric": "data-SFT generation (sft_compute_sfts)", "value": x.numel() / (ms * 1e-3), "unit": "samples/s",
-                      "ms_per_step": ms, "steps": args.steps, "warmup": args.warmup, "dtype": "f32 (f64 input)", "data": "synthetic",
-                      "config": {"workload": "config2-shaped series", "n_sft": n_sft, "n": n, "band": [k_lo, k_hi],
-                                 "cache": "l2_flush_between_steps; includes the twiddle-table kernel and the end-of-call sync"},
-                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
-                                   "traffic": None, "peak_source": src, "alg_bytes": nbytes}}), flush=True)
+    print(json.dumps(ingest_measurement(args.steps, args.warmup, dev, torch.cuda.current_stream(), flush)), flush=True)
 
 
 def main():
@@ -498,6 +625,7 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="config-5 scaling sweep (one JSON line per point)")
     ap.add_argument("--ingest", action="store_true", help="time the GPU data-SFT generation (NEXT-1)")
     ap.add_argument("--cpu-budget", type=float, default=12.0, dest="cpu_budget")
+    ap.add_argument("--no-aux", action="store_true", dest="no_aux", help="skip the config-3 and ingest side measurements")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

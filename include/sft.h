@@ -87,6 +87,9 @@ typedef struct {
   double resp_chi[SFT_MAX_CHANNELS]; /* SFT_RESP_ANNUAL: response phase per channel             */
   int32_t evaluator;   /* SFT_EVAL_*: how sum_k conj(x~) F / S and sum_k |F|^2 / S are evaluated for
                           |fdot| T^2 <= 1; results agree to ~1e-6 */
+  int32_t include_dc;  /* 0: bins k < 1 never contribute (DESIGN A6: int_0^inf of Eq.(1), PSDs diverging at f = 0);
+                          1: the bin k = 0 counts at full weight, as in the paper's sums ("d~[k] = 0 for k < 0") -
+                          needed by signals below the first bin (edge effects, section IV.D)    */
   int32_t device;      /* CUDA device ordinal                                             */
   void *stream;        /* cudaStream_t to order work on, or NULL for the legacy default stream */
 } sft_plan_desc;

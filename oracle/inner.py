@@ -58,6 +58,7 @@ class Plan:
     resp_depth: float = 0.3
     resp_psi: tuple = (0.0, 0.0)
     resp_chi: tuple = (0.0, 0.0)
+    include_dc: int = 0            # 0: bins k < 1 never contribute (reading A6); 1: k = 0 counts ("d~[k] = 0 for k < 0")
 
     @property
     def n_samp(self):
@@ -182,7 +183,7 @@ def band_terms_from_track(plan, store, t, A, phi, f, fdot, t_c, R):
     Fk = kernel_coefficients(plan, x[idx], b[idx])                    # [n_act][2K+1]
     m = np.arange(-K, K + 1, dtype=np.int64)
     k = k_c[idx][:, None] + m[None, :]                                # absolute bin index
-    valid = (k >= 1) & (k <= n // 2 - 1) & (k >= plan.k_lo) & (k < plan.k_hi)   # reading A6
+    valid = (k >= (0 if plan.include_dc else 1)) & (k <= n // 2 - 1) & (k >= plan.k_lo) & (k < plan.k_hi)   # reading A6
     col = np.clip(k - plan.k_lo, 0, plan.k_hi - plan.k_lo - 1)
     pref = A[idx] * np.exp(1j * phi[idx])                             # A_a e^{i phi_a}
     for c in range(C):
@@ -239,7 +240,7 @@ def xx_band(plan, store):
     """<x,x> restricted to the stored band: 4 df sum |x~|^2/S over present SFTs and valid bins."""
     n = plan.n_samp
     k = np.arange(plan.k_lo, plan.k_hi)
-    valid = (k >= 1) & (k <= n // 2 - 1)
+    valid = (k >= (0 if plan.include_dc else 1)) & (k <= n // 2 - 1)
     present = store.present()
     tot = 0.0
     for c in range(plan.n_channels):

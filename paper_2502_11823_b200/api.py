@@ -40,7 +40,7 @@ class PlanDesc(C.Structure):
                 ("f_lo", C.c_double), ("f_hi", C.c_double), ("f_ref", C.c_double),
                 ("resp_period", C.c_double), ("resp_depth", C.c_double),
                 ("resp_psi", C.c_double * MAX_CHANNELS), ("resp_chi", C.c_double * MAX_CHANNELS),
-                ("evaluator", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p)]
+                ("evaluator", C.c_int32), ("include_dc", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p)]
 
 
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
@@ -160,6 +160,7 @@ class Plan:
             pd.resp_chi[i] = float(v)
         ev = d.get("evaluator", "auto")
         pd.evaluator = EVALUATOR[ev] if isinstance(ev, str) else int(ev)
+        pd.include_dc = int(d.get("include_dc", 0))
         pd.device = int(device)
         pd.stream = C.c_void_p(int(stream)) if stream else None
         self.desc = pd

@@ -76,7 +76,11 @@ struct KParams {
   float b_table, b_table2; // B_TABLE, B_TABLE2 if the plan has the tables, else -1 (no |b| qualifies)
   double *part;            // [n_chunks][3][nT] chunk totals (xh, hh, xh_im)
   int *kc_out;             // [nT][C][n_sft] or null
-  float *loc_xh, *loc_hh;  // cumulative mode: [nT][n_sft] chunk-local prefix sums
+  // cumulative mode (MODE 1): single-pass scan over the SFT axis with decoupled look-back (one work unit = 32 SFT slots)
+  float *out_snr, *out_cx, *out_ch;   // [nT][n_sft] outputs, each nullable
+  double2 *scanA, *scanP;  // [n_chunks][nT] {xh, hh}: a unit's own totals (aggregate) / totals of all SFTs up to its end (inclusive)
+  unsigned *flagA, *flagP; // [n_chunks][nT]: == epoch once the entry of this call has been published
+  unsigned epoch;
 };
 
 __device__ __forceinline__ float rcp_approx(float x) {
@@ -1076,8 +1080,11 @@ __device__ __forceinline__ bool fast_coef(const KParams &p, const Tmpl &tm, int 
          eps <= POLY_EPS_MAX && eps > 0.0;
 }
 
-// The coefficients live in shared memory between the set-up of a block and its loop (26 registers per thread otherwise):
-// 7 x 16 bytes per thread, laid out [vector][thread] so that every LDS.128 / STS.128 of a warp is conflict free.
+// Kernel variants without CREG keep the coefficients in shared memory between the set-up of a block and its loop (26 registers
+// per thread otherwise): 7 x 16 bytes per thread, laid out [vector][thread] so that every LDS.128 / STS.128 of a warp is conflict
+// free.  Variants with CREG (compiled for 128 registers, 4 blocks per SM) keep them in registers: the loop of a clean block is
+// bound by the L1 data pipe (ncu: l1tex__data_pipe_lsu_wavefronts 80 % of peak; a 128-bit load costs four wavefronts whatever its
+// address pattern), and the 7 LDS.128 per two SFTs are a third of its wavefronts.
 constexpr int COEF_V = 7;
 __device__ __forceinline__ void coef_store(float4 *cs, const FastCoef &fc) {       // cs = slot of this thread
   *reinterpret_cast<double2 *>(cs) = make_double2(fc.p0, fc.p1);
@@ -1117,6 +1124,16 @@ __device__ __forceinline__ void ftrack_poly2(const float4 *cs, int jA, int jB, F
   ftrack_poly1(d0, d1, d2, f3, f4, f5, f6, jB, B);
 }
 
+// the same from coefficients held in registers (kernel variants with CREG)
+__device__ __forceinline__ void ftrack_poly2r(const FastCoef &fc, int jA, int jB, FTrack &A, FTrack &B) {
+  const double2 d0 = make_double2(fc.p0, fc.p1), d1 = make_double2(fc.p2, fc.y0), d2 = make_double2(fc.y1, fc.y2);
+  const float4 f3 = make_float4(fc.pt[0], fc.pt[1], fc.pt[2], fc.pt[3]), f4 = make_float4(fc.yt[0], fc.yt[1], fc.yt[2], fc.bc[0]);
+  const float4 f5 = make_float4(fc.bc[1], fc.bc[2], fc.ac[0], fc.ac[1]);
+  const float2 f6 = make_float2(fc.ac[2], fc.ac[3]);
+  ftrack_poly1(d0, d1, d2, f3, f4, f5, f6, jA, A);
+  ftrack_poly1(d0, d1, d2, f3, f4, f5, f6, jB, B);
+}
+
 template <class CFG>
 __device__ __forceinline__ void ftrack_closed(const KParams &p, const Tmpl &tm, double dalpha, float ascale, FTrack &t) {
   Track tr;
@@ -1129,11 +1146,11 @@ __device__ __forceinline__ void ftrack_closed(const KParams &p, const Tmpl &tm, 
 }
 
 // Is the block [g, ge) clean for this warp (see above)?  Returns 0 = no (generic loop), 1 = clean, closed-form track,
-// 2 = clean, polynomial track (coefficients in the thread's shared-memory slot cs).  `mask` receives the block's presence bits (any channel), usv[c] the
-// weight 1/s of SFT g + lane.
-template <int CT, class CFG>
+// 2 = clean, polynomial track (coefficients in fc and, unless CREG, in the thread's shared-memory slot cs).  `mask` receives the
+// block's presence bits (any channel), usv[c] the weight 1/s of SFT g + lane.
+template <int CT, class CFG, bool CREG>
 __device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int g, int ge, int lane, float ascale, float4 *cs,
-                                          unsigned &mask, float (&usv)[CT]) {
+                                          unsigned &mask, float (&usv)[CT], FastCoef &fc) {
   bool pres = false;
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
@@ -1143,7 +1160,6 @@ __device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int 
   mask = __ballot_sync(0xffffffffu, pres);
   if (mask == 0u || p.mtab == nullptr || cfg_phase<CFG>(p) != 0) return 0;
   const bool fres = cfg_kernel<CFG>(p) == 1;
-  FastCoef fc;
   const bool poly = __all_sync(0xffffffffu, fast_coef<CFG>(p, tm, g, ascale, fc));
   if (poly) {
     // the end SFTs from the polynomial itself (its error is far below the 1e-9 tie window of DESIGN A5/A12)
@@ -1167,7 +1183,7 @@ __device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int 
     const bool ok = tau_h > p.T && fl >= p.f_loT && fh + b_edge <= p.f_hiT && (unsigned)(kl - p.kwin0 - 2) <= (unsigned)p.jmax &&
                     (unsigned)(kh - p.kwin0 - 2) <= (unsigned)p.jmax && bl >= 0.f && bh >= bl && bh <= p.b_table && kh >= kl;
     if (!__all_sync(0xffffffffu, ok)) return 0;
-    coef_store(cs, fc);
+    if (!CREG) coef_store(cs, fc);
     return 2;
   }
   Track lo, hi;
@@ -1224,14 +1240,104 @@ __device__ __forceinline__ void finish_fast(const KParams &p, const Tmpl &tm, co
   }
 }
 
-// Transposed store of one tile of chunk-local prefix sums (MODE 1): rows = templates, 128-byte rows along the SFT axis.
-__device__ __forceinline__ void tile_store(const KParams &p, const float *txh, const float *thh, int tg, int g, int n, int lane) {
+// MODE 1, end of a work unit (32 SFT slots starting at g = 32 ch, n of them inside the data): the warp's tile holds the
+// unit-local inclusive prefix sums (fp32, rows = lanes = templates), (axh, ahh) the unit's totals (fp64).  Single-pass scan
+// with decoupled look-back along the SFT axis, one lane per template:
+//   1. publish the unit's totals (aggregate) - nobody is waited for before this, so every claimed unit publishes;
+//   2. walk back over the predecessors ch-1, ch-2, ... until one has published its INCLUSIVE totals (or the start is reached),
+//      waiting where neither entry of a predecessor is there yet: units are claimed in ascending order from one counter, so
+//      every predecessor is held by a resident warp that is past or on its way to step 1;
+//   3. carry = inclusive(k) + aggregate(k+1) + ... + aggregate(ch-1), added in ASCENDING order: the same fp64 sums whichever
+//      k the walk stopped at (run-to-run deterministic); publish carry + own totals as this unit's inclusive totals;
+//   4. store carry + local prefix (carry split into hi + lo floats: <= 1 ulp of the fp32 output) transposed, as 128-byte rows
+//      along the SFT axis, and snr = cum_xh / sqrt(cum_hh) (0 where cum_hh == 0).
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *q) {
+  unsigned v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(q) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_u32(unsigned *q, unsigned v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(q), "r"(v) : "memory");
+}
+__device__ __forceinline__ void scan_store(const KParams &p, float *txh, float *thh, int tg, int ch, int n, int lane, long long t,
+                                           double axh, double ahh, unsigned smask) {
+  const bool ok = t < p.nT;
+  const size_t nT = (size_t)p.nT;
+  double cx = 0.0, chh = 0.0;
+  if (ok) {
+    const size_t me = (size_t)ch * nT + (size_t)t;
+    p.scanA[me] = make_double2(axh, ahh);
+    st_release_u32(p.flagA + me, p.epoch);
+    int k = ch - 1;
+    while (k >= 0) {
+      const size_t e = (size_t)k * nT + (size_t)t;
+      if (ld_acquire_u32(p.flagP + e) == p.epoch) break;
+      if (ld_acquire_u32(p.flagA + e) == p.epoch) { --k; continue; }
+      __nanosleep(64);
+    }
+    if (k >= 0) {
+      const double2 v = __ldcg(p.scanP + (size_t)k * nT + (size_t)t);
+      cx = v.x; chh = v.y;
+    }
+    for (int j = k + 1; j < ch; ++j) {
+      const double2 v = __ldcg(p.scanA + (size_t)j * nT + (size_t)t);
+      cx += v.x; chh += v.y;
+    }
+    p.scanP[me] = make_double2(cx + axh, chh + ahh);
+    st_release_u32(p.flagP + me, p.epoch);
+  }
+  // carry of row r (hi + lo floats) comes from lane r
+  const float xhi = (float)cx, xlo = (float)(cx - (double)xhi), hhi = (float)chh, hlo = (float)(chh - (double)hhi);
   __syncwarp();
-  for (int r = 0; r < 32; ++r) {
-    const long long tt = (long long)tg * 32 + r;
-    if (tt < p.nT && lane < n) {
-      p.loc_xh[(size_t)tt * p.n_sft + g + lane] = txh[r * 33 + lane];
-      p.loc_hh[(size_t)tt * p.n_sft + g + lane] = thh[r * 33 + lane];
+  const int g = ch * 32;
+  // slot j shows the running sums of the last slot <= j that holds a value (smask), 0 if there is none
+  auto source = [&](int j) {
+    const unsigned m = smask & (0xffffffffu >> (31 - j));
+    return m ? 31 - __clz(m) : -1;
+  };
+  const size_t al = (size_t)p.out_snr | (size_t)p.out_cx | (size_t)p.out_ch;   // (null = aligned)
+  if ((p.n_sft & 3) == 0 && (al & 15) == 0) {
+    // 4 rows x 32 slots per step: lane = (row r0 + lane / 8, slots 4 (lane % 8) ... + 3), 16-byte stores
+    const int c4 = (lane & 7) * 4, rs = lane >> 3;
+    int src[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) src[j] = source(c4 + j);
+#pragma unroll 2
+    for (int r0 = 0; r0 < 32; r0 += 4) {
+      const int r = r0 + rs;
+      const long long tt = (long long)tg * 32 + r;
+      const float c0 = __shfl_sync(0xffffffffu, xhi, r), c1 = __shfl_sync(0xffffffffu, xlo, r);
+      const float c2 = __shfl_sync(0xffffffffu, hhi, r), c3 = __shfl_sync(0xffffffffu, hlo, r);
+      float x[4], h[4], q[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int sj = src[j] < 0 ? 0 : src[j];
+        const float lx = txh[r * 33 + sj], lh = thh[r * 33 + sj];
+        x[j] = c0 + (c1 + (src[j] < 0 ? 0.f : lx));
+        h[j] = c2 + (c3 + (src[j] < 0 ? 0.f : lh));
+        q[j] = h[j] > 0.f ? x[j] * rsqrt_approx(h[j]) : 0.f;
+      }
+      if (tt < p.nT && c4 < n) {
+        const size_t o = (size_t)tt * p.n_sft + g + c4;
+        if (p.out_snr) __stcs((float4 *)(p.out_snr + o), make_float4(q[0], q[1], q[2], q[3]));
+        if (p.out_cx) __stcs((float4 *)(p.out_cx + o), make_float4(x[0], x[1], x[2], x[3]));
+        if (p.out_ch) __stcs((float4 *)(p.out_ch + o), make_float4(h[0], h[1], h[2], h[3]));
+      }
+    }
+  } else {
+    const int sj = source(lane);
+    for (int r = 0; r < 32; ++r) {
+      const long long tt = (long long)tg * 32 + r;
+      const float c0 = __shfl_sync(0xffffffffu, xhi, r), c1 = __shfl_sync(0xffffffffu, xlo, r);
+      const float c2 = __shfl_sync(0xffffffffu, hhi, r), c3 = __shfl_sync(0xffffffffu, hlo, r);
+      if (tt < p.nT && lane < n) {
+        const float x = c0 + (c1 + (sj < 0 ? 0.f : txh[r * 33 + sj]));
+        const float h = c2 + (c3 + (sj < 0 ? 0.f : thh[r * 33 + sj]));
+        const size_t o = (size_t)tt * p.n_sft + g + lane;
+        if (p.out_snr) __stcs(p.out_snr + o, h > 0.f ? x * rsqrt_approx(h) : 0.f);
+        if (p.out_cx) __stcs(p.out_cx + o, x);
+        if (p.out_ch) __stcs(p.out_ch + o, h);
+      }
     }
   }
   __syncwarp();
@@ -1239,18 +1345,14 @@ __device__ __forceinline__ void tile_store(const KParams &p, const float *txh, c
 
 // The loop over the present SFTs of a clean block, two at a time.  Accumulates into axh / ahh / axi (fp64; fp32 partial
 // sums over the block).
-template <int CT, int MODE, class CFG, bool POLY>
-__device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, const float4 *cs, unsigned mask, const float (&usv)[CT],
+template <int CT, int MODE, class CFG, bool POLY, bool CREG>
+__device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, const float4 *cs, const FastCoef &fc, unsigned mask, const float (&usv)[CT],
                                            float ascale, int g, int ge, int tg, int lane, long long t, bool want_kc, double &axh,
                                            double &ahh, double &axi, float *txh, float *thh, unsigned long long *n_path) {
   const int n = ge - g;
   const unsigned row0 = (unsigned)g * p.mrow;
   const float2 *rt = p.rtab + g;
   int *kcp = (CFG::KC && want_kc) ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + g : nullptr;
-  if (MODE == 1) {                     // slots before the first present SFT keep the running sums
-    const int j0 = __ffs(mask) - 1;
-    for (int k = 0; k < j0; ++k) { txh[lane * 33 + k] = (float)axh; thh[lane * 33 + k] = (float)ahh; }
-  }
   if (CFG::KC && kcp && t < p.nT) {
     for (int k = 0; k < n; ++k)
 #pragma unroll
@@ -1265,7 +1367,8 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
     mask &= mask - 1;                  // (0 stays 0)
     FTrack A, B;
     if (POLY) {
-      ftrack_poly2(cs, jA, jB, A, B);
+      if (CREG) ftrack_poly2r(fc, jA, jB, A, B);
+      else ftrack_poly2(cs, jA, jB, A, B);
     } else {
       ftrack_closed<CFG>(p, tm, (double)(g + jA), ascale, A);
       ftrack_closed<CFG>(p, tm, (double)(g + jB), ascale, B);
@@ -1298,13 +1401,12 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
         if (vB && usB[c] > 0.f) kcp[(size_t)c * p.n_sft + jB] = B.kc;
       }
     }
-    if (MODE == 1) {
-      const int endA = vB ? jB : n, endB = mask ? __ffs(mask) - 1 : n;
+    if (MODE == 1) {                   // running sums at the present slots only: scan_store fills the gaps
       axh += (double)zrA; ahh += (double)hhA;
-      for (int k = jA; k < endA; ++k) { txh[lane * 33 + k] = (float)axh; thh[lane * 33 + k] = (float)ahh; }
+      txh[lane * 33 + jA] = (float)axh; thh[lane * 33 + jA] = (float)ahh;
       if (vB) {
         axh += (double)zrB; ahh += (double)hhB;
-        for (int k = jB; k < endB; ++k) { txh[lane * 33 + k] = (float)axh; thh[lane * 33 + k] = (float)ahh; }
+        txh[lane * 33 + jB] = (float)axh; thh[lane * 33 + jB] = (float)ahh;
       }
     } else {
       fxh += zrA + zrB;
@@ -1314,8 +1416,6 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
   }
   if (MODE == 0) {
     axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
-  } else {
-    tile_store(p, txh, thh, tg, g, n, lane);
   }
 }
 
@@ -1328,14 +1428,15 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
 // generic loop below, which runs in groups of GROUP SFTs: fp32 partial sums flushed into fp64 per group (MODE 0),
 // one transposed store per group (MODE 1).
 // ---------------------------------------------------------------------------------------------
-template <int KT, int CT, int MODE, class CFG, int MINB, bool DUO>
+template <int KT, int CT, int MODE, class CFG, int MINB, bool DUO, bool CREG>
 __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
   constexpr int GROUP = MODE == 1 ? 32 : FLUSH;
-  __shared__ float tile_s[MODE == 1 ? (TILE / 32) * 2 * 32 * 33 : 1];
-  __shared__ float4 coef_s[COEF_V * TILE];             // polynomial-track coefficients of the current block, per thread
-  float4 *cs = coef_s + threadIdx.x;
+  constexpr int TILE_F = 2 * 32 * 33;                  // two padded 32 x 32 tiles per warp
+  __shared__ float tile_s[MODE == 1 ? (TILE / 32) * TILE_F : 1];
+  __shared__ float4 coef_s[CREG ? 1 : COEF_V * TILE];  // polynomial-track coefficients of the current block, per thread
+  float4 *cs = coef_s + (CREG ? 0 : threadIdx.x);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  float *txh = tile_s + (MODE == 1 ? warp * 2 * 32 * 33 : 0);
+  float *txh = tile_s + (MODE == 1 ? warp * TILE_F : 0);
   float *thh = txh + (MODE == 1 ? 32 * 33 : 0);
   const bool want_kc = CFG::KC && p.kc_out != nullptr;
 
@@ -1344,13 +1445,15 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
     if (lane == 0) item = atomicAdd(p.counter, 1);
     item = __shfl_sync(0xffffffffu, item, 0);
     if (item >= p.n_items) break;
-    const int ch = p.n_chunks - 1 - item / p.n_tgroups;     // latest (most expensive) chunks first
+    // MODE 0: latest (most expensive) chunks first; MODE 1: ascending, as the look-back of scan_store needs
+    const int ch = MODE == 1 ? item / p.n_tgroups : p.n_chunks - 1 - item / p.n_tgroups;
     const int tg = item - (item / p.n_tgroups) * p.n_tgroups;
     const long long t = (long long)tg * 32 + lane;
     const int a0 = ch * p.chunk;
     const int a1 = min(a0 + p.chunk, p.n_sft);
     double axh = 0.0, ahh = 0.0, axi = 0.0;
     unsigned long long n_path[PATH_N] = {0, 0, 0, 0, 0, 0, 0};
+    unsigned smask = 0xffffffffu;      // MODE 1: slots of the unit's tile that were written (a clean block writes the present SFTs only)
 
     for (int gs = a0; gs < a1; gs += SUB) {
       const int gend = min(gs + SUB, a1);
@@ -1361,13 +1464,15 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
         float usv[CT];
         // where the template's amplitude constant is real (no response, one channel) it is folded into the amplitude
         const float ascale = (CFG::RESP == 0 && CT == 1) ? tm.AE[0].x : 1.0f;
-        const int kind = fast_setup<CT, CFG>(p, tm, gs, gend, lane, ascale, cs, mask, usv);
+        FastCoef fc;
+        const int kind = fast_setup<CT, CFG, CREG>(p, tm, gs, gend, lane, ascale, cs, mask, usv, fc);
+        if (kind != 0) smask = mask;
         if (kind == 2) {
-          fast_block<CT, MODE, CFG, true>(p, tm, cs, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
+          fast_block<CT, MODE, CFG, true, CREG>(p, tm, cs, fc, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
           continue;
         }
         if (kind == 1) {
-          fast_block<CT, MODE, CFG, false>(p, tm, cs, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
+          fast_block<CT, MODE, CFG, false, CREG>(p, tm, cs, fc, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
           continue;
         }
       }
@@ -1484,12 +1589,12 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
         }
         if (MODE == 0) {
           axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
-        } else {
-          tile_store(p, txh, thh, tg, g, ge - g, lane);
         }
       }
     }
-    if (t < p.nT) {
+    if (MODE == 1) {
+      scan_store(p, txh, thh, tg, ch, a1 - a0, lane, t, axh, ahh, smask);        // (the host sets chunk = SUB = 32 for MODE 1)
+    } else if (t < p.nT) {
       double *q = p.part + (size_t)ch * 3 * p.nT + t;
       q[0] = axh;
       q[p.nT] = ahh;
@@ -1544,60 +1649,6 @@ __global__ void sft_statistics_kernel(long long n, const double *xh, const doubl
   const double a = xh[t], b = xi[t], h = hh[t];
   if (loglike) loglike[t] = a - 0.5 * h;
   if (rho2max) rho2max[t] = h > 0.0 ? (a * a + b * b) / h : 0.0;
-}
-
-// Exclusive scan of the chunk totals along the chunk axis, in place, fp64 (the carries).
-__global__ void sft_scan_chunks_kernel(double *part, long long nT, int n_chunks) {
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nT) return;
-  double c0 = 0.0, c1 = 0.0;
-  for (int c = 0; c < n_chunks; ++c) {
-    double *q = part + (size_t)c * 3 * nT + t;
-    const double v0 = q[0], v1 = q[nT];
-    q[0] = c0;
-    q[nT] = c1;
-    c0 += v0;
-    c1 += v1;
-  }
-}
-
-// cum = carry (fp64) + chunk-local prefix (fp32);  snr = cum_xh / sqrt(cum_hh)  (0 where cum_hh == 0).
-// One warp per (template, chunk): the carry is split once into hi + lo floats, so that the per-element
-// work is two fp32 adds (error <= 1 ulp of the fp32 output) and the kernel runs at memory speed.
-// grid = (n_chunks, ceil(nT / 8)), block = 8 warps.
-__global__ void __launch_bounds__(256) sft_fixup_kernel(const double *part, long long nT, int n_sft, int chunk,
-                                                        const float *loc_xh, const float *loc_hh, float *snr,
-                                                        float *cum_xh, float *cum_hh) {
-  const int lane = threadIdx.x & 31, ch = blockIdx.x;
-  const long long t = (long long)blockIdx.y * 8 + (threadIdx.x >> 5);
-  if (t >= nT) return;
-  const double cx = part[(size_t)ch * 3 * nT + t], chh = part[(size_t)ch * 3 * nT + nT + t];
-  const float xh_hi = (float)cx, xh_lo = (float)(cx - (double)xh_hi);
-  const float hh_hi = (float)chh, hh_lo = (float)(chh - (double)hh_hi);
-  const int a0 = ch * chunk, a1 = min(a0 + chunk, n_sft);
-  const size_t row = (size_t)t * n_sft;
-  const size_t al = (size_t)loc_xh | (size_t)loc_hh | (size_t)snr | (size_t)cum_xh | (size_t)cum_hh;   // (null = aligned)
-  if (((n_sft | chunk) & 3) == 0 && (al & 15) == 0) {   // rows and chunk starts 16-byte aligned: 4 SFTs per lane
-    for (int a = a0 + 4 * lane; a < a1; a += 128) {
-      const float4 lx = __ldcs((const float4 *)(loc_xh + row + a)), lh = __ldcs((const float4 *)(loc_hh + row + a));
-      float4 x, h, q;
-      x.x = xh_hi + (xh_lo + lx.x); x.y = xh_hi + (xh_lo + lx.y); x.z = xh_hi + (xh_lo + lx.z); x.w = xh_hi + (xh_lo + lx.w);
-      h.x = hh_hi + (hh_lo + lh.x); h.y = hh_hi + (hh_lo + lh.y); h.z = hh_hi + (hh_lo + lh.z); h.w = hh_hi + (hh_lo + lh.w);
-      q.x = h.x > 0.f ? x.x * rsqrt_approx(h.x) : 0.f; q.y = h.y > 0.f ? x.y * rsqrt_approx(h.y) : 0.f;
-      q.z = h.z > 0.f ? x.z * rsqrt_approx(h.z) : 0.f; q.w = h.w > 0.f ? x.w * rsqrt_approx(h.w) : 0.f;
-      if (snr) __stcs((float4 *)(snr + row + a), q);
-      if (cum_xh) __stcs((float4 *)(cum_xh + row + a), x);
-      if (cum_hh) __stcs((float4 *)(cum_hh + row + a), h);
-    }
-    return;
-  }
-  for (int a = a0 + lane; a < a1; a += 32) {
-    const float x = xh_hi + (xh_lo + __ldcs(loc_xh + row + a));
-    const float h = hh_hi + (hh_lo + __ldcs(loc_hh + row + a));
-    if (snr) __stcs(snr + row + a, h > 0.f ? x * rsqrt_approx(h) : 0.f);
-    if (cum_xh) __stcs(cum_xh + row + a, x);
-    if (cum_hh) __stcs(cum_hh + row + a, h);
-  }
 }
 
 // Whitening of one channel at load time (Eq.(15); DESIGN "store"): writes both pair-planar

@@ -37,7 +37,8 @@ struct sft_plan {
   double *d_params = nullptr; size_t params_bytes = 0;
   void *d_out = nullptr; size_t out_bytes = 0;         // staging for host outputs
   void *h_pin = nullptr; size_t pin_bytes = 0;         // pinned host staging (params in, result vectors out)
-  float *loc = nullptr; size_t loc_bytes = 0;          // cumulative: chunk-local prefixes
+  void *scan = nullptr; size_t scan_bytes = 0;         // cumulative: look-back records {aggregate, inclusive} + flags per (unit, template)
+  unsigned epoch = 0;                                  // value of a published flag of the current cumulative call
   double *td = nullptr; size_t td_bytes = 0;           // per-template constants (sft_tmpl_kernel)
   float *tf = nullptr; size_t tf_bytes = 0;
   float4 *mtab = nullptr;                              // [C][n_sft][n_node][4] data-moment table (sft_table.cuh), or null
@@ -114,6 +115,7 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   if (!(d.f_ref > 0.0)) return fail(nullptr, SFT_EINVAL, "f_ref must be > 0");
   if (!(d.f_hi >= d.f_lo)) return fail(nullptr, SFT_EINVAL, "need f_lo <= f_hi");
   if (d.response == SFT_RESP_ANNUAL && !(d.resp_period > 0.0)) return fail(nullptr, SFT_EINVAL, "resp_period must be > 0");
+  if (d.include_dc != 0 && d.include_dc != 1) return fail(nullptr, SFT_EINVAL, "include_dc must be 0 or 1");
   if (d.evaluator < SFT_EVAL_AUTO || d.evaluator > SFT_EVAL_TABLE) return fail(nullptr, SFT_EINVAL, "unknown evaluator %d", d.evaluator);
   int ndev = 0;
   cudaError_t e = cudaGetDeviceCount(&ndev);
@@ -127,7 +129,8 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   p->d = d;
   p->nb = d.k_hi - d.k_lo;
   p->n_samp = (int)nearbyint(n);
-  p->kv_lo = d.k_lo > 1 ? d.k_lo : 1;                                   // DESIGN A6: 1 <= k <= n/2-1
+  const int k_first = d.include_dc ? 0 : 1;                             // DESIGN A6: 1 <= k <= n/2-1 (0 <= k with include_dc)
+  p->kv_lo = d.k_lo > k_first ? d.k_lo : k_first;
   p->kv_hi = d.k_hi < p->n_samp / 2 ? d.k_hi : p->n_samp / 2;
   p->stream = (cudaStream_t)d.stream;
   const size_t C = d.n_channels, N = d.n_sft, nb = p->nb;
@@ -208,7 +211,7 @@ SFT_API sft_status sft_plan_destroy(sft_plan *p) {
   cudaSetDevice(p->d.device);
   cudaStreamSynchronize(p->stream);
   cudaFree(p->Dp); cudaFree(p->ubp); cudaFree(p->us2); cudaFree(p->rtab);
-  cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->loc);
+  cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->scan);
   if (p->h_pin) cudaFreeHost(p->h_pin);
   cudaFree(p->td); cudaFree(p->tf); cudaFree(p->counter); cudaFree(p->path_counts);
   cudaFree(p->mtab); cudaFree(p->htab); cudaFree(p->ptab);
@@ -547,6 +550,9 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
 #ifndef SFT_DUO
 #define SFT_DUO true        // two consecutive SFTs per step through the tier-1 tables (sft_kernels.cuh :: duo_terms)
 #endif
+#ifndef SFT_CREG_BNS
+#define SFT_CREG_BNS true   // the config-2/3/5 variant keeps the polynomial-track coefficients in registers
+#endif
 #ifndef SFT_MINB
 #define SFT_MINB 5          // resident 128-thread blocks per SM the main kernel is compiled for
 #endif
@@ -562,9 +568,10 @@ using CfgLISA = sftk::Cfg<1, 1, 2, 0>;
 using CfgAny = sftk::Cfg<-1, -1, -1, 1, -1>;
 using CfgBNS32 = sftk::Cfg<1, 1, 0, 0, 1>;    // CfgBNS with the split-fp32 (double-float) phase track (config 5)
 
-template <int KT, int CT, int MODE, class CFG>
+// CREG: polynomial-track coefficients in registers (128 registers, 4 blocks per SM) instead of shared memory (96, 5 blocks)
+template <int KT, int CT, int MODE, class CFG, bool CREG = false>
 static void launch_variant(sft_plan *p, const KParams &k) {
-  auto kern = sftk::sft_main_kernel<KT, CT, MODE, CFG, SFT_MINB, SFT_DUO>;
+  auto kern = sftk::sft_main_kernel<KT, CT, MODE, CFG, CREG ? 4 : SFT_MINB, SFT_DUO, CREG>;
   int per_sm = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, sftk::TILE, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
   long long blocks = (long long)p->n_sm * per_sm;
@@ -585,11 +592,11 @@ static cudaError_t launch_main(sft_plan *p, const KParams &k) {
   const bool lisa = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 2;
 #ifdef SFT_FEW_VARIANTS      // development builds: only the config-2 variant and the single-channel run-time-flag variant
   (void)bns32; (void)newt; (void)lisa;
-  if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS>(p, k);
+  if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS, SFT_CREG_BNS>(p, k);
   else launch_variant<0, 1, MODE, CfgAny>(p, k);
 #else
   if (bns32) launch_variant<8, 1, MODE, CfgBNS32>(p, k);
-  else if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS>(p, k);
+  else if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS, SFT_CREG_BNS>(p, k);
   else if (bns && C == 1 && K == 16) launch_variant<16, 1, MODE, CfgBNS>(p, k);
   else if (bns && C == 1) launch_variant<0, 1, MODE, CfgBNS>(p, k);
   else if (newt && C == 1 && K == 4) launch_variant<4, 1, MODE, CfgNewt>(p, k);
@@ -624,13 +631,32 @@ static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t
     chunk = (int)((k.n_sft + want_chunks - 1) / want_chunks);
     if (chunk < 32) chunk = 32;
   }
-  if (cumulative) chunk = ((chunk + 31) / 32) * 32;
-  if (chunk > k.n_sft) chunk = cumulative ? ((k.n_sft + 31) / 32) * 32 : k.n_sft;
+  if (cumulative) chunk = sftk::SUB;          // single-pass scan: one work unit = one block of 32 SFT slots (scan_store)
+  if (chunk > k.n_sft && !cumulative) chunk = k.n_sft;
   k.chunk = chunk;
   k.n_chunks = (k.n_sft + chunk - 1) / chunk;
-  sft_status st = grow(p, (void **)&p->part, &p->part_bytes, (size_t)k.n_chunks * 3 * nT * sizeof(double));
-  if (st != SFT_OK) return st;
-  k.part = p->part;
+  sft_status st = SFT_OK;
+  if (cumulative) {
+    // look-back records: per (unit, template) two double2 and two flags.  A flag counts as published when it equals the
+    // epoch of this call, so nothing is cleared between calls; a fresh or regrown buffer is zeroed and the epoch restarts.
+    const size_t ent = (size_t)k.n_chunks * (size_t)nT, need = ent * (2 * sizeof(double2) + 2 * sizeof(unsigned));
+    if (p->scan_bytes < need || p->epoch == 0xffffffffu) {
+      st = grow(p, &p->scan, &p->scan_bytes, need);
+      if (st != SFT_OK) return st;
+      CU(p, cudaMemsetAsync(p->scan, 0, p->scan_bytes, p->stream));
+      p->epoch = 0;
+    }
+    p->epoch++;
+    k.scanA = (double2 *)p->scan;
+    k.scanP = k.scanA + ent;
+    k.flagA = (unsigned *)(k.scanP + ent);
+    k.flagP = k.flagA + ent;
+    k.epoch = p->epoch;
+  } else {
+    st = grow(p, (void **)&p->part, &p->part_bytes, (size_t)k.n_chunks * 3 * nT * sizeof(double));
+    if (st != SFT_OK) return st;
+    k.part = p->part;
+  }
   if ((double)k.n_tgroups * (double)k.n_chunks > 2.0e9) return fail(p, SFT_EINVAL, "too many work units: raise sfts_per_block");
   k.n_items = k.n_tgroups * k.n_chunks;
   k.counter = p->counter;
@@ -757,7 +783,6 @@ SFT_API sft_status sft_cumulative_snr(sft_plan *p, int64_t nT, const double *par
   sft_status st = prepare(p, nT, params, mem, k, true);
   if (st != SFT_OK) return st;
   const size_t N = p->d.n_sft, mat = (size_t)nT * N * sizeof(float);
-  // chunk-local prefixes: written into cum_xh/cum_hh when the caller gave device buffers, else scratch
   float *d_snr = snr, *d_cx = cum_xh, *d_ch = cum_hh;
   int n_out = (snr != nullptr) + (cum_xh != nullptr) + (cum_hh != nullptr);
   if (mem == SFT_MEM_HOST) {
@@ -768,22 +793,11 @@ SFT_API sft_status sft_cumulative_snr(sft_plan *p, int64_t nT, const double *par
     d_cx = cum_xh ? q : nullptr; if (cum_xh) q += (size_t)nT * N;
     d_ch = cum_hh ? q : nullptr;
   }
-  const int n_loc = (d_cx ? 0 : 1) + (d_ch ? 0 : 1);
-  if (n_loc) {
-    st = grow(p, (void **)&p->loc, &p->loc_bytes, (size_t)n_loc * mat);
-    if (st != SFT_OK) return st;
-  }
-  k.loc_xh = d_cx ? d_cx : p->loc;
-  k.loc_hh = d_ch ? d_ch : (d_cx ? p->loc : p->loc + (size_t)nT * N);
+  k.out_snr = d_snr;
+  k.out_cx = d_cx;
+  k.out_ch = d_ch;
   cudaError_t e = launch_main<1>(p, k);
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
-  sftk::sft_scan_chunks_kernel<<<(unsigned)((nT + 255) / 256), 256, 0, p->stream>>>(p->part, nT, k.n_chunks);
-  if ((nT + 7) / 8 > 65535) return fail(p, SFT_EUNSUPPORTED, "cumulative call: more than 524,280 templates per call");
-  dim3 fgrid((unsigned)k.n_chunks, (unsigned)((nT + 7) / 8));
-  sftk::sft_fixup_kernel<<<fgrid, 256, 0, p->stream>>>(p->part, nT, (int)N, k.chunk, k.loc_xh, k.loc_hh, d_snr, d_cx, d_ch);
-  p->launches += 2;
-  e = cudaGetLastError();
-  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "scan/fixup launch: %s", cudaGetErrorString(e));
   if (mem == SFT_MEM_HOST) {
     CU(p, cudaStreamSynchronize(p->stream));
     if (snr) CU(p, cudaMemcpyAsync(snr, d_snr, mat, cudaMemcpyDeviceToHost, p->stream));

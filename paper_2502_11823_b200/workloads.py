@@ -334,3 +334,57 @@ def config4(n_templates=65536, snr=50.0):
     return Workload(name="config4", desc=desc, bins=bins.astype(np.complex64),
                     psd_scale=np.ones((C, n_sft)), psd_shape=np.stack([S, S]), params=P, injection=inj,
                     notes=dict(tau_end=tau_end))
+
+
+# --------------------------------------------------------------------------------------------
+# accuracy experiment of section IV: a noiseless fiducial signal, r(delta, Delta k) of Eq.(36)
+# --------------------------------------------------------------------------------------------
+ACCURACY_EXAMPLES = {
+    # name: (m1, m2 [Msun], f_start, f_end [Hz], fs [Hz], modulation period [s])
+    "bns": (1.4, 1.4, 1.0, 10.0, 40.0, 86400.0),
+    "mbhb": (1e6, 1e6, 1e-4, 1.9e-3, 2.0, YEAR_S),
+}
+
+
+def accuracy_case(example, t_sft, K, f_start=None, pn1=1, kernel="fresnel"):
+    """One point of the paper's accuracy maps (Fig. 3 / Fig. 4) with this library's PN waveform in place of
+    IMRPhenomT (W1): the fiducial signal of section IV.B (``"bns"``: 1.4+1.4 Msun, 1 -> 10 Hz, fs = 40 Hz, daily
+    modulation) or IV.C (``"mbhb"``: 1e6+1e6 Msun, 1e-4 -> 1.9e-3 Hz, fs = 2 Hz, yearly modulation),
+    observed with the projector Lambda_t = [a(t) + b(t)](Re + Im), a = cos(2 pi t/P), b = sin(2 pi t/P), c_nu = 1
+    (Eq.(37)-(41)), i.e. h(t) = Re[R(t) A(t) e^{i phi(t)}] with R = (a + b)(1 - i) applied at every sample.  No noise, flat
+    PSD S = 1 (the experiment measures the loss of ([d,h]) against <d,h> for d = h).  ``t_sft`` is rounded to an even
+    number of samples; ``f_start`` above the example's own start shortens the signal (tests).  The template (row 0 of
+    ``params``) is the fiducial signal; its response table holds R at the SFT starts.
+    Returns a Workload whose ``series`` is the sampled signal over the whole SFTs and ``notes["xx_time"]`` the exact
+    time-domain product (2 dt / S) sum_j h_j^2 over the same samples (Eq.(1)/(14) for a flat PSD)."""
+    m1, m2, f0, f1, fs, period = ACCURACY_EXAMPLES[example]
+    if f_start is not None:
+        f0 = float(f_start)
+    eta = m1 * m2 / (m1 + m2) ** 2
+    mc = (m1 + m2) * eta ** 0.6
+    dt = 1.0 / fs
+    n = 2 * int(round(0.5 * t_sft * fs))
+    T = n * dt
+    tau0, tau1 = tau_for_frequency(f0, mc, eta, pn1), tau_for_frequency(f1, mc, eta, pn1)
+    n_sft = int((tau0 - tau1) // T)
+    T_obs = n_sft * T
+    inj = np.zeros(NPARAM)
+    inj[:5] = [mc, eta, tau0, 0.7, 1.0]                      # t = 0 at f_start; the data end where f_end is reached
+    f_ref = f1
+
+    def resp(tt):
+        ph = 2.0 * np.pi * tt / period
+        return (np.cos(ph) + np.sin(ph)) * (1.0 - 1.0j)
+
+    t = np.arange(n_sft * n, dtype=np.float64) * dt
+    h = inspiral_strain(t, inj, f_ref, pn1, resp)
+    _, fe = inspiral_phase_freq(np.float64(T_obs), mc, eta, inj[2], 0.0, pn1)
+    k_lo = max(0, int(np.floor(f0 * T)) - K - 2)
+    k_hi = min(n // 2, int(np.ceil(fe * T)) + K + 4)
+    bins = _segment_rfft_bins(h.reshape(n_sft, n), dt, k_lo, k_hi)[None].astype(np.complex64)
+    R = resp(np.arange(n_sft, dtype=np.float64) * T)[None].astype(np.complex64)
+    desc = dict(n_channels=1, n_sft=n_sft, t_sft=T, fs=fs, t0=0.0, k_lo=k_lo, k_hi=k_hi, K=K, kernel=kernel, pn1=pn1,
+                response="table", f_lo=0.0, f_hi=1e9, f_ref=f_ref)
+    return Workload(name=f"accuracy-{example}", desc=desc, bins=bins, psd_scale=np.ones((1, n_sft)),
+                    psd_shape=np.ones((1, k_hi - k_lo)), params=inj[None].copy(), response=R, injection=inj, series=h[None],
+                    notes=dict(xx_time=2.0 * dt * float(np.dot(h, h)), n=n, t_obs=T_obs, f_end=float(fe)))

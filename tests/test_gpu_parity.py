@@ -339,6 +339,75 @@ def test_errors_on_device(et_small):
     plan.close()
 
 
+def test_error_paths_leave_outputs_untouched(et_small):
+    """include/sft.h: "on error the outputs are untouched".  Every error return of the three compute calls, with NaN / -7
+    sentinels in the outputs (host and device buffers)."""
+    import ctypes as C
+    import torch
+    api = _api()
+    w = et_small
+    n = w.desc["n_sft"]
+    P = np.ascontiguousarray(w.params[:5])
+
+    def fresh():
+        return [np.full(5, np.nan) for _ in range(3)], np.full((5, 1, n), -7, np.int32), [np.full((5, n), np.nan, np.float32) for _ in range(3)]
+
+    def untouched(v, kc, m):
+        return all(np.isnan(a).all() for a in v) and (kc == -7).all() and all(np.isnan(a).all() for a in m)
+
+    # 1. no data loaded: SFT_ENODATA from both calls
+    plan = api.Plan(w.desc)
+    v, kc, m = fresh()
+    for call in (lambda: plan.inner_products(P, v[0], v[1], v[2], kc), lambda: plan.cumulative_snr(P, m[0], m[1], m[2])):
+        with pytest.raises(api.SftError) as ei:
+            call()
+        assert "SFT_ENODATA" in str(ei.value)
+    assert untouched(v, kc, m)
+    plan.close()
+    with api.plan_from_workload(w) as plan:
+        lib, h = plan.lib, plan._h
+        vp = lambda a: C.c_void_p(a.ctypes.data)
+        # 2. argument errors straight through the C ABI (the binding would refuse some of them itself)
+        assert lib.sft_inner_products(h, -1, vp(P), vp(v[0]), vp(v[1]), vp(v[2]), vp(kc), 0) == 1          # n_templates < 0
+        assert lib.sft_inner_products(h, 5, vp(P), vp(v[0]), vp(v[1]), vp(v[2]), vp(kc), 7) == 1           # bad mem
+        assert lib.sft_inner_products(h, 5, None, vp(v[0]), vp(v[1]), vp(v[2]), vp(kc), 0) == 1            # params NULL
+        assert lib.sft_inner_products(h, 5, vp(P), None, vp(v[1]), vp(v[2]), vp(kc), 0) == 1               # xh NULL
+        assert lib.sft_cumulative_snr(h, 5, vp(P), None, None, None, 0) == 1                               # no output at all
+        assert lib.sft_cumulative_snr(h, -2, vp(P), vp(m[0]), vp(m[1]), vp(m[2]), 0) == 1
+        assert lib.sft_cumulative_snr(h, 5, None, vp(m[0]), vp(m[1]), vp(m[2]), 0) == 1
+        assert lib.sft_cumulative_snr(h, 5, vp(P), vp(m[0]), vp(m[1]), vp(m[2]), 3) == 1
+        assert lib.sft_statistics(h, 5, vp(v[0]), vp(v[1]), vp(v[2]), None, None, 0) == 1                  # nothing asked for
+        assert lib.sft_statistics(h, 5, None, vp(v[1]), vp(v[2]), vp(v[0]), None, 0) == 1
+        assert b"" != lib.sft_last_error(h)
+        assert untouched(v, kc, m)
+        # n_templates == 0 is SFT_OK and touches nothing
+        assert lib.sft_inner_products(h, 0, vp(P), vp(v[0]), vp(v[1]), vp(v[2]), vp(kc), 0) == 0
+        assert lib.sft_cumulative_snr(h, 0, vp(P), vp(m[0]), vp(m[1]), vp(m[2]), 0) == 0
+        assert untouched(v, kc, m)
+        # 3. sft_load_data errors leave the channel as it was: the plan still computes the same numbers afterwards
+        plan.inner_products(P, v[0], v[1], v[2], None)
+        ref = [a.copy() for a in v]
+        bins = np.ascontiguousarray(w.bins[0], np.complex64)
+        scale = np.ascontiguousarray(w.psd_scale[0])
+        bad_shape = np.ascontiguousarray(w.psd_shape[0]).copy()
+        bad_shape[3] = -1.0
+        assert lib.sft_load_data(h, 0, vp(bins), vp(scale), vp(bad_shape), None, 0) == 1                   # non-positive PSD
+        assert lib.sft_load_data(h, 1, vp(bins), vp(scale), None, None, 0) == 1                            # channel out of range
+        assert lib.sft_load_data(h, 0, None, vp(scale), None, None, 0) == 1
+        assert lib.sft_load_data(h, 0, vp(bins), vp(scale), None, None, 9) == 1
+        v2 = [np.full(5, np.nan) for _ in range(3)]
+        plan.inner_products(P, v2[0], v2[1], v2[2], None)
+        assert all(np.array_equal(a, b) for a, b in zip(ref, v2))
+        # 4. device buffers: a failing call leaves them untouched as well
+        Pd = torch.from_numpy(P).cuda()
+        xd = torch.full((5,), float("nan"), dtype=torch.float64, device="cuda")
+        dp = lambda t: C.c_void_p(t.data_ptr())
+        assert lib.sft_inner_products(h, 5, dp(Pd), dp(xd), None, None, None, 1) == 1                      # hh NULL
+        assert lib.sft_cumulative_snr(h, 5, dp(Pd), None, None, None, 1) == 1
+        plan.sync()
+        assert bool(torch.isnan(xd).all())
+
+
 def test_evaluator_selection_by_memory():
     """SFT_EVAL_AUTO falls back to the direct evaluator when the moment tables would not fit in a quarter of the
     free device memory; SFT_EVAL_TABLE reports SFT_ENOMEM instead."""
