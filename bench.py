@@ -119,7 +119,7 @@ def time_oracle(w, budget_s=12.0, seed=99):
 # ---------------------------------------------------------------------------------------------
 class ClockSampler:
     """Samples SM clock and throttle reasons with NVML while the timed region runs."""
-    def __init__(self, index, period=0.01):
+    def __init__(self, index, period=0.002):
         self.samples, self.reasons, self.max_mhz = [], set(), None
         self.period, self._stop, self._th = period, threading.Event(), None
         try:

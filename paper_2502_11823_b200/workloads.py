@@ -388,3 +388,49 @@ def accuracy_case(example, t_sft, K, f_start=None, pn1=1, kernel="fresnel"):
     return Workload(name=f"accuracy-{example}", desc=desc, bins=bins, psd_scale=np.ones((1, n_sft)),
                     psd_shape=np.ones((1, k_hi - k_lo)), params=inj[None].copy(), response=R, injection=inj, series=h[None],
                     notes=dict(xx_time=2.0 * dt * float(np.dot(h, h)), n=n, t_obs=T_obs, f_end=float(fe)))
+
+
+# --------------------------------------------------------------------------------------------
+# F-statistic test case: a long signal with resolvable amplitude modulation, Eq.(10)-(12) P:107-118
+# --------------------------------------------------------------------------------------------
+def fstat_case(c_nu=(0.7, -0.4, 0.5, 0.9), n_templates=8, n_channels=1, noise=0.0, seed=12, K=6):
+    """A 0PN+1PN chirp (Mc 1.2, 7.4 -> 18 Hz over 2048 s, fs = 512 Hz: config 1's track) observed through the antenna-pattern
+    functions a_c(t) = cos(2 pi t/P + 0.4 c), b_c(t) = sin(2 pi t/P + 0.3 + 0.9 c), P = 3000 s (both vary by O(1) over the
+    data, so that the two polarisations are resolvable), with amplitudes ``c_nu`` of Eq.(10): h = sum_nu c_nu h_nu,
+    h_nu as in Eq.(11), evaluated at EVERY sample.  Optional white noise of standard deviation ``noise`` (seed); flat PSD
+    S = 2 noise^2 / fs (1 if noise = 0).  Bank: row 0 = the signal's intrinsic parameters, the rest perturbed as in config 1.
+    The Workload's ``response`` holds (a + i b) at the SFT starts: the pair (a, b) that ``sft_fstat`` reads."""
+    fs, T, N0 = 512.0, 8.0, 1 << 20
+    n = int(T * fs)
+    n_sft = N0 // n
+    k_lo, k_hi = 40, 176
+    f_ref, P_mod = 20.0, 3000.0
+    inj = np.zeros(NPARAM)
+    inj[:5] = [1.2, 0.25, N0 / fs + 216.0, 1.3, 1.0]
+    t = np.arange(N0, dtype=np.float64) / fs
+    c = np.asarray(c_nu, dtype=np.float64)
+    rng = np.random.default_rng(seed)
+    bins, resp_tab, series = [], [], []
+    for ch in range(n_channels):
+        a = lambda tt, ch=ch: np.cos(2.0 * np.pi * tt / P_mod + 0.4 * ch)
+        b = lambda tt, ch=ch: np.sin(2.0 * np.pi * tt / P_mod + 0.3 + 0.9 * ch)
+        x = inspiral_strain(t, inj, f_ref, 1, lambda tt: (c[0] * a(tt) + c[1] * b(tt)) - 1j * (c[2] * a(tt) + c[3] * b(tt)))
+        if noise > 0.0:
+            x = x + noise * rng.standard_normal(N0)
+        series.append(x)
+        bins.append(_segment_rfft_bins(x.reshape(n_sft, n), 1.0 / fs, k_lo, k_hi))
+        ta = np.arange(n_sft, dtype=np.float64) * T
+        resp_tab.append(a(ta) + 1j * b(ta))
+    rng = np.random.default_rng(seed + 1)
+    Pm = _rows(n_templates)
+    Pm[:] = inj
+    Pm[:, 0] *= 1.0 + 1e-4 * rng.standard_normal(n_templates)
+    Pm[:, 2] += 1e-3 * rng.standard_normal(n_templates)
+    Pm[:, 3] = rng.uniform(0.0, 2.0 * np.pi, n_templates)
+    Pm[0] = inj
+    S = 2.0 * noise * noise / fs if noise > 0.0 else 1.0
+    desc = dict(n_channels=n_channels, n_sft=n_sft, t_sft=T, fs=fs, t0=0.0, k_lo=k_lo, k_hi=k_hi, K=K, kernel="fresnel", pn1=1,
+                response="table", f_lo=5.0, f_hi=30.0, f_ref=f_ref)
+    return Workload(name="fstat", desc=desc, bins=np.stack(bins).astype(np.complex64), psd_scale=np.ones((n_channels, n_sft)),
+                    psd_shape=np.full((n_channels, k_hi - k_lo), S), params=Pm, response=np.stack(resp_tab).astype(np.complex64),
+                    injection=inj, series=np.stack(series), notes=dict(c_nu=c, S=S))

@@ -1,0 +1,74 @@
+"""Pins of the accuracy experiment (section IV, Eq.(36)) on the CPU oracle: what the paper prints and what the
+mathematics fixes.  The exact colour maps of Fig. 3 / Fig. 4 stay "parity unpinned" (different waveform model)."""
+import numpy as np
+import pytest
+
+from oracle import accuracy as oa, inner as oin, waveform as wf
+from paper_2502_11823_b200 import workloads as wl
+from _util import to_oracle
+
+
+def _t_sft(example, delta, pn1=1):
+    m1, m2, _, f1, _, _ = wl.ACCURACY_EXAMPLES[example]
+    eta = m1 * m2 / (m1 + m2) ** 2
+    mc = (m1 + m2) * eta ** 0.6
+    tau1 = wl.tau_for_frequency(f1, mc, eta, pn1)
+    return float(wf.t_sft_rule(delta, wf.taylor_t3_fddot(mc, eta, tau1, 0.0, pn1)))
+
+
+def _r(example, delta, K, **kw):
+    over = {k: kw.pop(k) for k in ("include_dc",) if k in kw}
+    w = wl.accuracy_case(example, _t_sft(example, delta), K, **kw)
+    w.desc = dict(w.desc, **over)
+    plan, store = to_oracle(w)
+    return oa.accuracy_point(plan, store, w.params, w.series[0], 1.0 / w.desc["fs"]), w
+
+
+def test_relative_error_definition():
+    """Eq.(36): r = 1 - sqrt(ratio); a negative ratio is reported, not rooted (reading A15)."""
+    assert oa.relative_error(0.81, 1.0) == (pytest.approx(0.1), pytest.approx(0.81))
+    r, ratio = oa.relative_error(-0.5, 1.0)
+    assert np.isnan(r) and ratio == -0.5
+
+
+def test_exact_product_is_the_matched_snr():
+    """<h,h> by direct integration for a slowly chirping cosine of amplitude A over T_obs: A^2 T_obs / S (flat S)."""
+    dt, n = 1.0 / 64.0, 64 * 600
+    t = np.arange(n) * dt
+    h = 0.3 * np.cos(2 * np.pi * (5.0 * t + 0.5 * 1e-3 * t * t))
+    assert oa.exact_product(h, h, dt, 2.0) == pytest.approx(0.09 * n * dt / 2.0, rel=2e-4)
+
+
+def test_bns_example_matches_the_printed_magnitudes():
+    """Section IV.B: Table I's SFT lengths through Eq.(34) (106 s / 73 s for delta = 3 / 1); "most configurations with
+    delta <~ 3 and Delta k >~ 20 yield r < 1 %"; delta = 1, Delta k = 200: r ~ 0.2 % (same order here); the
+    loss falls as the band widens."""
+    r3, w3 = _r("bns", 3.0, 10)
+    assert abs(w3.desc["t_sft"] - 106.0) < 1.5 and abs(w3.desc["n_sft"] - 4396) < 0.01 * 4396
+    assert 0.0 < r3["r"] < 0.01
+    r1, w1 = _r("bns", 1.0, 100)
+    assert abs(w1.desc["t_sft"] - 73.0) < 1.5
+    assert 1e-4 < r1["r"] < 4e-3
+    r_narrow, _ = _r("bns", 3.0, 1)
+    assert r_narrow["r"] > 3.0 * r3["r"]
+
+
+def test_mbhb_example_edge_effect_needs_the_dc_bin():
+    """Section IV.C/D: with the bin k = 0 in the sums, as in the paper, delta = 1 and Delta k = 200 give r ~ 3 %
+    ("an order of magnitude" above the BNS example) and delta = 0.05, Delta k ~ 100 a per-cent level loss;
+    under reading A6 (k >= 1 only) most of the signal, which sits below the first bin, is lost."""
+    r_dc, w = _r("mbhb", 1.0, 100, include_dc=1)
+    assert abs(w.desc["t_sft"] - 1735.0) < 0.25 * 1735.0            # Table II with IMRPhenomT; the 1PN expansion is poor at MECO
+    assert 0.015 < r_dc["r"] < 0.06
+    r_a6, _ = _r("mbhb", 1.0, 100, include_dc=0)
+    assert r_a6["r"] > 5.0 * r_dc["r"]
+    r_05, _ = _r("mbhb", 0.05, 50, include_dc=1)
+    assert 0.005 < r_05["r"] < 0.04
+
+
+def test_short_sfts_tend_to_the_dirichlet_truncation_loss():
+    """delta -> 0: the per-SFT signal is monochromatic, ([h,h]) / <h,h> -> captured Dirichlet power.  With the frequency
+    uniformly spread over a bin the captured power inside +-K is 1 - 1/(pi^2 K) + O(K^-2) on average."""
+    res, w = _r("bns", 0.002, 8, f_start=6.0)
+    cap = res["hh"] / res["exact"]
+    assert abs((1.0 - cap) - 1.0 / (np.pi ** 2 * 8.5)) < 0.004
