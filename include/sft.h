@@ -163,6 +163,21 @@ sft_status sft_cumulative_snr(sft_plan *plan, int64_t n_templates, const double 
 sft_status sft_statistics(sft_plan *plan, int64_t n_templates, const double *xh, const double *xh_im,
                           const double *hh, double *loglike, double *rho2_phase_max, int32_t mem);
 
+/* F-statistic (Eq.(10)-(13) P:107-122) for long signals whose two polarisations are resolved by the amplitude modulation of the
+ * detector: h = sum_nu c_nu h_nu with the four basis waveforms h_nu = A(t) [a cos(phi), b cos(phi), a sin(phi), b sin(phi)]
+ * (Eq.(11)); 2F = x^T M^-1 x with x_nu = ([x,h_nu]), M_numu = ([h_nu,h_mu]) is twice the log-likelihood Eq.(2) maximised over
+ * the four amplitudes c_nu (Eq.(13)).  Needs a plan with SFT_RESP_TABLE whose table holds, per (channel, SFT), the pair of
+ * antenna-pattern functions (a, b) at the SFT start (constant over the SFT) in the (re, im) slots of sft_load_data's
+ * `response`; at most 2 channels.  One pass of the fused kernel accumulates the 4 + 3 sums per template; in the SFT framework
+ * the products between a cos and a sin quadrature vanish and ([h_0,h_0]) = ([h_2,h_2]), ([h_1,h_1]) = ([h_3,h_3]),
+ * ([h_0,h_1]) = ([h_2,h_3]), so that M has three distinct entries.
+ *   twoF  [n_templates] (required); 0 where M is singular (no active SFT, or a and b proportional)
+ *   xnu   [4][n_templates] or NULL: ([x,h_nu]), nu = 0..3
+ *   mnu   [3][n_templates] or NULL: ([h_0,h_0]), ([h_1,h_1]), ([h_0,h_1])
+ * `params`, `mem` as in sft_inner_products (phi_c enters 2F only through rounding). */
+sft_status sft_fstat(sft_plan *plan, int64_t n_templates, const double *params, double *twoF,
+                     double *xnu, double *mnu, int32_t mem);
+
 /* Blocks until all work enqueued on the plan's stream has finished. */
 sft_status sft_plan_sync(sft_plan *plan);
 

@@ -46,7 +46,7 @@ class PlanDesc(C.Structure):
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
            "sft_plan_set_chunk", "sft_plan_path_counts", "sft_compute_sfts", "sft_ingest_timeseries",
-           "sft_tsft_rule", "sft_statistics", "sft_last_error", "sft_version",
+           "sft_tsft_rule", "sft_statistics", "sft_fstat", "sft_last_error", "sft_version",
            "sft_measure_alu_peaks"]
 
 _lib = None
@@ -76,6 +76,8 @@ def load_library(path=None):
     lib.sft_plan_path_counts.argtypes = [vp, C.POINTER(i64), i32]
     lib.sft_statistics.argtypes = [vp, i64, vp, vp, vp, vp, vp, i32]
     lib.sft_statistics.restype = i32
+    lib.sft_fstat.argtypes = [vp, i64, vp, vp, vp, vp, i32]
+    lib.sft_fstat.restype = i32
     lib.sft_tsft_rule.argtypes = [dbl, dbl, i32, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
     lib.sft_tsft_rule.restype = i32
     lib.sft_compute_sfts.argtypes = [i32, vp, vp, i64, i32, dbl, i32, i32, vp, i32]
@@ -238,6 +240,14 @@ class Plan:
             self._h, nT, _ptr(xh, np.float64, (nT,), "xh"), _ptr(xh_im, np.float64, (nT,), "xh_im"),
             _ptr(hh, np.float64, (nT,), "hh"), _ptr(loglike, np.float64, (nT,), "loglike"),
             _ptr(rho2_phase_max, np.float64, (nT,), "rho2_phase_max"), mem))
+
+    def fstat(self, params, twoF, xnu=None, mnu=None):
+        """``sft_fstat``: 2F [nT] and optionally ([x,h_nu]) [4][nT], (([h_0,h_0]), ([h_1,h_1]), ([h_0,h_1])) [3][nT]."""
+        nT = int(params.shape[0])
+        mem = _where([params, twoF, xnu, mnu])
+        self._check(self.lib.sft_fstat(
+            self._h, nT, _ptr(params, np.float64, (nT, NPARAM), "params"), _ptr(twoF, np.float64, (nT,), "twoF"),
+            _ptr(xnu, np.float64, (4, nT), "xnu"), _ptr(mnu, np.float64, (3, nT), "mnu"), mem))
 
     def sync(self):
         self._check(self.lib.sft_plan_sync(self._h))

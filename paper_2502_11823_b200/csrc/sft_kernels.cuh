@@ -834,10 +834,18 @@ __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, dou
 }
 
 // Phase, amplitude, response and noise weight applied to the contracted sums of one (template, SFT).
+// F-statistic variant (`fq` != nullptr, MODE 2 of the main kernel; Eq.(10)-(13) P:107-122): the plan's response table holds the
+// antenna-pattern functions (a, b)_{c,a}; with W = A e^{i phi} sum_k conj(x~) F / S and H = A^2 sum_k |F|^2 / S of the unit
+// response, the four basis waveforms h_nu = A [a cos, b cos, a sin, b sin](phi) = Re[(a, b, -i a, -i b) A e^{i phi}] give
+//   ([x,h_0]) + i ([x,h_2]) = sum a W,   ([x,h_1]) + i ([x,h_3]) = sum b W,
+//   ([h_0,h_0]) = ([h_2,h_2]) = sum a^2 H,  ([h_1,h_1]) = ([h_3,h_3]) = sum b^2 H,  ([h_0,h_1]) = ([h_2,h_3]) = sum a b H,
+// and the products between a cos and a sin quadrature vanish (Re[R_nu conj R_mu] = 0).  fq[0..6] receive this SFT's terms of
+// {Re sum a W, Im sum a W, Re sum b W, Im sum b W, sum a^2 H, sum b^2 H, sum a b H}, summed over the channels.
 template <int CT, class CFG>
 __device__ __forceinline__ void finish_terms(const KParams &p, const Tmpl &tm, const float2 *rt, const Track &tr, bool ok,
                                              float scale, float t, const float (&s1r)[CT], const float (&s1i)[CT],
-                                             const float (&s2)[CT], const float (&us2)[CT], float &zr, float &zi, float &hh) {
+                                             const float (&s2)[CT], const float (&us2)[CT], float &zr, float &zi, float &hh,
+                                             float *fq = nullptr) {
   // |t| <= 1 + 1/2 + |b|/4: the MUFU sin/cos argument reduction (x/2pi rounded to fp32) stays below 3e-7 rad
   float sp, cp_;
   sincospi_fast(t, sp, cp_);
@@ -850,7 +858,8 @@ __device__ __forceinline__ void finish_terms(const KParams &p, const Tmpl &tm, c
   for (int c = 0; c < CT; ++c) {
     // response (Eq.(5)-(6) P:80-85 as Lambda z = Re[R z]; DESIGN C3/D4)
     float2 R = tm.AE[c];
-    if (resp == 1) {
+    if (fq) {                          // unit response; (a, b) are applied to the sums below
+    } else if (resp == 1) {
       const float2 r = __ldg(rt + c * p.n_sft);
       R = make_float2(tm.AE[c].x * r.x, tm.AE[c].x * r.y);      // AE is real here
     } else if (resp == 2) {
@@ -859,13 +868,26 @@ __device__ __forceinline__ void finish_terms(const KParams &p, const Tmpl &tm, c
       R = make_float2(R.x * am, R.y * am);
     }
     float gr, gi, r2;
-    if (resp == 0) {                   // AE is real
+    if (resp == 0 || fq) {             // AE is real
       gr = R.x * er; gi = R.x * ei; r2 = R.x * R.x;
     } else {
       gr = R.x * er - R.y * ei; gi = R.x * ei + R.y * er; r2 = R.x * R.x + R.y * R.y;   // p_c = R * A e^{i phi} pref
     }
     const float cr = gr * s1r[c] - gi * s1i[c], ci = gr * s1i[c] + gi * s1r[c];
     const float chh = r2 * a2 * us2[c] * s2[c];
+    if (fq) {
+      const float2 ab = __ldg(rt + c * p.n_sft);
+      const bool on = ok && us2[c] > 0.f;
+      const float wa = on ? ab.x : 0.f, wb = on ? ab.y : 0.f, h_ = on ? chh : 0.f;
+      const float xr = on ? cr : 0.f, xi_ = on ? ci : 0.f;
+      if (c == 0) {
+        fq[0] = wa * xr; fq[1] = wa * xi_; fq[2] = wb * xr; fq[3] = wb * xi_;
+        fq[4] = wa * wa * h_; fq[5] = wb * wb * h_; fq[6] = wa * wb * h_;
+      } else {
+        fq[0] = fmaf(wa, xr, fq[0]); fq[1] = fmaf(wa, xi_, fq[1]); fq[2] = fmaf(wb, xr, fq[2]); fq[3] = fmaf(wb, xi_, fq[3]);
+        fq[4] = fmaf(wa * wa, h_, fq[4]); fq[5] = fmaf(wb * wb, h_, fq[5]); fq[6] = fmaf(wa * wb, h_, fq[6]);
+      }
+    }
     if (CT == 1) {
       sr = cr; si = ci; sh = chh;
     } else {
@@ -914,7 +936,7 @@ __device__ __forceinline__ void duo_terms(const KParams &p, const Tmpl &tm, cons
 template <int KT, int CT, class CFG>
 __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, const float4 *Drow0, const float4 *Mrow0,
                                            const float2 *rt, const Track &tr, bool go, float bmax, const float (&us2)[CT],
-                                           double dnext, Track &nxt, float &zr, float &zi, float &hh) {
+                                           double dnext, Track &nxt, float &zr, float &zi, float &hh, float *fq = nullptr) {
   // window start in the zero-padded row; windows that miss the stored band entirely contribute 0
   const int j0 = tr.kc - p.kwin0;                                  // kwin0 = k_lo + K - PAD
   const bool ok = go && (unsigned)(j0 - 2) <= (unsigned)p.jmax;    // 2 <= j0 <= nb - 1 + PAD  <=>  window overlaps the band
@@ -966,7 +988,7 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, con
       s2[c] = scale * (acc[c].W.x + acc[c].W.y);             // one of the two factors `scale` of |J|^2
     }
   }
-  finish_terms<CT, CFG>(p, tm, rt, tr, ok, scale, t, s1r, s1i, s2, us2, zr, zi, hh);
+  finish_terms<CT, CFG>(p, tm, rt, tr, ok, scale, t, s1r, s1i, s2, us2, zr, zi, hh, fq);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1451,6 +1473,9 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
     const long long t = (long long)tg * 32 + lane;
     const int a0 = ch * p.chunk;
     const int a1 = min(a0 + p.chunk, p.n_sft);
+    double afs[MODE == 2 ? 7 : 1];     // MODE 2: the seven sums of the F-statistic (finish_terms)
+#pragma unroll
+    for (int i = 0; i < (MODE == 2 ? 7 : 1); ++i) afs[i] = 0.0;
     double axh = 0.0, ahh = 0.0, axi = 0.0;
     unsigned long long n_path[PATH_N] = {0, 0, 0, 0, 0, 0, 0};
     unsigned smask = 0xffffffffu;      // MODE 1: slots of the unit's tile that were written (a clean block writes the present SFTs only)
@@ -1465,7 +1490,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
         // where the template's amplitude constant is real (no response, one channel) it is folded into the amplitude
         const float ascale = (CFG::RESP == 0 && CT == 1) ? tm.AE[0].x : 1.0f;
         FastCoef fc;
-        const int kind = fast_setup<CT, CFG, CREG>(p, tm, gs, gend, lane, ascale, cs, mask, usv, fc);
+        const int kind = MODE == 2 ? 0 : fast_setup<CT, CFG, CREG>(p, tm, gs, gend, lane, ascale, cs, mask, usv, fc);
         if (kind != 0) smask = mask;
         if (kind == 2) {
           fast_block<CT, MODE, CFG, true, CREG>(p, tm, cs, fc, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
@@ -1490,6 +1515,9 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
       for (int g = gs; g < gend; g += GROUP) {
         const int ge = min(g + GROUP, gend);
         float fxh = 0.f, fhh = 0.f, fxi = 0.f;
+        float ffs[MODE == 2 ? 7 : 1];
+#pragma unroll
+        for (int i = 0; i < (MODE == 2 ? 7 : 1); ++i) ffs[i] = 0.f;
         int alpha = g;
         while (alpha < ge) {
           float us2[CT], us2b[CT];
@@ -1503,7 +1531,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
           const float ab = (go && cfg_kernel<CFG>(p) == 1) ? fabsf(tr.b) : 0.f;
           // two SFTs at once when both are present and both go through the tier-1 tables
           bool duo = false, gob = false;
-          if (DUO && alpha + 1 < ge) {
+          if (DUO && MODE != 2 && alpha + 1 < ge) {
 #pragma unroll
             for (int c = 0; c < CT; ++c) {
               us2b[c] = __ldg(usp + c * p.n_sft + 1);
@@ -1560,8 +1588,12 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
               n_path[path_of(bmax, p.mtab != nullptr)] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * n_present);
             }
             float zr, zi, hh;
-            pair_terms<KT, CT, CFG>(p, tm, Drow0, Mrow0, rt, tr, go, bmax, us2, dalpha + 2.0, nxt, zr, zi, hh);
-            if (MODE == 1) {
+            float fq[7];
+            pair_terms<KT, CT, CFG>(p, tm, Drow0, Mrow0, rt, tr, go, bmax, us2, dalpha + 2.0, nxt, zr, zi, hh, MODE == 2 ? fq : nullptr);
+            if (MODE == 2) {
+#pragma unroll
+              for (int i = 0; i < 7; ++i) ffs[i] += fq[i];
+            } else if (MODE == 1) {
               axh += (double)zr;
               ahh += (double)hh;
             } else {
@@ -1590,10 +1622,20 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
         if (MODE == 0) {
           axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
         }
+        if (MODE == 2) {
+#pragma unroll
+          for (int i = 0; i < 7; ++i) afs[i] += (double)ffs[i];
+        }
       }
     }
     if (MODE == 1) {
       scan_store(p, txh, thh, tg, ch, a1 - a0, lane, t, axh, ahh, smask);        // (the host sets chunk = SUB = 32 for MODE 1)
+    } else if (MODE == 2) {
+      if (t < p.nT) {
+        double *q = p.part + (size_t)ch * 7 * p.nT + t;
+#pragma unroll
+        for (int i = 0; i < 7; ++i) q[(size_t)i * p.nT] = afs[i];
+      }
     } else if (t < p.nT) {
       double *q = p.part + (size_t)ch * 3 * p.nT + t;
       q[0] = axh;
@@ -1608,17 +1650,19 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
   }
 }
 
-// Sum of the chunk totals in fp64, fixed order (deterministic).  grid = (ceil(nT/32), 3 quantities),
+// Sum of the chunk totals in fp64, fixed order (deterministic).  grid = (ceil(nT/32), nq quantities),
 // block = 32 templates x RED_SLICES chunk slices; slice s sums the chunks c = s (mod RED_SLICES).
 constexpr int RED_SLICES = 16;
-__global__ void __launch_bounds__(32 * RED_SLICES) sft_reduce_kernel(const double *part, long long nT, int n_chunks,
-                                                                     double *xh, double *hh, double *xi) {
+struct RedOut {
+  double *q[7];          // output vector of quantity blockIdx.y (null: skipped)
+};
+__global__ void __launch_bounds__(32 * RED_SLICES) sft_reduce_kernel(const double *part, long long nT, int n_chunks, int nq, RedOut o) {
   __shared__ double sm[RED_SLICES][33];
   const int tx = threadIdx.x & 31, sl = threadIdx.x >> 5;
   const long long t = (long long)blockIdx.x * 32 + tx;
-  double *out = blockIdx.y == 0 ? xh : blockIdx.y == 1 ? hh : xi;
+  double *out = o.q[blockIdx.y];
   if (!out) return;
-  const size_t stride = (size_t)3 * nT;
+  const size_t stride = (size_t)nq * nT;
   double s0 = 0.0, s1 = 0.0;
   if (t < nT) {
     const double *q = part + (size_t)blockIdx.y * nT + t;
@@ -1637,6 +1681,20 @@ __global__ void __launch_bounds__(32 * RED_SLICES) sft_reduce_kernel(const doubl
     for (int j = 1; j < RED_SLICES; ++j) s += sm[j][tx];
     out[t] = s;
   }
+}
+
+// F-statistic from the seven sums (finish_terms): x = (Re Xa, Re Xb, Im Xa, Im Xb), M = [[A, C], [C, B]] (+) [[A, C], [C, B]],
+//   2F = x^T M^-1 x = [B (x0^2 + x2^2) + A (x1^2 + x3^2) - 2 C (x0 x1 + x2 x3)] / (A B - C^2)            (Eq.(13))
+// (0 where the determinant is not positive: no active SFT, or a and b proportional over the whole data).
+__global__ void sft_fstat_kernel(long long n, const double *sums, double *twoF, double *xnu, double *mnu) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const double x0 = sums[t], x2 = sums[n + t], x1 = sums[2 * n + t], x3 = sums[3 * n + t];
+  const double A = sums[4 * n + t], B = sums[5 * n + t], C = sums[6 * n + t];
+  const double D = A * B - C * C;
+  if (twoF) twoF[t] = D > 0.0 ? (B * (x0 * x0 + x2 * x2) + A * (x1 * x1 + x3 * x3) - 2.0 * C * (x0 * x1 + x2 * x3)) / D : 0.0;
+  if (xnu) { xnu[t] = x0; xnu[n + t] = x1; xnu[2 * n + t] = x2; xnu[3 * n + t] = x3; }
+  if (mnu) { mnu[t] = A; mnu[n + t] = B; mnu[2 * n + t] = C; }
 }
 
 // Statistics on top of the inner products: log-likelihood L = <x,h> - <h,h>/2 (Eq.(2)) and the

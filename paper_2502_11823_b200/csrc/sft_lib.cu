@@ -612,7 +612,7 @@ static cudaError_t launch_main(sft_plan *p, const KParams &k) {
   return cudaGetLastError();
 }
 
-static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t mem, KParams &k, bool cumulative) {
+static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t mem, KParams &k, bool cumulative, int nq = 3) {
   for (int c = 0; c < p->d.n_channels; ++c)
     if (!p->loaded[c]) return fail(p, SFT_ENODATA, "channel %d has no data (call sft_load_data)", c);
   if (nT > (1ll << 31) - 1) return fail(p, SFT_EINVAL, "n_templates too large");
@@ -653,7 +653,7 @@ static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t
     k.flagP = k.flagA + ent;
     k.epoch = p->epoch;
   } else {
-    st = grow(p, (void **)&p->part, &p->part_bytes, (size_t)k.n_chunks * 3 * nT * sizeof(double));
+    st = grow(p, (void **)&p->part, &p->part_bytes, (size_t)k.n_chunks * nq * nT * sizeof(double));
     if (st != SFT_OK) return st;
     k.part = p->part;
   }
@@ -710,8 +710,8 @@ SFT_API sft_status sft_inner_products(sft_plan *p, int64_t nT, const double *par
   if (d_kc) CU(p, cudaMemsetAsync(p->path_counts, 0, sftk::PATH_N * sizeof(unsigned long long), p->stream));
   cudaError_t e = launch_main<0>(p, k);
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
-  sftk::sft_reduce_kernel<<<dim3((unsigned)((nT + 31) / 32), 3), 32 * sftk::RED_SLICES, 0, p->stream>>>(p->part, nT, k.n_chunks, d_xh,
-                                                                                                        d_hh, d_xi);
+  sftk::RedOut ro = {{d_xh, d_hh, d_xi, nullptr, nullptr, nullptr, nullptr}};
+  sftk::sft_reduce_kernel<<<dim3((unsigned)((nT + 31) / 32), 3), 32 * sftk::RED_SLICES, 0, p->stream>>>(p->part, nT, k.n_chunks, 3, ro);
   p->launches++;
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "reduce kernel launch: %s", cudaGetErrorString(e));
@@ -766,6 +766,60 @@ SFT_API sft_status sft_statistics(sft_plan *p, int64_t nT, const double *xh, con
     if (loglike) CU(p, cudaMemcpyAsync(loglike, d_l, b, cudaMemcpyDeviceToHost, p->stream));
     if (rho2_phase_max) CU(p, cudaMemcpyAsync(rho2_phase_max, d_r, b, cudaMemcpyDeviceToHost, p->stream));
     CU(p, cudaStreamSynchronize(p->stream));
+  }
+  return SFT_OK;
+}
+
+// F-statistic, Eq.(10)-(13) P:107-122: one pass of the fused kernel (MODE 2) accumulates the seven sums per template.
+SFT_API sft_status sft_fstat(sft_plan *p, int64_t nT, const double *params, double *twoF, double *xnu, double *mnu, int32_t mem) {
+  if (!p) return SFT_EINVAL;
+  p->err[0] = 0;
+  if (nT < 0) return fail(p, SFT_EINVAL, "n_templates < 0");
+  if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(p, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
+  if (nT == 0) return SFT_OK;
+  if (!params || !twoF) return fail(p, SFT_EINVAL, "params and twoF are required");
+  if (p->d.response != SFT_RESP_TABLE)
+    return fail(p, SFT_EINVAL, "sft_fstat needs a plan with SFT_RESP_TABLE: the table holds the antenna-pattern functions (a, b)");
+  if (p->d.n_channels > 2) return fail(p, SFT_EUNSUPPORTED, "sft_fstat: at most 2 channels in this build");
+  KParams k;
+  sft_status st = prepare(p, nT, params, mem, k, false, 7);
+  if (st != SFT_OK) return st;
+  const size_t b_vec = (size_t)nT * sizeof(double);
+  // scratch: the 7 reduced sums, then (host calls) the 1 + 4 + 3 output vectors
+  st = grow(p, &p->d_out, &p->out_bytes, 15 * b_vec + 256);
+  if (st != SFT_OK) return st;
+  double *sums = (double *)p->d_out, *d_F = twoF, *d_x = xnu, *d_m = mnu;
+  if (mem == SFT_MEM_HOST) {
+    d_F = sums + 7 * nT;
+    d_x = xnu ? d_F + nT : nullptr;
+    d_m = mnu ? d_F + 5 * nT : nullptr;
+  }
+  k.kc_out = nullptr;
+  k.path_counts = nullptr;
+  cudaEventRecord(p->ev0, p->stream);
+  if (k.C == 1) launch_variant<0, 1, 2, CfgAny>(p, k);
+  else launch_variant<0, 2, 2, CfgAny>(p, k);
+  cudaEventRecord(p->ev1, p->stream);
+  p->timed = true;
+  p->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
+  sftk::RedOut ro;
+  for (int i = 0; i < 7; ++i) ro.q[i] = sums + (size_t)i * nT;
+  sftk::sft_reduce_kernel<<<dim3((unsigned)((nT + 31) / 32), 7), 32 * sftk::RED_SLICES, 0, p->stream>>>(p->part, nT, k.n_chunks, 7, ro);
+  sftk::sft_fstat_kernel<<<(unsigned)((nT + 255) / 256), 256, 0, p->stream>>>(nT, sums, d_F, d_x, d_m);
+  p->launches += 2;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "reduce / F-statistic kernel launch: %s", cudaGetErrorString(e));
+  if (mem == SFT_MEM_HOST) {
+    st = grow_pinned(p, 8 * b_vec);
+    if (st != SFT_OK) return st;
+    double *h = (double *)p->h_pin;
+    CU(p, cudaMemcpyAsync(h, d_F, 8 * b_vec, cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
+    memcpy(twoF, h, b_vec);
+    if (xnu) memcpy(xnu, h + nT, 4 * b_vec);
+    if (mnu) memcpy(mnu, h + 5 * nT, 3 * b_vec);
   }
   return SFT_OK;
 }

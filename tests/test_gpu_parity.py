@@ -265,6 +265,40 @@ def test_statistics_phase_maximised(et_small):
     assert np.abs(stat - stat_o).max() <= 1e-3 * stat_o.max()
 
 
+@pytest.mark.parametrize("n_channels,noise", [(1, 0.0), (1, 0.7), (2, 0.7)])
+def test_fstat_matches_oracle(n_channels, noise):
+    """sft_fstat (NEXT-3; Eq.(10)-(13) P:107-122): the 4 products ([x,h_nu]), the 3 distinct ([h_nu,h_mu]) and 2F against the
+    oracle, which sums all 4 + 10 products bin by bin and solves the 4 x 4 system; noiseless data return the injected c_nu."""
+    from oracle import stats as ost
+    api = _api()
+    w = wl.fstat_case(n_templates=70, n_channels=n_channels, noise=noise)
+    plan_o, store = to_oracle(w)
+    a, b = w.response.real.astype(np.float64), w.response.imag.astype(np.float64)
+    o = ost.fstat(plan_o, store, w.params, a, b)
+    xx = oin.xx_band(plan_o, store)
+    nT = w.n_templates
+    for ev in ("auto", "direct"):
+        with api.plan_from_workload(w, evaluator=ev) as plan:
+            F, x, m = np.full(nT, np.nan), np.full((4, nT), np.nan), np.full((3, nT), np.nan)
+            plan.fstat(np.ascontiguousarray(w.params), F, x, m)
+            F2 = np.full(nT, np.nan)
+            plan.fstat(np.ascontiguousarray(w.params), F2)
+        assert np.array_equal(F, F2)
+        Mo = o["M"]
+        for nu in range(4):
+            assert (np.abs(x[nu] - o["x"][:, nu]) / np.sqrt(xx * Mo[:, nu, nu])).max() <= REG
+        for i, (nu, mu) in enumerate(((0, 0), (1, 1), (0, 1))):
+            assert (np.abs(m[i] - Mo[:, nu, mu]) / np.sqrt(Mo[:, nu, nu] * Mo[:, mu, mu])).max() <= REG
+            assert (np.abs(m[i] - Mo[:, nu + 2, mu + 2]) / np.sqrt(Mo[:, nu, nu] * Mo[:, mu, mu])).max() <= REG
+        assert np.abs(Mo[:, :2, 2:]).max() <= 1e-10 * np.abs(Mo).max()                 # what the kernel does not compute is zero
+        # 2F: |d 2F| <= 2 sqrt(2F) |d x|_M  ->  bar REG sqrt(<x,x>) 2 sqrt(2F) (+ relative REG for the M part)
+        assert np.all(np.abs(F - o["twoF"]) <= 4.0 * REG * np.sqrt(xx * np.maximum(o["twoF"], 1e-300)) + 10 * REG * o["twoF"])
+    if noise == 0.0:
+        M = np.array([[m[0][0], m[2][0], 0, 0], [m[2][0], m[1][0], 0, 0], [0, 0, m[0][0], m[2][0]], [0, 0, m[2][0], m[1][0]]])
+        c = np.linalg.solve(M, x[:, 0])
+        assert np.abs(c - w.notes["c_nu"]).max() < 0.02
+
+
 def test_response_table():
     """SFT_RESP_TABLE: an arbitrary complex per-(channel, SFT) response."""
     w = wl.config4(n_templates=40)
