@@ -53,7 +53,8 @@ typedef enum {
 enum { SFT_KERNEL_DIRICHLET = 0, /* F(a,0) = e^{i pi a} sinc(a), Eq.(B2)          */
        SFT_KERNEL_FRESNEL = 1 }; /* F(a,b), Eq.(28)-(32) P:215-236                      */
 enum { SFT_WF_PN0 = 0,           /* Newtonian restricted TaylorT3 inspiral              */
-       SFT_WF_PN1 = 1 };         /* + 1PN phase and frequency terms                     */
+       SFT_WF_PN1 = 1,           /* + 1PN phase and frequency terms                     */
+       SFT_WF_PN15 = 2 };        /* + 1.5PN (tail) terms: phase -(3 pi/4) Theta^(1/4), frequency -(3 pi/10) Theta^(-3/4)  */
 enum { SFT_PHASE_FP64 = 0,       /* phase/frequency track evaluated in fp64             */
        SFT_PHASE_SPLIT32 = 1 };  /* track evaluated in double-float (2 x fp32) arithmetic: same bins,
                                     phases to ~1e-7 rad; slower on B200       */
@@ -162,6 +163,16 @@ sft_status sft_cumulative_snr(sft_plan *plan, int64_t n_templates, const double 
  *                   over distance and initial phase (Eq.(7)-(9) P:97-101; 0 where hh == 0), nullable */
 sft_status sft_statistics(sft_plan *plan, int64_t n_templates, const double *xh, const double *xh_im,
                           const double *hh, double *loglike, double *rho2_phase_max, int32_t mem);
+
+/* Validity of the per-SFT signal model for each template (Eq.(33)-(34) P:244-248): the quadratic phase model of Eq.(17) is good
+ * over one SFT while 1/2 T_SFT^2 max fddot <= delta df; per template
+ *   delta_eff [n_templates] doubles or NULL: 1/2 T_SFT^3 fddot at the template's last active SFT (DESIGN A12), where fddot is
+ *             largest - the delta at which Eq.(33) holds with equality on this plan's T_SFT; 0 for a template with no active SFT
+ *   flags     [n_templates] bytes or NULL: 1 where delta_eff > delta_max (the template leaves the regime the plan's SFT length
+ *             was chosen for: expect a loss r, Eq.(36), above the one of the paper's Fig. 3/4 at that delta), else 0
+ * Needs no data (channels may be unloaded).  At least one output must be non-NULL. */
+sft_status sft_validity(sft_plan *plan, int64_t n_templates, const double *params, double delta_max,
+                        double *delta_eff, uint8_t *flags, int32_t mem);
 
 /* F-statistic (Eq.(10)-(13) P:107-122) for long signals whose two polarisations are resolved by the amplitude modulation of the
  * detector: h = sum_nu c_nu h_nu with the four basis waveforms h_nu = A(t) [a cos(phi), b cos(phi), a sin(phi), b sin(phi)]

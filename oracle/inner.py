@@ -249,3 +249,20 @@ def xx_band(plan, store):
             w = np.where(valid[None, :] & present[c][:, None], 1.0 / S, 0.0)
         tot += 4.0 / plan.t_sft * float(np.sum(np.abs(np.asarray(store.bins[c], np.complex128)) ** 2 * w))
     return tot
+
+
+def validity(plan, params):
+    """Eq.(33)-(34) P:244-248 per template: ``delta_eff = 1/2 T_SFT^3 max_a fddot_a`` over the template's active SFTs (the
+    delta at which Eq.(33) ``1/2 T^2 max fddot <= delta df`` holds with equality on the plan's SFT length); 0 where no SFT is
+    active.  [T]"""
+    params = np.atleast_2d(np.asarray(params, dtype=np.float64))
+    t = sft_times(plan)
+    out = np.zeros(params.shape[0])
+    for i, p in enumerate(params):
+        phi, f, fdot = wf.taylor_t3(p[0], p[1], p[2], p[3], t, plan.pn1)
+        _, _, _, active, _ = select_bins(plan, t, f, fdot, p[2])
+        if active.any():
+            with np.errstate(invalid="ignore"):
+                fdd = wf.taylor_t3_fddot(p[0], p[1], p[2], t, plan.pn1)
+            out[i] = 0.5 * plan.t_sft ** 3 * np.max(fdd[active])
+    return out

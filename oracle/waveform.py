@@ -24,6 +24,9 @@ C_PHI_0 = 3715.0 / 8064.0
 C_PHI_1 = 55.0 / 96.0
 C_F_0 = 743.0 / 2688.0
 C_F_1 = 11.0 / 32.0
+#: 1.5PN (tail) terms of TaylorT3 relative to the leading one, in Theta^(-3/8): phase -3 pi/4, frequency -3 pi/10
+C15_PHI = -0.75 * np.pi
+C15_F = -0.3 * np.pi
 
 
 def total_mass_seconds(m_chirp, eta):
@@ -34,7 +37,9 @@ def total_mass_seconds(m_chirp, eta):
 def taylor_t3(m_chirp, eta, t_c, phi_c, t, pn1):
     """Phase [rad], frequency [Hz], frequency derivative [Hz/s] at times ``t``.
 
-    ``pn1`` in {0, 1} switches the 1PN terms.  Where ``t >= t_c`` the outputs are NaN
+    ``pn1`` is the PN order code: 0 = 0PN, 1 = + 1PN terms, 2 = + 1.5PN (tail) terms
+    ``phi += (2/eta)(3 pi/4) Theta^{1/4}``, ``f -= (3 pi/10) Theta^{-3/4}/(8 pi M)`` (the textbook TaylorT3 coefficients;
+    ``dphi/dt = 2 pi f`` holds order by order, pinned numerically).  Where ``t >= t_c`` the outputs are NaN
     (the template has ended; such SFTs are inactive, reading A12).
     """
     t = np.asarray(t, dtype=np.float64)
@@ -45,10 +50,12 @@ def taylor_t3(m_chirp, eta, t_c, phi_c, t, pn1):
         cphi = C_PHI_0 + C_PHI_1 * eta
         cf = C_F_0 + C_F_1 * eta
         th_m14 = theta ** (-0.25)
-        phi = phi_c - (2.0 / eta) * theta ** 0.625 * (1.0 + pn1 * cphi * th_m14)
-        f = theta ** (-0.375) / (8.0 * np.pi * M) * (1.0 + pn1 * cf * th_m14)
+        th_m38 = theta ** (-0.375)
+        p1, p15 = float(pn1 >= 1), float(pn1 >= 2)
+        phi = phi_c - (2.0 / eta) * theta ** 0.625 * (1.0 + p1 * cphi * th_m14 + p15 * C15_PHI * th_m38)
+        f = theta ** (-0.375) / (8.0 * np.pi * M) * (1.0 + p1 * cf * th_m14 + p15 * C15_F * th_m38)
         fdot = (eta / (5.0 * M)) / (8.0 * np.pi * M) * (
-            0.375 * theta ** (-1.375) + 0.625 * pn1 * cf * theta ** (-1.625))
+            0.375 * theta ** (-1.375) + 0.625 * p1 * cf * theta ** (-1.625) + 0.75 * p15 * C15_F * theta ** (-1.75))
     return phi, f, fdot
 
 
@@ -60,7 +67,8 @@ def taylor_t3_fddot(m_chirp, eta, t_c, t, pn1):
     cf = C_F_0 + C_F_1 * eta
     k = eta / (5.0 * M)
     return k * k / (8.0 * np.pi * M) * (
-        0.375 * 1.375 * theta ** (-2.375) + 0.625 * 1.625 * pn1 * cf * theta ** (-2.625))
+        0.375 * 1.375 * theta ** (-2.375) + 0.625 * 1.625 * float(pn1 >= 1) * cf * theta ** (-2.625)
+        + 0.75 * 1.75 * float(pn1 >= 2) * C15_F * theta ** (-2.75))
 
 
 def amplitude(amp, f, f_ref):

@@ -46,7 +46,7 @@ class PlanDesc(C.Structure):
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
            "sft_plan_set_chunk", "sft_plan_path_counts", "sft_compute_sfts", "sft_ingest_timeseries",
-           "sft_tsft_rule", "sft_statistics", "sft_fstat", "sft_last_error", "sft_version",
+           "sft_tsft_rule", "sft_statistics", "sft_fstat", "sft_validity", "sft_last_error", "sft_version",
            "sft_measure_alu_peaks"]
 
 _lib = None
@@ -78,6 +78,8 @@ def load_library(path=None):
     lib.sft_statistics.restype = i32
     lib.sft_fstat.argtypes = [vp, i64, vp, vp, vp, vp, i32]
     lib.sft_fstat.restype = i32
+    lib.sft_validity.argtypes = [vp, i64, vp, dbl, vp, vp, i32]
+    lib.sft_validity.restype = i32
     lib.sft_tsft_rule.argtypes = [dbl, dbl, i32, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
     lib.sft_tsft_rule.restype = i32
     lib.sft_compute_sfts.argtypes = [i32, vp, vp, i64, i32, dbl, i32, i32, vp, i32]
@@ -118,7 +120,7 @@ def _ptr(a, dtype, shape=None, name="array"):
     if _is_torch(a):
         import torch
         want = {np.float32: torch.float32, np.float64: torch.float64, np.int32: torch.int32,
-                np.complex64: torch.complex64}[dtype]
+                np.complex64: torch.complex64, np.uint8: torch.uint8}[dtype]
         if a.dtype != want or not a.is_contiguous():
             raise TypeError("%s must be a contiguous %s tensor" % (name, want))
         if shape is not None and tuple(a.shape) != tuple(shape):
@@ -248,6 +250,14 @@ class Plan:
         self._check(self.lib.sft_fstat(
             self._h, nT, _ptr(params, np.float64, (nT, NPARAM), "params"), _ptr(twoF, np.float64, (nT,), "twoF"),
             _ptr(xnu, np.float64, (4, nT), "xnu"), _ptr(mnu, np.float64, (3, nT), "mnu"), mem))
+
+    def validity(self, params, delta_max, delta_eff=None, flags=None):
+        """``sft_validity``: delta_eff [nT] float64 and / or flags [nT] uint8 (delta_eff > delta_max)."""
+        nT = int(params.shape[0])
+        mem = _where([params, delta_eff, flags])
+        self._check(self.lib.sft_validity(
+            self._h, nT, _ptr(params, np.float64, (nT, NPARAM), "params"), float(delta_max),
+            _ptr(delta_eff, np.float64, (nT,), "delta_eff"), _ptr(flags, np.uint8, (nT,), "flags"), mem))
 
     def sync(self):
         self._check(self.lib.sft_plan_sync(self._h))

@@ -37,6 +37,8 @@ constexpr int MAXC = 4;              // SFT_MAX_CHANNELS
 constexpr int FLUSH = 8;             // SFTs summed in fp32 before the fp64 accumulators are touched
 constexpr double GMSUN_S = 4.925491025543576e-6;   // G Msun / c^3 [s]
 constexpr float PI_F = 3.14159265358979f;
+// 1.5PN ("tail") coefficients of TaylorT3 in Theta^(-3/8) relative to the leading term: phase -3 pi/4, frequency -3 pi/10
+constexpr double C15_PHI = -0.75 * 3.141592653589793, C15_F = -0.3 * 3.141592653589793;
 constexpr float INV_2PI_F = 0.15915494309189535f;
 
 // b = fdot T^2 thresholds of the coefficient evaluator (DESIGN "kernel evaluator"): the power
@@ -152,6 +154,7 @@ struct Cfg {
 };
 template <class CFG> __device__ __forceinline__ int cfg_phase(const KParams &p) { return CFG::PHASE >= 0 ? CFG::PHASE : p.phase_path; }
 template <class CFG> __device__ __forceinline__ int cfg_kernel(const KParams &p) { return CFG::KERNEL >= 0 ? CFG::KERNEL : p.kernel; }
+// PN order code of the waveform: 0 = 0PN, 1 = 0PN+1PN, 2 = 0PN+1PN+1.5PN (SFT_WF_*)
 template <class CFG> __device__ __forceinline__ int cfg_pn1(const KParams &p) { return CFG::PN1 >= 0 ? CFG::PN1 : p.pn1; }
 template <class CFG> __device__ __forceinline__ int cfg_resp(const KParams &p) { return CFG::RESP >= 0 ? CFG::RESP : p.response; }
 
@@ -318,14 +321,21 @@ __device__ __forceinline__ void track_eval_split32(const KParams &p, const Tmpl 
   const float sr = fmaf(r.h, 9.0f / 128.0f, 0.125f) * r.h;          // s = r/8 + 9 r^2/128, |s| ~ 1e-6: fp32 suffices
   const df32 q = df_add(y, df_mul_f(y, sr));                        // Theta^(-1/8), error ~ y * 6e-8 * |s| ~ 1e-13
   const df32 q2 = df_mul(q, q), q3 = df_mul(q2, q), q4 = df_mul(q2, q2), q8 = df_mul(q4, q4), q11 = df_mul(q8, q3);
-  const bool pn1 = cfg_pn1<CFG>(p) != 0;
+  const bool pn1 = cfg_pn1<CFG>(p) != 0, pn15 = cfg_pn1<CFG>(p) >= 2;
   df32 ph, fT, b;
   const df32 thq3 = df_mul(theta, q3);
   if (pn1) {
-    ph = df_add(c.phic_cyc, df_neg(df_mul(df_mul(c.cphase, thq3), df_add(one, df_mul(c.cphi, q2)))));
-    fT = df_mul(df_mul(c.F0T, q3), df_add(one, df_mul(c.cf, q2)));
+    df32 gp = df_add(one, df_mul(c.cphi, q2)), gf = df_add(one, df_mul(c.cf, q2));
     const df32 k375 = {0.375f, 0.f};
-    b = df_mul(df_mul(c.bscale, q11), df_add(k375, df_mul_f(df_mul(c.cf, q2), 0.625f)));
+    df32 gb = df_add(k375, df_mul_f(df_mul(c.cf, q2), 0.625f));
+    if (pn15) {
+      gp = df_add(gp, df_mul(df_from(C15_PHI), q3));
+      gf = df_add(gf, df_mul(df_from(C15_F), q3));
+      gb = df_add(gb, df_mul(df_from(0.75 * C15_F), q3));
+    }
+    ph = df_add(c.phic_cyc, df_neg(df_mul(df_mul(c.cphase, thq3), gp)));
+    fT = df_mul(df_mul(c.F0T, q3), gf);
+    b = df_mul(df_mul(c.bscale, q11), gb);
   } else {
     ph = df_add(c.phic_cyc, df_neg(df_mul(c.cphase, thq3)));
     fT = df_mul(c.F0T, q3);
@@ -347,7 +357,7 @@ __device__ __forceinline__ void track_eval_split32(const KParams &p, const Tmpl 
   tr.frac = fr - rintf(fr);
   const float q2f = y0 * y0;
   float a = q2f;
-  if (pn1) a *= ex2_approx((2.0f / 3.0f) * lg2_approx(fmaf(tm.cf32, q2f, 1.0f)));
+  if (pn1) a *= ex2_approx((2.0f / 3.0f) * lg2_approx(fmaf(tm.cf32, q2f, 1.0f) + (pn15 ? (float)C15_F * (q2f * y0) : 0.f)));
   tr.amp = a;
 }
 
@@ -371,12 +381,18 @@ __device__ __forceinline__ void track_eval_fp64(const KParams &p, const Tmpl &tm
   const double s = fma(r, 9.0 / 128.0, 0.125) * r;
   const double q = fma(y, s, y);                  // Theta^(-1/8)
   const double q2 = q * q, q3 = q2 * q, q4 = q2 * q2, q8 = q4 * q4;
-  const bool pn1 = cfg_pn1<CFG>(p) != 0;
+  const bool pn1 = cfg_pn1<CFG>(p) != 0, pn15 = cfg_pn1<CFG>(p) >= 2;
   double ph, fT, b;
   if (pn1) {
-    ph = fma(-tm.cphase * (theta * q3), fma(tm.cphi, q2, 1.0), tm.phic_cyc);   // cycles
-    fT = tm.F0T * q3 * fma(tm.cf, q2, 1.0);
-    b = tm.bscale * (q8 * q3) * fma(0.625 * tm.cf, q2, 0.375);
+    double gp = fma(tm.cphi, q2, 1.0), gf = fma(tm.cf, q2, 1.0), gb = fma(0.625 * tm.cf, q2, 0.375);
+    if (pn15) {                                     // 1.5PN tail terms, relative order Theta^(-3/8) = q^3
+      gp = fma(C15_PHI, q3, gp);
+      gf = fma(C15_F, q3, gf);
+      gb = fma(0.75 * C15_F, q3, gb);
+    }
+    ph = fma(-tm.cphase * (theta * q3), gp, tm.phic_cyc);   // cycles
+    fT = tm.F0T * q3 * gf;
+    b = tm.bscale * (q8 * q3) * gb;
   } else {
     ph = fma(-tm.cphase, theta * q3, tm.phic_cyc);
     fT = tm.F0T * q3;
@@ -393,7 +409,7 @@ __device__ __forceinline__ void track_eval_fp64(const KParams &p, const Tmpl &tm
   // amplitude (f_a/F0)^(2/3) = q^2 (1 + cf q^2)^(2/3): the seed is good enough (1e-6 relative)
   const float q2f = y0 * y0;
   float a = q2f;
-  if (pn1) a *= ex2_approx((2.0f / 3.0f) * lg2_approx(fmaf(tm.cf32, q2f, 1.0f)));
+  if (pn1) a *= ex2_approx((2.0f / 3.0f) * lg2_approx(fmaf(tm.cf32, q2f, 1.0f) + (pn15 ? (float)C15_F * (q2f * y0) : 0.f)));
   tr.amp = a;
 }
 
@@ -1052,7 +1068,7 @@ struct FTrack {
 // `ascale` multiplies the amplitude polynomial.
 template <class CFG>
 __device__ __forceinline__ bool fast_coef(const KParams &p, const Tmpl &tm, int g, float ascale, FastCoef &fc) {
-  const bool pn1 = cfg_pn1<CFG>(p) != 0, fres = cfg_kernel<CFG>(p) == 1;
+  const bool pn1 = cfg_pn1<CFG>(p) != 0, pn15 = cfg_pn1<CFG>(p) >= 2, fres = cfg_kernel<CFG>(p) == 1;
   const double tau = fma(-(double)(g + 16), p.T, tm.tau0);
   const double theta = tm.cTheta * tau;
   const float y0 = ex2_approx(-0.125f * lg2_approx((float)theta));
@@ -1065,14 +1081,16 @@ __device__ __forceinline__ bool fast_coef(const KParams &p, const Tmpl &tm, int 
   const double me = -eps;
   double A = theta * q3;                                             // Theta^(5/8)
   double B = pn1 ? tm.cphi * (theta * (q3 * q2)) : 0.0;              // c_phi Theta^(3/8)
+  double Cq = pn15 ? C15_PHI * (theta * (q3 * q3)) : 0.0;            // -3 pi/4 Theta^(1/4)
   const double mc = -tm.cphase;
   double pk[8];
-  pk[0] = fma(mc, A + B, tm.phic_cyc);
+  pk[0] = fma(mc, A + B + Cq, tm.phic_cyc);
 #pragma unroll
   for (int k = 1; k <= 7; ++k) {
     A *= me * ((0.625 - (double)(k - 1)) / (double)k);               // binom(5/8, k) (-eps)^k Theta_m^(5/8)
     if (pn1) B *= me * ((0.375 - (double)(k - 1)) / (double)k);
-    pk[k] = mc * (A + B);
+    if (pn15) Cq *= me * ((0.25 - (double)(k - 1)) / (double)k);
+    pk[k] = mc * (A + B + Cq);
   }
   double yk[6];
 #pragma unroll
@@ -1091,9 +1109,9 @@ __device__ __forceinline__ bool fast_coef(const KParams &p, const Tmpl &tm, int 
   // amplitude q^2 (1 + cf q^2)^(2/3) = a_m (1 - eps u)^(-s1),  s1 = -dln a/dln Theta = (1 + 2 w/3)/4,  w = cf q^2/(1 + cf q^2)
   double am = q2, s1 = 0.25;
   if (pn1) {
-    const double gq = fma(tm.cf, q2, 1.0);
-    am = q2 * (double)cbrtf((float)(gq * gq));                       // (1 + cf q^2)^(2/3) ~ 1.0x: fp32 cube root, 1e-7 relative
-    s1 = 0.25 * fma(2.0 / 3.0, tm.cf * q2 / gq, 1.0);
+    const double gq = fma(tm.cf, q2, 1.0) + (pn15 ? C15_F * q3 : 0.0);
+    am = q2 * (double)cbrtf((float)(gq * gq));                       // (1 + cf q^2 [+ c15 q^3])^(2/3) ~ 1.0x: fp32 cube root, 1e-7 relative
+    s1 = 0.25 + (2.0 / 3.0) * (0.25 * tm.cf * q2 + (pn15 ? 0.375 * C15_F * q3 : 0.0)) / gq;
   }
   am *= (double)ascale;
   const double a1 = am * s1 * eps, a2 = a1 * (0.5 * (s1 + 1.0)) * eps, a3 = a2 * ((s1 + 2.0) * (1.0 / 3.0)) * eps;
@@ -1695,6 +1713,42 @@ __global__ void sft_fstat_kernel(long long n, const double *sums, double *twoF, 
   if (twoF) twoF[t] = D > 0.0 ? (B * (x0 * x0 + x2 * x2) + A * (x1 * x1 + x3 * x3) - 2.0 * C * (x0 * x1 + x2 * x3)) / D : 0.0;
   if (xnu) { xnu[t] = x0; xnu[n + t] = x1; xnu[2 * n + t] = x2; xnu[3 * n + t] = x3; }
   if (mnu) { mnu[t] = A; mnu[n + t] = B; mnu[2 * n + t] = C; }
+}
+
+// Validity of the per-SFT signal model, Eq.(33)-(34) P:244-248: the quadratic phase model Eq.(17) holds over
+// one SFT while 1/2 T^2 max fddot <= delta df, i.e. delta_eff = 1/2 T^3 fddot <= delta.  fddot grows monotonically along an
+// inspiral, so the largest value over a template's active SFTs (DESIGN A12) is the one of its LAST active SFT: the upper
+// conditions (t_a + T < t_c, f_a + fdot_a T <= f_hi) hold up to some SFT index found by bisection, the lower one (f_lo <= f_a)
+// from some index on.  One thread per template; pow() is fine here (once per template and bisection step).
+__global__ void sft_validity_kernel(const KParams p, double delta_max, double *delta_eff, unsigned char *flags) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= p.nT) return;
+  const double *row = p.params + t * 8;
+  const double mc = row[0], eta = row[1], tau0 = row[2] - p.t0;
+  const double M = mc * pow(eta, -0.6) * GMSUN_S;
+  const double k = eta / (5.0 * M), F0 = 1.0 / (8.0 * 3.141592653589793 * M);
+  const double cf = p.pn1 >= 1 ? (743.0 / 2688.0 + 11.0 / 32.0 * eta) : 0.0, c15 = p.pn1 >= 2 ? C15_F : 0.0;
+  auto eval = [&](int a, double &fT, double &b, double &fdd) {
+    const double tau = tau0 - (double)a * p.T;
+    const double q = pow(k * tau, -0.125), q2 = q * q, q3 = q2 * q, q8 = q2 * q2 * q2 * q2;
+    fT = F0 * p.T * q3 * (1.0 + cf * q2 + c15 * q3);
+    b = F0 * k * p.T * p.T * (q8 * q3) * (0.375 + 0.625 * cf * q2 + 0.75 * c15 * q3);
+    fdd = F0 * k * k * (q8 * q8 * q3) * (0.375 * 1.375 + 0.625 * 1.625 * cf * q2 + 0.75 * 1.75 * c15 * q3);
+    return tau > p.T && fT + b <= p.f_hiT;                 // (NaN for tau <= 0 fails)
+  };
+  double fT, b, fdd, de = 0.0;
+  if (eval(0, fT, b, fdd)) {
+    int lo = 0, hi = p.n_sft - 1;                          // invariant: upper conditions hold at lo
+    if (eval(hi, fT, b, fdd)) lo = hi;
+    while (hi - lo > 1) {
+      const int mid = lo + (hi - lo) / 2;
+      if (eval(mid, fT, b, fdd)) lo = mid; else hi = mid;
+    }
+    eval(lo, fT, b, fdd);
+    if (fT >= p.f_loT) de = 0.5 * p.T * p.T * p.T * fdd;
+  }
+  if (delta_eff) delta_eff[t] = de;
+  if (flags) flags[t] = de > delta_max ? 1 : 0;
 }
 
 // Statistics on top of the inner products: log-likelihood L = <x,h> - <h,h>/2 (Eq.(2)) and the

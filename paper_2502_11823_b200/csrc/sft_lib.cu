@@ -109,7 +109,7 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   if (d.k_lo < 0 || d.k_hi <= d.k_lo) return fail(nullptr, SFT_ESHAPE, "stored band [k_lo=%d, k_hi=%d) is empty or negative", d.k_lo, d.k_hi);
   if (d.K < 0 || d.K > SFT_MAX_K) return fail(nullptr, SFT_EINVAL, "K=%d outside 0..%d", d.K, SFT_MAX_K);
   if (d.kernel != SFT_KERNEL_DIRICHLET && d.kernel != SFT_KERNEL_FRESNEL) return fail(nullptr, SFT_EINVAL, "unknown kernel %d", d.kernel);
-  if (d.waveform != SFT_WF_PN0 && d.waveform != SFT_WF_PN1) return fail(nullptr, SFT_EINVAL, "unknown waveform %d", d.waveform);
+  if (d.waveform < SFT_WF_PN0 || d.waveform > SFT_WF_PN15) return fail(nullptr, SFT_EINVAL, "unknown waveform %d", d.waveform);
   if (d.phase_path != SFT_PHASE_FP64 && d.phase_path != SFT_PHASE_SPLIT32) return fail(nullptr, SFT_EINVAL, "unknown phase_path %d", d.phase_path);
   if (d.response < SFT_RESP_NONE || d.response > SFT_RESP_ANNUAL) return fail(nullptr, SFT_EINVAL, "unknown response %d", d.response);
   if (!(d.f_ref > 0.0)) return fail(nullptr, SFT_EINVAL, "f_ref must be > 0");
@@ -257,17 +257,19 @@ SFT_API sft_status sft_tsft_rule(double m_chirp, double eta, int32_t waveform, d
   if (!t_sft) return fail(nullptr, SFT_EINVAL, "sft_tsft_rule: t_sft is NULL");
   if (!(m_chirp > 0.0) || !(eta > 0.0) || !(eta <= 0.25) || !(f_max > 0.0) || !(delta > 0.0))
     return fail(nullptr, SFT_EINVAL, "sft_tsft_rule: need m_chirp, f_max, delta > 0 and 0 < eta <= 1/4");
-  if (waveform != SFT_WF_PN0 && waveform != SFT_WF_PN1) return fail(nullptr, SFT_EINVAL, "unknown waveform %d", waveform);
+  if (waveform < SFT_WF_PN0 || waveform > SFT_WF_PN15) return fail(nullptr, SFT_EINVAL, "unknown waveform %d", waveform);
   const double PI = 3.141592653589793;
   const double M = m_chirp * pow(eta, -0.6) * sftk::GMSUN_S;
-  const double cf = waveform == SFT_WF_PN1 ? 743.0 / 2688.0 + 11.0 / 32.0 * eta : 0.0;
+  const double cf = waveform >= SFT_WF_PN1 ? 743.0 / 2688.0 + 11.0 / 32.0 * eta : 0.0;
+  const double c15 = waveform >= SFT_WF_PN15 ? sftk::C15_F : 0.0;
   // Theta at which f(Theta) = Theta^(-3/8) (1 + cf Theta^(-1/4)) / (8 pi M) reaches f_max: f falls monotonically with Theta;
   // start from the 0PN root (where the 1PN f is higher, i.e. the root lies at larger Theta) and use Newton's method in
-  // u = Theta^(-1/8):  g(u) = u^3 (1 + cf u^2) - 8 pi M f_max
+  // u = Theta^(-1/8):  g(u) = u^3 (1 + cf u^2 + c15 u^3) - 8 pi M f_max
   const double target = 8.0 * PI * M * f_max;
   double u = cbrt(target);
   for (int it = 0; it < 60; ++it) {
-    const double g = u * u * u * (1.0 + cf * u * u) - target, dg = 3.0 * u * u + 5.0 * cf * u * u * u * u;
+    const double u2 = u * u, u3 = u2 * u;
+    const double g = u3 * (1.0 + cf * u2 + c15 * u3) - target, dg = 3.0 * u2 + 5.0 * cf * u2 * u2 + 6.0 * c15 * u2 * u3;
     const double un = u - g / dg;
     if (fabs(un - u) <= 1e-15 * fabs(u)) { u = un; break; }
     u = un;
@@ -276,7 +278,7 @@ SFT_API sft_status sft_tsft_rule(double m_chirp, double eta, int32_t waveform, d
   // d^2 f / dt^2 = k^2/(8 pi M) [ (3/8)(11/8) Theta^(-19/8) + (5/8)(13/8) cf Theta^(-21/8) ],  k = eta/(5M), Theta^(-1/8) = u
   const double k = eta / (5.0 * M);
   const double u19 = pow(u, 19.0), u21 = u19 * u * u;
-  const double fdd = k * k / (8.0 * PI * M) * (0.375 * 1.375 * u19 + 0.625 * 1.625 * cf * u21);
+  const double fdd = k * k / (8.0 * PI * M) * (0.375 * 1.375 * u19 + 0.625 * 1.625 * cf * u21 + 0.75 * 1.75 * c15 * u21 * u);
   if (fddot_max) *fddot_max = fdd;
   *t_sft = cbrt(2.0 * delta / fdd);
   return SFT_OK;
@@ -521,7 +523,7 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.cstrideD = (unsigned)(p->d.n_channels * p->d.n_sft * p->npair);
   k.cstrideU = (unsigned)(p->d.n_channels * p->npair);
   k.kernel = p->d.kernel;
-  k.pn1 = p->d.waveform == SFT_WF_PN1;
+  k.pn1 = p->d.waveform;                          // PN order code: 0, 1 (1PN), 2 (1.5PN)
   k.response = p->d.response;
   k.phase_path = p->d.phase_path;
   k.T = p->d.t_sft;
@@ -766,6 +768,53 @@ SFT_API sft_status sft_statistics(sft_plan *p, int64_t nT, const double *xh, con
     if (loglike) CU(p, cudaMemcpyAsync(loglike, d_l, b, cudaMemcpyDeviceToHost, p->stream));
     if (rho2_phase_max) CU(p, cudaMemcpyAsync(rho2_phase_max, d_r, b, cudaMemcpyDeviceToHost, p->stream));
     CU(p, cudaStreamSynchronize(p->stream));
+  }
+  return SFT_OK;
+}
+
+// Validity flags of Eq.(33)-(34) P:244-248 per template (no data needed).
+SFT_API sft_status sft_validity(sft_plan *p, int64_t nT, const double *params, double delta_max, double *delta_eff,
+                                uint8_t *flags, int32_t mem) {
+  if (!p) return SFT_EINVAL;
+  p->err[0] = 0;
+  if (nT < 0) return fail(p, SFT_EINVAL, "n_templates < 0");
+  if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(p, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
+  if (nT == 0) return SFT_OK;
+  if (!params) return fail(p, SFT_EINVAL, "params is required");
+  if (!delta_eff && !flags) return fail(p, SFT_EINVAL, "at least one of delta_eff, flags must be non-NULL");
+  if (!(delta_max >= 0.0)) return fail(p, SFT_EINVAL, "delta_max must be >= 0");
+  if (nT > (1ll << 31) - 1) return fail(p, SFT_EINVAL, "n_templates too large");
+  CU(p, cudaSetDevice(p->d.device));
+  KParams k;
+  fill_kparams(p, k);
+  k.nT = nT;
+  double *d_de = delta_eff;
+  unsigned char *d_fl = flags;
+  const size_t b_de = (size_t)nT * sizeof(double), b_par = (size_t)nT * SFT_NPARAM * sizeof(double);
+  sft_status st;
+  if (mem == SFT_MEM_HOST) {
+    st = grow(p, (void **)&p->d_params, &p->params_bytes, b_par);
+    if (st != SFT_OK) return st;
+    st = grow(p, &p->d_out, &p->out_bytes, b_de + (size_t)nT + 256);
+    if (st != SFT_OK) return st;
+    CU(p, cudaMemcpyAsync(p->d_params, params, b_par, cudaMemcpyHostToDevice, p->stream));
+    k.params = p->d_params;
+    d_de = (double *)p->d_out;
+    d_fl = (unsigned char *)p->d_out + b_de;
+  } else {
+    k.params = params;
+  }
+  sftk::sft_validity_kernel<<<(unsigned)((nT + 127) / 128), 128, 0, p->stream>>>(k, delta_max, d_de, d_fl);
+  p->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "validity kernel launch: %s", cudaGetErrorString(e));
+  if (mem == SFT_MEM_HOST) {
+    st = grow_pinned(p, b_de + (size_t)nT);
+    if (st != SFT_OK) return st;
+    CU(p, cudaMemcpyAsync(p->h_pin, d_de, b_de + (size_t)nT, cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
+    if (delta_eff) memcpy(delta_eff, p->h_pin, b_de);
+    if (flags) memcpy(flags, (char *)p->h_pin + b_de, (size_t)nT);
   }
   return SFT_OK;
 }

@@ -25,17 +25,21 @@ NPARAM = 8
 # the signal that is put into the data: a continuously sampled PN inspiral strain
 # --------------------------------------------------------------------------------------------
 def _pn_coeffs(eta, pn1):
-    return pn1 * (3715.0 / 8064.0 + 55.0 / 96.0 * eta), pn1 * (743.0 / 2688.0 + 11.0 / 32.0 * eta)
+    """1PN coefficients (pn1 >= 1) of phase and frequency, and the 1.5PN tail coefficients (pn1 >= 2)."""
+    p1, p15 = float(pn1 >= 1), float(pn1 >= 2)
+    return (p1 * (3715.0 / 8064.0 + 55.0 / 96.0 * eta), p1 * (743.0 / 2688.0 + 11.0 / 32.0 * eta),
+            -0.75 * np.pi * p15, -0.3 * np.pi * p15)
 
 
 def inspiral_phase_freq(t, m_chirp, eta, t_c, phi_c, pn1):
     """phi(t) [rad] and f(t) [Hz] of the injected inspiral at sample times t < t_c."""
     M = m_chirp * eta ** (-0.6) * GMSUN_S
-    cphi, cf = _pn_coeffs(eta, pn1)
+    cphi, cf, tphi, tf = _pn_coeffs(eta, pn1)
     L = np.log(eta * (t_c - t) / (5.0 * M))
     q = np.exp(-0.25 * L)
-    phi = phi_c - (2.0 / eta) * np.exp(0.625 * L) * (1.0 + cphi * q)
-    f = np.exp(-0.375 * L) / (8.0 * np.pi * M) * (1.0 + cf * q)
+    q15 = np.exp(-0.375 * L)
+    phi = phi_c - (2.0 / eta) * np.exp(0.625 * L) * (1.0 + cphi * q + tphi * q15)
+    f = q15 / (8.0 * np.pi * M) * (1.0 + cf * q + tf * q15)
     return phi, f
 
 

@@ -299,6 +299,40 @@ def test_fstat_matches_oracle(n_channels, noise):
         assert np.abs(c - w.notes["c_nu"]).max() < 0.02
 
 
+def test_validity_flags(et_small):
+    """sft_validity (NEXT-2; Eq.(33)-(34) P:244-248) against its oracle twin on a wide bank (ended, never-active and full-span
+    templates), for all three PN orders; device and host buffers."""
+    import torch
+    api = _api()
+    w = wl.et_bns_wide_bank(et_small, 300)
+    for pn in (0, 1, 2):
+        o, xx, plan_o, store = _oracle(w, pn1=pn)
+        d_o = oin.validity(plan_o, w.params)
+        with api.Plan(dict(w.desc, pn1=pn)) as plan:                       # no data loaded: not needed
+            d, fl = np.full(300, np.nan), np.full(300, 9, np.uint8)
+            plan.validity(np.ascontiguousarray(w.params), 0.25, d, fl)
+            Pd = torch.from_numpy(np.ascontiguousarray(w.params)).cuda()
+            dd = torch.full((300,), float("nan"), dtype=torch.float64, device="cuda")
+            plan.validity(Pd, 0.25, dd, None)
+            plan.sync()
+        assert np.allclose(d, d_o, rtol=1e-9, atol=0.0) and np.array_equal(dd.cpu().numpy(), d)
+        assert np.array_equal(fl, (d_o > 0.25).astype(np.uint8)) and 0 < fl.sum() < 300
+
+
+def test_pn15_waveform(et_small):
+    """SFT_WF_PN15 (NEXT-2): the 1.5PN tail terms in the closed-form track, the polynomial track of the clean blocks and the
+    double-float track, against the oracle; k_c bit-exact.  The data hold a 1PN signal: the templates need not match it."""
+    w = et_small
+    P = w.params[:96]
+    o, xx, _, _ = _oracle(w, params=P, pn1=2)
+    assert np.abs(o["xh"] - _oracle(w, params=P)[0]["xh"]).max() > 1.0          # the tail terms matter
+    _check(w, _run_gpu(w, params=P, pn1=2), o, xx)
+    _check(w, _run_gpu(w, params=P, pn1=2, phase_path="split32"), o, xx)
+    ww = wl.et_bns_wide_bank(w, 64)
+    o2, xx2, _, _ = _oracle(ww, pn1=2)
+    _check(ww, _run_gpu(ww, pn1=2), o2, xx2)
+
+
 def test_response_table():
     """SFT_RESP_TABLE: an arbitrary complex per-(channel, SFT) response."""
     w = wl.config4(n_templates=40)

@@ -358,3 +358,34 @@ def test_xx_band_is_the_plain_product_of_the_data_with_itself():
     p0.k_lo, p0.k_hi = 0, 3
     s0 = oin.Store(bins=np.ones((1, plan.n_sft, 3), complex), psd_scale=store.psd_scale, psd_shape=np.ones((1, 3)))
     assert abs(oin.xx_band(p0, s0) - 4.0 / T * plan.n_sft * 2) < 1e-9                   # k = 0 excluded, k = 1, 2 counted
+
+
+def test_validity_delta_eff_closed_form_and_paper_table():
+    """oracle.inner.validity (Eq.(33)-(34) P:244-248).  (i) 0PN closed form: fddot = (11/3) fdot^2 / f with
+    fdot = (96/5) pi^(8/3) Mc^(5/3) f^(11/3), evaluated at the last active SFT; with T_SFT = 8 s and Mc = 1.2 Msun
+    delta_eff reaches 1 at ~28.7 Hz.  (ii) the paper's Table I: the BNS example analysed with the SFT length of
+    delta = 1 (73 s) has delta_eff ~ 1; a template with no active SFT has 0."""
+    from oracle import waveform as wf
+    mc = 1.2
+    plan = oin.Plan(n_channels=1, n_sft=256, t_sft=8.0, fs=512.0, t0=0.0, k_lo=40, k_hi=400, K=4, kernel="fresnel", pn1=0,
+                    f_lo=5.0, f_hi=1e3, f_ref=20.0)
+    tau_end = float(wf.tau_newtonian(28.7, mc))                      # f = 28.7 Hz at the start of the last SFT
+    P = np.zeros((2, 8))
+    P[0, :5] = [mc, 0.25, 255 * 8.0 + tau_end, 0.0, 1.0]
+    P[1, :5] = [mc, 0.25, -5.0, 0.0, 1.0]                            # ended before the data: never active
+    d = oin.validity(plan, P)
+    f = 28.7
+    fdot = 96.0 / 5.0 * np.pi ** (8.0 / 3.0) * (mc * wf.GMSUN_S) ** (5.0 / 3.0) * f ** (11.0 / 3.0)
+    assert d[0] == pytest.approx(0.5 * 8.0 ** 3 * (11.0 / 3.0) * fdot ** 2 / f, rel=2e-3)
+    assert abs(d[0] - 1.0) < 0.03 and d[1] == 0.0
+    eta, mcb = 0.25, 2.8 * 0.25 ** 0.6
+    for pn in (0, 1, 2):
+        tau10 = wl.tau_for_frequency(10.0, mcb, eta, pn)
+        T = float(wf.t_sft_rule(1.0, wf.taylor_t3_fddot(mcb, eta, tau10, 0.0, pn)))
+        assert abs(T - 73.0) < 2.5                                    # Table I, delta = 1
+        planb = oin.Plan(n_channels=1, n_sft=100, t_sft=T, fs=40.0, t0=0.0, k_lo=0, k_hi=800, K=4, kernel="fresnel", pn1=pn,
+                         f_lo=0.0, f_hi=1e3, f_ref=10.0)
+        Pb = np.zeros((1, 8))
+        Pb[0, :5] = [mcb, eta, 100 * T + tau10, 0.0, 1.0]            # 10 Hz at the end of the last SFT
+        db = oin.validity(planb, Pb)[0]
+        assert 0.8 < db < 1.0                                         # fddot at the START of the last SFT: somewhat below 1

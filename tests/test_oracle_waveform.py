@@ -8,7 +8,7 @@ from oracle import waveform as wf
 GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.json")))
 
 
-@pytest.mark.parametrize("pn1", [0, 1])
+@pytest.mark.parametrize("pn1", [0, 1, 2])
 @pytest.mark.parametrize("mc,eta,tau", [(1.2188, 0.25, 5000.0), (1.2188, 0.25, 200.0), (4.06e5, 0.2222, 1e6), (30.0, 0.2, 50.0)])
 def test_P6_derivative_consistency(pn1, mc, eta, tau):
     """dphi/dt = 2 pi f, df/dt = fdot, d2f/dt2 = fddot by central differences (f = phi-dot)."""
@@ -48,6 +48,25 @@ def test_P6_1pn_chirp_time_textbook():
     (r1, x1), (r2, x2) = res
     assert abs(r1) < 20 * x1 ** 2 and abs(r2) < 20 * x2 ** 2
     assert abs(np.log(abs(r2 / r1)) / np.log(x2 / x1) - 2.0) < 0.15   # residual ~ x^2 = (pi M f)^(4/3)
+
+
+def test_P6_15pn_chirp_time_textbook():
+    """1.5PN (order code 2): t_c - t(f) = tau0 [1 + (4/3)(743/336 + 11 eta/4) x - (32 pi/5) x^(3/2)] + O(x^2), x = (pi M f)^(2/3)
+    (the textbook chirp times tau0 + tau1 - tau1.5): pins the sign and size of the tail terms; the residual scales as x^2."""
+    mc, eta = 1.2188, 0.25
+    M = wf.total_mass_seconds(mc, eta)
+    res = []
+    for tau in (1e5, 1e3):
+        _, f, _ = wf.taylor_t3(mc, eta, tau, 0.0, 0.0, 2)
+        x = (np.pi * M * f) ** (2.0 / 3.0)
+        pred = wf.tau_newtonian(f, mc) * (1 + 4.0 / 3.0 * (743.0 / 336.0 + 11.0 * eta / 4.0) * x - 32.0 * np.pi / 5.0 * x ** 1.5)
+        res.append((pred / tau - 1, x))
+        # without the tail term the mismatch is of order x^(3/2), far above the residual
+        _, f1, _ = wf.taylor_t3(mc, eta, tau, 0.0, 0.0, 1)
+        assert abs(f / f1 - 1) > 0.05 * x ** 1.5
+    (r1, x1), (r2, x2) = res
+    assert abs(r1) < 40 * x1 ** 2 and abs(r2) < 40 * x2 ** 2
+    assert abs(np.log(abs(r2 / r1)) / np.log(x2 / x1) - 2.0) < 0.25
 
 
 def test_P7_bns_printed_values():
