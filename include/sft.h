@@ -118,6 +118,15 @@ sft_status sft_load_data(sft_plan *plan, int32_t channel, const float *sft_bins,
                          const double *psd_scale, const double *psd_shape,
                          const float *response, int32_t mem);
 
+/* Streaming ("SFTs ... can be computed online and in parallel as data arrives", section V.A): replaces the SFT slots
+ * first_sft <= a < first_sft + n_new of a channel that sft_load_data has loaded before (typically with the slots still to come
+ * marked as gaps), in place: the rows of the whitened store and of the moment tables of these slots only.  The channel keeps the
+ * PSD shape S_c(f_k) of its sft_load_data call.
+ *   sft_bins   complex64 [n_new][k_hi-k_lo], psd_scale [n_new] (<= 0 or non-finite => gap), response complex64 [n_new] (iff
+ *   SFT_RESP_TABLE); `mem` as in sft_load_data.  SFT_ESHAPE if the slots do not fit the plan, SFT_ENODATA before sft_load_data. */
+sft_status sft_append_sfts(sft_plan *plan, int32_t channel, int64_t first_sft, int64_t n_new,
+                           const float *sft_bins, const double *psd_scale, const float *response, int32_t mem);
+
 /* Data SFTs from a time series (Eq.(26), section V.A): for each of n_sft disjoint segments of n
  * samples (a trailing partial segment is ignored, DESIGN A13)
  *     bins[a][k - k_lo] = dt sum_{j<n} x[a n + j] exp(-2 pi i j k / n),   k_lo <= k < k_hi,
@@ -127,9 +136,22 @@ sft_status sft_load_data(sft_plan *plan, int32_t channel, const float *sft_bins,
 sft_status sft_compute_sfts(int32_t device, void *stream, const double *x, int64_t n_sft, int32_t n,
                             double dt, int32_t k_lo, int32_t k_hi, float *bins, int32_t mem);
 
+/* Per-SFT noise level from the data themselves ("whitening data on a per-SFT basis"): with S_a(f_k) = s_a S(f_k)
+ * (DESIGN A9) and Gaussian noise, |x~_{a,k}|^2 / (S(f_k) T_SFT / 2) is s_a times a unit exponential variate (median ln 2), so
+ *     psd_scale[a] = median{ |x~_{a',k}|^2 / (S(f_k) T_SFT/2) : |a' - a| <= half_window, a' not a gap, 1 <= k <= n_samp/2 - 1 } / ln 2
+ * - a median over the band (and 2 half_window + 1 neighbouring SFTs), insensitive to a narrow signal crossing it.  An SFT whose
+ * bins are all exactly zero is a gap: psd_scale = 0, and it does not enter its neighbours' pools.
+ *   sft_bins complex64 [n_sft][k_hi-k_lo]; psd_shape [k_hi-k_lo] or NULL (= 1); psd_scale [n_sft] out; `mem` for all three.
+ * No plan needed; blocks until done.  At most 8192 pooled values per SFT (SFT_EUNSUPPORTED beyond). */
+sft_status sft_estimate_psd_scale(int32_t device, void *stream, const float *sft_bins, int64_t n_sft, int32_t k_lo,
+                                  int32_t k_hi, int32_t n_samp, double t_sft, const double *psd_shape,
+                                  int32_t half_window, double *psd_scale, int32_t mem);
+
 /* sft_compute_sfts + sft_load_data in one call: channel `channel` of the plan from its strain time series
  * x[n_samples] (n_samples >= n_sft * t_sft * fs; sample j of SFT a is x[a n + j], t = t0 + (a n + j)/fs).
- * The SFT bins never leave the device.  Noise description and `mem` as in sft_load_data. */
+ * The SFT bins never leave the device.  Noise description and `mem` as in sft_load_data, except that psd_scale may be NULL:
+ * the per-SFT noise levels are then estimated from the data (sft_estimate_psd_scale with half_window = 0) and segments whose
+ * samples are all zero become gaps. */
 sft_status sft_ingest_timeseries(sft_plan *plan, int32_t channel, const double *x, int64_t n_samples,
                                  const double *psd_scale, const double *psd_shape,
                                  const float *response, int32_t mem);

@@ -52,3 +52,26 @@ def full_band_product(xs, hs, S, df, ks, n, half_weight_edges=False):
     if half_weight_edges:
         w = np.where((ks == 0) | (ks == n // 2), 0.5, w)
     return 4.0 * df * float(np.sum(w * np.real(np.conj(xs) * hs) / S))
+
+
+def psd_scale_estimate(bins, psd_shape, t_sft, k_lo, n_samp, half_window=0):
+    """Per-SFT noise level from the data ("whitening data on a per-SFT basis"): with ``S_a(f_k) = s_a S(f_k)`` and
+    Gaussian noise ``|x~_{a,k}|^2 / (S(f_k) T/2)`` is ``s_a`` times a unit exponential variate, whose median is ln 2, so
+    ``s^_a = median{...} / ln 2`` over the valid bins ``1 <= k <= n/2 - 1`` of the SFTs ``|a' - a| <= half_window`` that are not
+    gaps (a gap = all bins exactly zero; its own estimate is 0).  Plain numpy.  Pin: tests/test_oracle_sft.py (recovers the
+    lognormal scales of the config-2 recipe without bias; scaling law; gaps)."""
+    bins = np.asarray(bins)
+    n_sft, nb = bins.shape
+    S = np.ones(nb) if psd_shape is None else np.asarray(psd_shape, np.float64)
+    k = k_lo + np.arange(nb)
+    valid = (k >= 1) & (k <= n_samp // 2 - 1)
+    v = (bins.real.astype(np.float64) ** 2 + bins.imag.astype(np.float64) ** 2) / (S * 0.5 * t_sft)
+    present = np.any(bins != 0, axis=1)
+    out = np.zeros(n_sft)
+    for a in range(n_sft):
+        if not present[a]:
+            continue
+        rows = [b for b in range(max(0, a - half_window), min(n_sft - 1, a + half_window) + 1) if present[b]]
+        pool = v[rows][:, valid].ravel()
+        out[a] = np.median(pool) / np.log(2.0) if pool.size else 0.0
+    return out

@@ -46,7 +46,7 @@ class PlanDesc(C.Structure):
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
            "sft_plan_set_chunk", "sft_plan_path_counts", "sft_compute_sfts", "sft_ingest_timeseries",
-           "sft_tsft_rule", "sft_statistics", "sft_fstat", "sft_validity", "sft_last_error", "sft_version",
+           "sft_tsft_rule", "sft_statistics", "sft_fstat", "sft_validity", "sft_append_sfts", "sft_estimate_psd_scale", "sft_last_error", "sft_version",
            "sft_measure_alu_peaks"]
 
 _lib = None
@@ -80,6 +80,10 @@ def load_library(path=None):
     lib.sft_fstat.restype = i32
     lib.sft_validity.argtypes = [vp, i64, vp, dbl, vp, vp, i32]
     lib.sft_validity.restype = i32
+    lib.sft_append_sfts.argtypes = [vp, i32, i64, i64, vp, vp, vp, i32]
+    lib.sft_append_sfts.restype = i32
+    lib.sft_estimate_psd_scale.argtypes = [i32, vp, vp, i64, i32, i32, i32, dbl, vp, i32, vp, i32]
+    lib.sft_estimate_psd_scale.restype = i32
     lib.sft_tsft_rule.argtypes = [dbl, dbl, i32, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
     lib.sft_tsft_rule.restype = i32
     lib.sft_compute_sfts.argtypes = [i32, vp, vp, i64, i32, dbl, i32, i32, vp, i32]
@@ -204,7 +208,15 @@ class Plan:
             _ptr(psd_shape, np.float64, (self.nb,), "psd_shape"),
             _ptr(response, np.complex64, (self.n_sft,), "response"), mem))
 
-    def ingest_timeseries(self, channel, x, psd_scale, psd_shape=None, response=None):
+    def append_sfts(self, channel, first_sft, sft_bins, psd_scale, response=None):
+        """``sft_append_sfts``: replaces slots [first_sft, first_sft + n_new) of a loaded channel in place."""
+        n_new = int(sft_bins.shape[0])
+        mem = _where([sft_bins, psd_scale, response])
+        self._check(self.lib.sft_append_sfts(
+            self._h, int(channel), int(first_sft), n_new, _ptr(sft_bins, np.complex64, (n_new, self.nb), "sft_bins"),
+            _ptr(psd_scale, np.float64, (n_new,), "psd_scale"), _ptr(response, np.complex64, (n_new,), "response"), mem))
+
+    def ingest_timeseries(self, channel, x, psd_scale=None, psd_shape=None, response=None):
         """``sft_ingest_timeseries``: float64 strain series [>= n_sft * n] instead of precomputed SFT bins."""
         mem = _where([x, psd_scale, psd_shape, response])
         ns = int(x.shape[0])
@@ -312,6 +324,26 @@ def compute_sfts(x, n_sft, n, dt, k_lo, k_hi, bins, device=0, stream=None):
                               _ptr(bins, np.complex64, (int(n_sft), int(k_hi) - int(k_lo)), "bins"), mem)
     if st != 0:
         raise SftError(st, lib.sft_last_error(None).decode())
+
+
+def estimate_psd_scale(sft_bins, k_lo, n_samp, t_sft, psd_shape=None, half_window=0, out=None, device=0, stream=None):
+    """``sft_estimate_psd_scale``: per-SFT noise level [n_sft] (float64) from complex64 ``sft_bins`` [n_sft][nb]."""
+    lib = load_library()
+    n_sft, nb = int(sft_bins.shape[0]), int(sft_bins.shape[1])
+    if out is None:
+        if _is_torch(sft_bins):
+            import torch
+            out = torch.empty(n_sft, dtype=torch.float64, device=sft_bins.device)
+        else:
+            out = np.empty(n_sft, dtype=np.float64)
+    mem = _where([sft_bins, psd_shape, out])
+    st = lib.sft_estimate_psd_scale(int(device), C.c_void_p(int(stream)) if stream else None,
+                                    _ptr(sft_bins, np.complex64, (n_sft, nb), "sft_bins"), n_sft, int(k_lo), int(k_lo) + nb,
+                                    int(n_samp), float(t_sft), _ptr(psd_shape, np.float64, (nb,), "psd_shape"), int(half_window),
+                                    _ptr(out, np.float64, (n_sft,), "psd_scale"), mem)
+    if st != 0:
+        raise SftError(st, lib.sft_last_error(None).decode())
+    return out
 
 
 def measure_alu_peaks(device=0):

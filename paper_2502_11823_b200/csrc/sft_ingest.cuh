@@ -171,4 +171,74 @@ __global__ void __launch_bounds__(256) sft_dft_band_kernel(const double *x, int 
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Per-SFT noise level from the data themselves ("whitening data on a per-SFT basis").  With the
+// separable noise model S_a(f_k) = s_a S(f_k) (DESIGN A9) and Gaussian noise, |x~_{a,k}|^2 / (S(f_k) T/2) is s_a times a unit
+// exponential variate, whose median is ln 2:
+//   s^_a = median{ |x~_{a',k}|^2 / (S(f_k) T/2) : |a' - a| <= w, a' not a gap, k valid } / ln 2.
+// The median over the band (and over 2w+1 neighbouring SFTs) is insensitive to a narrow-band signal crossing it.  An SFT whose
+// bins are all exactly zero is a gap (s^ = 0) and does not enter its neighbours' pools.
+constexpr int PSD_MAX_VALUES = 8192;
+
+__global__ void sft_nonzero_kernel(const float2 *bins, int nb, unsigned char *flag) {
+  __shared__ int any;
+  if (threadIdx.x == 0) any = 0;
+  __syncthreads();
+  const float2 *row = bins + (size_t)blockIdx.x * nb;
+  int a = 0;
+  for (int q = threadIdx.x; q < nb; q += blockDim.x) a |= (row[q].x != 0.f) | (row[q].y != 0.f);
+  if (a) any = 1;
+  __syncthreads();
+  if (threadIdx.x == 0) flag[blockIdx.x] = (unsigned char)any;
+}
+
+// One block per SFT; npow2 = the power of two >= the largest pool size (<= PSD_MAX_VALUES); bitonic sort in shared memory.
+__global__ void __launch_bounds__(256) sft_psd_scale_kernel(const float2 *bins, const unsigned char *flag, const double *shape,
+                                                            int n_sft, int nb, int k_lo, int n_samp, double half_T, int w, int npow2,
+                                                            double *scale) {
+  extern __shared__ float vals[];
+  __shared__ int count;
+  const int a = blockIdx.x;
+  if (!flag[a]) {
+    if (threadIdx.x == 0) scale[a] = 0.0;
+    return;
+  }
+  if (threadIdx.x == 0) count = 0;
+  __syncthreads();
+  const int q0 = max(0, 1 - k_lo), q1 = min(nb, n_samp / 2 - k_lo);        // valid bins 1 <= k <= n/2 - 1
+  const int nv = max(0, q1 - q0);
+  int slot = 0;                                                            // pool layout: [present neighbour][valid bin]
+  for (int b = max(0, a - w); b <= min(n_sft - 1, a + w); ++b) {
+    if (!flag[b]) continue;
+    const float2 *row = bins + (size_t)b * nb;
+    for (int q = threadIdx.x; q < nv; q += blockDim.x) {
+      const float2 v = row[q0 + q];
+      const double Sk = shape ? shape[q0 + q] : 1.0;
+      vals[slot * nv + q] = (float)(((double)v.x * (double)v.x + (double)v.y * (double)v.y) / (Sk * half_T));
+    }
+    ++slot;
+  }
+  const int cnt = slot * nv;
+  for (int i = cnt + threadIdx.x; i < npow2; i += blockDim.x) vals[i] = __int_as_float(0x7f800000);   // +inf padding
+  __syncthreads();
+  for (int k = 2; k <= npow2; k <<= 1) {
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int i = threadIdx.x; i < npow2; i += blockDim.x) {
+        const int l = i ^ j;
+        if (l > i) {
+          const float x = vals[i], y = vals[l];
+          const bool up = (i & k) == 0;
+          if ((x > y) == up) { vals[i] = y; vals[l] = x; }
+        }
+      }
+      __syncthreads();
+    }
+  }
+  if (threadIdx.x == 0) {
+    double med = 0.0;
+    if (cnt > 0) med = (cnt & 1) ? (double)vals[cnt / 2] : 0.5 * ((double)vals[cnt / 2 - 1] + (double)vals[cnt / 2]);
+    scale[a] = med / 0.6931471805599453;
+  }
+}
+
 }  // namespace sftk

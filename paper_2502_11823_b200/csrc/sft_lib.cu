@@ -31,6 +31,9 @@ struct sft_plan {
   float *us2 = nullptr;   // [C][n_sft]
   float2 *rtab = nullptr; // [C][n_sft]
   double sigma[SFT_MAX_CHANNELS] = {0, 0, 0, 0};
+  double s_ref[SFT_MAX_CHANNELS] = {1, 1, 1, 1};       // reference PSD level of the channel's shape (sft_load_data)
+  double *shape_dev = nullptr;                         // [C][nb] device copy of the PSD shapes (sft_append_sfts reuses them)
+  bool has_shape[SFT_MAX_CHANNELS] = {false, false, false, false};
   bool loaded[SFT_MAX_CHANNELS] = {false, false, false, false};
   // scratch, grown on demand
   double *part = nullptr; size_t part_bytes = 0;
@@ -150,6 +153,7 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   alloc((void **)&p->ubp, 2 * C * npair * sizeof(float2));
   alloc((void **)&p->us2, C * N * sizeof(float));
   alloc((void **)&p->rtab, C * N * sizeof(float2));
+  alloc((void **)&p->shape_dev, C * (size_t)p->nb * sizeof(double));
   // moment tables (sft_table.cuh): 64 bytes per node, TAB_R nodes per window position and SFT.  AUTO takes
   // them when they fit in a quarter of the free device memory, TABLE insists, DIRECT never builds them.
   p->n_kc = p->nb + 2 * d.K;
@@ -210,7 +214,7 @@ SFT_API sft_status sft_plan_destroy(sft_plan *p) {
   if (!p) return SFT_OK;
   cudaSetDevice(p->d.device);
   cudaStreamSynchronize(p->stream);
-  cudaFree(p->Dp); cudaFree(p->ubp); cudaFree(p->us2); cudaFree(p->rtab);
+  cudaFree(p->Dp); cudaFree(p->ubp); cudaFree(p->us2); cudaFree(p->rtab); cudaFree(p->shape_dev);
   cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->scan);
   if (p->h_pin) cudaFreeHost(p->h_pin);
   cudaFree(p->td); cudaFree(p->tf); cudaFree(p->counter); cudaFree(p->path_counts);
@@ -365,6 +369,7 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
         d_shape, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi, p->PAD, p->npair, S_ref, p->ubp + (size_t)channel * npair,
         p->ubp + (C + (size_t)channel) * npair);
     p->launches += 2;
+    if (d_shape) ok(cudaMemcpyAsync(p->shape_dev + (size_t)channel * nb, d_shape, nb * sizeof(double), cudaMemcpyDeviceToDevice, p->stream));
     if (p->mtab) {
       const size_t per_chan = N * (size_t)p->n_node * ((sftk::TAB_Q + 1) / 2);
       sftk::sft_mtab_kernel<<<(unsigned)(bpr * N), 256, 0, p->stream>>>(
@@ -381,7 +386,71 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "sft_load_data (copy/launch): %s", cudaGetErrorString(e));
   if (e2 != cudaSuccess) return fail(p, SFT_ECUDA, "sft_load_data: %s", cudaGetErrorString(e2));
   p->sigma[channel] = sqrt(p->d.t_sft / S_ref);
+  p->s_ref[channel] = S_ref;
+  p->has_shape[channel] = psd_shape != nullptr;
   p->loaded[channel] = true;
+  return SFT_OK;
+}
+
+// Streaming (section V.A: SFTs "can be computed online and in parallel as data arrives"): replaces the SFT slots
+// [first_sft, first_sft + n_new) of a loaded channel - whitening with the channel's PSD shape, the rows of the pair-planar
+// store and of the moment table - in place; nothing else of the plan is touched or rebuilt.
+SFT_API sft_status sft_append_sfts(sft_plan *p, int32_t channel, int64_t first_sft, int64_t n_new, const float *sft_bins,
+                                   const double *psd_scale, const float *response, int32_t mem) {
+  if (!p) return SFT_EINVAL;
+  p->err[0] = 0;
+  if (channel < 0 || channel >= p->d.n_channels) return fail(p, SFT_EINVAL, "channel %d outside 0..%d", channel, p->d.n_channels - 1);
+  if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(p, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
+  if (n_new < 0 || first_sft < 0 || first_sft + n_new > p->d.n_sft)
+    return fail(p, SFT_ESHAPE, "slots [%lld, %lld) outside the plan's %lld SFT slots", (long long)first_sft, (long long)(first_sft + n_new),
+                (long long)p->d.n_sft);
+  if (!p->loaded[channel]) return fail(p, SFT_ENODATA, "channel %d has no data yet: sft_load_data fixes its PSD shape first", channel);
+  if (n_new == 0) return SFT_OK;
+  if (!sft_bins || !psd_scale) return fail(p, SFT_EINVAL, "sft_bins and psd_scale are required");
+  if (p->d.response == SFT_RESP_TABLE && !response) return fail(p, SFT_EINVAL, "response table required by SFT_RESP_TABLE");
+  CU(p, cudaSetDevice(p->d.device));
+  const size_t N = p->d.n_sft, nb = p->nb, nn = (size_t)n_new, a0 = (size_t)first_sft, C = p->d.n_channels, npair = p->npair;
+  unsigned bpr = 0;
+  if (p->mtab) {
+    bpr = ((unsigned)p->n_node * (sftk::TAB_Q + 1) + 255) / 256;
+    if ((double)bpr * (double)nn > 2.0e9) return fail(p, SFT_EUNSUPPORTED, "moment-table build grid too large");
+  }
+  const float2 *d_raw = (const float2 *)sft_bins;
+  const double *d_scale = psd_scale;
+  void *tmp = nullptr;
+  cudaError_t e = cudaSuccess;
+  auto ok = [&](cudaError_t r) { if (e == cudaSuccess && r != cudaSuccess) e = r; return e == cudaSuccess; };
+  if (mem == SFT_MEM_HOST) {
+    const size_t b_raw = nn * nb * sizeof(float2), o_scale = (b_raw + 255) & ~size_t(255);
+    cudaError_t ea = cudaMalloc(&tmp, o_scale + nn * sizeof(double) + 256);
+    if (ea != cudaSuccess) return fail(p, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(ea));
+    ok(cudaMemcpyAsync(tmp, sft_bins, b_raw, cudaMemcpyHostToDevice, p->stream));
+    ok(cudaMemcpyAsync((char *)tmp + o_scale, psd_scale, nn * sizeof(double), cudaMemcpyHostToDevice, p->stream));
+    d_raw = (const float2 *)tmp;
+    d_scale = (const double *)((char *)tmp + o_scale);
+  }
+  if (p->d.response == SFT_RESP_TABLE)
+    ok(cudaMemcpyAsync(p->rtab + (size_t)channel * N + a0, response, nn * sizeof(float2),
+                       mem == SFT_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, p->stream));
+  if (e == cudaSuccess) {
+    const double *d_shape = p->has_shape[channel] ? p->shape_dev + (size_t)channel * nb : nullptr;
+    float4 *D0 = p->Dp + ((size_t)channel * N + a0) * npair, *D1 = p->Dp + ((C + (size_t)channel) * N + a0) * npair;
+    sftk::sft_whiten_kernel<<<(unsigned)nn, 128, 0, p->stream>>>(d_raw, d_scale, d_shape, (int)nn, (int)nb, p->d.k_lo, p->kv_lo, p->kv_hi,
+                                                                 p->PAD, p->npair, p->d.t_sft, p->s_ref[channel], D0, D1,
+                                                                 p->us2 + (size_t)channel * N + a0);
+    p->launches++;
+    if (p->mtab) {
+      const size_t per_chan = N * (size_t)p->n_node * ((sftk::TAB_Q + 1) / 2), per_row = (size_t)p->n_node * ((sftk::TAB_Q + 1) / 2);
+      sftk::sft_mtab_kernel<<<(unsigned)(bpr * nn), 256, 0, p->stream>>>(D0, p->npair, p->n_node, p->d.K, p->ptab, bpr,
+                                                                        (float2 *)(p->mtab + (size_t)channel * per_chan + a0 * per_row));
+      p->launches++;
+    }
+    ok(cudaGetLastError());
+  }
+  cudaError_t e2 = (tmp || e != cudaSuccess) ? cudaStreamSynchronize(p->stream) : cudaSuccess;   // host staging in flight
+  if (tmp) cudaFree(tmp);
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "sft_append_sfts (copy/launch): %s", cudaGetErrorString(e));
+  if (e2 != cudaSuccess) return fail(p, SFT_ECUDA, "sft_append_sfts: %s", cudaGetErrorString(e2));
   return SFT_OK;
 }
 
@@ -454,13 +523,69 @@ SFT_API sft_status sft_compute_sfts(int32_t device, void *stream, const double *
   return SFT_OK;
 }
 
+// Per-SFT noise level from the data (sft_ingest.cuh).  Device pointers.
+static cudaError_t estimate_scale_device(cudaStream_t st, const float2 *bins, int64_t n_sft, int nb, const double *shape, double T,
+                                         int k_lo, int n_samp, int w, double *scale, unsigned char *flag, int pool_max) {
+  int npow2 = 1;
+  while (npow2 < pool_max) npow2 <<= 1;
+  sftk::sft_nonzero_kernel<<<(unsigned)n_sft, 128, 0, st>>>(bins, nb, flag);
+  sftk::sft_psd_scale_kernel<<<(unsigned)n_sft, 256, (size_t)npow2 * sizeof(float), st>>>(bins, flag, shape, (int)n_sft, nb, k_lo, n_samp,
+                                                                                          0.5 * T, w, npow2, scale);
+  return cudaGetLastError();
+}
+
+SFT_API sft_status sft_estimate_psd_scale(int32_t device, void *stream, const float *sft_bins, int64_t n_sft, int32_t k_lo,
+                                          int32_t k_hi, int32_t n_samp, double t_sft, const double *psd_shape, int32_t half_window,
+                                          double *psd_scale, int32_t mem) {
+  g_create_err[0] = 0;
+  if (!sft_bins || !psd_scale) return fail(nullptr, SFT_EINVAL, "sft_estimate_psd_scale: sft_bins and psd_scale are required");
+  if (n_sft < 1 || n_sft > (1ll << 30) || k_lo < 0 || k_hi <= k_lo || n_samp < 2 || !(t_sft > 0.0) || half_window < 0)
+    return fail(nullptr, SFT_EINVAL, "sft_estimate_psd_scale: need n_sft >= 1, 0 <= k_lo < k_hi, n_samp >= 2, t_sft > 0, half_window >= 0");
+  if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(nullptr, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
+  const int nb = k_hi - k_lo;
+  const int q0 = k_lo < 1 ? 1 - k_lo : 0, q1 = nb < n_samp / 2 - k_lo ? nb : n_samp / 2 - k_lo;
+  const long long pool = (long long)(2 * half_window + 1) * (q1 > q0 ? q1 - q0 : 0);
+  if (pool > sftk::PSD_MAX_VALUES)
+    return fail(nullptr, SFT_EUNSUPPORTED, "pool of %lld values per SFT exceeds %d: use a smaller half_window or band", pool, sftk::PSD_MAX_VALUES);
+  CU(nullptr, cudaSetDevice(device));
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t b_bins = (size_t)n_sft * nb * sizeof(float2), b_shape = psd_shape ? nb * sizeof(double) : 0, b_scale = (size_t)n_sft * sizeof(double);
+  void *tmp = nullptr;
+  const size_t o_shape = (b_bins + 255) & ~size_t(255), o_scale = (o_shape + b_shape + 255) & ~size_t(255), o_flag = o_scale + b_scale;
+  cudaError_t e = cudaMalloc(&tmp, (mem == SFT_MEM_HOST ? o_flag : 0) + (size_t)n_sft + 512);
+  if (e != cudaSuccess) return fail(nullptr, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(e));
+  const float2 *d_bins = (const float2 *)sft_bins;
+  const double *d_shape = psd_shape;
+  double *d_scale = psd_scale;
+  unsigned char *d_flag = (unsigned char *)tmp;
+  if (mem == SFT_MEM_HOST) {
+    char *base = (char *)tmp;
+    e = cudaMemcpyAsync(base, sft_bins, b_bins, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && psd_shape) e = cudaMemcpyAsync(base + o_shape, psd_shape, b_shape, cudaMemcpyHostToDevice, st);
+    d_bins = (const float2 *)base;
+    d_shape = psd_shape ? (const double *)(base + o_shape) : nullptr;
+    d_scale = (double *)(base + o_scale);
+    d_flag = (unsigned char *)(base + o_flag);
+  }
+  if (e == cudaSuccess) e = estimate_scale_device(st, d_bins, n_sft, nb, d_shape, t_sft, k_lo, n_samp, half_window, d_scale, d_flag, (int)(pool > 1 ? pool : 1));
+  if (e == cudaSuccess && mem == SFT_MEM_HOST) e = cudaMemcpyAsync(psd_scale, d_scale, b_scale, cudaMemcpyDeviceToHost, st);
+  cudaError_t e2 = cudaStreamSynchronize(st);
+  cudaFree(tmp);
+  if (e != cudaSuccess || e2 != cudaSuccess) return fail(nullptr, SFT_ECUDA, "sft_estimate_psd_scale: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+  return SFT_OK;
+}
+
 SFT_API sft_status sft_ingest_timeseries(sft_plan *p, int32_t channel, const double *x, int64_t n_samples,
                                          const double *psd_scale, const double *psd_shape, const float *response, int32_t mem) {
   if (!p) return SFT_EINVAL;
   p->err[0] = 0;
-  if (!x || !psd_scale) return fail(p, SFT_EINVAL, "x and psd_scale are required");
+  if (!x) return fail(p, SFT_EINVAL, "x is required");
   if (mem != SFT_MEM_HOST && mem != SFT_MEM_DEVICE) return fail(p, SFT_EINVAL, "mem must be SFT_MEM_HOST or SFT_MEM_DEVICE");
   const size_t N = p->d.n_sft, n = p->n_samp, nb = p->nb;
+  if (!psd_scale) {                      // estimated from the data: one median over the band per SFT (sft_estimate_psd_scale)
+    const long long pool = (long long)p->kv_hi - p->kv_lo;
+    if (pool > sftk::PSD_MAX_VALUES) return fail(p, SFT_EUNSUPPORTED, "psd_scale = NULL: the band holds more than %d bins", sftk::PSD_MAX_VALUES);
+  }
   if (n_samples < (int64_t)(N * n)) return fail(p, SFT_ESHAPE, "%lld samples < n_sft * n = %zu", (long long)n_samples, N * n);
   CU(p, cudaSetDevice(p->d.device));
   const size_t b_x = N * n * sizeof(double), b_bins = N * nb * sizeof(float2);
@@ -482,17 +607,24 @@ SFT_API sft_status sft_ingest_timeseries(sft_plan *p, int32_t channel, const dou
   void *tmp2 = nullptr;
   const double *d_scale = psd_scale, *d_shape = psd_shape;
   const float *d_resp = response;
-  if (mem == SFT_MEM_HOST) {
-    const size_t b_scale = N * sizeof(double), b_shape = psd_shape ? nb * sizeof(double) : 0;
-    const size_t b_resp = (response && p->d.response == SFT_RESP_TABLE) ? N * sizeof(float2) : 0;
-    e = cudaMalloc(&tmp2, b_scale + b_shape + b_resp + 768);
+  if (mem == SFT_MEM_HOST || !psd_scale) {
+    const bool host = mem == SFT_MEM_HOST;
+    const size_t b_scale = N * sizeof(double), b_shape = (psd_shape && host) ? nb * sizeof(double) : 0;
+    const size_t b_resp = (response && host && p->d.response == SFT_RESP_TABLE) ? N * sizeof(float2) : 0;
+    e = cudaMalloc(&tmp2, b_scale + b_shape + b_resp + N + 1024);
     if (e != cudaSuccess) { cudaStreamSynchronize(p->stream); cudaFree(tmp); return fail(p, SFT_ENOMEM, "cudaMalloc staging: %s", cudaGetErrorString(e)); }
     char *q = (char *)tmp2;
-    e = cudaMemcpyAsync(q, psd_scale, b_scale, cudaMemcpyHostToDevice, p->stream);
-    d_scale = (const double *)q;
+    e = psd_scale && host ? cudaMemcpyAsync(q, psd_scale, b_scale, cudaMemcpyHostToDevice, p->stream) : cudaSuccess;
+    if (!psd_scale || host) d_scale = (const double *)q;
+    double *est = (double *)q;
     q += (b_scale + 255) & ~size_t(255);
     if (psd_shape && e == cudaSuccess) { e = cudaMemcpyAsync(q, psd_shape, b_shape, cudaMemcpyHostToDevice, p->stream); d_shape = (const double *)q; q += (b_shape + 255) & ~size_t(255); }
-    if (b_resp && e == cudaSuccess) { e = cudaMemcpyAsync(q, response, b_resp, cudaMemcpyHostToDevice, p->stream); d_resp = (const float *)q; }
+    if (b_resp && e == cudaSuccess) { e = cudaMemcpyAsync(q, response, b_resp, cudaMemcpyHostToDevice, p->stream); d_resp = (const float *)q; q += (b_resp + 255) & ~size_t(255); }
+    if (!psd_scale && e == cudaSuccess) {
+      e = estimate_scale_device(p->stream, d_bins, (int64_t)N, (int)nb, d_shape, p->d.t_sft, p->d.k_lo, p->n_samp, 0, est, (unsigned char *)q,
+                                p->kv_hi > p->kv_lo ? p->kv_hi - p->kv_lo : 1);
+      p->launches += 2;
+    }
     if (e != cudaSuccess) {
       cudaStreamSynchronize(p->stream); cudaFree(tmp); cudaFree(tmp2);
       return fail(p, SFT_ECUDA, "noise-description copy: %s", cudaGetErrorString(e));

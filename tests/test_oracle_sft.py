@@ -78,3 +78,31 @@ def test_P4_sft_folded_equals_full_resolution():
                                   np.full(kN.shape, S), 1 / (N * dt), kN, N, True)
     tdp = osft.time_domain_product(x[:N], h[:N], dt, S)
     assert abs(folded - tdp) < 1e-11 * abs(tdp) and abs(full - tdp) < 1e-11 * abs(tdp)
+
+
+def test_psd_scale_estimate_recovers_the_per_sft_noise_level():
+    """oracle.sft.psd_scale_estimate ("whitening data on a per-SFT basis") on the config-2 noise recipe (coloured PSD
+    shape x lognormal per-SFT scale, 10 % gaps, no signal): unbiased (the median of a unit exponential variate is ln 2) with the
+    scatter of a sample median over the band, ~1/sqrt(n_bins); pooling neighbours tightens it; gaps stay gaps; scaling the
+    data by c scales the estimate by c^2; a strong narrow line does not move it."""
+    from paper_2502_11823_b200 import workloads as wl
+    w = wl.et_bns(n_templates=1, n_sft=600, K=8, inject=False, name="noise-only")
+    bins, s_true, S = w.bins[0].astype(np.complex128), w.psd_scale[0], w.psd_shape[0]
+    n = int(w.desc["t_sft"] * w.desc["fs"])
+    est = osft.psd_scale_estimate(bins, S, w.desc["t_sft"], w.desc["k_lo"], n, 0)
+    pres = s_true > 0
+    assert np.all(est[~pres] == 0.0) and np.all(est[pres] > 0.0)
+    ratio = est[pres] / s_true[pres]
+    nb = bins.shape[1]
+    assert abs(ratio.mean() - 1.0) < 4.0 / np.sqrt(nb * pres.sum())          # unbiased
+    assert 0.7 / np.sqrt(nb) < ratio.std() < 1.6 / np.sqrt(nb)                # sample median of Exp(1): sd = 1/(ln 2 sqrt(n)) x ln2... ~1/sqrt(n)
+    est2 = osft.psd_scale_estimate(bins, S, w.desc["t_sft"], w.desc["k_lo"], n, 2)
+    assert np.all(est2[~pres] == 0.0)
+    assert np.allclose(osft.psd_scale_estimate(3.0 * bins, S, w.desc["t_sft"], w.desc["k_lo"], n, 0), 9.0 * est)
+    line = bins.copy()
+    line[:, 40:43] *= 100.0
+    est_line = osft.psd_scale_estimate(line, S, w.desc["t_sft"], w.desc["k_lo"], n, 0)
+    assert np.abs(est_line[pres] / est[pres] - 1.0).mean() < 0.06          # 3 of 153 bins boosted x 1e4 in power: a mean would move x 200
+    # textbook check of the statistic itself: |CN(0, v)|^2 / v has median ln 2
+    z = np.random.default_rng(0).standard_normal((200000, 2)).view(np.complex128)[:, 0] / np.sqrt(2.0)
+    assert abs(np.median(np.abs(z) ** 2) - np.log(2.0)) < 0.01
