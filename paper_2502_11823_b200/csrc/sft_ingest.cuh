@@ -92,12 +92,21 @@ __device__ __forceinline__ void dif_pass(float2 *z, const double *seg, const flo
   }
 }
 
-// One block per segment.  Dynamic shared memory: (n/2 + n/32) float2.
-__global__ void __launch_bounds__(256) sft_rfft_band_kernel(const double *x, int n, int log2m, double dt, int k_lo, int nb,
+// Persistent blocks (grid = SMs x resident blocks), each walking the segments s = blockIdx.x, + gridDim.x, ...  Before it
+// starts on a segment a block asks the TMA unit to pull its NEXT segment from HBM into L2 (cp.async.bulk.prefetch.L2, one
+// instruction for the whole 8 n bytes): the HBM reads of the next segment then run under the butterflies of the current one,
+// and its first pass finds the samples in L2.  (All resident blocks together hold <= 444 x 128 KB = 57 MB of prefetched
+// segments, under half of B200's L2.)  Dynamic shared memory: (n/2 + n/32) float2.
+__global__ void __launch_bounds__(256) sft_rfft_band_kernel(const double *x, int n_sft, int n, int log2m, double dt, int k_lo, int nb,
                                                             const float2 *W, float2 *bins) {
   extern __shared__ float2 z[];
   const int m = n >> 1;
-  const double *seg = x + (size_t)blockIdx.x * n;
+  for (int sidx = blockIdx.x; sidx < n_sft; sidx += gridDim.x) {
+  const double *seg = x + (size_t)sidx * n;
+  if (threadIdx.x == 0 && sidx + (int)gridDim.x < n_sft) {
+    const double *nxt = x + (size_t)(sidx + gridDim.x) * n;
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nxt), "r"((unsigned)(n * 8)) : "memory");
+  }
   // in-place radix-2 DIF network over m points, up to four consecutive stages at a time in registers.  The first pass
   // reads the series from global memory (the only HBM traffic of the kernel) and leaves its output in shared memory.
   int h = m >> 1;                                    // half-block of the next stage
@@ -121,7 +130,7 @@ __global__ void __launch_bounds__(256) sft_rfft_band_kernel(const double *x, int
     return (pos & 1) ? make_float2(w2.x - v.x, w2.y - v.y) : make_float2(v.x + w2.x, v.y + w2.y);
   };
   // band bins from the bit-reversed m-point spectrum
-  float2 *out = bins + (size_t)blockIdx.x * nb;
+  float2 *out = bins + (size_t)sidx * nb;
   const float fdt = (float)dt;
   for (int q = threadIdx.x; q < nb; q += blockDim.x) {
     const int k = k_lo + q;
@@ -139,6 +148,8 @@ __global__ void __launch_bounds__(256) sft_rfft_band_kernel(const double *x, int
       X = make_float2(0.5f * fdt * (S.x + tr), 0.5f * fdt * (S.y + ti));
     }
     out[q] = X;
+  }
+  __syncthreads();                                   // the work array is reused by the next segment
   }
 }
 

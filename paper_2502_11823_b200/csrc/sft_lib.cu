@@ -485,7 +485,12 @@ static cudaError_t compute_sfts_device(cudaStream_t stream, const double *x, int
     while ((1 << log2m) < n / 2) ++log2m;
     const size_t smem = (size_t)(n / 2 + n / 32 + 1) * sizeof(float2);
     cudaFuncSetAttribute(sftk::sft_rfft_band_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    sftk::sft_rfft_band_kernel<<<(unsigned)n_sft, 256, smem, stream>>>(x, n, log2m, dt, k_lo, nb, W, bins);
+    int per_sm = 1, n_sm = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sftk::sft_rfft_band_kernel, 256, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    long long grid = (long long)n_sm * per_sm;
+    if (grid > n_sft) grid = n_sft;
+    sftk::sft_rfft_band_kernel<<<(unsigned)grid, 256, smem, stream>>>(x, (int)n_sft, n, log2m, dt, k_lo, nb, W, bins);
     if (launches) *launches += 1;
     return cudaGetLastError();
   }
