@@ -443,9 +443,11 @@ def run_ours(args, rank, world, local_rank):
 # DRAM bytes (read + write) of one main-kernel launch, from the committed ncu --set full captures (dram__bytes_read.sum +
 # dram__bytes_write.sum): NOT measured by this run - the source capture is named in roofline.traffic_source.
 NCU_TRAFFIC = {
-    ("config2-F", "auto"): (2.219008e6 + 0.401408e6, "profiles/r02a_main_fastpath.md"),
-    ("config2-F", "table"): (2.219008e6 + 0.401408e6, "profiles/r02a_main_fastpath.md"),
+    ("config2-F", "auto"): (2.103296e6 + 7.424e3, "profiles/r02_main_kernel.md"),
+    ("config2-F", "table"): (2.103296e6 + 7.424e3, "profiles/r02_main_kernel.md"),
     ("config2-F", "direct"): (8.213504e6 + 10.752e3, "profiles/r01d_kernel_v7_tables.md"),
+    ("config3-F", "auto"): (5.682176e6 + 872.57728e6, "profiles/r02_main_kernel.md"),
+    ("config4", "auto"): (6.582272e6 + 2.335232e6, "profiles/r02_main_kernel.md"),
 }
 
 # Algorithmic work per active pair and the ALU peak: DESIGN.md section 7.
