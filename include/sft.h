@@ -238,6 +238,19 @@ sft_status sft_plan_path_counts(sft_plan *plan, int64_t *out, int32_t n_out);
 sft_status sft_tsft_rule(double m_chirp, double eta, int32_t waveform, double f_max, double delta,
                          double *t_sft, double *fddot_max);
 
+/* Moment tables for a bank around a known track ("Fourier transforms of the data will be computed once and will be valid for any
+ * template within a given parameter-space region").  By default the tables of the table evaluator cover every window
+ * position k_c of the stored band at every SFT (128 bytes x 4 nodes x (k_hi - k_lo + 2K) x n_sft per channel: 1.1 GB for
+ * config 2, and out of reach for wide bands).  With a fiducial template (one parameter row, host pointer) they cover, per block
+ * of 32 SFT slots, only the positions its k_c sweeps in that block +- half_width bins: templates whose windows stay inside take
+ * the tables, all others the direct evaluator for those SFTs (same results within the evaluators' ~1e-6).  NULL restores the full
+ * tables.  Replaces the tables: every channel must be loaded (again) afterwards.  SFT_ENOMEM if SFT_EVAL_TABLE was asked for and
+ * the tables still do not fit. */
+sft_status sft_plan_set_table_track(sft_plan *plan, const double *fiducial_params, int32_t half_width);
+
+/* Bytes of device memory held by the data-moment tables (0: the plan uses the direct evaluator). */
+int64_t sft_plan_table_bytes(const sft_plan *plan);
+
 /* Tuning knob: SFTs per work unit along the time axis (0 = automatic).  Results do not depend on it
  * beyond fp64 summation order. */
 sft_status sft_plan_set_chunk(sft_plan *plan, int32_t sfts_per_unit);

@@ -46,7 +46,7 @@ class PlanDesc(C.Structure):
 EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_products",
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
            "sft_plan_set_chunk", "sft_plan_path_counts", "sft_compute_sfts", "sft_ingest_timeseries",
-           "sft_tsft_rule", "sft_statistics", "sft_fstat", "sft_validity", "sft_append_sfts", "sft_estimate_psd_scale", "sft_last_error", "sft_version",
+           "sft_tsft_rule", "sft_statistics", "sft_fstat", "sft_validity", "sft_append_sfts", "sft_estimate_psd_scale", "sft_plan_set_table_track", "sft_plan_table_bytes", "sft_last_error", "sft_version",
            "sft_measure_alu_peaks"]
 
 _lib = None
@@ -84,6 +84,10 @@ def load_library(path=None):
     lib.sft_append_sfts.restype = i32
     lib.sft_estimate_psd_scale.argtypes = [i32, vp, vp, i64, i32, i32, i32, dbl, vp, i32, vp, i32]
     lib.sft_estimate_psd_scale.restype = i32
+    lib.sft_plan_set_table_track.argtypes = [vp, vp, i32]
+    lib.sft_plan_set_table_track.restype = i32
+    lib.sft_plan_table_bytes.argtypes = [vp]
+    lib.sft_plan_table_bytes.restype = i64
     lib.sft_tsft_rule.argtypes = [dbl, dbl, i32, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
     lib.sft_tsft_rule.restype = i32
     lib.sft_compute_sfts.argtypes = [i32, vp, vp, i64, i32, dbl, i32, i32, vp, i32]
@@ -271,6 +275,14 @@ class Plan:
             self._h, nT, _ptr(params, np.float64, (nT, NPARAM), "params"), float(delta_max),
             _ptr(delta_eff, np.float64, (nT,), "delta_eff"), _ptr(flags, np.uint8, (nT,), "flags"), mem))
 
+    def set_table_track(self, fiducial_params, half_width):
+        """``sft_plan_set_table_track``: tables only along the track of ``fiducial_params`` (+- half_width bins); None = full."""
+        fp = None if fiducial_params is None else np.ascontiguousarray(fiducial_params, dtype=np.float64)
+        self._check(self.lib.sft_plan_set_table_track(self._h, _ptr(fp, np.float64, (NPARAM,), "fiducial_params"), int(half_width)))
+
+    def table_bytes(self):
+        return int(self.lib.sft_plan_table_bytes(self._h))
+
     def sync(self):
         self._check(self.lib.sft_plan_sync(self._h))
 
@@ -294,7 +306,10 @@ def plan_from_workload(w, device=0, stream=None, **override):
     """Creates a plan for a ``workloads.Workload`` and loads all its channels (host arrays)."""
     d = dict(w.desc)
     d.update(override)
+    track = d.pop("table_track", None)               # (fiducial parameter row, half width in bins) or None
     plan = Plan(d, device=device, stream=stream)
+    if track is not None:
+        plan.set_table_track(track[0], track[1])
     for c in range(plan.n_channels):
         resp = None if w.response is None else np.ascontiguousarray(w.response[c], dtype=np.complex64)
         plan.load_data(c, np.ascontiguousarray(w.bins[c], dtype=np.complex64),

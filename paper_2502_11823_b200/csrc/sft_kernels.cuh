@@ -73,7 +73,14 @@ struct KParams {
   // moment-table evaluator (sft_table.cuh); mtab == nullptr: direct evaluator only
   const float4 *mtab;      // [C][n_sft][n_node][4]   8 complex64 moments per node, node = kcidx * TAB_R + cell
   const float4 *htab;      // [C][n_kc * HTAB_R][4]   <h,h> polynomial per node
-  unsigned mrow, mchan;    // float4 entries per SFT row (n_node * 4) and per channel (n_sft * mrow), hchan likewise
+  // The moment table is laid out per block of 32 SFT slots (tblk[a >> 5]): rows of W window positions starting at
+  // position kb (counted from k_lo - K), so that a bank around a known track needs only the band the track sweeps
+  // (sft_plan_set_table_track); without a track every block covers all n_kc positions.
+  const int4 *tblk;        // per block {x: float4 index of the block's first row (channel 0), y: kb, z: W, w: float4 per row}
+  int banded;              // 0: every block covers all window positions (the in-band test implies the in-table test)
+  unsigned mrow0;          // float4 per row of the full (not banded) layout: kernel variants compiled with BAND = false use it
+                           // as a constant-bank operand instead of the per-block record
+  unsigned mchan;          // float4 entries per channel of mtab; hchan likewise for htab
   unsigned hchan;
   float b_table, b_table2; // B_TABLE, B_TABLE2 if the plan has the tables, else -1 (no |b| qualifies)
   double *part;            // [n_chunks][3][nT] chunk totals (xh, hh, xh_im)
@@ -715,7 +722,7 @@ struct TableData {
 
 // node look-up and loads
 template <int CT, int TIER>
-__device__ __forceinline__ void table_load(const KParams &p, float xp, float b, int kcidx, const float4 *Mrow,
+__device__ __forceinline__ void table_load(const KParams &p, float xp, float b, int kcidx, int kb, const float4 *Mrow,
                                            TableData<CT, TIER> &d) {
   // node of the <h,h> table: cellH = floor((xp + 1/2) HTAB_R) by the 1.5 * 2^23 rounding trick, clamped (xp = 1/2
   // exactly, NaN lanes); the data-moment node is cellH >> HTAB_SHIFT.  The offset HTAB_R/2 - 1/2 must be added
@@ -727,7 +734,7 @@ __device__ __forceinline__ void table_load(const KParams &p, float xp, float b, 
   const int cellH = __float_as_int(cm) & (HTAB_R - 1);
   const int cell = cellH >> HTAB_SHIFT;
   const float cHf = cm - RM;                                   // (float)cellH
-  const float4 *mp = Mrow + (unsigned)(kcidx * TAB_R + cell) * (unsigned)((TAB_Q + 1) / 2);
+  const float4 *mp = Mrow + (unsigned)((kcidx - kb) * TAB_R + cell) * (unsigned)((TAB_Q + 1) / 2);    // row of the block: positions kb ...
   const float4 *hp = p.htab + (unsigned)(kcidx * HTAB_R + cellH) * (unsigned)(HTAB_W / 4);
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
@@ -841,10 +848,10 @@ __device__ __forceinline__ void table_math2(const TableData<CT, TIER> &dA, const
 
 template <int CT, class CFG, int TIER>
 __device__ __forceinline__ void table_eval(const KParams &p, const Tmpl &tm, double dnext, Track &nxt, float xp, float b,
-                                           int kcidx, const float4 *Mrow, float (&s1r)[CT], float (&s1i)[CT],
+                                           int kcidx, int kb, const float4 *Mrow, float (&s1r)[CT], float (&s1i)[CT],
                                            float (&s2)[CT]) {
   TableData<CT, TIER> d;
-  table_load<CT, TIER>(p, xp, b, kcidx, Mrow, d);
+  table_load<CT, TIER>(p, xp, b, kcidx, kb, Mrow, d);
   track_eval<CFG>(p, tm, dnext, nxt);
   table_math<CT, TIER>(d, s1r, s1i, s2);
 }
@@ -922,7 +929,7 @@ __device__ __forceinline__ void finish_terms(const KParams &p, const Tmpl &tm, c
 // independent work in one straight-line block (the fp64 tracks of alpha + 2 and alpha + 3 included), so that the
 // fixed-latency dependency chains of one fill the issue gaps of the other.
 template <int CT, class CFG>
-__device__ __forceinline__ void duo_terms(const KParams &p, const Tmpl &tm, const float4 *Mrow0, const float2 *rt,
+__device__ __forceinline__ void duo_terms(const KParams &p, const Tmpl &tm, const float4 *Mrow0, int4 tb, const float2 *rt,
                                           const Track &trA, const Track &trB, bool goA, bool goB, const float (&usA)[CT],
                                           const float (&usB)[CT], double dnext, Track &nA, Track &nB, float &zrA, float &ziA,
                                           float &hhA, float &zrB, float &ziB, float &hhB) {
@@ -931,8 +938,8 @@ __device__ __forceinline__ void duo_terms(const KParams &p, const Tmpl &tm, cons
   const bool fres = (cfg_kernel<CFG>(p) == 1);
   const float bA = fres ? trA.b : 0.f, bB = fres ? trB.b : 0.f;
   TableData<CT, 1> dA, dB;
-  table_load<CT, 1>(p, fmaf(0.5f, bA, trA.x), bA, okA ? j0A - 2 : 0, Mrow0, dA);
-  table_load<CT, 1>(p, fmaf(0.5f, bB, trB.x), bB, okB ? j0B - 2 : 0, Mrow0 + p.mrow, dB);
+  table_load<CT, 1>(p, fmaf(0.5f, bA, trA.x), bA, okA ? j0A - 2 : tb.y, tb.y, Mrow0, dA);
+  table_load<CT, 1>(p, fmaf(0.5f, bB, trB.x), bB, okB ? j0B - 2 : tb.y, tb.y, Mrow0 + (unsigned)tb.w, dB);
   track_eval<CFG>(p, tm, dnext, nA);
   track_eval<CFG>(p, tm, dnext + 1.0, nB);
   float s1rA[CT], s1iA[CT], s2A[CT], s1rB[CT], s1iB[CT], s2B[CT];
@@ -950,8 +957,8 @@ __device__ __forceinline__ void duo_terms(const KParams &p, const Tmpl &tm, cons
 // of SFT alpha, channel 0, in the pair-planar store / the moment table.  Also evaluates the track of the
 // next SFT (see series_pairs).
 template <int KT, int CT, class CFG>
-__device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, const float4 *Drow0, const float4 *Mrow0,
-                                           const float2 *rt, const Track &tr, bool go, float bmax, const float (&us2)[CT],
+__device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, const float4 *Drow0, const float4 *Mrow0, int kb,
+                                           float bt1, float bt2, const float2 *rt, const Track &tr, bool go, float bmax, const float (&us2)[CT],
                                            double dnext, Track &nxt, float &zr, float &zi, float &hh, float *fq = nullptr) {
   // window start in the zero-padded row; windows that miss the stored band entirely contribute 0
   const int j0 = tr.kc - p.kwin0;                                  // kwin0 = k_lo + K - PAD
@@ -962,10 +969,11 @@ __device__ __forceinline__ void pair_terms(const KParams &p, const Tmpl &tm, con
   float s1r[CT], s1i[CT], s2[CT];
   float scale;                 // the series evaluators return 2 pi J
   float t;                     // total phase / pi:  2 frac (= phi_a/pi) + prefactor phase / pi
-  if (bmax <= p.b_table2) {
+  if (bmax <= bt2) {                   // bt1 / bt2: B_TABLE / B_TABLE2 where the warp's windows lie inside the block's table rows, else -1
     const float xp = fmaf(0.5f, b, tr.x);
-    if (bmax <= p.b_table) table_eval<CT, CFG, 1>(p, tm, dnext, nxt, xp, b, j0c - 2, Mrow0, s1r, s1i, s2);
-    else table_eval<CT, CFG, 2>(p, tm, dnext, nxt, xp, b, j0c - 2, Mrow0, s1r, s1i, s2);
+    const int kci = ok ? j0 - 2 : kb;
+    if (bmax <= bt1) table_eval<CT, CFG, 1>(p, tm, dnext, nxt, xp, b, kci, kb, Mrow0, s1r, s1i, s2);
+    else table_eval<CT, CFG, 2>(p, tm, dnext, nxt, xp, b, kci, kb, Mrow0, s1r, s1i, s2);
     scale = 1.0f;
     t = fmaf(2.0f, tr.frac, fmaf(0.25f, b, tr.x));           // prefactor e^{i pi (x + b/4)}
   } else {
@@ -1188,9 +1196,9 @@ __device__ __forceinline__ void ftrack_closed(const KParams &p, const Tmpl &tm, 
 // Is the block [g, ge) clean for this warp (see above)?  Returns 0 = no (generic loop), 1 = clean, closed-form track,
 // 2 = clean, polynomial track (coefficients in fc and, unless CREG, in the thread's shared-memory slot cs).  `mask` receives the
 // block's presence bits (any channel), usv[c] the weight 1/s of SFT g + lane.
-template <int CT, class CFG, bool CREG>
+template <int CT, class CFG, bool CREG, bool BAND>
 __device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int g, int ge, int lane, float ascale, float4 *cs,
-                                          unsigned &mask, float (&usv)[CT], FastCoef &fc) {
+                                          unsigned &mask, float (&usv)[CT], FastCoef &fc, int4 &tb) {
   bool pres = false;
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
@@ -1199,6 +1207,14 @@ __device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int 
   }
   mask = __ballot_sync(0xffffffffu, pres);
   if (mask == 0u || p.mtab == nullptr || cfg_phase<CFG>(p) != 0) return 0;
+  if (BAND) {
+    if ((g >> 5) != ((ge - 1) >> 5)) return 0;                     // (work units that are not aligned to the table's blocks of 32 SFTs)
+    tb = __ldg(p.tblk + (g >> 5));
+    if (tb.z <= 0) return 0;
+  } else {                                                         // full layout: row of SFT a at a * mrow0, all positions present
+    tb = make_int4(0, 0, p.jmax + 1, 0);
+  }
+  const int kofs = p.kwin0 + 2 + tb.y;                              // window position of k_c inside the block's rows: k_c - kofs in [0, W)
   const bool fres = cfg_kernel<CFG>(p) == 1;
   const bool poly = __all_sync(0xffffffffu, fast_coef<CFG>(p, tm, g, ascale, fc));
   if (poly) {
@@ -1220,8 +1236,8 @@ __device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int 
     const double tau_h = fma(-(double)(ge - 1), p.T, tm.tau0);
     // Dirichlet kernel: the band edge test needs fdot T^2 although the evaluator does not (2 p_2 at the centre; +-1e-9 ties are flagged)
     const double b_edge = fres ? (double)bh : 2.0 * fc.p2;
-    const bool ok = tau_h > p.T && fl >= p.f_loT && fh + b_edge <= p.f_hiT && (unsigned)(kl - p.kwin0 - 2) <= (unsigned)p.jmax &&
-                    (unsigned)(kh - p.kwin0 - 2) <= (unsigned)p.jmax && bl >= 0.f && bh >= bl && bh <= p.b_table && kh >= kl;
+    const bool ok = tau_h > p.T && fl >= p.f_loT && fh + b_edge <= p.f_hiT && (unsigned)(kl - kofs) < (unsigned)tb.z &&
+                    (unsigned)(kh - kofs) < (unsigned)tb.z && bl >= 0.f && bh >= bl && bh <= p.b_table && kh >= kl;
     if (!__all_sync(0xffffffffu, ok)) return 0;
     if (!CREG) coef_store(cs, fc);
     return 2;
@@ -1230,8 +1246,7 @@ __device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int 
   track_eval_fp64<CFG>(p, tm, (double)g, lo);
   track_eval_fp64<CFG>(p, tm, (double)(ge - 1), hi);
   const float bl = fres ? lo.b : 0.f, bh = fres ? hi.b : 0.f;
-  const int j0l = lo.kc - p.kwin0, j0h = hi.kc - p.kwin0;
-  const bool ok = lo.active && hi.active && (unsigned)(j0l - 2) <= (unsigned)p.jmax && (unsigned)(j0h - 2) <= (unsigned)p.jmax &&
+  const bool ok = lo.active && hi.active && (unsigned)(lo.kc - kofs) < (unsigned)tb.z && (unsigned)(hi.kc - kofs) < (unsigned)tb.z &&
                   bl >= 0.f && bh >= bl && bh <= p.b_table && hi.kc >= lo.kc;
   return __all_sync(0xffffffffu, ok) ? 1 : 0;
 }
@@ -1385,12 +1400,15 @@ __device__ __forceinline__ void scan_store(const KParams &p, float *txh, float *
 
 // The loop over the present SFTs of a clean block, two at a time.  Accumulates into axh / ahh / axi (fp64; fp32 partial
 // sums over the block).
-template <int CT, int MODE, class CFG, bool POLY, bool CREG>
-__device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, const float4 *cs, const FastCoef &fc, unsigned mask, const float (&usv)[CT],
+template <int CT, int MODE, class CFG, bool POLY, bool CREG, bool BAND>
+__device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, const float4 *cs, const FastCoef &fc, int4 tb, unsigned mask, const float (&usv)[CT],
                                            float ascale, int g, int ge, int tg, int lane, long long t, bool want_kc, double &axh,
                                            double &ahh, double &axi, float *txh, float *thh, unsigned long long *n_path) {
   const int n = ge - g;
-  const unsigned row0 = (unsigned)g * p.mrow;
+  // first row of the block's table rows, shifted so that the GLOBAL window position indexes it (arithmetic mod 2^32)
+  const unsigned mrow = BAND ? (unsigned)tb.w : p.mrow0;
+  const unsigned row0 = BAND ? (unsigned)tb.x + (unsigned)(g & 31) * mrow - (unsigned)tb.y * (unsigned)(TAB_R * ((TAB_Q + 1) / 2))
+                             : (unsigned)g * p.mrow0;
   const float2 *rt = p.rtab + g;
   int *kcp = (CFG::KC && want_kc) ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + g : nullptr;
   if (CFG::KC && kcp && t < p.nT) {
@@ -1420,8 +1438,8 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
       usB[c] = vB ? __shfl_sync(0xffffffffu, usv[c], jB) : 0.f;
     }
     TableData<CT, 1> dA, dB;
-    table_load_fast<CT>(p, A.xp, A.b, A.kc - p.kwin0 - 2, row0 + (unsigned)jA * p.mrow, dA);
-    table_load_fast<CT>(p, B.xp, B.b, B.kc - p.kwin0 - 2, row0 + (unsigned)jB * p.mrow, dB);
+    table_load_fast<CT>(p, A.xp, A.b, A.kc - p.kwin0 - 2, row0 + (unsigned)jA * mrow, dA);
+    table_load_fast<CT>(p, B.xp, B.b, B.kc - p.kwin0 - 2, row0 + (unsigned)jB * mrow, dB);
     float s1rA[CT], s1iA[CT], s2A[CT], s1rB[CT], s1iB[CT], s2B[CT];
     table_math2<CT, 1>(dA, dB, s1rA, s1iA, s2A, s1rB, s1iB, s2B);
     float zrA, ziA, hhA, zrB, ziB, hhB;
@@ -1468,7 +1486,7 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
 // generic loop below, which runs in groups of GROUP SFTs: fp32 partial sums flushed into fp64 per group (MODE 0),
 // one transposed store per group (MODE 1).
 // ---------------------------------------------------------------------------------------------
-template <int KT, int CT, int MODE, class CFG, int MINB, bool DUO, bool CREG>
+template <int KT, int CT, int MODE, class CFG, int MINB, bool DUO, bool CREG, bool BAND = true>
 __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
   constexpr int GROUP = MODE == 1 ? 32 : FLUSH;
   constexpr int TILE_F = 2 * 32 * 33;                  // two padded 32 x 32 tiles per warp
@@ -1508,14 +1526,15 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
         // where the template's amplitude constant is real (no response, one channel) it is folded into the amplitude
         const float ascale = (CFG::RESP == 0 && CT == 1) ? tm.AE[0].x : 1.0f;
         FastCoef fc;
-        const int kind = MODE == 2 ? 0 : fast_setup<CT, CFG, CREG>(p, tm, gs, gend, lane, ascale, cs, mask, usv, fc);
+        int4 tbf;
+        const int kind = MODE == 2 ? 0 : fast_setup<CT, CFG, CREG, BAND>(p, tm, gs, gend, lane, ascale, cs, mask, usv, fc, tbf);
         if (kind != 0) smask = mask;
         if (kind == 2) {
-          fast_block<CT, MODE, CFG, true, CREG>(p, tm, cs, fc, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
+          fast_block<CT, MODE, CFG, true, CREG, BAND>(p, tm, cs, fc, tbf, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
           continue;
         }
         if (kind == 1) {
-          fast_block<CT, MODE, CFG, false, CREG>(p, tm, cs, fc, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
+          fast_block<CT, MODE, CFG, false, CREG, BAND>(p, tm, cs, fc, tbf, mask, usv, ascale, gs, gend, tg, lane, t, want_kc, axh, ahh, axi, txh, thh, n_path);
           continue;
         }
       }
@@ -1524,8 +1543,13 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
       const float *usp = p.us2 + gs;
       const float2 *rt = p.rtab + gs;
       const float4 *Drow0 = p.Dp + (size_t)gs * p.npair;
-      const float4 *Mrow0 = p.mtab ? p.mtab + (size_t)gs * p.mrow : nullptr;
       int *kcp = want_kc ? p.kc_out + ((size_t)(t < p.nT ? t : 0) * CT) * p.n_sft + gs : nullptr;
+      // table rows: one layout record per block of 32 SFT slots; [gs, gend) lies inside one block unless the work units are
+      // not aligned to 32 (sft_plan_set_chunk), in which case the record is re-read per SFT
+      const bool one_blk = (gs >> 5) == ((gend - 1) >> 5);
+      int4 tb = !p.mtab ? make_int4(0, 0, 0, 0)
+                : BAND  ? __ldg(p.tblk + (gs >> 5))
+                        : make_int4((int)((unsigned)(gs & ~31) * p.mrow0), 0, p.jmax + 1, (int)p.mrow0);
       Track tr, tr2;                                   // tracks of SFT alpha and alpha + 1
       track_eval<CFG>(p, tm, dalpha, tr);
       track_eval<CFG>(p, tm, dalpha + 1.0, tr2);
@@ -1547,9 +1571,20 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
           }
           const bool go = any && tr.active;
           const float ab = (go && cfg_kernel<CFG>(p) == 1) ? fabsf(tr.b) : 0.f;
+          // the table rows of this SFT (block alpha >> 5) and whether the windows of all active lanes lie inside them
+          if (!one_blk && p.mtab) {
+            if (BAND) tb = __ldg(p.tblk + (alpha >> 5));
+            else tb.x = (int)((unsigned)(alpha & ~31) * p.mrow0);
+          }
+          const float4 *Mrow0 = p.mtab + ((unsigned)tb.x + (unsigned)(alpha & 31) * (unsigned)tb.w);
+          const int kci = tr.kc - p.kwin0 - 2;
+          const bool tabok = !p.banded ? p.mtab != nullptr
+                                       : (tb.z > 0 && __all_sync(0xffffffffu, !(go && (unsigned)kci <= (unsigned)p.jmax) ||
+                                                                                  (unsigned)(kci - tb.y) < (unsigned)tb.z));
+          const float bt1 = tabok ? p.b_table : -1.f, bt2 = tabok ? p.b_table2 : -1.f;
           // two SFTs at once when both are present and both go through the tier-1 tables
           bool duo = false, gob = false;
-          if (DUO && MODE != 2 && alpha + 1 < ge) {
+          if (DUO && MODE != 2 && alpha + 1 < ge && tabok && (alpha & 31) != 31) {
 #pragma unroll
             for (int c = 0; c < CT; ++c) {
               us2b[c] = __ldg(usp + c * p.n_sft + 1);
@@ -1558,12 +1593,14 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
             gob = anyb && tr2.active;
             const float abb = (gob && cfg_kernel<CFG>(p) == 1) ? fabsf(tr2.b) : 0.f;
             const float bm2 = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(ab, abb))));
-            duo = bm2 <= p.b_table && __any_sync(0xffffffffu, go) && __any_sync(0xffffffffu, gob);
+            const int kcb = tr2.kc - p.kwin0 - 2;
+            const bool tabokb = !p.banded || __all_sync(0xffffffffu, !(gob && (unsigned)kcb <= (unsigned)p.jmax) || (unsigned)(kcb - tb.y) < (unsigned)tb.z);
+            duo = tabokb && bm2 <= p.b_table && __any_sync(0xffffffffu, go) && __any_sync(0xffffffffu, gob);
           }
           if (duo) {
             Track nA, nB;
             float zrA, ziA, hhA, zrB, ziB, hhB;
-            duo_terms<CT, CFG>(p, tm, Mrow0, rt, tr, tr2, go, gob, us2, us2b, dalpha + 2.0, nA, nB, zrA, ziA, hhA, zrB, ziB, hhB);
+            duo_terms<CT, CFG>(p, tm, Mrow0, tb, rt, tr, tr2, go, gob, us2, us2b, dalpha + 2.0, nA, nB, zrA, ziA, hhA, zrB, ziB, hhB);
             if (CFG::KC && p.path_counts) {
               int npa = 0, npb = 0;
 #pragma unroll
@@ -1593,7 +1630,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
               fhh += hhA + hhB;
             }
             tr = nA; tr2 = nB;
-            alpha += 2; dalpha += 2.0; usp += 2; rt += 2; Drow0 += 2 * p.npair; Mrow0 += 2 * p.mrow;
+            alpha += 2; dalpha += 2.0; usp += 2; rt += 2; Drow0 += 2 * p.npair;
             continue;
           }
           Track nxt;                                               // track of SFT alpha + 2
@@ -1603,11 +1640,11 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
               int n_present = 0;
 #pragma unroll
               for (int c = 0; c < CT; ++c) n_present += us2[c] > 0.f;
-              n_path[path_of(bmax, p.mtab != nullptr)] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * n_present);
+              n_path[path_of(bmax, tabok)] += (unsigned)(__popc(__ballot_sync(0xffffffffu, go)) * n_present);
             }
             float zr, zi, hh;
             float fq[7];
-            pair_terms<KT, CT, CFG>(p, tm, Drow0, Mrow0, rt, tr, go, bmax, us2, dalpha + 2.0, nxt, zr, zi, hh, MODE == 2 ? fq : nullptr);
+            pair_terms<KT, CT, CFG>(p, tm, Drow0, Mrow0, tb.y, bt1, bt2, rt, tr, go, bmax, us2, dalpha + 2.0, nxt, zr, zi, hh, MODE == 2 ? fq : nullptr);
             if (MODE == 2) {
 #pragma unroll
               for (int i = 0; i < 7; ++i) ffs[i] += fq[i];
@@ -1635,7 +1672,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
             txh[lane * 33 + (alpha - g)] = (float)axh;
             thh[lane * 33 + (alpha - g)] = (float)ahh;
           }
-          ++alpha; dalpha += 1.0; ++usp; ++rt; Drow0 += p.npair; Mrow0 += p.mrow;
+          ++alpha; dalpha += 1.0; ++usp; ++rt; Drow0 += p.npair;
         }
         if (MODE == 0) {
           axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;

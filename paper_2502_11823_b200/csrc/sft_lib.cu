@@ -48,6 +48,10 @@ struct sft_plan {
   float4 *htab = nullptr;                              // [C][n_kc * HTAB_R][4] <h,h> table
   float2 *ptab = nullptr;                              // [(2K+1)][TAB_R][TAB_Q+1] kernel moments at the nodes
   int n_kc = 0, n_node = 0;
+  int4 *tblk = nullptr;                                // [ceil(n_sft/32)] layout of the moment table per block of 32 SFT slots (sft_kernels.cuh)
+  size_t m_f4_chan = 0;                                // float4 entries of mtab per channel
+  int w_max = 0;                                       // widest block (window positions)
+  bool banded = false;                                 // layout from sft_plan_set_table_track
   int *counter = nullptr;                              // work-unit counter of the persistent main kernel
   unsigned long long *path_counts = nullptr;           // [PATH_N] diagnostic counters
   int n_sm = 0;
@@ -97,6 +101,44 @@ static sft_status grow(sft_plan *p, void **ptr, size_t *have, size_t need) {
 SFT_API const char *sft_version(void) { return "sft_b200 0.1 (sm_100a)"; }
 
 SFT_API const char *sft_last_error(const sft_plan *plan) { return plan ? plan->err : g_create_err; }
+
+// Lays out and allocates the data-moment table (replacing any previous one).  `kb` / `w` [n_blocks]: first window position
+// (counted from k_lo - K) and number of positions of every block of 32 SFT slots; null = all n_kc positions everywhere.
+// SFT_ENOMEM (plan left without a table) if it does not fit in a quarter of the free device memory or in 32-bit indexing.
+static sft_status table_layout(sft_plan *p, const int *kb, int /*unused*/, const int *w) {
+  const size_t N = p->d.n_sft, C = p->d.n_channels, nblk = (N + 31) / 32, f4_node = (sftk::TAB_Q + 1) / 2;
+  std::vector<int4> h(nblk);
+  size_t off = 0;
+  int wmax = 0;
+  for (size_t b = 0; b < nblk; ++b) {
+    const int kbb = kb ? kb[b] : 0, wb = w ? w[b] : p->n_kc;
+    const size_t rows = (b + 1 < nblk) ? 32 : N - 32 * b, mrow = (size_t)wb * sftk::TAB_R * f4_node;
+    if (off + rows * mrow >= 4000000000ull) { off = ~size_t(0) / 2; break; }
+    h[b] = make_int4((int)(unsigned)off, kbb, wb, (int)mrow);
+    off += rows * mrow;
+    if (wb > wmax) wmax = wb;
+  }
+  cudaFree(p->mtab); p->mtab = nullptr;
+  cudaFree(p->tblk); p->tblk = nullptr;
+  p->m_f4_chan = 0;
+  size_t free_b = 0, total_b = 0;
+  cudaMemGetInfo(&free_b, &total_b);
+  const double m_bytes = (double)C * (double)off * 16.0;
+  if (off >= 4000000000ull || (double)C * (double)off >= 4.0e9 || m_bytes > 0.25 * (double)free_b)
+    return fail(p, SFT_ENOMEM, "moment tables of %.3g bytes do not fit (free %.3g)", m_bytes, (double)free_b);
+  if (cudaMalloc((void **)&p->mtab, (size_t)m_bytes + 256) != cudaSuccess || cudaMalloc((void **)&p->tblk, nblk * sizeof(int4)) != cudaSuccess) {
+    cudaFree(p->mtab); p->mtab = nullptr;
+    cudaFree(p->tblk); p->tblk = nullptr;
+    cudaGetLastError();
+    return fail(p, SFT_ENOMEM, "cudaMalloc of the moment tables (%.3g bytes) failed", m_bytes);
+  }
+  cudaError_t e = cudaMemcpyAsync(p->tblk, h.data(), nblk * sizeof(int4), cudaMemcpyHostToDevice, p->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);          // (h is a local)
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "table layout copy: %s", cudaGetErrorString(e));
+  p->m_f4_chan = off;
+  p->w_max = wmax;
+  return SFT_OK;
+}
 
 SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   g_create_err[0] = 0;
@@ -159,14 +201,10 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
   p->n_kc = p->nb + 2 * d.K;
   p->n_node = p->n_kc * sftk::TAB_R;
   if (st == SFT_OK && d.evaluator != SFT_EVAL_DIRECT) {
-    const double m_bytes = (double)C * (double)N * p->n_node * (8.0 * (sftk::TAB_Q + 1));
-    size_t free_b = 0, total_b = 0;
-    cudaMemGetInfo(&free_b, &total_b);
-    const bool fits = m_bytes <= 0.25 * (double)free_b && (double)C * (double)N * p->n_node * ((sftk::TAB_Q + 1) / 2) < 4.0e9;
-    if (!fits && d.evaluator == SFT_EVAL_TABLE)
-      st = fail(nullptr, SFT_ENOMEM, "moment tables of %.3g bytes do not fit (free %.3g)", m_bytes, (double)free_b);
-    if (fits) {
-      alloc((void **)&p->mtab, (size_t)m_bytes + (size_t)p->n_node * 8 * (sftk::TAB_Q + 1));   // (+ one spare row)
+    st = table_layout(p, nullptr, 0, nullptr);         // every block covers all n_kc window positions
+    if (st == SFT_ENOMEM && d.evaluator == SFT_EVAL_AUTO) st = SFT_OK;   // does not fit: direct evaluator (mtab stays null)
+    if (st != SFT_OK) memcpy(g_create_err, p->err, 512);
+    if (st == SFT_OK) {
       alloc((void **)&p->htab, C * (size_t)p->n_kc * sftk::HTAB_R * sftk::HTAB_W * sizeof(float));
       alloc((void **)&p->ptab, (size_t)(2 * d.K + 1) * sftk::TAB_R * (sftk::TAB_Q + 1) * sizeof(float2));
       if (st == SFT_OK) {
@@ -218,7 +256,7 @@ SFT_API sft_status sft_plan_destroy(sft_plan *p) {
   cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->scan);
   if (p->h_pin) cudaFreeHost(p->h_pin);
   cudaFree(p->td); cudaFree(p->tf); cudaFree(p->counter); cudaFree(p->path_counts);
-  cudaFree(p->mtab); cudaFree(p->htab); cudaFree(p->ptab);
+  cudaFree(p->mtab); cudaFree(p->htab); cudaFree(p->ptab); cudaFree(p->tblk);
   if (p->ev0) cudaEventDestroy(p->ev0);
   if (p->ev1) cudaEventDestroy(p->ev1);
   delete p;
@@ -288,6 +326,60 @@ SFT_API sft_status sft_tsft_rule(double m_chirp, double eta, int32_t waveform, d
   return SFT_OK;
 }
 
+// Moment tables restricted to the band a known track sweeps.  The k_c of the fiducial template at the first and last SFT of
+// every block of 32 slots (host double arithmetic of the same closed form as the kernels: DESIGN W1/W2, A5) +- half_width
+// bins gives the block's window positions; blocks the fiducial signal does not reach get no rows.
+SFT_API sft_status sft_plan_set_table_track(sft_plan *p, const double *fiducial, int32_t half_width) {
+  if (!p) return SFT_EINVAL;
+  p->err[0] = 0;
+  if (p->d.evaluator == SFT_EVAL_DIRECT) return SFT_OK;             // no tables: nothing to lay out
+  if (half_width < 0) return fail(p, SFT_EINVAL, "half_width must be >= 0");
+  CU(p, cudaSetDevice(p->d.device));
+  CU(p, cudaStreamSynchronize(p->stream));
+  const size_t N = p->d.n_sft, nblk = (N + 31) / 32;
+  std::vector<int> kb, w;
+  if (fiducial) {
+    kb.assign(nblk, 0);
+    w.assign(nblk, 0);
+    const double mc = fiducial[0], eta = fiducial[1], tau0 = fiducial[2] - p->d.t0, T = p->d.t_sft;
+    if (!(mc > 0.0) || !(eta > 0.0) || !(eta <= 0.25) || !isfinite(tau0)) return fail(p, SFT_EINVAL, "fiducial template: need m_chirp > 0, 0 < eta <= 1/4");
+    const double M = mc * pow(eta, -0.6) * sftk::GMSUN_S, k = eta / (5.0 * M), F0T = T / (8.0 * 3.141592653589793 * M);
+    const double cf = p->d.waveform >= SFT_WF_PN1 ? 743.0 / 2688.0 + 11.0 / 32.0 * eta : 0.0, c15 = p->d.waveform >= SFT_WF_PN15 ? sftk::C15_F : 0.0;
+    auto kc_of = [&](size_t a, long long &kc) {
+      const double tau = tau0 - (double)a * T;
+      if (!(tau > T)) return false;
+      const double q = pow(k * tau, -0.125), q2 = q * q, q3 = q2 * q, q8 = q2 * q2 * q2 * q2;
+      const double fT = F0T * q3 * (1.0 + cf * q2 + c15 * q3), b = F0T * k * T * (q8 * q3) * (0.375 + 0.625 * cf * q2 + 0.75 * c15 * q3);
+      const double y = p->d.kernel == SFT_KERNEL_FRESNEL ? fT + 0.5 * b : fT;
+      if (!isfinite(y) || fabs(y) > 1.0e9) return false;
+      kc = (long long)floor(y + 0.5);
+      return true;
+    };
+    const long long base = (long long)p->d.k_lo - p->d.K;                // window position 0
+    for (size_t b = 0; b < nblk; ++b) {
+      const size_t a0 = 32 * b, a1 = (a0 + 31 < N ? a0 + 31 : N - 1);
+      long long k0, k1;
+      if (!kc_of(a0, k0)) continue;                                       // ended before the block starts: no rows
+      size_t al = a1;
+      while (al > a0 && !kc_of(al, k1)) --al;                              // (the signal may end inside the block)
+      if (al == a0) k1 = k0;
+      long long lo = k0 - half_width - base, hi = k1 + half_width - base;
+      if (lo < 0) lo = 0;
+      if (hi > p->n_kc - 1) hi = p->n_kc - 1;
+      if (hi >= lo) { kb[b] = (int)lo; w[b] = (int)(hi - lo + 1); }
+    }
+  }
+  sft_status st = table_layout(p, fiducial ? kb.data() : nullptr, 0, fiducial ? w.data() : nullptr);
+  for (int c = 0; c < p->d.n_channels; ++c) p->loaded[c] = false;        // the tables are gone: sft_load_data again
+  p->banded = fiducial != nullptr && st == SFT_OK;
+  if (st == SFT_ENOMEM && p->d.evaluator == SFT_EVAL_AUTO) return SFT_OK; // no tables: the direct evaluator serves
+  return st;
+}
+
+SFT_API int64_t sft_plan_table_bytes(const sft_plan *p) {
+  return p && p->mtab ? (int64_t)(p->m_f4_chan * 16 * (size_t)p->d.n_channels) : 0;
+}
+
 SFT_API sft_status sft_plan_set_chunk(sft_plan *p, int32_t c) {
   if (!p) return SFT_EINVAL;
   if (c < 0) return fail(p, SFT_EINVAL, "sfts_per_block must be >= 0");
@@ -328,8 +420,9 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
   // limits are checked before anything is enqueued or allocated (outputs/plan untouched on error)
   unsigned bpr = 0;
   if (p->mtab) {
-    const unsigned outs = (unsigned)p->n_node * (sftk::TAB_Q + 1);
+    const unsigned outs = (unsigned)p->w_max * sftk::TAB_R * (sftk::TAB_Q + 1);
     bpr = (outs + 255) / 256;
+    if (bpr < 1) bpr = 1;
     if ((double)bpr * (double)N > 2.0e9) return fail(p, SFT_EUNSUPPORTED, "moment-table build grid too large");
   }
   const float2 *d_raw = nullptr;
@@ -371,9 +464,8 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
     p->launches += 2;
     if (d_shape) ok(cudaMemcpyAsync(p->shape_dev + (size_t)channel * nb, d_shape, nb * sizeof(double), cudaMemcpyDeviceToDevice, p->stream));
     if (p->mtab) {
-      const size_t per_chan = N * (size_t)p->n_node * ((sftk::TAB_Q + 1) / 2);
       sftk::sft_mtab_kernel<<<(unsigned)(bpr * N), 256, 0, p->stream>>>(
-          p->Dp + (size_t)channel * N * npair, p->npair, p->n_node, p->d.K, p->ptab, bpr, (float2 *)(p->mtab + (size_t)channel * per_chan));
+          p->Dp + (size_t)channel * N * npair, p->npair, p->tblk, 0, p->d.K, p->ptab, bpr, (float2 *)(p->mtab + (size_t)channel * p->m_f4_chan));
       sftk::sft_htab_kernel<<<(unsigned)(p->n_kc * sftk::HTAB_R), 64, 0, p->stream>>>(
           p->ubp + (size_t)channel * npair, p->d.K, (float *)(p->htab + (size_t)channel * p->n_kc * sftk::HTAB_R * (sftk::HTAB_W / 4)));
       p->launches += 2;
@@ -412,7 +504,8 @@ SFT_API sft_status sft_append_sfts(sft_plan *p, int32_t channel, int64_t first_s
   const size_t N = p->d.n_sft, nb = p->nb, nn = (size_t)n_new, a0 = (size_t)first_sft, C = p->d.n_channels, npair = p->npair;
   unsigned bpr = 0;
   if (p->mtab) {
-    bpr = ((unsigned)p->n_node * (sftk::TAB_Q + 1) + 255) / 256;
+    bpr = ((unsigned)p->w_max * sftk::TAB_R * (sftk::TAB_Q + 1) + 255) / 256;
+    if (bpr < 1) bpr = 1;
     if ((double)bpr * (double)nn > 2.0e9) return fail(p, SFT_EUNSUPPORTED, "moment-table build grid too large");
   }
   const float2 *d_raw = (const float2 *)sft_bins;
@@ -440,9 +533,8 @@ SFT_API sft_status sft_append_sfts(sft_plan *p, int32_t channel, int64_t first_s
                                                                  p->us2 + (size_t)channel * N + a0);
     p->launches++;
     if (p->mtab) {
-      const size_t per_chan = N * (size_t)p->n_node * ((sftk::TAB_Q + 1) / 2), per_row = (size_t)p->n_node * ((sftk::TAB_Q + 1) / 2);
-      sftk::sft_mtab_kernel<<<(unsigned)(bpr * nn), 256, 0, p->stream>>>(D0, p->npair, p->n_node, p->d.K, p->ptab, bpr,
-                                                                        (float2 *)(p->mtab + (size_t)channel * per_chan + a0 * per_row));
+      sftk::sft_mtab_kernel<<<(unsigned)(bpr * nn), 256, 0, p->stream>>>(D0, p->npair, p->tblk, (int)a0, p->d.K, p->ptab, bpr,
+                                                                        (float2 *)(p->mtab + (size_t)channel * p->m_f4_chan));
       p->launches++;
     }
     ok(cudaGetLastError());
@@ -675,8 +767,10 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.depth = (float)p->d.resp_depth;
   k.mtab = p->mtab;
   k.htab = p->htab;
-  k.mrow = p->mtab ? (unsigned)p->n_node * (unsigned)((sftk::TAB_Q + 1) / 2) : 0u;
-  k.mchan = p->mtab ? (unsigned)(p->d.n_sft * p->n_node * ((sftk::TAB_Q + 1) / 2)) : 0u;
+  k.tblk = p->tblk;
+  k.banded = p->banded ? 1 : 0;
+  k.mrow0 = (unsigned)p->n_node * (unsigned)((sftk::TAB_Q + 1) / 2);
+  k.mchan = p->mtab ? (unsigned)p->m_f4_chan : 0u;
   k.hchan = (unsigned)(p->n_kc * sftk::HTAB_R * (sftk::HTAB_W / 4));
   k.b_table = p->mtab ? sftk::B_TABLE : -1.0f;
   k.b_table2 = p->mtab ? sftk::B_TABLE2 : -1.0f;
@@ -691,6 +785,9 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
 #endif
 #ifndef SFT_CREG_BNS
 #define SFT_CREG_BNS true   // the config-2/3/5 variant keeps the polynomial-track coefficients in registers
+#endif
+#ifndef SFT_CREG_MINB
+#define SFT_CREG_MINB 4     // resident blocks per SM of the CREG variants (128 registers)
 #endif
 #ifndef SFT_MINB
 #define SFT_MINB 5          // resident 128-thread blocks per SM the main kernel is compiled for
@@ -708,9 +805,11 @@ using CfgAny = sftk::Cfg<-1, -1, -1, 1, -1>;
 using CfgBNS32 = sftk::Cfg<1, 1, 0, 0, 1>;    // CfgBNS with the split-fp32 (double-float) phase track (config 5)
 
 // CREG: polynomial-track coefficients in registers (128 registers, 4 blocks per SM) instead of shared memory (96, 5 blocks)
-template <int KT, int CT, int MODE, class CFG, bool CREG = false>
+// BAND = false: specialisation for the full table layout (no sft_plan_set_table_track): row addresses from a constant-bank operand
+template <int KT, int CT, int MODE, class CFG, bool CREG = false, bool BAND = true>
 static void launch_variant(sft_plan *p, const KParams &k) {
-  auto kern = sftk::sft_main_kernel<KT, CT, MODE, CFG, CREG ? 4 : SFT_MINB, SFT_DUO, CREG>;
+  if (CREG && BAND && !p->banded) return launch_variant<KT, CT, MODE, CFG, CREG, false>(p, k);   // (only the CREG variants have it)
+  auto kern = sftk::sft_main_kernel<KT, CT, MODE, CFG, CREG ? SFT_CREG_MINB : SFT_MINB, SFT_DUO, CREG, BAND>;
   int per_sm = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, sftk::TILE, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
   long long blocks = (long long)p->n_sm * per_sm;
@@ -769,6 +868,7 @@ static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t
     if (want_chunks < 1) want_chunks = 1;
     chunk = (int)((k.n_sft + want_chunks - 1) / want_chunks);
     if (chunk < 32) chunk = 32;
+    chunk = ((chunk + 31) / 32) * 32;            // work units aligned to the blocks of 32 SFT slots of the fast path / table layout
   }
   if (cumulative) chunk = sftk::SUB;          // single-pass scan: one work unit = one block of 32 SFT slots (scan_store)
   if (chunk > k.n_sft && !cumulative) chunk = k.n_sft;

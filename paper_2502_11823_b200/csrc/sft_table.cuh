@@ -92,30 +92,33 @@ __global__ void sft_ptab_kernel(int K, float2 *ptab) {
   }
 }
 
-// Data-moment table of one channel: mtab[a][node][q], node = kcidx * TAB_R + cell, kcidx = kc - (k_lo - K).
-// 1-D grid of n_sft * bpr blocks (bpr = ceil(n_node * 8 / 256) blocks per SFT row); the padded whitened row of SFT a is read from copy 0 of the
-// pair-planar store (neighbouring threads share a window: L1 broadcast), ptab through L1 (consecutive
-// threads read consecutive entries).
-__global__ void __launch_bounds__(256) sft_mtab_kernel(const float4 *Dp0, int npair, int n_node, int K, const float2 *ptab,
-                                                       unsigned bpr, float2 *mtab) {
-  const unsigned a = blockIdx.x / bpr, bx = blockIdx.x - a * bpr;
-  const float4 *src = Dp0 + (size_t)a * npair;
+// Data-moment table of one channel.  Layout per block of 32 SFT slots, tblk[a >> 5] = {float4 index of the block's first row,
+// kb, W, float4 per row}: the row of SFT a holds the nodes of the W window positions kb .. kb + W - 1 (counted from k_lo - K),
+// node = (kcidx - kb) * TAB_R + cell, TAB_Q + 1 complex64 moments each.  Grid: n_rows * bpr blocks (bpr = blocks per row for
+// the widest block); `a_first` = SFT slot of the first row handled (sft_append_sfts builds a range), Dp0 = its padded whitened
+// row in copy 0 of the pair-planar store (neighbouring threads share a window: L1 broadcast), ptab through L1.
+__global__ void __launch_bounds__(256) sft_mtab_kernel(const float4 *Dp0, int npair, const int4 *tblk, int a_first, int K,
+                                                       const float2 *ptab, unsigned bpr, float2 *mtab) {
+  const unsigned al = blockIdx.x / bpr, bx = blockIdx.x - al * bpr;
+  const int a = a_first + (int)al;
+  const int4 tb = __ldg(tblk + (a >> 5));
+  const float4 *src = Dp0 + (size_t)al * npair;
   constexpr int nq = TAB_Q + 1, per_bin = TAB_R * nq;
   const int o = bx * blockDim.x + threadIdx.x;                // (node, q) flattened
-  if (o >= n_node * nq) return;
-  const int kcidx = o / per_bin, cq = o - kcidx * per_bin;     // cq = cell * nq + q
+  if (o >= tb.z * per_bin) return;
+  const int kcl = o / per_bin, cq = o - kcl * per_bin;         // cq = cell * nq + q
   const float2 *pp = ptab + cq;
   float re = 0.f, im = 0.f;
   const int nb = 2 * K + 1;
   for (int mi = 0; mi < nb; ++mi) {
-    const int j = kcidx + 2 + mi;                              // window start j0 = kcidx + 2
+    const int j = tb.y + kcl + 2 + mi;                         // window start j0 = kcidx + 2
     const float4 d4 = __ldg(src + (j >> 1));
     const float dx = (j & 1) ? d4.y : d4.x, dy = (j & 1) ? d4.w : d4.z;
     const float2 pv = __ldg(pp + (size_t)mi * per_bin);
     re = fmaf(dx, pv.x, re); re = fmaf(-dy, pv.y, re);
     im = fmaf(dx, pv.y, im); im = fmaf(dy, pv.x, im);
   }
-  mtab[((size_t)a * n_node) * nq + o] = make_float2(re, im);
+  mtab[2 * ((size_t)(unsigned)tb.x + (size_t)(a & 31) * (unsigned)tb.w) + o] = make_float2(re, im);
 }
 
 // <h,h> table of one channel: htab[nodeH][HTAB_W], nodeH = kcidx * HTAB_R + cell.  One block per node,

@@ -476,6 +476,59 @@ def test_error_paths_leave_outputs_untouched(et_small):
         assert bool(torch.isnan(xd).all())
 
 
+def test_table_track_banded_tables(et_small):
+    """sft_plan_set_table_track: moment tables only along the track of a fiducial template (the SFTs serve "any template
+    within a given parameter-space region").  (i) For the +-1e-3 bank the banded tables give bit-identical results to the full
+    ones, for both calls, at a fraction of the memory, and the same evaluator paths; (ii) a wide bank, most of whose lanes
+    leave the band of the track, falls back to the direct evaluator for those SFTs and still matches the oracle; (iii) a plan
+    whose full tables could never fit (4000-bin band x 200,000 SFTs: 411 GB) gets tables with a track."""
+    api = _api()
+    w = et_small
+    n = w.desc["n_sft"]
+    P = np.ascontiguousarray(w.params)
+    nT = len(P)
+    def run(plan):
+        xh, hh, xi = np.empty(nT), np.empty(nT), np.empty(nT)
+        kc = np.empty((nT, 1, n), np.int32)
+        plan.inner_products(P, xh, hh, xi, kc)
+        paths = plan.path_counts()
+        snr = np.empty((nT, n), np.float32)
+        plan.cumulative_snr(P, snr)
+        xh2, hh2 = np.empty(nT), np.empty(nT)
+        plan.inner_products(P, xh2, hh2)
+        return xh, hh, xi, kc, snr, xh2, hh2, paths
+    with api.plan_from_workload(w) as plan:
+        full = run(plan)
+        full_bytes = plan.table_bytes()
+        plan.set_table_track(w.injection, 3)                      # replaces the tables: data must be loaded again
+        with pytest.raises(api.SftError) as ei:
+            plan.inner_products(P, np.empty(nT), np.empty(nT))
+        assert "SFT_ENODATA" in str(ei.value)
+    with api.plan_from_workload(w, table_track=(w.injection, 3)) as plan:
+        band = run(plan)
+        assert 0 < plan.table_bytes() < 0.2 * full_bytes
+    for i, (a, b) in enumerate(zip(full[:-1], band[:-1])):
+        if i == 4:          # the SNR matrix: the two layouts run two instantiations of the cumulative kernel (fp32 rounding of the running sums)
+            assert np.abs(a - b).max() <= 2e-6 * np.abs(a).max()
+        else:
+            assert np.array_equal(a, b)
+    assert full[-1] == band[-1] and band[-1]["table"] > 0
+    ww = wl.et_bns_wide_bank(w, 96)
+    ww.params = np.concatenate([w.params[:64], ww.params])          # two warps inside the band of the track, three wide ones
+    o, xx, _, _ = _oracle(ww)
+    g = _run_gpu(ww, table_track=(w.injection, 3))
+    _check(ww, g, o, xx)
+    assert g["paths"]["table"] > 0 and g["paths"]["series1"] + g["paths"]["series2"] + g["paths"]["series3"] > 0
+    desc = dict(n_channels=1, n_sft=200000, t_sft=8.0, fs=2048.0, t0=0.0, k_lo=10, k_hi=4010, K=8, kernel="fresnel",
+                pn1=1, response="none", f_lo=0.0, f_hi=1e9, f_ref=10.0)
+    fid = w.injection.copy()
+    fid[2] = 200000 * 8.0 + 300.0
+    with api.Plan(dict(desc, evaluator="auto")) as plan:
+        assert plan.table_bytes() == 0
+        plan.set_table_track(fid, 8)
+        assert 0 < plan.table_bytes() < 8e9
+
+
 def test_evaluator_selection_by_memory():
     """SFT_EVAL_AUTO falls back to the direct evaluator when the moment tables would not fit in a quarter of the
     free device memory; SFT_EVAL_TABLE reports SFT_ENOMEM instead."""
