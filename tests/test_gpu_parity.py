@@ -519,6 +519,24 @@ def test_table_track_banded_tables(et_small):
     g = _run_gpu(ww, table_track=(w.injection, 3))
     _check(ww, g, o, xx)
     assert g["paths"]["table"] > 0 and g["paths"]["series1"] + g["paths"]["series2"] + g["paths"]["series3"] > 0
+    # two channels with the annual response (config-4 recipe), tables along the injection's track
+    w4 = wl.config4(n_templates=100)
+    o4, xx4, _, _ = _oracle(w4)
+    g4 = _run_gpu(w4, table_track=(w4.injection, 2))
+    _check(w4, g4, o4, xx4)
+    assert g4["paths"]["table"] > 0
+    # streaming append into banded tables = one-shot load
+    bins, scale, shape = np.ascontiguousarray(w.bins[0], np.complex64), np.ascontiguousarray(w.psd_scale[0]), np.ascontiguousarray(w.psd_shape[0])
+    with api.Plan(w.desc) as plan:
+        plan.set_table_track(w.injection, 3)
+        ps, pb = scale.copy(), bins.copy()
+        ps[500:] = 0.0
+        pb[500:] = 0.0
+        plan.load_data(0, pb, ps, shape)
+        plan.append_sfts(0, 500, np.ascontiguousarray(bins[500:]), np.ascontiguousarray(scale[500:]))
+        xh, hh = np.empty(nT), np.empty(nT)
+        plan.inner_products(P, xh, hh)
+    assert np.array_equal(xh, band[5]) and np.array_equal(hh, band[6])
     desc = dict(n_channels=1, n_sft=200000, t_sft=8.0, fs=2048.0, t0=0.0, k_lo=10, k_hi=4010, K=8, kernel="fresnel",
                 pn1=1, response="none", f_lo=0.0, f_hi=1e9, f_ref=10.0)
     fid = w.injection.copy()
