@@ -17,6 +17,10 @@ order (citations ``P:NNN`` are line numbers of ``/root/reference/PAPER.md``):
   time-domain / full-band inner products Eq.(1), Eq.(14) P:149.
 * ``oracle.inner``     – the method itself, Eq.(20)/(24)/(35) P:178-259 with the band
   truncation of P:238, and the cumulative-over-SFTs variant.
+* ``oracle.stats``     – log-likelihood Eq.(2), phase-maximised statistic Eq.(7)-(9), F-statistic Eq.(10)-(13) P:63-122
+  (all 4 + 10 products bin by bin, plain 4 x 4 solve).
+* ``oracle.accuracy``  – the accuracy experiment of section IV: ``<d,h>`` by direct integration and ``r`` of Eq.(36) P:274.
+  (``oracle.sft`` also holds the per-SFT noise-level estimate of P:139, ``oracle.inner`` the validity measure of Eq.(33).)
 
 Pins (tests/test_oracle_*.py, all ``-m "not gpu"``) tie each function to something
 other than itself; a function without such a pin says "parity unpinned" in its
