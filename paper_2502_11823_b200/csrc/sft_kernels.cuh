@@ -262,14 +262,15 @@ __global__ void sft_tmpl_kernel(const KParams p, double *td, float *tf) {
   }
 }
 
-// Lanes beyond the last template get tau0 = -1: never active.
+// Lanes beyond the last template run as copies of the last one (so that a ragged last warp, or a bank smaller than a warp, still
+// takes the clean-block path); nothing of theirs is ever stored or counted (every output is guarded by t < nT).
 template <int CT>
 __device__ __forceinline__ void tmpl_load(const KParams &p, long long t, Tmpl &tm) {
   const bool ok = t < p.nT;
-  const long long n = p.nT, tt = ok ? t : 0;
+  const long long n = p.nT, tt = ok ? t : n - 1;
   const double *d = p.td + tt;
   const float *f = p.tf + tt;
-  tm.tau0 = ok ? __ldg(d + TD_TAU0 * n) : -1.0;
+  tm.tau0 = __ldg(d + TD_TAU0 * n);
   tm.cTheta = __ldg(d + TD_CTHETA * n);
   tm.phic_cyc = __ldg(d + TD_PHIC * n);
   tm.cphase = __ldg(d + TD_CPHASE * n);
@@ -1450,7 +1451,7 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
       int np_ = 0;
 #pragma unroll
       for (int c = 0; c < CT; ++c) np_ += (usA[c] > 0.f) + (vB && usB[c] > 0.f);
-      n_path[PATH_TABLE] += 32u * (unsigned)np_;
+      n_path[PATH_TABLE] += (unsigned)__popc(__ballot_sync(0xffffffffu, t < p.nT)) * (unsigned)np_;
     }
     if (CFG::KC && kcp && t < p.nT) {
 #pragma unroll
@@ -1569,7 +1570,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
             us2[c] = __ldg(usp + c * p.n_sft);
             any |= us2[c] > 0.f;                                   // warp-uniform
           }
-          const bool go = any && tr.active;
+          const bool go = any && tr.active && t < p.nT;
           const float ab = (go && cfg_kernel<CFG>(p) == 1) ? fabsf(tr.b) : 0.f;
           // the table rows of this SFT (block alpha >> 5) and whether the windows of all active lanes lie inside them
           if (!one_blk && p.mtab) {
@@ -1590,7 +1591,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
               us2b[c] = __ldg(usp + c * p.n_sft + 1);
               anyb |= us2b[c] > 0.f;
             }
-            gob = anyb && tr2.active;
+            gob = anyb && tr2.active && t < p.nT;
             const float abb = (gob && cfg_kernel<CFG>(p) == 1) ? fabsf(tr2.b) : 0.f;
             const float bm2 = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(ab, abb))));
             const int kcb = tr2.kc - p.kwin0 - 2;
