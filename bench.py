@@ -444,11 +444,11 @@ def run_ours(args, rank, world, local_rank):
 # DRAM bytes (read + write) of one main-kernel launch, from the committed ncu --set full captures (dram__bytes_read.sum +
 # dram__bytes_write.sum): NOT measured by this run - the source capture is named in roofline.traffic_source.
 NCU_TRAFFIC = {
-    ("config2-F", "auto"): (2.103296e6 + 7.424e3, "profiles/r02_main_kernel.md"),
-    ("config2-F", "table"): (2.103296e6 + 7.424e3, "profiles/r02_main_kernel.md"),
+    ("config2-F", "auto"): (2.103552e6 + 10.496e3, "profiles/r02_main_kernel.md"),
+    ("config2-F", "table"): (2.103552e6 + 10.496e3, "profiles/r02_main_kernel.md"),
     ("config2-F", "direct"): (8.213504e6 + 10.752e3, "profiles/r01d_kernel_v7_tables.md"),
-    ("config3-F", "auto"): (5.682176e6 + 872.57728e6, "profiles/r02_main_kernel.md"),
-    ("config4", "auto"): (6.582272e6 + 2.335232e6, "profiles/r02_main_kernel.md"),
+    ("config3-F", "auto"): (5.656064e6 + 872.535296e6, "profiles/r02_main_kernel.md"),
+    ("config4", "auto"): (6.583040e6 + 2.189312e6, "profiles/r02_main_kernel.md"),
 }
 
 # Algorithmic work per active pair and the ALU peak: DESIGN.md section 7.
@@ -477,13 +477,13 @@ def alg_instr_per_pair(path, K, C):
 
 def kernel_instr_per_pair(path, K, C, strict=False):
     """What the CURRENT kernel issues per pair on its common path (clean block, polynomial track, tier-1 tables; counted
-    in the SASS of the hot loop, profiles/r02a_main_fastpath.md): track 29 (11 fp64, 3 conversions, 13 fp32, 2 constant
-    loads), S1 29 C (19 packed FMAs + 10 scalings), H 8 C, 6 C table loads, prefactor 15 + 12 (C - 1), accumulation 3;
-    plus - not in the strict count - node / address arithmetic 19 C and the loop over the presence mask 9.  Other paths as
-    in alg_instr_per_pair with the cheaper track (-21) where the block is clean."""
+    in the SASS of the hot loop, profiles/r02_main_kernel.md: 225 instructions per two SFTs): track 29 (11 fp64, 3
+    conversions, 13 fp32, 2 constant loads), S1 29 C (19 packed FMAs + 10 scalings), H 4 C (compact node), 5 C table loads,
+    prefactor 15 + 12 (C - 1), accumulation 3; plus - not in the strict count - node / address arithmetic 18 C and the loop
+    over the presence mask 9.5.  Other paths as in alg_instr_per_pair."""
     if path == "table":
-        core = 29 + (29 + 8 + 6) * C + 15 + 12 * (C - 1) + 3
-        return core if strict else core + 19 * C + 9
+        core = 29 + (29 + 4 + 5) * C + 15 + 12 * (C - 1) + 3
+        return core if strict else core + 18 * C + 9.5
     full = alg_instr_per_pair(path, K, C)
     return full - 34 if strict else full           # strict: without the 13 loop + 21 node/constant instructions
 

@@ -72,7 +72,9 @@ struct KParams {
   unsigned long long *path_counts;   // nullable [PATH_N]: active pairs per evaluator path (diagnostic)
   // moment-table evaluator (sft_table.cuh); mtab == nullptr: direct evaluator only
   const float4 *mtab;      // [C][n_sft][n_node][4]   8 complex64 moments per node, node = kcidx * TAB_R + cell
-  const float4 *htab;      // [C][n_kc * HTAB_R][4]   <h,h> polynomial per node
+  const float4 *htab;      // [C][n_kc * HTAB_R][4]   <h,h> polynomial per node (tier 2)
+  const float4 *htab1;     // [C][n_kc * HT1_R]       compact tier-1 <h,h> node {h_00, h_10, h_20, h_02}
+  unsigned h1chan;         // entries of htab1 per channel
   // The moment table is laid out per block of 32 SFT slots (tblk[a >> 5]): rows of W window positions starting at
   // position kb (counted from k_lo - K), so that a bank around a known track needs only the band the track sweeps
   // (sft_plan_set_table_track); without a track every block covers all n_kc positions.
@@ -715,8 +717,8 @@ template <int CT, int TIER>
 struct TableData {
   static constexpr int Q = TIER == 1 ? TAB_Q1 : TAB_Q;          // highest moment
   static constexpr int NL = (Q + 1) / 2;                         // float4 loads of moments per channel
-  static constexpr int NHB = TIER == 1 ? 2 : HTAB_NB;            // powers of beta^2 in H
-  static constexpr int NHL = (NHB * (HTAB_P + 1) + 3) / 4;       // float4 loads of H coefficients
+  static constexpr int NHB = HTAB_NB;                            // powers of beta^2 in H (tier 2)
+  static constexpr int NHL = TIER == 1 ? 1 : (NHB * (HTAB_P + 1) + 3) / 4;   // float4 loads of H coefficients (tier 1: the compact node)
   float4 Mq[CT][NL], Hq[CT][NHL];
   float a, aH, be;
 };
@@ -730,22 +732,25 @@ __device__ __forceinline__ void table_load(const KParams &p, float xp, float b, 
   // BEFORE the magic constant: 31.5 + 1.5 * 2^23 is not representable (ulp 1) and would turn the floor into a round-to-
   // nearest, i.e. nodes half a cell off.  (At an exact cell edge the rounding may pick either neighbour: same bound.)
   constexpr float RM = 12582912.0f;
-  float cm = fmaf(xp, (float)HTAB_R, 0.5f * HTAB_R - 0.5f) + RM;
-  cm = fminf(fmaxf(cm, RM), RM + (float)(HTAB_R - 1));
-  const int cellH = __float_as_int(cm) & (HTAB_R - 1);
-  const int cell = cellH >> HTAB_SHIFT;
+  constexpr int HR = TIER == 1 ? HT1_R : HTAB_R, HS = TIER == 1 ? HT1_SHIFT : HTAB_SHIFT;   // tier 1: compact node on the finer grid
+  float cm = fmaf(xp, (float)HR, 0.5f * HR - 0.5f) + RM;
+  cm = fminf(fmaxf(cm, RM), RM + (float)(HR - 1));
+  const int cellH = __float_as_int(cm) & (HR - 1);
+  const int cell = cellH >> HS;
   const float cHf = cm - RM;                                   // (float)cellH
   const float4 *mp = Mrow + (unsigned)((kcidx - kb) * TAB_R + cell) * (unsigned)((TAB_Q + 1) / 2);    // row of the block: positions kb ...
-  const float4 *hp = p.htab + (unsigned)(kcidx * HTAB_R + cellH) * (unsigned)(HTAB_W / 4);
+  const float4 *hp = TIER == 1 ? p.htab1 + (unsigned)(kcidx * HT1_R + cellH)
+                               : p.htab + (unsigned)(kcidx * HTAB_R + cellH) * (unsigned)(HTAB_W / 4);
+  const unsigned hch = TIER == 1 ? p.h1chan : p.hchan;
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
 #pragma unroll
     for (int i = 0; i < TableData<CT, TIER>::NL; ++i) d.Mq[c][i] = __ldg(mp + c * p.mchan + i);
 #pragma unroll
-    for (int i = 0; i < TableData<CT, TIER>::NHL; ++i) d.Hq[c][i] = __ldg(hp + c * p.hchan + i);
+    for (int i = 0; i < TableData<CT, TIER>::NHL; ++i) d.Hq[c][i] = __ldg(hp + c * hch + i);
   }
   // a = 2 pi (xp - node centre):  centre_H = (cellH + 1/2)/HTAB_R - 1/2,  centre_M = (cell + 1/2)/TAB_R - 1/2
-  d.aH = fmaf(cHf, -(2.0f * PI_F) / HTAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / HTAB_R)));
+  d.aH = fmaf(cHf, -(2.0f * PI_F) / HR, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / HR)));
   d.a = fmaf((float)cell, -(2.0f * PI_F) / TAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / TAB_R)));
   d.be = PI_F * b;
 }
@@ -779,15 +784,19 @@ __device__ __forceinline__ void table_math(const TableData<CT, TIER> &d, float (
     }
     s1r[c] = S.x;
     s1i[c] = S.y;
-    // H = sum_P aH^P sum_N beta^(2N) h_{P,2N};  floats: [N][P], P fastest
+    // H = sum_P aH^P sum_N beta^(2N) h_{P,2N};  floats: [N][P], P fastest (tier 1: the compact node {h_00, h_10, h_20, h_02})
     const float *hf = (const float *)&d.Hq[c][0];
     float h = 0.f;
+    if (TIER == 1) {
+      h = fmaf(be2, hf[3], fmaf(fmaf(hf[2], aH, hf[1]), aH, hf[0]));
+    } else {
 #pragma unroll
-    for (int P = HTAB_P; P >= 0; --P) {
-      float g = hf[(NHB - 1) * (HTAB_P + 1) + P];
+      for (int P = HTAB_P; P >= 0; --P) {
+        float g = hf[(NHB - 1) * (HTAB_P + 1) + P];
 #pragma unroll
-      for (int N = NHB - 2; N >= 0; --N) g = fmaf(g, be2, hf[N * (HTAB_P + 1) + P]);
-      h = P == HTAB_P ? g : fmaf(h, aH, g);
+        for (int N = NHB - 2; N >= 0; --N) g = fmaf(g, be2, hf[N * (HTAB_P + 1) + P]);
+        h = P == HTAB_P ? g : fmaf(h, aH, g);
+      }
     }
     s2[c] = h;
   }
@@ -831,16 +840,21 @@ __device__ __forceinline__ void table_math2(const TableData<CT, TIER> &dA, const
     s1rB[c] = SB.x; s1iB[c] = SB.y;
     const float *hA = (const float *)&dA.Hq[c][0], *hB = (const float *)&dB.Hq[c][0];
     float ha = 0.f, hb = 0.f;
+    if (TIER == 1) {
+      ha = fmaf(be2A, hA[3], fmaf(fmaf(hA[2], dA.aH, hA[1]), dA.aH, hA[0]));
+      hb = fmaf(be2B, hB[3], fmaf(fmaf(hB[2], dB.aH, hB[1]), dB.aH, hB[0]));
+    } else {
 #pragma unroll
-    for (int P = HTAB_P; P >= 0; --P) {
-      float gA = hA[(NHB - 1) * (HTAB_P + 1) + P], gB = hB[(NHB - 1) * (HTAB_P + 1) + P];
+      for (int P = HTAB_P; P >= 0; --P) {
+        float gA = hA[(NHB - 1) * (HTAB_P + 1) + P], gB = hB[(NHB - 1) * (HTAB_P + 1) + P];
 #pragma unroll
-      for (int N = NHB - 2; N >= 0; --N) {
-        gA = fmaf(gA, be2A, hA[N * (HTAB_P + 1) + P]);
-        gB = fmaf(gB, be2B, hB[N * (HTAB_P + 1) + P]);
+        for (int N = NHB - 2; N >= 0; --N) {
+          gA = fmaf(gA, be2A, hA[N * (HTAB_P + 1) + P]);
+          gB = fmaf(gB, be2B, hB[N * (HTAB_P + 1) + P]);
+        }
+        ha = P == HTAB_P ? gA : fmaf(ha, dA.aH, gA);
+        hb = P == HTAB_P ? gB : fmaf(hb, dB.aH, gB);
       }
-      ha = P == HTAB_P ? gA : fmaf(ha, dA.aH, gA);
-      hb = P == HTAB_P ? gB : fmaf(hb, dB.aH, gB);
     }
     s2A[c] = ha;
     s2B[c] = hb;
@@ -1257,22 +1271,22 @@ __device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int 
 template <int CT>
 __device__ __forceinline__ void table_load_fast(const KParams &p, float xp, float b, int kcidx, unsigned row, TableData<CT, 1> &d) {
   constexpr float RM = 12582912.0f;
-  const float cm = fmaf(xp, (float)HTAB_R * (1.0f - 9.5367431640625e-7f), 0.5f * HTAB_R - 0.5f) + RM;
+  const float cm = fmaf(xp, (float)HT1_R * (1.0f - 9.5367431640625e-7f), 0.5f * HT1_R - 0.5f) + RM;
   const unsigned cb = __float_as_uint(cm);
-  const unsigned cellH = cb & (unsigned)(HTAB_R - 1);
+  const unsigned cellH = cb & (unsigned)(HT1_R - 1);
   const float cHf = cm - RM;                                                      // (float)cellH
-  const float cSf = __uint_as_float(cb & ~(unsigned)((1 << HTAB_SHIFT) - 1)) - RM;   // cell << HTAB_SHIFT, cell = data-moment node
-  const float4 *mp = p.mtab + (row + ((unsigned)kcidx * TAB_R + (cellH >> HTAB_SHIFT)) * (unsigned)((TAB_Q + 1) / 2));
-  const float4 *hp = p.htab + ((unsigned)kcidx * HTAB_R + cellH) * (unsigned)(HTAB_W / 4);
+  const float cSf = __uint_as_float(cb & ~(unsigned)((1 << HT1_SHIFT) - 1)) - RM;    // cell << HT1_SHIFT, cell = data-moment node
+  const float4 *mp = p.mtab + (row + ((unsigned)kcidx * TAB_R + (cellH >> HT1_SHIFT)) * (unsigned)((TAB_Q + 1) / 2));
+  const float4 *hp = p.htab1 + ((unsigned)kcidx * HT1_R + cellH);
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
 #pragma unroll
     for (int i = 0; i < TableData<CT, 1>::NL; ++i) d.Mq[c][i] = __ldg(mp + c * p.mchan + i);
 #pragma unroll
-    for (int i = 0; i < TableData<CT, 1>::NHL; ++i) d.Hq[c][i] = __ldg(hp + c * p.hchan + i);
+    for (int i = 0; i < TableData<CT, 1>::NHL; ++i) d.Hq[c][i] = __ldg(hp + c * p.h1chan + i);
   }
-  d.aH = fmaf(cHf, -(2.0f * PI_F) / HTAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / HTAB_R)));
-  d.a = fmaf(cSf, -(2.0f * PI_F) / HTAB_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / TAB_R)));
+  d.aH = fmaf(cHf, -(2.0f * PI_F) / HT1_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / HT1_R)));
+  d.a = fmaf(cSf, -(2.0f * PI_F) / HT1_R, fmaf(xp, 2.0f * PI_F, (2.0f * PI_F) * (0.5f - 0.5f / TAB_R)));
   d.be = PI_F * b;
 }
 

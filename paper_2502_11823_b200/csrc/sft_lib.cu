@@ -46,6 +46,7 @@ struct sft_plan {
   float *tf = nullptr; size_t tf_bytes = 0;
   float4 *mtab = nullptr;                              // [C][n_sft][n_node][4] data-moment table (sft_table.cuh), or null
   float4 *htab = nullptr;                              // [C][n_kc * HTAB_R][4] <h,h> table
+  float4 *htab1 = nullptr;                             // [C][n_kc * HT1_R] compact tier-1 <h,h> table
   float2 *ptab = nullptr;                              // [(2K+1)][TAB_R][TAB_Q+1] kernel moments at the nodes
   int n_kc = 0, n_node = 0;
   int4 *tblk = nullptr;                                // [ceil(n_sft/32)] layout of the moment table per block of 32 SFT slots (sft_kernels.cuh)
@@ -206,6 +207,7 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
     if (st != SFT_OK) memcpy(g_create_err, p->err, 512);
     if (st == SFT_OK) {
       alloc((void **)&p->htab, C * (size_t)p->n_kc * sftk::HTAB_R * sftk::HTAB_W * sizeof(float));
+      alloc((void **)&p->htab1, C * (size_t)p->n_kc * sftk::HT1_R * sizeof(float4));
       alloc((void **)&p->ptab, (size_t)(2 * d.K + 1) * sftk::TAB_R * (sftk::TAB_Q + 1) * sizeof(float2));
       if (st == SFT_OK) {
         const int n = (2 * d.K + 1) * sftk::TAB_R;
@@ -256,7 +258,7 @@ SFT_API sft_status sft_plan_destroy(sft_plan *p) {
   cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->scan);
   if (p->h_pin) cudaFreeHost(p->h_pin);
   cudaFree(p->td); cudaFree(p->tf); cudaFree(p->counter); cudaFree(p->path_counts);
-  cudaFree(p->mtab); cudaFree(p->htab); cudaFree(p->ptab); cudaFree(p->tblk);
+  cudaFree(p->mtab); cudaFree(p->htab); cudaFree(p->htab1); cudaFree(p->ptab); cudaFree(p->tblk);
   if (p->ev0) cudaEventDestroy(p->ev0);
   if (p->ev1) cudaEventDestroy(p->ev1);
   delete p;
@@ -468,7 +470,9 @@ SFT_API sft_status sft_load_data(sft_plan *p, int32_t channel, const float *sft_
           p->Dp + (size_t)channel * N * npair, p->npair, p->tblk, 0, p->d.K, p->ptab, bpr, (float2 *)(p->mtab + (size_t)channel * p->m_f4_chan));
       sftk::sft_htab_kernel<<<(unsigned)(p->n_kc * sftk::HTAB_R), 64, 0, p->stream>>>(
           p->ubp + (size_t)channel * npair, p->d.K, (float *)(p->htab + (size_t)channel * p->n_kc * sftk::HTAB_R * (sftk::HTAB_W / 4)));
-      p->launches += 2;
+      sftk::sft_htab1_kernel<<<(unsigned)(p->n_kc * sftk::HT1_R), 64, 0, p->stream>>>(
+          p->ubp + (size_t)channel * npair, p->d.K, p->htab1 + (size_t)channel * p->n_kc * sftk::HT1_R);
+      p->launches += 3;
     }
     ok(cudaGetLastError());
   }
@@ -767,6 +771,8 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.depth = (float)p->d.resp_depth;
   k.mtab = p->mtab;
   k.htab = p->htab;
+  k.htab1 = p->htab1;
+  k.h1chan = (unsigned)(p->n_kc * sftk::HT1_R);
   k.tblk = p->tblk;
   k.banded = p->banded ? 1 : 0;
   k.mrow0 = (unsigned)p->n_node * (unsigned)((sftk::TAB_Q + 1) / 2);

@@ -23,11 +23,12 @@ def test_counts_are_ordered_and_mix_weighted():
             strict = bench.kernel_instr_per_pair(path, K, C, strict=True)
             assert 0 < strict < kern <= fixed, (path, K, C)
     paths = dict(series0=0, series1=0, series2=0, series3=0, fresnel=106496, table=39080960, table2=626688)   # config 2-F
-    r = bench.roofline(_w(), 39813120 + 0 * 106496, 0.2623, paths, "auto", dict(ffma=34700.0, table_mix_ipc=0.9))
+    r = bench.roofline(_w(), 39813120, 0.2588, paths, "auto", dict(ffma=34700.0, table_mix_ipc=0.9))
     assert abs(r["alg_instr_per_pair"] - 149.42) < 0.05
     assert r["frac_strict"] < r["frac_kernel_count"] < r["frac"] < r["frac_of_measured_ffma_issue"] < r["frac_of_mix_ceiling"] < 1.0
     assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and abs(r["peak"] - 148 * 4 * 32 * 1.965) < 1e-9
-    assert abs(r["frac"] - 0.609) < 0.003                       # the committed line (profiles/r02_bench.json.txt)
+    assert abs(r["frac"] - 0.618) < 0.003                       # the committed line (profiles/r02_bench.json.txt)
+    assert abs(r["kernel_instr_per_pair"] - 117.5) < 0.5        # 112.5 on the common path (225 SASS instructions per two SFTs), path-mix average
     assert bench.roofline(_w(), 1, None, paths) is None and bench.roofline(_w(), 1, 0.1, None) is None
 
 
@@ -36,4 +37,4 @@ def test_traffic_figures_cite_committed_captures():
         assert bytes_ > 0 and os.path.exists(os.path.join(ROOT, src)), src
     txt = open(os.path.join(ROOT, "profiles", "r02_main_kernel.md")).read()
     m = re.search(r"`dram__bytes_read.sum` \| Mbyte \| ([0-9.]+)", txt)
-    assert m and abs(float(m.group(1)) * 1e6 - (bench.NCU_TRAFFIC[("config2-F", "auto")][0] - 7.424e3)) < 2e5
+    assert m and abs(float(m.group(1)) * 1e6 - bench.NCU_TRAFFIC[("config2-F", "auto")][0]) < 2e5
