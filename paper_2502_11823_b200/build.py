@@ -12,7 +12,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsft_b200.so")
-SOURCES = [os.path.join(CSRC, "sft_lib.cu")]
+SOURCES = [os.path.join(CSRC, f) for f in ("sft_lib.cu", "sft_var_bns.cu", "sft_var_misc.cu", "sft_var_lisa.cu", "sft_var_any1.cu", "sft_var_any2.cu", "sft_var_any3.cu",
+                                             "sft_var_any4.cu")]
+OBJ = os.path.join(HERE, "_obj")
 
 
 def deps():
@@ -23,8 +25,7 @@ def deps():
 
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",
-              "-cudart", "static"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
 
 def nvcc():
@@ -42,18 +43,33 @@ def up_to_date():
 
 
 def build(force=False, verbose=False, extra=()):
-    """Compiles the library if it is missing or older than its sources.  Returns its path."""
+    """Compiles the library if it is missing or older than its sources.  The variants of the fused kernel are spread over
+    several translation units, compiled side by side (one nvcc process each), then linked.  Returns the library's path."""
     if not force and up_to_date():
         return LIB
     extra = list(extra) + os.environ.get("SFT_NVCC_EXTRA", "").split()      # e.g. -DSFT_MINB=4
-    cmd = [nvcc()] + NVCC_FLAGS + extra + ["-o", LIB] + SOURCES
-    if verbose:
-        print(" ".join(cmd), flush=True)
+    os.makedirs(OBJ, exist_ok=True)
+    procs = []
+    for src in SOURCES:
+        obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")
+        cmd = [nvcc()] + NVCC_FLAGS + extra + ["-c", "-o", obj, src]
+        if verbose:
+            print(" ".join(cmd), flush=True)
+        procs.append((obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
+    objs, log, bad = [], "", False
+    for obj, pr in procs:
+        out, _ = pr.communicate()
+        log += out
+        bad |= pr.returncode != 0
+        objs.append(obj)
+    if bad:
+        raise RuntimeError("nvcc failed:\n" + log)
+    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static", "-o", LIB] + objs
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + r.stdout + r.stderr)
-    if verbose and (r.stdout or r.stderr):
-        print(r.stdout + r.stderr)
+        raise RuntimeError("link failed:\n" + r.stdout + r.stderr)
+    if verbose and log:
+        print(log)
     return LIB
 
 

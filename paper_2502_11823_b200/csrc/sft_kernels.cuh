@@ -222,6 +222,7 @@ struct Tmpl {
   TmplS s;
 };
 
+#ifndef SFT_MAIN_ONLY      // (the translation units that only instantiate sft_main_kernel skip the small kernels)
 // One thread per template, once per call.
 __global__ void sft_tmpl_kernel(const KParams p, double *td, float *tf) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -263,6 +264,8 @@ __global__ void sft_tmpl_kernel(const KParams p, double *td, float *tf) {
     tf[(TF_AE + 2 * c + 1) * n + t] = ae.y;
   }
 }
+
+#endif  // SFT_MAIN_ONLY
 
 // Lanes beyond the last template run as copies of the last one (so that a ragged last warp, or a bank smaller than a warp, still
 // takes the clean-block path); nothing of theirs is ever stored or counted (every output is guarded by t < nT).
@@ -1060,9 +1063,9 @@ constexpr double POLY_Y3_MAX = 5e-4 / 4096.0;                   //              
 constexpr double POLY_EPS_MAX = 0.03 / 16.0;                    // amplitude after u^3: quartic term 0.08 (16 eps)^4 <= 7e-8
 
 // u = j - 16 for slot j of a block: as double, and {u, u^3} as floats
-__constant__ double c_ud[SUB] = {-16., -15., -14., -13., -12., -11., -10., -9., -8., -7., -6., -5., -4., -3., -2., -1.,
+static __constant__ double c_ud[SUB] = {-16., -15., -14., -13., -12., -11., -10., -9., -8., -7., -6., -5., -4., -3., -2., -1.,
                                  0.,   1.,   2.,   3.,   4.,   5.,   6.,   7.,  8.,  9.,  10., 11., 12., 13., 14., 15.};
-__constant__ float2 c_uf[SUB] = {{-16.f, -4096.f}, {-15.f, -3375.f}, {-14.f, -2744.f}, {-13.f, -2197.f}, {-12.f, -1728.f}, {-11.f, -1331.f},
+static __constant__ float2 c_uf[SUB] = {{-16.f, -4096.f}, {-15.f, -3375.f}, {-14.f, -2744.f}, {-13.f, -2197.f}, {-12.f, -1728.f}, {-11.f, -1331.f},
                                  {-10.f, -1000.f}, {-9.f, -729.f},   {-8.f, -512.f},   {-7.f, -343.f},   {-6.f, -216.f},   {-5.f, -125.f},
                                  {-4.f, -64.f},    {-3.f, -27.f},    {-2.f, -8.f},     {-1.f, -1.f},     {0.f, 0.f},       {1.f, 1.f},
                                  {2.f, 8.f},       {3.f, 27.f},      {4.f, 64.f},      {5.f, 125.f},     {6.f, 216.f},     {7.f, 343.f},
@@ -1720,6 +1723,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
   }
 }
 
+#ifndef SFT_MAIN_ONLY
 // Sum of the chunk totals in fp64, fixed order (deterministic).  grid = (ceil(nT/32), nq quantities),
 // block = 32 templates x RED_SLICES chunk slices; slice s sums the chunks c = s (mod RED_SLICES).
 constexpr int RED_SLICES = 16;
@@ -1864,5 +1868,7 @@ __global__ void sft_annual_table_kernel(int n_sft, double t0, double T, double p
   sincos(2.0 * 3.141592653589793 * ((t0 + (double)a * T) / period) + psi, &s, &c);
   out[a] = make_float2((float)c, (float)s);
 }
+
+#endif  // SFT_MAIN_ONLY
 
 }  // namespace sftk

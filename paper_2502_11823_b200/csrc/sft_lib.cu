@@ -12,6 +12,7 @@
 
 #include "../../include/sft.h"
 #include "sft_kernels.cuh"
+#include "sft_launch.cuh"
 #include "alu_peaks.cuh"
 #include "sft_ingest.cuh"
 
@@ -786,74 +787,27 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.rtab = p->rtab;
 }
 
-#ifndef SFT_DUO
-#define SFT_DUO true        // two consecutive SFTs per step through the tier-1 tables (sft_kernels.cuh :: duo_terms)
-#endif
-#ifndef SFT_CREG_BNS
-#define SFT_CREG_BNS true   // the config-2/3/5 variant keeps the polynomial-track coefficients in registers
-#endif
-#ifndef SFT_CREG_MINB
-#define SFT_CREG_MINB 4     // resident blocks per SM of the CREG variants (128 registers)
-#endif
-#ifndef SFT_MINB
-#define SFT_MINB 5          // resident 128-thread blocks per SM the main kernel is compiled for
-#endif
-
-// Compile-time flag sets of the hot variants (everything else takes the run-time-flag variant):
-//   CfgBNS  = Fresnel kernel, 0PN+1PN, no response      (configs 2, 3, 5)
-//   CfgNewt = Fresnel kernel, 0PN, no response          (config 1)
-//   CfgLISA = Fresnel kernel, 0PN+1PN, annual response  (config 4)
-//   CfgAny  = run-time flags (incl. the phase path), optional k_c output and path counters
-using CfgBNS = sftk::Cfg<1, 1, 0, 0>;
-using CfgNewt = sftk::Cfg<1, 0, 0, 0>;
-using CfgLISA = sftk::Cfg<1, 1, 2, 0>;
-using CfgAny = sftk::Cfg<-1, -1, -1, 1, -1>;
-using CfgBNS32 = sftk::Cfg<1, 1, 0, 0, 1>;    // CfgBNS with the split-fp32 (double-float) phase track (config 5)
-
-// CREG: polynomial-track coefficients in registers (128 registers, 4 blocks per SM) instead of shared memory (96, 5 blocks)
-// BAND = false: specialisation for the full table layout (no sft_plan_set_table_track): row addresses from a constant-bank operand
-template <int KT, int CT, int MODE, class CFG, bool CREG = false, bool BAND = true>
-static void launch_variant(sft_plan *p, const KParams &k) {
-  if (CREG && BAND && !p->banded) return launch_variant<KT, CT, MODE, CFG, CREG, false>(p, k);   // (only the CREG variants have it)
-  auto kern = sftk::sft_main_kernel<KT, CT, MODE, CFG, CREG ? SFT_CREG_MINB : SFT_MINB, SFT_DUO, CREG, BAND>;
-  int per_sm = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, sftk::TILE, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
-  long long blocks = (long long)p->n_sm * per_sm;
-  const long long need = ((long long)k.n_items + sftk::TILE / 32 - 1) / (sftk::TILE / 32);
-  if (blocks > need) blocks = need;
-  kern<<<(unsigned)blocks, sftk::TILE, 0, p->stream>>>(k);
-}
-
-template <int MODE>
-static cudaError_t launch_main(sft_plan *p, const KParams &k) {
+// The variants of the fused main kernel live in sft_var_*.cu (sft_launch.cuh): ask the units in turn.
+static cudaError_t launch_main(sft_plan *p, const KParams &k, int mode) {
   cudaEventRecord(p->ev0, p->stream);             // (the work-unit counter was zeroed by sft_tmpl_kernel)
-  const int C = k.C, K = k.K;
   const bool diag = k.kc_out != nullptr || k.path_counts != nullptr || k.phase_path != 0;
-  const bool bns32 = k.kc_out == nullptr && k.path_counts == nullptr && k.phase_path == 1 && k.kernel == 1 && k.pn1 == 1 &&
-                     k.response == 0 && C == 1 && K == 8;
-  const bool bns = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 0;
-  const bool newt = !diag && k.kernel == 1 && k.pn1 == 0 && k.response == 0;
-  const bool lisa = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 2;
-#ifdef SFT_FEW_VARIANTS      // development builds: only the config-2 variant and the single-channel run-time-flag variant
-  (void)bns32; (void)newt; (void)lisa;
-  if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS, SFT_CREG_BNS>(p, k);
-  else launch_variant<0, 1, MODE, CfgAny>(p, k);
-#else
-  if (bns32) launch_variant<8, 1, MODE, CfgBNS32>(p, k);
-  else if (bns && C == 1 && K == 8) launch_variant<8, 1, MODE, CfgBNS, SFT_CREG_BNS>(p, k);
-  else if (bns && C == 1 && K == 16) launch_variant<16, 1, MODE, CfgBNS>(p, k);
-  else if (bns && C == 1) launch_variant<0, 1, MODE, CfgBNS>(p, k);
-  else if (newt && C == 1 && K == 4) launch_variant<4, 1, MODE, CfgNewt>(p, k);
-  else if (lisa && C == 2 && K == 16) launch_variant<16, 2, MODE, CfgLISA>(p, k);
-  else if (C == 1) launch_variant<0, 1, MODE, CfgAny>(p, k);
-  else if (C == 2) launch_variant<0, 2, MODE, CfgAny>(p, k);
-  else if (C == 3) launch_variant<0, 3, MODE, CfgAny>(p, k);
-  else launch_variant<0, 4, MODE, CfgAny>(p, k);
-#endif
+  sftl::Key key;
+  key.mode = mode;
+  key.C = k.C;
+  key.K = k.K;
+  key.bns32 = mode != 2 && k.kc_out == nullptr && k.path_counts == nullptr && k.phase_path == 1 && k.kernel == 1 && k.pn1 == 1 &&
+              k.response == 0 && k.C == 1 && k.K == 8;
+  key.bns = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 0;
+  key.newt = !diag && k.kernel == 1 && k.pn1 == 0 && k.response == 0;
+  key.lisa = !diag && k.kernel == 1 && k.pn1 == 1 && k.response == 2;
+  const sftl::Ctx ctx = {p->stream, p->n_sm, p->banded};
+  const bool done = sftl::launch_bns(key, ctx, k) || sftl::launch_misc(key, ctx, k) || sftl::launch_lisa(key, ctx, k) ||
+                    sftl::launch_any1(key, ctx, k) || sftl::launch_any2(key, ctx, k) || sftl::launch_any3(key, ctx, k) ||
+                    sftl::launch_any4(key, ctx, k);
   cudaEventRecord(p->ev1, p->stream);
   p->timed = true;
   p->launches++;
-  return cudaGetLastError();
+  return done ? cudaGetLastError() : cudaErrorInvalidConfiguration;
 }
 
 static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t mem, KParams &k, bool cumulative, int nq = 3) {
@@ -953,7 +907,7 @@ SFT_API sft_status sft_inner_products(sft_plan *p, int64_t nT, const double *par
   k.kc_out = d_kc;
   k.path_counts = d_kc ? p->path_counts : nullptr;     // the diagnostic call also counts the evaluator paths
   if (d_kc) CU(p, cudaMemsetAsync(p->path_counts, 0, sftk::PATH_N * sizeof(unsigned long long), p->stream));
-  cudaError_t e = launch_main<0>(p, k);
+  cudaError_t e = launch_main(p, k, 0);
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
   sftk::RedOut ro = {{d_xh, d_hh, d_xi, nullptr, nullptr, nullptr, nullptr}};
   sftk::sft_reduce_kernel<<<dim3((unsigned)((nT + 31) / 32), 3), 32 * sftk::RED_SLICES, 0, p->stream>>>(p->part, nT, k.n_chunks, 3, ro);
@@ -1088,13 +1042,7 @@ SFT_API sft_status sft_fstat(sft_plan *p, int64_t nT, const double *params, doub
   }
   k.kc_out = nullptr;
   k.path_counts = nullptr;
-  cudaEventRecord(p->ev0, p->stream);
-  if (k.C == 1) launch_variant<0, 1, 2, CfgAny>(p, k);
-  else launch_variant<0, 2, 2, CfgAny>(p, k);
-  cudaEventRecord(p->ev1, p->stream);
-  p->timed = true;
-  p->launches++;
-  cudaError_t e = cudaGetLastError();
+  cudaError_t e = launch_main(p, k, 2);
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
   sftk::RedOut ro;
   for (int i = 0; i < 7; ++i) ro.q[i] = sums + (size_t)i * nT;
@@ -1142,7 +1090,7 @@ SFT_API sft_status sft_cumulative_snr(sft_plan *p, int64_t nT, const double *par
   k.out_snr = d_snr;
   k.out_cx = d_cx;
   k.out_ch = d_ch;
-  cudaError_t e = launch_main<1>(p, k);
+  cudaError_t e = launch_main(p, k, 1);
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
   if (mem == SFT_MEM_HOST) {
     CU(p, cudaStreamSynchronize(p->stream));

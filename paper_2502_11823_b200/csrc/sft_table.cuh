@@ -49,6 +49,7 @@ static_assert(HT1_R == (TAB_R << HT1_SHIFT), "table geometry");
 constexpr float B_TABLE = 0.12f;    // tier 1: moments q <= 7, H to beta^2
 constexpr float B_TABLE2 = 1.0f;    // tier 2: moments q <= 15, H to beta^6
 
+#ifndef SFT_MAIN_ONLY
 // sigma_q(a') with rho_q = sigma_q (q even), i sigma_q (q odd):  sigma_q = int v^q cos(w v) dv (q even), int v^q sin(w v) dv (q odd),
 // w = 2 pi a', over [-1/2, 1/2].  |a'| >= 1.5: integration by parts upwards in q (each step multiplies
 // the error by q/w < 1); below: power series in w (|w|/2 < 4.8: 40 terms leave < 1e-17).
@@ -197,5 +198,7 @@ __global__ void __launch_bounds__(64) sft_htab1_kernel(const float2 *ub0, int K,
   __syncthreads();
   if (threadIdx.x == 0) htab1[node] = make_float4((float)red[0], (float)red[1], (float)red[2], (float)red[3]);
 }
+
+#endif  // SFT_MAIN_ONLY
 
 }  // namespace sftk
