@@ -1363,11 +1363,15 @@ __device__ __forceinline__ void scan_store(const KParams &p, float *txh, float *
   const float xhi = (float)cx, xlo = (float)(cx - (double)xhi), hhi = (float)chh, hlo = (float)(chh - (double)hhi);
   __syncwarp();
   const int g = ch * 32;
-  // slot j shows the running sums of the last slot <= j that holds a value (smask), 0 if there is none
-  auto source = [&](int j) {
-    const unsigned m = smask & (0xffffffffu >> (31 - j));
-    return m ? 31 - __clz(m) : -1;
-  };
+  // slot j shows the running sums of the last slot <= j that holds a value (smask); slots before the first one show 0:
+  // slot 0 is made to hold that 0, so that every slot has a source
+  if (!(smask & 1u)) {
+    txh[lane * 33] = 0.f;
+    thh[lane * 33] = 0.f;
+    smask |= 1u;
+    __syncwarp();
+  }
+  auto source = [&](int j) { return 31 - __clz(smask & (0xffffffffu >> (31 - j))); };
   const size_t al = (size_t)p.out_snr | (size_t)p.out_cx | (size_t)p.out_ch;   // (null = aligned)
   if ((p.n_sft & 3) == 0 && (al & 15) == 0) {
     // 4 rows x 32 slots per step: lane = (row r0 + lane / 8, slots 4 (lane % 8) ... + 3), 16-byte stores
@@ -1384,10 +1388,8 @@ __device__ __forceinline__ void scan_store(const KParams &p, float *txh, float *
       float x[4], h[4], q[4];
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
-        const int sj = src[j] < 0 ? 0 : src[j];
-        const float lx = txh[r * 33 + sj], lh = thh[r * 33 + sj];
-        x[j] = c0 + (c1 + (src[j] < 0 ? 0.f : lx));
-        h[j] = c2 + (c3 + (src[j] < 0 ? 0.f : lh));
+        x[j] = c0 + (c1 + txh[r * 33 + src[j]]);
+        h[j] = c2 + (c3 + thh[r * 33 + src[j]]);
         q[j] = h[j] > 0.f ? x[j] * rsqrt_approx(h[j]) : 0.f;
       }
       if (tt < p.nT && c4 < n) {
@@ -1404,8 +1406,8 @@ __device__ __forceinline__ void scan_store(const KParams &p, float *txh, float *
       const float c0 = __shfl_sync(0xffffffffu, xhi, r), c1 = __shfl_sync(0xffffffffu, xlo, r);
       const float c2 = __shfl_sync(0xffffffffu, hhi, r), c3 = __shfl_sync(0xffffffffu, hlo, r);
       if (tt < p.nT && lane < n) {
-        const float x = c0 + (c1 + (sj < 0 ? 0.f : txh[r * 33 + sj]));
-        const float h = c2 + (c3 + (sj < 0 ? 0.f : thh[r * 33 + sj]));
+        const float x = c0 + (c1 + txh[r * 33 + sj]);
+        const float h = c2 + (c3 + thh[r * 33 + sj]);
         const size_t o = (size_t)tt * p.n_sft + g + lane;
         if (p.out_snr) __stcs(p.out_snr + o, h > 0.f ? x * rsqrt_approx(h) : 0.f);
         if (p.out_cx) __stcs(p.out_cx + o, x);
