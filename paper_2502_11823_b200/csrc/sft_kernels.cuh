@@ -1479,12 +1479,12 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
         if (vB && usB[c] > 0.f) kcp[(size_t)c * p.n_sft + jB] = B.kc;
       }
     }
-    if (MODE == 1) {                   // running sums at the present slots only: scan_store fills the gaps
-      axh += (double)zrA; ahh += (double)hhA;
-      txh[lane * 33 + jA] = (float)axh; thh[lane * 33 + jA] = (float)ahh;
+    if (MODE == 1) {                   // running sums at the present slots only: scan_store fills the gaps.  fp32 inside the
+      fxh += zrA; fhh += hhA;          // unit (<= 32 terms, as MODE 0 sums 8 SFTs in fp32); the carries across units are fp64
+      txh[lane * 33 + jA] = fxh; thh[lane * 33 + jA] = fhh;
       if (vB) {
-        axh += (double)zrB; ahh += (double)hhB;
-        txh[lane * 33 + jB] = (float)axh; thh[lane * 33 + jB] = (float)ahh;
+        fxh += zrB; fhh += hhB;
+        txh[lane * 33 + jB] = fxh; thh[lane * 33 + jB] = fhh;
       }
     } else {
       fxh += zrA + zrB;
@@ -1494,6 +1494,8 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
   }
   if (MODE == 0) {
     axh += (double)fxh; axi += (double)fxi; ahh += (double)fhh;
+  } else if (MODE == 1) {
+    axh += (double)fxh; ahh += (double)fhh;      // (one block per unit: axh, ahh were 0)
   }
 }
 
