@@ -444,11 +444,11 @@ def run_ours(args, rank, world, local_rank):
 # DRAM bytes (read + write) of one main-kernel launch, from the committed ncu --set full captures (dram__bytes_read.sum +
 # dram__bytes_write.sum): NOT measured by this run - the source capture is named in roofline.traffic_source.
 NCU_TRAFFIC = {
-    ("config2-F", "auto"): (2.103552e6 + 10.496e3, "profiles/r02_main_kernel.md"),
-    ("config2-F", "table"): (2.103552e6 + 10.496e3, "profiles/r02_main_kernel.md"),
+    ("config2-F", "auto"): (2.104832e6 + 84.48e3, "profiles/r02_main_kernel.md"),
+    ("config2-F", "table"): (2.104832e6 + 84.48e3, "profiles/r02_main_kernel.md"),
     ("config2-F", "direct"): (8.213504e6 + 10.752e3, "profiles/r01d_kernel_v7_tables.md"),
-    ("config3-F", "auto"): (5.656064e6 + 872.535296e6, "profiles/r02_main_kernel.md"),
-    ("config4", "auto"): (6.583040e6 + 2.189312e6, "profiles/r02_main_kernel.md"),
+    ("config3-F", "auto"): (6.057728e6 + 872.374272e6, "profiles/r02_main_kernel.md"),
+    ("config4", "auto"): (6.319616e6 + 229.888e3, "profiles/r02_main_kernel.md"),
 }
 
 # Algorithmic work per active pair and the ALU peak: DESIGN.md section 7.
