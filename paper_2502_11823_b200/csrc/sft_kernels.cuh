@@ -1502,8 +1502,12 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
 // ---------------------------------------------------------------------------------------------
 // Main fused kernel.  Persistent grid; every warp draws (32 templates) x (SFT chunk) work units from
 // p.counter.  CT == number of channels (exactly).
-// MODE 0: chunk totals only.  MODE 1 (cumulative): additionally writes chunk-local inclusive prefix
-// sums, transposed through shared memory so that global stores are 128-byte rows along the SFT axis.
+// MODE 0: chunk totals only (sft_reduce_kernel sums the chunks in fixed order).
+// MODE 1 (cumulative): one work unit is one 32-SFT block; units are drawn in ascending SFT order, each
+// publishes its aggregate and picks up the carry of all earlier units by decoupled look-back (scan_store),
+// then writes the final cumulative <x,h>, <h,h> and SNR, transposed through shared memory so that global
+// stores are 128-byte rows along the SFT axis.  One pass, no second kernel.
+// MODE 2 (F-statistic): chunk totals of the seven sums of sft.h (sft_fstat).
 // A work unit is walked in blocks of SUB = 32 SFT slots: clean blocks take the fast path above, all others the
 // generic loop below, which runs in groups of GROUP SFTs: fp32 partial sums flushed into fp64 per group (MODE 0),
 // one transposed store per group (MODE 1).
