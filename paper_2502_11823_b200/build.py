@@ -1,6 +1,11 @@
 """Builds ``libsft_b200.so`` (the C-ABI library of include/sft.h) in-tree with nvcc for sm_100a.
 
-    python -m paper_2502_11823_b200.build [--force]
+    python -m paper_2502_11823_b200.build [--force] [--checked]
+
+``--checked`` builds the same library with -DSFT_CHECKED: every indexed global access of the main path is tested against the
+extent of its buffer and a call whose kernel tripped a test returns SFT_ECUDA (sft_kernels.cuh, SFT_CHK).  For running the GPU
+tests once after a change of the index arithmetic; slower, never the library that is timed.  ``sft_version()`` says which one
+is loaded.
 
 The shared library is written next to this file so that it travels with the source tree (it is
 git-ignored).  nvcc cross-compiles without a GPU.
@@ -74,5 +79,5 @@ def build(force=False, verbose=False, extra=()):
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True,
-                extra=["-Xptxas", "-v"] if "--ptxas-v" in sys.argv else ()))
+    print(build(force="--force" in sys.argv or "--checked" in sys.argv, verbose=True,
+                extra=(["-Xptxas", "-v"] if "--ptxas-v" in sys.argv else []) + (["-DSFT_CHECKED"] if "--checked" in sys.argv else [])))

@@ -92,7 +92,28 @@ struct KParams {
   double2 *scanA, *scanP;  // [n_chunks][nT] {xh, hh}: a unit's own totals (aggregate) / totals of all SFTs up to its end (inclusive)
   unsigned *flagA, *flagP; // [n_chunks][nT]: == epoch once the entry of this call has been published
   unsigned epoch;
+#ifdef SFT_CHECKED
+  // checked build (build.py --checked): every indexed global access of the main path is tested against the extent of
+  // its buffer (entries, counted in the pointer's element type); the first failing site leaves its code in *chk and the
+  // call returns SFT_ECUDA.  The sizes below are those of the allocations in sft_lib.cu, not derived from the indices.
+  unsigned *chk;
+  unsigned long long n_Dp, n_ubp, n_sl, n_mtab, n_htab, n_htab1, n_tblk, n_out, n_scan, n_part, n_kc;
+#endif
 };
+
+// SFT_CHK(p, condition, site): no code at all in the product build
+#ifdef SFT_CHECKED
+#define SFT_CHK(p, cond, site) do { if (!(cond)) atomicCAS((p).chk, 0u, (unsigned)(site)); } while (0)
+#define SFT_CHK_TB(p, a) ((unsigned long long)((a) >> 5) < (p).n_tblk ? 0u : atomicCAS((p).chk, 0u, (unsigned)CHK_TBLK))
+#else
+#define SFT_CHK(p, cond, site) do { } while (0)
+#define SFT_CHK_TB(p, a) 0
+#endif
+// entries [ptr, ptr + cnt) inside [base, base + n)
+#define SFT_CHK_RANGE(p, ptr, cnt, base, n, site) \
+  SFT_CHK(p, (unsigned long long)((ptr) - (base)) + (unsigned long long)(cnt) <= (unsigned long long)(n) && (ptr) >= (base), site)
+enum ChkSite { CHK_TMPL = 1, CHK_DP, CHK_UBP, CHK_MTAB, CHK_HTAB, CHK_MTAB_FAST, CHK_HTAB1_FAST, CHK_RESP, CHK_US2, CHK_TBLK,
+               CHK_SCAN, CHK_OUT, CHK_PART, CHK_KC };
 
 __device__ __forceinline__ float rcp_approx(float x) {
   float r;
@@ -275,6 +296,7 @@ __device__ __forceinline__ void tmpl_load(const KParams &p, long long t, Tmpl &t
   const long long n = p.nT, tt = ok ? t : n - 1;
   const double *d = p.td + tt;
   const float *f = p.tf + tt;
+  SFT_CHK(p, tt >= 0 && tt < n, CHK_TMPL);
   tm.tau0 = __ldg(d + TD_TAU0 * n);
   tm.cTheta = __ldg(d + TD_CTHETA * n);
   tm.phic_cyc = __ldg(d + TD_PHIC * n);
@@ -602,6 +624,8 @@ __device__ __forceinline__ void mac_pair(const KParams &p, const Win &w, int i, 
   const float2 mag = __ffma2_rn(Ji, Ji, __fmul2_rn(Jr, Jr));
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
+    SFT_CHK_RANGE(p, dp + c * p.dstride, 1, p.Dp, p.n_Dp, CHK_DP);
+    SFT_CHK_RANGE(p, up + c * p.npair, 1, p.ubp, p.n_ubp, CHK_UBP);
     const float4 d = __ldg(dp + c * p.dstride);
     const float2 u = __ldg(up + c * p.npair);
     const float2 dre = make_float2(d.x, d.y), dim = make_float2(d.z, d.w);
@@ -621,6 +645,8 @@ __device__ __forceinline__ void mac_single(const KParams &p, const Win &w, int i
   const float mag = fmaf(Ji, Ji, Jr * Jr);
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
+    SFT_CHK_RANGE(p, dp + c * p.dstride, 1, p.Dp, p.n_Dp, CHK_DP);
+    SFT_CHK_RANGE(p, up + c * p.npair, 1, p.ubp, p.n_ubp, CHK_UBP);
     const float4 d = __ldg(dp + c * p.dstride);
     const float2 u = __ldg(up + c * p.npair);
     acc[c].A.x = fmaf(d.x, Jr, acc[c].A.x);
@@ -747,6 +773,8 @@ __device__ __forceinline__ void table_load(const KParams &p, float xp, float b, 
   const unsigned hch = TIER == 1 ? p.h1chan : p.hchan;
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
+    SFT_CHK_RANGE(p, mp + c * p.mchan, (TableData<CT, TIER>::NL), p.mtab, p.n_mtab, CHK_MTAB);
+    SFT_CHK_RANGE(p, hp + c * hch, (TableData<CT, TIER>::NHL), TIER == 1 ? p.htab1 : p.htab, TIER == 1 ? p.n_htab1 : p.n_htab, CHK_HTAB);
 #pragma unroll
     for (int i = 0; i < TableData<CT, TIER>::NL; ++i) d.Mq[c][i] = __ldg(mp + c * p.mchan + i);
 #pragma unroll
@@ -901,9 +929,11 @@ __device__ __forceinline__ void finish_terms(const KParams &p, const Tmpl &tm, c
     float2 R = tm.AE[c];
     if (fq) {                          // unit response; (a, b) are applied to the sums below
     } else if (resp == 1) {
+      SFT_CHK_RANGE(p, rt + c * p.n_sft, 1, p.rtab, p.n_sl, CHK_RESP);
       const float2 r = __ldg(rt + c * p.n_sft);
       R = make_float2(tm.AE[c].x * r.x, tm.AE[c].x * r.y);      // AE is real here
     } else if (resp == 2) {
+      SFT_CHK_RANGE(p, rt + c * p.n_sft, 1, p.rtab, p.n_sl, CHK_RESP);
       const float2 cs = __ldg(rt + c * p.n_sft);
       const float am = fmaf(p.depth, cs.x * tm.cl - cs.y * tm.sl, 1.0f);
       R = make_float2(R.x * am, R.y * am);
@@ -917,6 +947,7 @@ __device__ __forceinline__ void finish_terms(const KParams &p, const Tmpl &tm, c
     const float cr = gr * s1r[c] - gi * s1i[c], ci = gr * s1i[c] + gi * s1r[c];
     const float chh = r2 * a2 * us2[c] * s2[c];
     if (fq) {
+      SFT_CHK_RANGE(p, rt + c * p.n_sft, 1, p.rtab, p.n_sl, CHK_RESP);
       const float2 ab = __ldg(rt + c * p.n_sft);
       const bool on = ok && us2[c] > 0.f;
       const float wa = on ? ab.x : 0.f, wb = on ? ab.y : 0.f, h_ = on ? chh : 0.f;
@@ -1220,6 +1251,7 @@ __device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int 
   bool pres = false;
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
+    SFT_CHK(p, g + lane >= ge || (unsigned long long)c * p.n_sft + g + lane < p.n_sl, CHK_US2);
     usv[c] = (g + lane < ge) ? __ldg(p.us2 + (size_t)c * p.n_sft + g + lane) : 0.f;
     pres |= usv[c] > 0.f;
   }
@@ -1227,6 +1259,7 @@ __device__ __forceinline__ int fast_setup(const KParams &p, const Tmpl &tm, int 
   if (mask == 0u || p.mtab == nullptr || cfg_phase<CFG>(p) != 0) return 0;
   if (BAND) {
     if ((g >> 5) != ((ge - 1) >> 5)) return 0;                     // (work units that are not aligned to the table's blocks of 32 SFTs)
+    SFT_CHK(p, (unsigned long long)(g >> 5) < p.n_tblk, CHK_TBLK);
     tb = __ldg(p.tblk + (g >> 5));
     if (tb.z <= 0) return 0;
   } else {                                                         // full layout: row of SFT a at a * mrow0, all positions present
@@ -1283,6 +1316,8 @@ __device__ __forceinline__ void table_load_fast(const KParams &p, float xp, floa
   const float4 *hp = p.htab1 + ((unsigned)kcidx * HT1_R + cellH);
 #pragma unroll
   for (int c = 0; c < CT; ++c) {
+    SFT_CHK_RANGE(p, mp + c * p.mchan, (TableData<CT, 1>::NL), p.mtab, p.n_mtab, CHK_MTAB_FAST);
+    SFT_CHK_RANGE(p, hp + c * p.h1chan, 1, p.htab1, p.n_htab1, CHK_HTAB1_FAST);
 #pragma unroll
     for (int i = 0; i < TableData<CT, 1>::NL; ++i) d.Mq[c][i] = __ldg(mp + c * p.mchan + i);
 #pragma unroll
@@ -1339,6 +1374,7 @@ __device__ __forceinline__ void scan_store(const KParams &p, float *txh, float *
   double cx = 0.0, chh = 0.0;
   if (ok) {
     const size_t me = (size_t)ch * nT + (size_t)t;
+    SFT_CHK(p, me < p.n_scan, CHK_SCAN);
     p.scanA[me] = make_double2(axh, ahh);
     st_release_u32(p.flagA + me, p.epoch);
     int k = ch - 1;
@@ -1394,6 +1430,7 @@ __device__ __forceinline__ void scan_store(const KParams &p, float *txh, float *
       }
       if (tt < p.nT && c4 < n) {
         const size_t o = (size_t)tt * p.n_sft + g + c4;
+        SFT_CHK(p, o + 4 <= p.n_out, CHK_OUT);
         if (p.out_snr) __stcs((float4 *)(p.out_snr + o), make_float4(q[0], q[1], q[2], q[3]));
         if (p.out_cx) __stcs((float4 *)(p.out_cx + o), make_float4(x[0], x[1], x[2], x[3]));
         if (p.out_ch) __stcs((float4 *)(p.out_ch + o), make_float4(h[0], h[1], h[2], h[3]));
@@ -1409,6 +1446,7 @@ __device__ __forceinline__ void scan_store(const KParams &p, float *txh, float *
         const float x = c0 + (c1 + txh[r * 33 + sj]);
         const float h = c2 + (c3 + thh[r * 33 + sj]);
         const size_t o = (size_t)tt * p.n_sft + g + lane;
+        SFT_CHK(p, o < p.n_out, CHK_OUT);
         if (p.out_snr) __stcs(p.out_snr + o, h > 0.f ? x * rsqrt_approx(h) : 0.f);
         if (p.out_cx) __stcs(p.out_cx + o, x);
         if (p.out_ch) __stcs(p.out_ch + o, h);
@@ -1434,7 +1472,10 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
   if (CFG::KC && kcp && t < p.nT) {
     for (int k = 0; k < n; ++k)
 #pragma unroll
-      for (int c = 0; c < CT; ++c) kcp[(size_t)c * p.n_sft + k] = -1;
+      for (int c = 0; c < CT; ++c) {
+        SFT_CHK_RANGE(p, kcp + (size_t)c * p.n_sft + k, 1, p.kc_out, p.n_kc, CHK_KC);
+        kcp[(size_t)c * p.n_sft + k] = -1;
+      }
   }
   float fxh = 0.f, fhh = 0.f, fxi = 0.f;
   while (mask) {
@@ -1475,6 +1516,8 @@ __device__ __forceinline__ void fast_block(const KParams &p, const Tmpl &tm, con
     if (CFG::KC && kcp && t < p.nT) {
 #pragma unroll
       for (int c = 0; c < CT; ++c) {
+        SFT_CHK_RANGE(p, kcp + (size_t)c * p.n_sft + jA, 1, p.kc_out, p.n_kc, CHK_KC);
+        SFT_CHK(p, !vB || (unsigned long long)(kcp + (size_t)c * p.n_sft + jB - p.kc_out) < p.n_kc, CHK_KC);
         if (usA[c] > 0.f) kcp[(size_t)c * p.n_sft + jA] = A.kc;
         if (vB && usB[c] > 0.f) kcp[(size_t)c * p.n_sft + jB] = B.kc;
       }
@@ -1574,7 +1617,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
       // not aligned to 32 (sft_plan_set_chunk), in which case the record is re-read per SFT
       const bool one_blk = (gs >> 5) == ((gend - 1) >> 5);
       int4 tb = !p.mtab ? make_int4(0, 0, 0, 0)
-                : BAND  ? __ldg(p.tblk + (gs >> 5))
+                : BAND  ? (SFT_CHK_TB(p, gs), __ldg(p.tblk + (gs >> 5)))
                         : make_int4((int)((unsigned)(gs & ~31) * p.mrow0), 0, p.jmax + 1, (int)p.mrow0);
       Track tr, tr2;                                   // tracks of SFT alpha and alpha + 1
       track_eval<CFG>(p, tm, dalpha, tr);
@@ -1592,6 +1635,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
           bool any = false, anyb = false;
 #pragma unroll
           for (int c = 0; c < CT; ++c) {
+            SFT_CHK_RANGE(p, usp + c * p.n_sft, 1, p.us2, p.n_sl, CHK_US2);
             us2[c] = __ldg(usp + c * p.n_sft);
             any |= us2[c] > 0.f;                                   // warp-uniform
           }
@@ -1599,7 +1643,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
           const float ab = (go && cfg_kernel<CFG>(p) == 1) ? fabsf(tr.b) : 0.f;
           // the table rows of this SFT (block alpha >> 5) and whether the windows of all active lanes lie inside them
           if (!one_blk && p.mtab) {
-            if (BAND) tb = __ldg(p.tblk + (alpha >> 5));
+            if (BAND) { SFT_CHK_TB(p, alpha); tb = __ldg(p.tblk + (alpha >> 5)); }
             else tb.x = (int)((unsigned)(alpha & ~31) * p.mrow0);
           }
           const float4 *Mrow0 = p.mtab + ((unsigned)tb.x + (unsigned)(alpha & 31) * (unsigned)tb.w);
@@ -1613,6 +1657,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
           if (DUO && MODE != 2 && alpha + 1 < ge && tabok && (alpha & 31) != 31) {
 #pragma unroll
             for (int c = 0; c < CT; ++c) {
+              SFT_CHK_RANGE(p, usp + c * p.n_sft + 1, 1, p.us2, p.n_sl, CHK_US2);
               us2b[c] = __ldg(usp + c * p.n_sft + 1);
               anyb |= us2b[c] > 0.f;
             }
@@ -1637,6 +1682,7 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
               if (t < p.nT) {
 #pragma unroll
                 for (int c = 0; c < CT; ++c) {
+                  SFT_CHK_RANGE(p, kcp + (size_t)c * p.n_sft, 2, p.kc_out, p.n_kc, CHK_KC);
                   kcp[(size_t)c * p.n_sft] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
                   kcp[(size_t)c * p.n_sft + 1] = (tr2.active && us2b[c] > 0.f) ? tr2.kc : -1;
                 }
@@ -1688,7 +1734,10 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
           if (CFG::KC && want_kc) {
             if (t < p.nT) {
 #pragma unroll
-              for (int c = 0; c < CT; ++c) kcp[(size_t)c * p.n_sft] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
+              for (int c = 0; c < CT; ++c) {
+                SFT_CHK_RANGE(p, kcp + (size_t)c * p.n_sft, 1, p.kc_out, p.n_kc, CHK_KC);
+                kcp[(size_t)c * p.n_sft] = (tr.active && us2[c] > 0.f) ? tr.kc : -1;
+              }
             }
             ++kcp;
           }
@@ -1714,11 +1763,13 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
     } else if (MODE == 2) {
       if (t < p.nT) {
         double *q = p.part + (size_t)ch * 7 * p.nT + t;
+        SFT_CHK_RANGE(p, q + 6 * (size_t)p.nT, 1, p.part, p.n_part, CHK_PART);
 #pragma unroll
         for (int i = 0; i < 7; ++i) q[(size_t)i * p.nT] = afs[i];
       }
     } else if (t < p.nT) {
       double *q = p.part + (size_t)ch * 3 * p.nT + t;
+      SFT_CHK_RANGE(p, q + 2 * (size_t)p.nT, 1, p.part, p.n_part, CHK_PART);
       q[0] = axh;
       q[p.nT] = ahh;
       q[2 * p.nT] = axi;

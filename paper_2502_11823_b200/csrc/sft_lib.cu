@@ -55,6 +55,7 @@ struct sft_plan {
   int w_max = 0;                                       // widest block (window positions)
   bool banded = false;                                 // layout from sft_plan_set_table_track
   int *counter = nullptr;                              // work-unit counter of the persistent main kernel
+  unsigned *chk = nullptr;                             // checked build only (SFT_CHECKED): first failing bounds-check site
   unsigned long long *path_counts = nullptr;           // [PATH_N] diagnostic counters
   int n_sm = 0;
   int chunk_user = 0;
@@ -100,7 +101,11 @@ static sft_status grow(sft_plan *p, void **ptr, size_t *have, size_t need) {
   return SFT_OK;
 }
 
+#ifdef SFT_CHECKED
+SFT_API const char *sft_version(void) { return "sft_b200 0.1 (sm_100a, checked build: bounds tests on)"; }
+#else
 SFT_API const char *sft_version(void) { return "sft_b200 0.1 (sm_100a)"; }
+#endif
 
 SFT_API const char *sft_last_error(const sft_plan *plan) { return plan ? plan->err : g_create_err; }
 
@@ -220,6 +225,10 @@ SFT_API sft_status sft_plan_create(const sft_plan_desc *desc, sft_plan **out) {
     }
   }
   alloc((void **)&p->counter, sizeof(int));
+#ifdef SFT_CHECKED
+  alloc((void **)&p->chk, sizeof(unsigned));
+  if (st == SFT_OK && cudaMemset(p->chk, 0, sizeof(unsigned)) != cudaSuccess) st = fail(nullptr, SFT_ECUDA, "plan set-up: cudaMemset");
+#endif
   alloc((void **)&p->path_counts, sftk::PATH_N * sizeof(unsigned long long));
   if (st == SFT_OK) {
     cudaError_t e2 = cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, d.device);
@@ -258,7 +267,7 @@ SFT_API sft_status sft_plan_destroy(sft_plan *p) {
   cudaFree(p->Dp); cudaFree(p->ubp); cudaFree(p->us2); cudaFree(p->rtab); cudaFree(p->shape_dev);
   cudaFree(p->part); cudaFree(p->d_params); cudaFree(p->d_out); cudaFree(p->scan);
   if (p->h_pin) cudaFreeHost(p->h_pin);
-  cudaFree(p->td); cudaFree(p->tf); cudaFree(p->counter); cudaFree(p->path_counts);
+  cudaFree(p->td); cudaFree(p->tf); cudaFree(p->counter); cudaFree(p->path_counts); cudaFree(p->chk);
   cudaFree(p->mtab); cudaFree(p->htab); cudaFree(p->htab1); cudaFree(p->ptab); cudaFree(p->tblk);
   if (p->ev0) cudaEventDestroy(p->ev0);
   if (p->ev1) cudaEventDestroy(p->ev1);
@@ -785,6 +794,19 @@ static void fill_kparams(const sft_plan *p, KParams &k) {
   k.ubp = p->ubp;
   k.us2 = p->us2;
   k.rtab = p->rtab;
+#ifdef SFT_CHECKED
+  {                                                    // extents of the allocations (sft_plan_create, table_layout), in entries
+    const unsigned long long C = p->d.n_channels, N = p->d.n_sft;
+    k.chk = p->chk;
+    k.n_Dp = (2 * C * N + 1) * (unsigned long long)p->npair;
+    k.n_ubp = 2 * C * (unsigned long long)p->npair;
+    k.n_sl = C * N;
+    k.n_mtab = p->mtab ? C * (unsigned long long)p->m_f4_chan : 0;
+    k.n_htab = p->htab ? C * (unsigned long long)p->n_kc * sftk::HTAB_R * (sftk::HTAB_W / 4) : 0;
+    k.n_htab1 = p->htab1 ? C * (unsigned long long)p->n_kc * sftk::HT1_R : 0;
+    k.n_tblk = p->tblk ? (N + 31) / 32 : 0;
+  }
+#endif
 }
 
 // The variants of the fused main kernel live in sft_var_*.cu (sft_launch.cuh): ask the units in turn.
@@ -807,6 +829,19 @@ static cudaError_t launch_main(sft_plan *p, const KParams &k, int mode) {
   cudaEventRecord(p->ev1, p->stream);
   p->timed = true;
   p->launches++;
+#ifdef SFT_CHECKED
+  if (done) {                                          // the site (sftk::ChkSite) of the first failed bounds check, if any
+    unsigned site = 0;
+    cudaError_t ec = cudaStreamSynchronize(p->stream);
+    if (ec == cudaSuccess) ec = cudaMemcpy(&site, p->chk, sizeof(site), cudaMemcpyDeviceToHost);
+    if (ec != cudaSuccess) return ec;
+    if (site != 0) {
+      fprintf(stderr, "sft_b200 (checked build): bounds check failed at site %u (sftk::ChkSite)\n", site);
+      cudaMemset(p->chk, 0, sizeof(unsigned));
+      return cudaErrorAssert;
+    }
+  }
+#endif
   return done ? cudaGetLastError() : cudaErrorInvalidConfiguration;
 }
 
@@ -851,10 +886,16 @@ static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t
     k.flagA = (unsigned *)(k.scanP + ent);
     k.flagP = k.flagA + ent;
     k.epoch = p->epoch;
+#ifdef SFT_CHECKED
+    k.n_scan = ent;
+#endif
   } else {
     st = grow(p, (void **)&p->part, &p->part_bytes, (size_t)k.n_chunks * nq * nT * sizeof(double));
     if (st != SFT_OK) return st;
     k.part = p->part;
+#ifdef SFT_CHECKED
+    k.n_part = (unsigned long long)k.n_chunks * nq * nT;
+#endif
   }
   if ((double)k.n_tgroups * (double)k.n_chunks > 2.0e9) return fail(p, SFT_EINVAL, "too many work units: raise sfts_per_block");
   k.n_items = k.n_tgroups * k.n_chunks;
@@ -905,6 +946,9 @@ SFT_API sft_status sft_inner_products(sft_plan *p, int64_t nT, const double *par
     d_kc = kc_out ? (int *)(d_xi + nT) : nullptr;
   }
   k.kc_out = d_kc;
+#ifdef SFT_CHECKED
+  k.n_kc = d_kc ? (unsigned long long)nT * C * N : 0;
+#endif
   k.path_counts = d_kc ? p->path_counts : nullptr;     // the diagnostic call also counts the evaluator paths
   if (d_kc) CU(p, cudaMemsetAsync(p->path_counts, 0, sftk::PATH_N * sizeof(unsigned long long), p->stream));
   cudaError_t e = launch_main(p, k, 0);
@@ -1090,6 +1134,9 @@ SFT_API sft_status sft_cumulative_snr(sft_plan *p, int64_t nT, const double *par
   k.out_snr = d_snr;
   k.out_cx = d_cx;
   k.out_ch = d_ch;
+#ifdef SFT_CHECKED
+  k.n_out = (unsigned long long)nT * N;
+#endif
   cudaError_t e = launch_main(p, k, 1);
   if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
   if (mem == SFT_MEM_HOST) {
