@@ -170,6 +170,29 @@ sft_status sft_inner_products(sft_plan *plan, int64_t n_templates, const double 
                               double *xh, double *hh, double *xh_im, int32_t *kc_out,
                               int32_t mem);
 
+/* sft_inner_products for callers that may not allocate device memory inside the call (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the same kernels and the same results (Eq.(35)), but the scratch
+ * of the call - per-template constants, the per-chunk totals that the final reduction sums, the work-unit counter - lives in
+ * one file-scope device array of SFT_STATIC_SCRATCH_BYTES inside the library, which every GPU that loads the library holds
+ * until the process exits.  The call issues no cudaMalloc / cudaFree / allocating library routine, whatever the plan did
+ * before.
+ *   params, xh, hh, xh_im (nullable): DEVICE pointers, shapes as in sft_inner_products; results are complete when the
+ *           plan's stream reaches this point (the call returns after enqueueing; sft_plan_sync to wait).
+ *   n_templates <= SFT_STATIC_MAX_TEMPLATES, else SFT_EUNSUPPORTED (outputs untouched); 0 is SFT_OK.  Larger banks: several
+ *           calls on slices, or sft_inner_products.
+ * The SFT axis is cut into fewer, longer chunks than sft_inner_products uses when the scratch would not hold its chunk
+ * totals; the fp64 sums are then taken in a different order (differences at the 1e-15 relative level).
+ * The scratch is SHARED by every plan and every call on a device and keeps the previous call's contents; the call itself
+ * clears the one word that must start at zero.  Calls that overlap on the GPU (two plans on different streams, or two
+ * host threads) race on it: order them on one stream or with events.  sft_static_setup(device, &bytes) resolves the
+ * array's address on that device ahead of time (the first call on a device does it otherwise; do it before a capture
+ * begins) and reports the size; it allocates nothing either. */
+#define SFT_STATIC_MAX_TEMPLATES 4096
+#define SFT_STATIC_SCRATCH_BYTES 8388608
+sft_status sft_static_setup(int32_t device, int64_t *scratch_bytes /* nullable */);
+sft_status sft_inner_products_static(sft_plan *plan, int64_t n_templates, const double *params,
+                                     double *xh, double *hh, double *xh_im);
+
 /* Early-warning variant ("accumulating the result over time"): inclusive prefix
  * sums over the SFT index of the per-SFT terms (summed over channels; gaps and inactive SFTs
  * add 0), carried in fp64 and stored in fp32:

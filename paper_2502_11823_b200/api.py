@@ -47,7 +47,7 @@ EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_pr
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
            "sft_plan_set_chunk", "sft_plan_path_counts", "sft_compute_sfts", "sft_ingest_timeseries",
            "sft_tsft_rule", "sft_statistics", "sft_fstat", "sft_validity", "sft_append_sfts", "sft_estimate_psd_scale", "sft_plan_set_table_track", "sft_plan_table_bytes", "sft_last_error", "sft_version",
-           "sft_measure_alu_peaks"]
+           "sft_measure_alu_peaks", "sft_static_setup", "sft_inner_products_static"]
 
 _lib = None
 
@@ -94,6 +94,10 @@ def load_library(path=None):
     lib.sft_ingest_timeseries.argtypes = [vp, i32, vp, i64, vp, vp, vp, i32]
     lib.sft_measure_alu_peaks.argtypes = [i32, C.POINTER(dbl), i32]
     lib.sft_measure_alu_peaks.restype = i32
+    lib.sft_static_setup.argtypes = [i32, C.POINTER(i64)]
+    lib.sft_static_setup.restype = i32
+    lib.sft_inner_products_static.argtypes = [vp, i64, vp, vp, vp, vp]
+    lib.sft_inner_products_static.restype = i32
     lib.sft_last_error.argtypes = [vp]
     lib.sft_last_error.restype = C.c_char_p
     lib.sft_version.restype = C.c_char_p
@@ -240,6 +244,16 @@ class Plan:
             _ptr(xh_im, np.float64, (nT,), "xh_im"),
             _ptr(kc_out, np.int32, (nT, self.n_channels, self.n_sft), "kc_out"), mem))
 
+    def inner_products_static(self, params, xh, hh, xh_im=None):
+        """``sft_inner_products_static``: the allocation-free call (device tensors only, at most STATIC_MAX_TEMPLATES rows)."""
+        nT = int(params.shape[0])
+        if _where([params, xh, hh, xh_im]) != MEM_DEVICE:
+            raise ValueError("sft_inner_products_static takes device tensors only")
+        self._check(self.lib.sft_inner_products_static(
+            self._h, nT, _ptr(params, np.float64, (nT, NPARAM), "params"),
+            _ptr(xh, np.float64, (nT,), "xh"), _ptr(hh, np.float64, (nT,), "hh"),
+            _ptr(xh_im, np.float64, (nT,), "xh_im")))
+
     def cumulative_snr(self, params, snr=None, cum_xh=None, cum_hh=None):
         """``sft_cumulative_snr`` into caller-allocated float32 [nT][n_sft] outputs."""
         nT = int(params.shape[0])
@@ -369,6 +383,19 @@ def measure_alu_peaks(device=0):
     if st != 0:
         raise SftError(st, lib.sft_last_error(None).decode())
     return dict(zip(("ffma", "ffma2", "dfma", "mufu_rcp", "ffma_mufu_mix", "table_mix_ipc"), [float(v) for v in out]))
+
+
+STATIC_MAX_TEMPLATES = 4096          # SFT_STATIC_MAX_TEMPLATES of include/sft.h
+
+
+def static_setup(device=0):
+    """``sft_static_setup``: resolves the library's static scratch on ``device``; returns its size in bytes."""
+    lib = load_library()
+    n = C.c_int64(0)
+    st = lib.sft_static_setup(int(device), C.byref(n))
+    if st != 0:
+        raise SftError(st, lib.sft_last_error(None).decode())
+    return int(n.value)
 
 
 def version():

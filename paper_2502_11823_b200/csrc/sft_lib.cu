@@ -1214,3 +1214,112 @@ SFT_API sft_status sft_measure_alu_peaks(int32_t device, double *out, int32_t n_
   if (n_out > 5) out[5] = mix_ipc;
   return SFT_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// sft_inner_products_static: sft_inner_products for callers that may not allocate (CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc).  The scratch of the call - per-template constants td/tf, the chunk totals `part` that
+// sft_reduce_kernel sums, the work-unit counter - lives in the file-scope device array below instead of the plan's grown
+// buffers; every GPU that loads the library holds SFT_STATIC_SCRATCH_BYTES of it until exit.
+//   In host code `g_static_scratch` is the host-side stand-in of the symbol, NOT a device address: the address on a device
+// comes from cudaGetSymbolAddress with that device current (static_scratch_ptr, once per device).
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_static_scratch[SFT_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int STATIC_MAX_DEV = 64;
+constexpr size_t STATIC_HEAD = 256;                       // [0, 256): work-unit counter (zeroed by sft_tmpl_kernel on every call)
+std::mutex g_static_mu;
+unsigned char *g_static_ptr[STATIC_MAX_DEV] = {nullptr};
+
+constexpr size_t align256(size_t b) { return (b + 255) & ~size_t(255); }
+
+// device address of g_static_scratch on `device` (made current here); resolved once per device
+cudaError_t static_scratch_ptr(int device, unsigned char **out) {
+  if (device < 0 || device >= STATIC_MAX_DEV) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  cudaError_t e = cudaSetDevice(device);
+  if (e != cudaSuccess) return e;
+  if (!g_static_ptr[device]) {
+    void *q = nullptr;
+    e = cudaGetSymbolAddress(&q, g_static_scratch);
+    if (e != cudaSuccess) return e;
+    g_static_ptr[device] = (unsigned char *)q;
+  }
+  *out = g_static_ptr[device];
+  return cudaSuccess;
+}
+}  // namespace
+
+SFT_API sft_status sft_static_setup(int32_t device, int64_t *scratch_bytes) {
+  g_create_err[0] = 0;
+  unsigned char *q = nullptr;
+  const cudaError_t e = static_scratch_ptr(device, &q);
+  if (e != cudaSuccess) return fail(nullptr, e == cudaErrorInvalidDevice ? SFT_EINVAL : SFT_ECUDA, "static scratch of device %d: %s", device, cudaGetErrorString(e));
+  if (scratch_bytes) *scratch_bytes = (int64_t)SFT_STATIC_SCRATCH_BYTES;
+  return SFT_OK;
+}
+
+SFT_API sft_status sft_inner_products_static(sft_plan *p, int64_t nT, const double *params, double *xh, double *hh, double *xh_im) {
+  if (!p) return SFT_EINVAL;
+  p->err[0] = 0;
+  if (nT < 0) return fail(p, SFT_EINVAL, "n_templates < 0");
+  if (nT == 0) return SFT_OK;
+  if (!params || !xh || !hh) return fail(p, SFT_EINVAL, "params, xh and hh are required (device pointers)");
+  if (nT > SFT_STATIC_MAX_TEMPLATES)
+    return fail(p, SFT_EUNSUPPORTED, "sft_inner_products_static: n_templates = %lld exceeds SFT_STATIC_MAX_TEMPLATES = %d "
+                "(static scratch of %d bytes); split the bank or use sft_inner_products", (long long)nT,
+                (int)SFT_STATIC_MAX_TEMPLATES, (int)SFT_STATIC_SCRATCH_BYTES);
+  for (int c = 0; c < p->d.n_channels; ++c)
+    if (!p->loaded[c]) return fail(p, SFT_ENODATA, "channel %d has no data (call sft_load_data)", c);
+  unsigned char *base = nullptr;
+  cudaError_t e = static_scratch_ptr(p->d.device, &base);          // (makes the plan's device current)
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "static scratch of device %d: %s", p->d.device, cudaGetErrorString(e));
+  // carve the scratch: counter | td [TD_N][nT] fp64 | tf [TF_N][nT] fp32 | part [n_chunks][3][nT] fp64
+  const size_t o_td = STATIC_HEAD, o_tf = o_td + align256((size_t)sftk::TD_N * nT * sizeof(double));
+  const size_t o_part = o_tf + align256((size_t)sftk::TF_N * nT * sizeof(float));
+  const size_t row = 3 * (size_t)nT * sizeof(double);                // chunk totals of one chunk
+  if (o_part + row > (size_t)SFT_STATIC_SCRATCH_BYTES) return fail(p, SFT_EUNSUPPORTED, "static scratch too small for %lld templates", (long long)nT);
+  const long long max_chunks = (long long)(((size_t)SFT_STATIC_SCRATCH_BYTES - o_part) / row);
+  KParams k;
+  fill_kparams(p, k);
+  k.nT = nT;
+  k.n_tgroups = (int)((nT + 31) / 32);
+  // SFTs per work unit: the rule of prepare(), with the number of chunks capped by what the scratch holds
+  const long long target_units = 16ll * p->n_sm * 24;
+  long long want_chunks = (target_units + k.n_tgroups - 1) / k.n_tgroups;
+  if (want_chunks > max_chunks) want_chunks = max_chunks;
+  if (want_chunks < 1) want_chunks = 1;
+  int chunk = (int)((k.n_sft + want_chunks - 1) / want_chunks);
+  if (chunk < 32) chunk = 32;
+  chunk = ((chunk + 31) / 32) * 32;                                  // aligned to the blocks of 32 SFT slots (fast path, table layout)
+  if (chunk > k.n_sft) chunk = k.n_sft;
+  k.chunk = chunk;
+  k.n_chunks = (k.n_sft + chunk - 1) / chunk;
+  if (k.n_chunks > max_chunks) return fail(p, SFT_EUNSUPPORTED, "static scratch too small: %d chunks of %d SFTs needed, room for %lld", k.n_chunks, chunk, max_chunks);
+  k.n_items = k.n_tgroups * k.n_chunks;
+  k.counter = (int *)base;
+  double *td = (double *)(base + o_td);
+  float *tf = (float *)(base + o_tf);
+  double *part = (double *)(base + o_part);
+  k.td = td;
+  k.tf = tf;
+  k.part = part;
+  k.params = params;
+#ifdef SFT_CHECKED
+  k.n_part = (unsigned long long)k.n_chunks * 3 * nT;
+#endif
+  // nothing in the scratch needs to start at zero except the counter, which sft_tmpl_kernel clears; td, tf and every
+  // (chunk, quantity, template) entry of part that the reduction reads are written by this call before they are read
+  sftk::sft_tmpl_kernel<<<(unsigned)((nT + 127) / 128), 128, 0, p->stream>>>(k, td, tf);
+  p->launches++;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "template kernel launch: %s", cudaGetErrorString(e));
+  e = launch_main(p, k, 0);
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
+  sftk::RedOut ro = {{xh, hh, xh_im, nullptr, nullptr, nullptr, nullptr}};
+  sftk::sft_reduce_kernel<<<dim3((unsigned)((nT + 31) / 32), 3), 32 * sftk::RED_SLICES, 0, p->stream>>>(part, nT, k.n_chunks, 3, ro);
+  p->launches++;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "reduce kernel launch: %s", cudaGetErrorString(e));
+  return SFT_OK;
+}
