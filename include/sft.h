@@ -278,6 +278,15 @@ int64_t sft_plan_table_bytes(const sft_plan *plan);
  * beyond fp64 summation order. */
 sft_status sft_plan_set_chunk(sft_plan *plan, int32_t sfts_per_unit);
 
+/* Tuning knob of sft_cumulative_snr with HOST outputs: the bank is processed in slabs of `templates_per_slab` templates
+ * (rounded down to a multiple of 32, at least 32) and the matrices of a finished slab are copied to the host on a second
+ * stream while the next slab is computed, so that the copy - 4 n_sft bytes per template and matrix, the part that bounds
+ * the call end to end - starts after the first slab instead of after the whole bank.  0 = automatic (about 64 MB per
+ * matrix and slab).  Results do not depend on it.  The copies overlap only if the host matrices are pinned
+ * (cudaHostAlloc / cudaHostRegister); pageable memory works, without overlap.  If the call fails half-way, slabs already
+ * finished may have been written to the host matrices. */
+sft_status sft_plan_set_host_slab(sft_plan *plan, int64_t templates_per_slab);
+
 /* Diagnostic: measures the plain-ALU pipe rates of `device` that bound this path (the
  * data store is L2 resident, so FP32 / FP64 / XU issue rates, not HBM, are the roofline).  Writes up
  * to 6 doubles, in 1e9 lane-operations per second (one FMA = one operation):

@@ -47,7 +47,8 @@ EXPORTS = ["sft_plan_create", "sft_plan_destroy", "sft_load_data", "sft_inner_pr
            "sft_cumulative_snr", "sft_plan_sync", "sft_plan_launch_count", "sft_plan_last_kernel_ms",
            "sft_plan_set_chunk", "sft_plan_path_counts", "sft_compute_sfts", "sft_ingest_timeseries",
            "sft_tsft_rule", "sft_statistics", "sft_fstat", "sft_validity", "sft_append_sfts", "sft_estimate_psd_scale", "sft_plan_set_table_track", "sft_plan_table_bytes", "sft_last_error", "sft_version",
-           "sft_measure_alu_peaks", "sft_static_setup", "sft_inner_products_static"]
+           "sft_measure_alu_peaks", "sft_static_setup", "sft_inner_products_static",
+           "sft_plan_set_host_slab"]
 
 _lib = None
 
@@ -73,6 +74,8 @@ def load_library(path=None):
     lib.sft_plan_last_kernel_ms.argtypes = [vp]
     lib.sft_plan_last_kernel_ms.restype = dbl
     lib.sft_plan_set_chunk.argtypes = [vp, i32]
+    lib.sft_plan_set_host_slab.argtypes = [vp, i64]
+    lib.sft_plan_set_host_slab.restype = i32
     lib.sft_plan_path_counts.argtypes = [vp, C.POINTER(i64), i32]
     lib.sft_statistics.argtypes = [vp, i64, vp, vp, vp, vp, vp, i32]
     lib.sft_statistics.restype = i32
@@ -308,6 +311,10 @@ class Plan:
 
     def set_chunk(self, sfts_per_unit):
         self._check(self.lib.sft_plan_set_chunk(self._h, int(sfts_per_unit)))
+
+    def set_host_slab(self, templates_per_slab):
+        """``sft_plan_set_host_slab``: templates per slab of ``cumulative_snr`` with host outputs (0 = automatic)."""
+        self._check(self.lib.sft_plan_set_host_slab(self._h, int(templates_per_slab)))
 
     def path_counts(self):
         """``sft_plan_path_counts``: dict path name -> active pairs of the last call that had kc_out."""

@@ -59,6 +59,9 @@ struct sft_plan {
   unsigned long long *path_counts = nullptr;           // [PATH_N] diagnostic counters
   int n_sm = 0;
   int chunk_user = 0;
+  long long slab_user = 0;                             // sft_plan_set_host_slab: templates per slab of the host-output pipeline (0 = auto)
+  cudaStream_t copy_stream = nullptr;                  // sft_cumulative_snr with host outputs: device-to-host copies of finished slabs
+  cudaEvent_t ev_slab[2] = {nullptr, nullptr};
   long long launches = 0;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
@@ -269,6 +272,8 @@ SFT_API sft_status sft_plan_destroy(sft_plan *p) {
   if (p->h_pin) cudaFreeHost(p->h_pin);
   cudaFree(p->td); cudaFree(p->tf); cudaFree(p->counter); cudaFree(p->path_counts); cudaFree(p->chk);
   cudaFree(p->mtab); cudaFree(p->htab); cudaFree(p->htab1); cudaFree(p->ptab); cudaFree(p->tblk);
+  if (p->copy_stream) { cudaStreamSynchronize(p->copy_stream); cudaStreamDestroy(p->copy_stream); }
+  for (int i = 0; i < 2; ++i) if (p->ev_slab[i]) cudaEventDestroy(p->ev_slab[i]);
   if (p->ev0) cudaEventDestroy(p->ev0);
   if (p->ev1) cudaEventDestroy(p->ev1);
   delete p;
@@ -396,6 +401,13 @@ SFT_API sft_status sft_plan_set_chunk(sft_plan *p, int32_t c) {
   if (!p) return SFT_EINVAL;
   if (c < 0) return fail(p, SFT_EINVAL, "sfts_per_block must be >= 0");
   p->chunk_user = c;
+  return SFT_OK;
+}
+
+SFT_API sft_status sft_plan_set_host_slab(sft_plan *p, int64_t templates) {
+  if (!p) return SFT_EINVAL;
+  if (templates < 0) return fail(p, SFT_EINVAL, "templates_per_slab must be >= 0");
+  p->slab_user = templates;
   return SFT_OK;
 }
 
@@ -1117,36 +1129,82 @@ SFT_API sft_status sft_cumulative_snr(sft_plan *p, int64_t nT, const double *par
   if (nT == 0) return SFT_OK;
   if (!params) return fail(p, SFT_EINVAL, "params is required");
   if (!snr && !cum_xh && !cum_hh) return fail(p, SFT_EINVAL, "at least one of snr, cum_xh, cum_hh must be non-NULL");
-  KParams k;
-  sft_status st = prepare(p, nT, params, mem, k, true);
-  if (st != SFT_OK) return st;
   const size_t N = p->d.n_sft, mat = (size_t)nT * N * sizeof(float);
-  float *d_snr = snr, *d_cx = cum_xh, *d_ch = cum_hh;
-  int n_out = (snr != nullptr) + (cum_xh != nullptr) + (cum_hh != nullptr);
-  if (mem == SFT_MEM_HOST) {
-    st = grow(p, &p->d_out, &p->out_bytes, (size_t)n_out * mat);
+  const int n_out = (snr != nullptr) + (cum_xh != nullptr) + (cum_hh != nullptr);
+  sft_status st = SFT_OK;
+  if (mem == SFT_MEM_DEVICE) {
+    KParams k;
+    st = prepare(p, nT, params, mem, k, true);
     if (st != SFT_OK) return st;
-    float *q = (float *)p->d_out;
-    d_snr = snr ? q : nullptr; if (snr) q += (size_t)nT * N;
-    d_cx = cum_xh ? q : nullptr; if (cum_xh) q += (size_t)nT * N;
-    d_ch = cum_hh ? q : nullptr;
-  }
-  k.out_snr = d_snr;
-  k.out_cx = d_cx;
-  k.out_ch = d_ch;
+    k.out_snr = snr;
+    k.out_cx = cum_xh;
+    k.out_ch = cum_hh;
 #ifdef SFT_CHECKED
-  k.n_out = (unsigned long long)nT * N;
+    k.n_out = (unsigned long long)nT * N;
 #endif
-  cudaError_t e = launch_main(p, k, 1);
-  if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
-  if (mem == SFT_MEM_HOST) {
-    CU(p, cudaStreamSynchronize(p->stream));
-    if (snr) CU(p, cudaMemcpyAsync(snr, d_snr, mat, cudaMemcpyDeviceToHost, p->stream));
-    if (cum_xh) CU(p, cudaMemcpyAsync(cum_xh, d_cx, mat, cudaMemcpyDeviceToHost, p->stream));
-    if (cum_hh) CU(p, cudaMemcpyAsync(cum_hh, d_ch, mat, cudaMemcpyDeviceToHost, p->stream));
-    CU(p, cudaStreamSynchronize(p->stream));
+    cudaError_t e = launch_main(p, k, 1);
+    if (e != cudaSuccess) return fail(p, SFT_ECUDA, "main kernel launch: %s", cudaGetErrorString(e));
+    return SFT_OK;
   }
-  return SFT_OK;
+  // Host outputs: the bank is cut into slabs of templates; slab i + 1 is computed while the matrices of slab i travel to the
+  // host on a second stream (the output, 4 n_sft bytes per template and matrix, is what bounds this call end to end).
+  // One slab when the whole output is small.
+  long long slab = p->slab_user;
+  if (slab <= 0) slab = (long long)((64u << 20) / (N * sizeof(float)));            // ~64 MB per matrix and slab
+  slab = (slab / 32) * 32;
+  if (slab < 32) slab = 32;
+  if (slab > nT) slab = nT;
+  if (slab < nT && !p->copy_stream) {
+    CU(p, cudaSetDevice(p->d.device));
+    CU(p, cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) CU(p, cudaEventCreateWithFlags(&p->ev_slab[i], cudaEventDisableTiming));
+  }
+  st = grow(p, &p->d_out, &p->out_bytes, (size_t)n_out * mat);
+  if (st != SFT_OK) return st;
+  float *q = (float *)p->d_out;
+  float *d_snr = snr ? q : nullptr; if (snr) q += (size_t)nT * N;
+  float *d_cx = cum_xh ? q : nullptr; if (cum_xh) q += (size_t)nT * N;
+  float *d_ch = cum_hh ? q : nullptr;
+  float *const dev[3] = {d_snr, d_cx, d_ch};
+  float *const host[3] = {snr, cum_xh, cum_hh};
+  auto copy_slab = [&](long long t0, long long n, int i) -> cudaError_t {          // slab i: after its kernel (ev_slab[i & 1])
+    cudaStream_t cs = slab < nT ? p->copy_stream : p->stream;
+    cudaError_t e = cudaSuccess;
+    if (slab < nT) e = cudaStreamWaitEvent(cs, p->ev_slab[i & 1], 0);
+    for (int j = 0; j < 3 && e == cudaSuccess; ++j)
+      if (host[j]) e = cudaMemcpyAsync(host[j] + (size_t)t0 * N, dev[j] + (size_t)t0 * N, (size_t)n * N * sizeof(float), cudaMemcpyDeviceToHost, cs);
+    return e;
+  };
+  long long prev_t0 = 0, prev_n = 0;
+  int i = 0;
+  for (long long t0 = 0; t0 < nT; t0 += slab, ++i) {
+    const long long n = nT - t0 < slab ? nT - t0 : slab;
+    KParams k;
+    st = prepare(p, n, params + (size_t)t0 * SFT_NPARAM, mem, k, true);
+    if (st != SFT_OK) break;
+    k.out_snr = d_snr ? d_snr + (size_t)t0 * N : nullptr;
+    k.out_cx = d_cx ? d_cx + (size_t)t0 * N : nullptr;
+    k.out_ch = d_ch ? d_ch + (size_t)t0 * N : nullptr;
+#ifdef SFT_CHECKED
+    k.n_out = (unsigned long long)n * N;
+#endif
+    cudaError_t e = launch_main(p, k, 1);
+    if (e == cudaSuccess && slab < nT) e = cudaEventRecord(p->ev_slab[i & 1], p->stream);
+    // the previous slab's copy is issued after this slab's kernel: with pageable host memory cudaMemcpyAsync blocks the host
+    if (e == cudaSuccess && i > 0) e = copy_slab(prev_t0, prev_n, i - 1);
+    if (e != cudaSuccess) { st = fail(p, SFT_ECUDA, "cumulative slab %d: %s", i, cudaGetErrorString(e)); break; }
+    prev_t0 = t0; prev_n = n;
+  }
+  if (st == SFT_OK) {
+    cudaError_t e = copy_slab(prev_t0, prev_n, i - 1);
+    if (e != cudaSuccess) st = fail(p, SFT_ECUDA, "cumulative slab %d copy: %s", i - 1, cudaGetErrorString(e));
+  }
+  // (on an error part of the slabs may already have been written to the host matrices)
+  cudaError_t e1 = p->copy_stream ? cudaStreamSynchronize(p->copy_stream) : cudaSuccess;
+  cudaError_t e2 = cudaStreamSynchronize(p->stream);
+  if (st == SFT_OK && (e1 != cudaSuccess || e2 != cudaSuccess))
+    st = fail(p, SFT_ECUDA, "cumulative: %s", cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+  return st;
 }
 
 // ---------------------------------------------------------------------------------------------

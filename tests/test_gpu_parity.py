@@ -376,6 +376,34 @@ def test_cumulative_small(et_small):
         assert np.allclose(cx[:, -1], ref["xh"], rtol=0, atol=1e-4 * norm.max())
 
 
+def test_cumulative_host_slabs(et_small):
+    """sft_cumulative_snr with host outputs runs the bank in slabs of templates (copy of slab i under the compute of slab
+    i + 1, sft_plan_set_host_slab): the matrices must not depend on the slab size - pageable and pinned host memory, a ragged
+    last slab, one and three outputs."""
+    import torch
+    api = _api()
+    w = et_small
+    nT, n = 150, w.desc["n_sft"]
+    P = np.ascontiguousarray(w.params[:nT])
+    with api.plan_from_workload(w) as plan:
+        Pd = torch.from_numpy(P).cuda()
+        ref = [torch.full((nT, n), float("nan"), dtype=torch.float32, device="cuda") for _ in range(3)]
+        plan.cumulative_snr(Pd, *ref)
+        plan.sync()
+        ref = [r.cpu().numpy() for r in ref]
+        for slab in (0, 32, 64, 100, 4096):                            # 100 -> 96: slabs of 96 + 54 templates
+            plan.set_host_slab(slab)
+            out = [np.full((nT, n), np.nan, np.float32) for _ in range(3)]
+            plan.cumulative_snr(P, *out)
+            for a, b in zip(out, ref):
+                assert np.array_equal(a, b), slab
+            pin = torch.full((nT, n), float("nan"), dtype=torch.float32).pin_memory()
+            plan.cumulative_snr(P, pin.numpy(), None, None)
+            assert np.array_equal(pin.numpy(), ref[0]), slab
+        with pytest.raises(api.SftError):
+            plan.set_host_slab(-1)
+
+
 def test_device_pointers_and_edge_sizes(et_small):
     """Device-resident params/outputs (torch tensors), n_templates in {0, 1, 129}."""
     import torch
@@ -687,7 +715,11 @@ def test_config3_full_size_all_templates():
         g_snr = torch.gather(snr, 1, i).cpu().numpy()
         g_cx = torch.gather(cx, 1, i).cpu().numpy()
         g_ch = torch.gather(ch, 1, i).cpu().numpy()
-        del snr, cx, ch, snr_only
+        # the same call with a host matrix (slabs of templates, copies under the next slab's compute): same bits
+        snr_host = np.empty((nT, N), dtype=np.float32)
+        plan.cumulative_snr(P, snr_host, None, None)
+        assert bool(torch.equal(torch.from_numpy(snr_host), snr.cpu()))
+        del snr, cx, ch, snr_only, snr_host
     from _util import oracle_cumulative_at_parallel
     o_cx, o_ch, o_snr, o_xh, o_hh = oracle_cumulative_at_parallel(w, P, idx)
     plan_o, store = to_oracle(w)
