@@ -153,6 +153,119 @@ __global__ void __launch_bounds__(256) sft_rfft_band_kernel(const double *x, int
   }
 }
 
+// Second radix-16 pass of the narrow-band kernel below: groups {base + j B}, j < 16, of one 16 B-point block, pos = g mod B.
+// Same network and output order as dif_pass<4, false> with h = 8 B, but the twiddle is applied once, after the four
+// stages (which then contain sixteenth-turn rotations only): output j carries w^(pos bitrev4(j)), w = exp(-2 pi i / 16 B),
+// read from the table tw[j][pos] in shared memory - pos = tid mod B is the same for every group a thread ever sees.
+template <int LOG2B>
+__device__ __forceinline__ void dif16_table_pass(float2 *z, const float2 *tw, int m, int tid, int nthr) {
+  constexpr int B = 1 << LOG2B;
+  const int pos = tid & (B - 1);
+  for (int g = tid; g < (m >> 4); g += nthr) {
+    const int base = ((g - pos) << 4) + pos;
+    float2 v[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) v[j] = z[padi(base + j * B)];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      const int hj = 8 >> s;
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        if ((j / hj) & 1) continue;
+        const float2 u = v[j], w2 = v[j + hj];
+        v[j] = make_float2(u.x + w2.x, u.y + w2.y);
+        v[j + hj] = rot16(make_float2(u.x - w2.x, u.y - w2.y), (j % hj) * (8 / hj));
+      }
+    }
+    z[padi(base)] = v[0];
+#pragma unroll
+    for (int j = 1; j < 16; ++j) z[padi(base + j * B)] = cmul(v[j], tw[j * B + pos]);
+  }
+}
+
+// Narrow band (at most 256 bins, 1 <= k_lo, k_hi <= m = n/2): output-pruned version of the kernel above.  After the first eight
+// DIF stages (two radix-16 passes) the work array is 256 independent blocks of B = m/256 points: block b holds the sub-problem
+// of the outputs k = r + 256 k'', r = bitrev8(b), and  Z[k] = sum_{j<B} y_b[j] exp(-2 pi i j k''/B).  A band of <= 256 bins
+// meets every residue r at most once, and so does its mirror image m - k (needed by the real-input split): instead of running
+// the remaining log2(B) stages over all m points, thread b sums its block once for each of the (at most two) outputs asked of
+// it - 2 B complex multiply-adds per thread against the third radix-16 pass, the last radix-2 stage and the bit-reversed
+// gather.  Twiddles of the four values k'' can take come from a table in shared memory (T, filled once per block); the
+// k'' = 0 sums of a band below bin 256 need none.  blockDim.x == 256.  Dynamic shared memory: (n/2 + n/32 + 1 + 20 B) float2.
+template <int LOG2B>
+__global__ void __launch_bounds__(256) sft_rfft_lowband_kernel(const double *x, int n_sft, int n, double dt, int k_lo, int nb,
+                                                               const float2 *W, float2 *bins) {
+  constexpr int B = 1 << LOG2B, log2m = LOG2B + 8;
+  extern __shared__ float2 z[];
+  const int m = n >> 1, k_hi = k_lo + nb;
+  float2 *T = z + (m + (m >> 4) + 1);                   // [4][B]: slots {a0, a0 + 1, c0, c0 + 1}
+  float2 *T2 = T + 4 * B;                               // [16][B]: twiddles of the second pass (dif16_table_pass)
+  for (int t = threadIdx.x; t < 16 * B; t += blockDim.x) {
+    const int j = t >> LOG2B, pos = t & (B - 1);
+    const int q = (int)(__brev((unsigned)j) >> 28);     // exp(-2 pi i pos q / 16 B) = W[pos q n / 16 B], pos q < 16 B / 2 ... 16 B
+    const int e = pos * q;                              // < 16 B
+    const float2 w = __ldg(W + (e & (8 * B - 1)) * (n >> (LOG2B + 4)));
+    T2[t] = (e & (8 * B)) ? make_float2(-w.x, -w.y) : w;
+  }
+  const int a0 = k_lo >> 8, c0 = (m - k_hi + 1) >> 8;
+  for (int t = threadIdx.x; t < 4 * B; t += blockDim.x) {
+    const int slot = t >> LOG2B, j = t & (B - 1);
+    const int kpp = ((slot < 2 ? a0 : c0) + (slot & 1)) & (B - 1);
+    const int e = (j * kpp) & (B - 1);                  // exp(-2 pi i e / B) = +- W[(e mod B/2) n/B]
+    const float2 w = __ldg(W + (e & (B / 2 - 1)) * (n >> LOG2B));
+    T[t] = (e & (B / 2)) ? make_float2(-w.x, -w.y) : w;
+  }
+  // the outputs asked of this thread's block (the same for every segment)
+  const int b = threadIdx.x, r = (int)(__brev((unsigned)b) >> 24);
+  const int kA = k_lo + ((r - k_lo) & 255), kM = k_lo + ((-r - k_lo) & 255);       // band bins with k = r, m - k = r (mod 256)
+  const bool hasA = kA < k_hi, hasM = kM < k_hi;
+  const float2 *TA = T + (((kA >> 8) - a0) & 1) * B, *TM = T + (2 + ((((m - kM) >> 8) - c0) & 1)) * B;
+  const bool plainA = k_hi <= 256;                      // every k'' of the band itself is 0
+  const float2 *blk = z + (b * B + ((b * B) >> 4));
+  const float fdt = (float)dt;
+  __syncthreads();
+  for (int sidx = blockIdx.x; sidx < n_sft; sidx += gridDim.x) {
+    const double *seg = x + (size_t)sidx * n;
+    if (threadIdx.x == 0 && sidx + (int)gridDim.x < n_sft) {
+      const double *nxt = x + (size_t)(sidx + gridDim.x) * n;
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nxt), "r"((unsigned)(n * 8)) : "memory");
+    }
+    dif_pass<4, true>(z, seg, W, m, n, m >> 1, threadIdx.x, blockDim.x);
+    __syncthreads();
+    dif16_table_pass<LOG2B>(z, T2, m, threadIdx.x, blockDim.x);
+    __syncthreads();
+    float2 sA = make_float2(0.f, 0.f), sM = sA;
+#pragma unroll
+    for (int j = 0; j < B; ++j) {
+      const float2 v = blk[j + (j >> 4)];
+      if (plainA) {
+        sA.x += v.x; sA.y += v.y;
+      } else {
+        const float2 t = TA[j];
+        sA.x = fmaf(v.x, t.x, fmaf(-v.y, t.y, sA.x)); sA.y = fmaf(v.x, t.y, fmaf(v.y, t.x, sA.y));
+      }
+      const float2 u = TM[j];
+      sM.x = fmaf(v.x, u.x, fmaf(-v.y, u.y, sM.x)); sM.y = fmaf(v.x, u.y, fmaf(v.y, u.x, sM.y));
+    }
+    __syncthreads();                                   // every block has been read: the array now takes the results
+    // (slot q of the band is kept at q ^ (q >> 4): the threads of a warp hold residues that differ in their high bits only)
+    if (hasA) z[(kA - k_lo) ^ ((kA - k_lo) >> 4)] = sA;                 // Z[k]
+    if (hasM) z[256 + ((kM - k_lo) ^ ((kM - k_lo) >> 4))] = sM;         // Z[m - k]
+    __syncthreads();
+    float2 *out = bins + (size_t)sidx * nb;
+    for (int q = threadIdx.x; q < nb; q += blockDim.x) {
+      const int k = k_lo + q;
+      const float2 A = z[q ^ (q >> 4)], Bc = z[256 + (q ^ (q >> 4))];
+      const float2 Bv = make_float2(Bc.x, -Bc.y);                 // conj Z[m-k]
+      const float2 S = make_float2(A.x + Bv.x, A.y + Bv.y), D = make_float2(A.x - Bv.x, A.y - Bv.y);
+      float2 w;                                                  // w^k, k <= m = n/2
+      if (k < m) w = __ldg(W + k); else w = make_float2(-1.f, 0.f);
+      const float tr = w.x * D.y + w.y * D.x, ti = -(w.x * D.x - w.y * D.y);
+      out[q] = make_float2(0.5f * fdt * (S.x + tr), 0.5f * fdt * (S.y + ti));
+    }
+    __syncthreads();                                   // the work array is reused by the next segment
+  }
+}
+
 // Direct band DFT for any n: block per segment, one thread per bin, samples staged through shared memory.
 __global__ void __launch_bounds__(256) sft_dft_band_kernel(const double *x, int n, double dt, int k_lo, int nb, float2 *bins) {
   __shared__ double xs[1024];
