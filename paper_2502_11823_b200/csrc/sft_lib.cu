@@ -612,15 +612,24 @@ static cudaError_t compute_sfts_device(cudaStream_t stream, const double *x, int
       if (grid > n_sft) grid = n_sft;
       kernel<<<(unsigned)grid, 256, smem, stream>>>(args...);
     };
+    auto launch_lb = [&](auto kernel, size_t smem, auto... args) {
+      cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      int per_sm = 1;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, 256, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+      // persistent blocks, prefetch distance = one round of the grid (one block per segment measured 4 % slower)
+      const long long resident = (long long)n_sm * per_sm, grid = resident < n_sft ? resident : n_sft;
+      kernel<<<(unsigned)grid, 256, smem, stream>>>(args..., (int)grid);
+    };
     const size_t smem = (size_t)(n / 2 + n / 32 + 1) * sizeof(float2);
-    // a band of at most 256 bins inside [1, n/2]: output-pruned transform (two radix-16 passes, then one sum per output)
+    // a band of at most 256 bins inside [1, n/2]: output-pruned transform (two radix-16 passes, then one sum per output).
+    // SFT_INGEST_FULL_FFT in the environment forces the full transform (measurement switch, profiles/r02_ingest.md).
     const bool narrow = nb <= 256 && k_lo >= 1 && k_hi <= n / 2 && log2m >= 11 && log2m <= 13 && !getenv("SFT_INGEST_FULL_FFT");
     if (narrow && log2m == 13)
-      launch(sftk::sft_rfft_lowband_kernel<5>, smem + 20 * 32 * sizeof(float2), x, (int)n_sft, n, dt, k_lo, nb, (const float2 *)W, bins);
+      launch_lb(sftk::sft_rfft_lowband_kernel<5>, smem + 20 * 32 * sizeof(float2), x, (int)n_sft, dt, k_lo, nb, (const float2 *)W, bins);
     else if (narrow && log2m == 12)
-      launch(sftk::sft_rfft_lowband_kernel<4>, smem + 20 * 16 * sizeof(float2), x, (int)n_sft, n, dt, k_lo, nb, (const float2 *)W, bins);
+      launch_lb(sftk::sft_rfft_lowband_kernel<4>, smem + 20 * 16 * sizeof(float2), x, (int)n_sft, dt, k_lo, nb, (const float2 *)W, bins);
     else if (narrow)
-      launch(sftk::sft_rfft_lowband_kernel<3>, smem + 20 * 8 * sizeof(float2), x, (int)n_sft, n, dt, k_lo, nb, (const float2 *)W, bins);
+      launch_lb(sftk::sft_rfft_lowband_kernel<3>, smem + 20 * 8 * sizeof(float2), x, (int)n_sft, dt, k_lo, nb, (const float2 *)W, bins);
     else
       launch(sftk::sft_rfft_band_kernel, smem, x, (int)n_sft, n, log2m, dt, k_lo, nb, (const float2 *)W, bins);
     if (launches) *launches += 1;
