@@ -248,6 +248,27 @@ __global__ void __launch_bounds__(256, 3) sft_rfft_lowband_kernel(const double *
   const float2 *blk = z + (b * B + ((b * B) >> 4));
   const float fdt = (float)dt;
   __syncthreads();
+  // Results: slot p = q ^ (q >> 4) for band offset q (the threads of a warp hold residues that differ in their high bits
+  // only), the mirror sums 256 slots further.  With m/16 >= 512 the slots are the padding entries of the work array (index
+  // 17 p + 16), which no pass ever touches: no barrier before the result write and none after the read-out (three barriers
+  // per segment instead of five: 0.283 -> 0.276 ms).  Smaller transforms keep the results in the first 512 entries, between
+  // two extra barriers.  (Deferring the read-out of segment s to just after the first barrier of the block's next segment
+  // saves the third barrier as well; measured the same, 0.277 ms, so not kept.)
+  constexpr bool PADRES = m / 16 >= 512;
+  auto slot = [](int p) { return PADRES ? 17 * p + 16 : p; };
+  auto read_out = [&](int sdone) {
+    float2 *out = bins + (size_t)sdone * nb;
+    for (int q = threadIdx.x; q < nb; q += blockDim.x) {
+      const int k = k_lo + q;
+      const float2 A = z[slot(q ^ (q >> 4))], Bc = z[slot(256 + (q ^ (q >> 4)))];
+      const float2 Bv = make_float2(Bc.x, -Bc.y);                 // conj Z[m-k]
+      const float2 S = make_float2(A.x + Bv.x, A.y + Bv.y), D = make_float2(A.x - Bv.x, A.y - Bv.y);
+      float2 w;                                                  // w^k, k <= m = n/2
+      if (k < m) w = __ldg(W + k); else w = make_float2(-1.f, 0.f);
+      const float tr = w.x * D.y + w.y * D.x, ti = -(w.x * D.x - w.y * D.y);
+      out[q] = make_float2(0.5f * fdt * (S.x + tr), 0.5f * fdt * (S.y + ti));
+    }
+  };
   for (int sidx = blockIdx.x; sidx < n_sft; sidx += gridDim.x) {
     const double *seg = x + (size_t)sidx * n;
     dif_pass<4, true>(z, seg, W, m, n, m >> 1, threadIdx.x, blockDim.x);
@@ -269,23 +290,12 @@ __global__ void __launch_bounds__(256, 3) sft_rfft_lowband_kernel(const double *
       const float2 u = TM[j];
       sM.x = fmaf(v.x, u.x, fmaf(-v.y, u.y, sM.x)); sM.y = fmaf(v.x, u.y, fmaf(v.y, u.x, sM.y));
     }
-    __syncthreads();                                   // every block has been read: the array now takes the results
-    // (slot q of the band is kept at q ^ (q >> 4): the threads of a warp hold residues that differ in their high bits only)
-    if (hasA) z[(kA - k_lo) ^ ((kA - k_lo) >> 4)] = sA;                 // Z[k]
-    if (hasM) z[256 + ((kM - k_lo) ^ ((kM - k_lo) >> 4))] = sM;         // Z[m - k]
+    if (!PADRES) __syncthreads();                      // every block has been read: the array now takes the results
+    if (hasA) z[slot((kA - k_lo) ^ ((kA - k_lo) >> 4))] = sA;                 // Z[k]
+    if (hasM) z[slot(256 + ((kM - k_lo) ^ ((kM - k_lo) >> 4)))] = sM;         // Z[m - k]
     __syncthreads();
-    float2 *out = bins + (size_t)sidx * nb;
-    for (int q = threadIdx.x; q < nb; q += blockDim.x) {
-      const int k = k_lo + q;
-      const float2 A = z[q ^ (q >> 4)], Bc = z[256 + (q ^ (q >> 4))];
-      const float2 Bv = make_float2(Bc.x, -Bc.y);                 // conj Z[m-k]
-      const float2 S = make_float2(A.x + Bv.x, A.y + Bv.y), D = make_float2(A.x - Bv.x, A.y - Bv.y);
-      float2 w;                                                  // w^k, k <= m = n/2
-      if (k < m) w = __ldg(W + k); else w = make_float2(-1.f, 0.f);
-      const float tr = w.x * D.y + w.y * D.x, ti = -(w.x * D.x - w.y * D.y);
-      out[q] = make_float2(0.5f * fdt * (S.x + tr), 0.5f * fdt * (S.y + ti));
-    }
-    __syncthreads();                                   // the work array is reused by the next segment
+    read_out(sidx);
+    if (!PADRES) __syncthreads();                      // the work array is reused by the next segment
   }
 }
 
