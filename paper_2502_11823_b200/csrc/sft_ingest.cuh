@@ -240,7 +240,13 @@ __global__ void __launch_bounds__(256, 3) sft_rfft_lowband_kernel(const double *
     T[t] = (e & (B / 2)) ? make_float2(-w.x, -w.y) : w;
   }
   // the outputs asked of this thread's block (the same for every segment)
-  const int b = threadIdx.x, r = (int)(__brev((unsigned)b) >> 24);
+  // Block b of this thread: for B >= 16 one of the 32 blocks that its own warp writes in the second pass (B = 32: warp w
+  // transforms the 512-point chunks w and w + 8 = blocks 16 w .. 16 w + 15 and 16 (w + 8) ..; B = 16: chunks 2 w, 2 w + 1 =
+  // blocks 32 w .. 32 w + 31), so that the sums need a __syncwarp() after that pass, not a block-wide barrier.
+  constexpr bool WARP_LOCAL = LOG2B >= 4;
+  const int lane_ = threadIdx.x & 31, warp_ = threadIdx.x >> 5;
+  const int b = LOG2B == 5 ? 16 * (warp_ + 8 * (lane_ >> 4)) + (lane_ & 15) : (int)threadIdx.x;
+  const int r = (int)(__brev((unsigned)b) >> 24);
   const int kA = k_lo + ((r - k_lo) & 255), kM = k_lo + ((-r - k_lo) & 255);       // band bins with k = r, m - k = r (mod 256)
   const bool hasA = kA < k_hi, hasM = kM < k_hi;
   const float2 *TA = T + (((kA >> 8) - a0) & 1) * B, *TM = T + (2 + ((((m - kM) >> 8) - c0) & 1)) * B;
@@ -275,7 +281,7 @@ __global__ void __launch_bounds__(256, 3) sft_rfft_lowband_kernel(const double *
     __syncthreads();
     SFT_PF(0, n * 4);                                  // first half of this block's next segment -> L2 (see SFT_PF)
     dif16_table_pass<LOG2B>(z, T2, m, threadIdx.x, blockDim.x);
-    __syncthreads();
+    if (WARP_LOCAL) __syncwarp(); else __syncthreads();
     SFT_PF(n / 2, n * 4);                              // second half
     float2 sA = make_float2(0.f, 0.f), sM = sA;
 #pragma unroll
