@@ -256,11 +256,19 @@ __global__ void __launch_bounds__(256, 3) sft_rfft_lowband_kernel(const double *
   __syncthreads();
   // Results: slot p = q ^ (q >> 4) for band offset q (the threads of a warp hold residues that differ in their high bits
   // only), the mirror sums 256 slots further.  With m/16 >= 512 the slots are the padding entries of the work array (index
-  // 17 p + 16), which no pass ever touches: no barrier before the result write and none after the read-out (three barriers
-  // per segment instead of five: 0.283 -> 0.276 ms).  Smaller transforms keep the results in the first 512 entries, between
-  // two extra barriers.  (Deferring the read-out of segment s to just after the first barrier of the block's next segment
-  // saves the third barrier as well; measured the same, 0.277 ms, so not kept.)
+  // 17 p + 16), which no pass ever touches, and the read-out of segment s (split + store of the band) is deferred to just
+  // after the first barrier of the block's next segment, which already orders it after every thread's result write.  The
+  // opposite order - no thread may overwrite the slots before every thread has read them - is kept by an mbarrier on which
+  // all threads arrive after their read-out and wait before their next result write; that wait is over long before it is
+  // reached (a second pass and the block sums lie in between).  One block-wide barrier per segment is left, after the first
+  // pass (five before: 0.283 -> 0.266 ms).  Smaller transforms keep the results in the first 512 entries, between barriers.
   constexpr bool PADRES = m / 16 >= 512;
+  __shared__ unsigned long long bar_mem;
+  const unsigned bar_s = (unsigned)__cvta_generic_to_shared(&bar_mem);
+  if (PADRES && threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared.b64 [%0], %1;" ::"r"(bar_s), "r"(256) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
   auto slot = [](int p) { return PADRES ? 17 * p + 16 : p; };
   auto read_out = [&](int sdone) {
     float2 *out = bins + (size_t)sdone * nb;
@@ -275,11 +283,18 @@ __global__ void __launch_bounds__(256, 3) sft_rfft_lowband_kernel(const double *
       out[q] = make_float2(0.5f * fdt * (S.x + tr), 0.5f * fdt * (S.y + ti));
     }
   };
+  int pending = -1;                                    // PADRES: segment whose results wait in the padding entries
+  unsigned phase = 0;                                  // parity of the mbarrier phase to wait for
   for (int sidx = blockIdx.x; sidx < n_sft; sidx += gridDim.x) {
     const double *seg = x + (size_t)sidx * n;
     dif_pass<4, true>(z, seg, W, m, n, m >> 1, threadIdx.x, blockDim.x);
     __syncthreads();
     SFT_PF(0, n * 4);                                  // first half of this block's next segment -> L2 (see SFT_PF)
+    if (PADRES) {
+      // read-out of the block's previous segment: this barrier already orders it after every thread's result write
+      if (pending >= 0) read_out(pending);
+      asm volatile("{ .reg .b64 t; mbarrier.arrive.shared.b64 t, [%0]; }" ::"r"(bar_s) : "memory");   // "I have read the results"
+    }
     dif16_table_pass<LOG2B>(z, T2, m, threadIdx.x, blockDim.x);
     if (WARP_LOCAL) __syncwarp(); else __syncthreads();
     SFT_PF(n / 2, n * 4);                              // second half
@@ -297,11 +312,27 @@ __global__ void __launch_bounds__(256, 3) sft_rfft_lowband_kernel(const double *
       sM.x = fmaf(v.x, u.x, fmaf(-v.y, u.y, sM.x)); sM.y = fmaf(v.x, u.y, fmaf(v.y, u.x, sM.y));
     }
     if (!PADRES) __syncthreads();                      // every block has been read: the array now takes the results
+    if (PADRES) {                                      // every thread has read the previous results (long ago, as a rule)
+      unsigned ok;
+      do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(bar_s), "r"(phase) : "memory");
+      } while (!ok);
+      phase ^= 1u;
+    }
     if (hasA) z[slot((kA - k_lo) ^ ((kA - k_lo) >> 4))] = sA;                 // Z[k]
     if (hasM) z[slot(256 + ((kM - k_lo) ^ ((kM - k_lo) >> 4)))] = sM;         // Z[m - k]
+    if (PADRES) {
+      pending = sidx;
+    } else {
+      __syncthreads();
+      read_out(sidx);
+      __syncthreads();                                 // the work array is reused by the next segment
+    }
+  }
+  if (PADRES && pending >= 0) {
     __syncthreads();
-    read_out(sidx);
-    if (!PADRES) __syncthreads();                      // the work array is reused by the next segment
+    read_out(pending);
   }
 }
 
