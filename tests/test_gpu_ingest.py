@@ -32,7 +32,8 @@ def _check_bins(g, o, tol):
 # bins; 257 bins (back to the full transform); more segments than resident blocks (persistent loop).
 @pytest.mark.parametrize("n,n_sft,k_lo,k_hi", [(4096, 19, 48, 168), (16384, 5, 7, 219), (64, 33, 0, 33), (1024, 3, 500, 513),
                                                (8192, 7, 1, 257), (16384, 4, 3000, 3200), (16384, 3, 7936, 8192),
-                                               (4096, 5, 1900, 2048), (16384, 2, 200, 457), (16384, 450, 5, 187)])
+                                               (4096, 5, 1900, 2048), (16384, 2, 200, 457), (16384, 450, 5, 187),
+                                               (16384, 1, 100, 101), (16384, 889, 255, 258)])
 def test_fft_path_matches_direct_dft(n, n_sft, k_lo, k_hi):
     api = _api()
     rng = np.random.default_rng(n + n_sft)
