@@ -89,9 +89,8 @@ struct KParams {
   int *kc_out;             // [nT][C][n_sft] or null
   // cumulative mode (MODE 1): single-pass scan over the SFT axis with decoupled look-back (one work unit = 32 SFT slots)
   float *out_snr, *out_cx, *out_ch;   // [nT][n_sft] outputs, each nullable
-  double2 *scanA, *scanP;  // [n_chunks][nT] {xh, hh}: a unit's own totals (aggregate) / totals of all SFTs up to its end (inclusive)
-  unsigned *flagA, *flagP; // [n_chunks][nT]: == epoch once the entry of this call has been published
-  unsigned epoch;
+  double2 *scanA, *scanP;  // [n_chunks][nT] {xh, hh} + tag: a unit's own totals (aggregate) / totals of all SFTs up to its end (inclusive)
+  unsigned epoch;          // 16-bit tag (1 ... 65534) carried by every entry published in this call (scan_publish)
 #ifdef SFT_CHECKED
   // checked build (build.py --checked): every indexed global access of the main path is tested against the extent of
   // its buffer (entries, counted in the pointer's element type); the first failing site leaves its code in *chk and the
@@ -1359,13 +1358,25 @@ __device__ __forceinline__ void finish_fast(const KParams &p, const Tmpl &tm, co
 //      k the walk stopped at (run-to-run deterministic); publish carry + own totals as this unit's inclusive totals;
 //   4. store carry + local prefix (carry split into hi + lo floats: <= 1 ulp of the fp32 output) transposed, as 128-byte rows
 //      along the SFT axis, and snr = cum_xh / sqrt(cum_hh) (0 where cum_hh == 0).
-__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *q) {
-  unsigned v;
-  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(q) : "memory");
-  return v;
+// Records: a published entry is ONE 16-byte word {xh, hh} written and read by single 128-bit accesses, with the 16-bit
+// epoch of the call in the low 8 mantissa bits of each double (2^-45 relative: invisible in the fp32 outputs).  A reader that
+// finds the tag has the values, so no fence orders "data before flag" - a release fence here would wait for the 128 KB of
+// output stores of the warp's previous unit to drain, 12 % of the kernel's stall samples when it was there.  Every sum is
+// truncated to the 44-bit mantissa again (scan_trunc) so that a stored value equals the value its writer went on with.
+__device__ __forceinline__ double scan_trunc(double v) {
+  return __longlong_as_double(__double_as_longlong(v) & ~0xffll);
 }
-__device__ __forceinline__ void st_release_u32(unsigned *q, unsigned v) {
-  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(q), "r"(v) : "memory");
+__device__ __forceinline__ void scan_publish(double2 *q, double xh, double hh, unsigned epoch) {      // xh, hh truncated
+  const unsigned long long lo = (unsigned long long)__double_as_longlong(xh) | (epoch & 0xffu);
+  const unsigned long long hi = (unsigned long long)__double_as_longlong(hh) | ((epoch >> 8) & 0xffu);
+  asm volatile("{ .reg .b128 q; mov.b128 q, {%1, %2}; st.relaxed.gpu.global.b128 [%0], q; }" ::"l"(q), "l"(lo), "l"(hi) : "memory");
+}
+__device__ __forceinline__ bool scan_read(const double2 *q, unsigned epoch, double &xh, double &hh) {
+  unsigned long long lo, hi;
+  asm volatile("{ .reg .b128 q; ld.relaxed.gpu.global.b128 q, [%2]; mov.b128 {%0, %1}, q; }" : "=l"(lo), "=l"(hi) : "l"(q) : "memory");
+  xh = __longlong_as_double((long long)(lo & ~0xffull));
+  hh = __longlong_as_double((long long)(hi & ~0xffull));
+  return (unsigned)((lo & 0xffu) | ((hi & 0xffu) << 8)) == epoch;
 }
 __device__ __forceinline__ void scan_store(const KParams &p, float *txh, float *thh, int tg, int ch, int n, int lane, long long t,
                                            double axh, double ahh, unsigned smask) {
@@ -1375,25 +1386,22 @@ __device__ __forceinline__ void scan_store(const KParams &p, float *txh, float *
   if (ok) {
     const size_t me = (size_t)ch * nT + (size_t)t;
     SFT_CHK(p, me < p.n_scan, CHK_SCAN);
-    p.scanA[me] = make_double2(axh, ahh);
-    st_release_u32(p.flagA + me, p.epoch);
+    axh = scan_trunc(axh);
+    ahh = scan_trunc(ahh);
+    scan_publish(p.scanA + me, axh, ahh, p.epoch);
     int k = ch - 1;
+    double vx, vh;
     while (k >= 0) {
       const size_t e = (size_t)k * nT + (size_t)t;
-      if (ld_acquire_u32(p.flagP + e) == p.epoch) break;
-      if (ld_acquire_u32(p.flagA + e) == p.epoch) { --k; continue; }
+      if (scan_read(p.scanP + e, p.epoch, vx, vh)) { cx = vx; chh = vh; break; }
+      if (scan_read(p.scanA + e, p.epoch, vx, vh)) { --k; continue; }
       __nanosleep(64);
     }
-    if (k >= 0) {
-      const double2 v = __ldcg(p.scanP + (size_t)k * nT + (size_t)t);
-      cx = v.x; chh = v.y;
+    for (int j = k + 1; j < ch; ++j) {                  // (their tags were seen above: published, and written once per call)
+      scan_read(p.scanA + (size_t)j * nT + (size_t)t, p.epoch, vx, vh);
+      cx = scan_trunc(cx + vx); chh = scan_trunc(chh + vh);
     }
-    for (int j = k + 1; j < ch; ++j) {
-      const double2 v = __ldcg(p.scanA + (size_t)j * nT + (size_t)t);
-      cx += v.x; chh += v.y;
-    }
-    p.scanP[me] = make_double2(cx + axh, chh + ahh);
-    st_release_u32(p.flagP + me, p.epoch);
+    scan_publish(p.scanP + me, scan_trunc(cx + axh), scan_trunc(chh + ahh), p.epoch);
   }
   // carry of row r (hi + lo floats) comes from lane r
   const float xhi = (float)cx, xlo = (float)(cx - (double)xhi), hhi = (float)chh, hlo = (float)(chh - (double)hhi);

@@ -42,8 +42,8 @@ struct sft_plan {
   double *d_params = nullptr; size_t params_bytes = 0;
   void *d_out = nullptr; size_t out_bytes = 0;         // staging for host outputs
   void *h_pin = nullptr; size_t pin_bytes = 0;         // pinned host staging (params in, result vectors out)
-  void *scan = nullptr; size_t scan_bytes = 0;         // cumulative: look-back records {aggregate, inclusive} + flags per (unit, template)
-  unsigned epoch = 0;                                  // value of a published flag of the current cumulative call
+  void *scan = nullptr; size_t scan_bytes = 0;         // cumulative: look-back records {aggregate, inclusive} per (unit, template), 16 bytes each
+  unsigned epoch = 0;                                  // 16-bit tag of the entries published by the current cumulative call (1 ... 65534)
   double *td = nullptr; size_t td_bytes = 0;           // per-template constants (sft_tmpl_kernel)
   float *tf = nullptr; size_t tf_bytes = 0;
   float4 *mtab = nullptr;                              // [C][n_sft][n_node][4] data-moment table (sft_table.cuh), or null
@@ -906,10 +906,11 @@ static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t
   k.n_chunks = (k.n_sft + chunk - 1) / chunk;
   sft_status st = SFT_OK;
   if (cumulative) {
-    // look-back records: per (unit, template) two double2 and two flags.  A flag counts as published when it equals the
-    // epoch of this call, so nothing is cleared between calls; a fresh or regrown buffer is zeroed and the epoch restarts.
-    const size_t ent = (size_t)k.n_chunks * (size_t)nT, need = ent * (2 * sizeof(double2) + 2 * sizeof(unsigned));
-    if (p->scan_bytes < need || p->epoch == 0xffffffffu) {
+    // look-back records: per (unit, template) two 16-byte words {xh, hh} (aggregate, inclusive), each carrying the 16-bit tag
+    // of the call that wrote it (scan_publish), so nothing is cleared between calls; a fresh or regrown buffer is zeroed (tag 0
+    // is never used) and so is the buffer when the tag wraps.
+    const size_t ent = (size_t)k.n_chunks * (size_t)nT, need = ent * 2 * sizeof(double2);
+    if (p->scan_bytes < need || p->epoch >= 0xfffeu) {
       st = grow(p, &p->scan, &p->scan_bytes, need);
       if (st != SFT_OK) return st;
       CU(p, cudaMemsetAsync(p->scan, 0, p->scan_bytes, p->stream));
@@ -918,8 +919,6 @@ static sft_status prepare(sft_plan *p, int64_t nT, const double *params, int32_t
     p->epoch++;
     k.scanA = (double2 *)p->scan;
     k.scanP = k.scanA + ent;
-    k.flagA = (unsigned *)(k.scanP + ent);
-    k.flagP = k.flagA + ent;
     k.epoch = p->epoch;
 #ifdef SFT_CHECKED
     k.n_scan = ent;
