@@ -447,7 +447,7 @@ NCU_TRAFFIC = {
     ("config2-F", "auto"): (2.104832e6 + 84.48e3, "profiles/r02_main_kernel.md"),
     ("config2-F", "table"): (2.104832e6 + 84.48e3, "profiles/r02_main_kernel.md"),
     ("config2-F", "direct"): (8.213504e6 + 10.752e3, "profiles/r01d_kernel_v7_tables.md"),
-    ("config3-F", "auto"): (6.057728e6 + 872.374272e6, "profiles/r02_main_kernel.md"),
+    ("config3-F", "auto"): (14.8288e6 + 830.107904e6, "profiles/r02_main_kernel.md"),
     ("config4", "auto"): (6.319616e6 + 229.888e3, "profiles/r02_main_kernel.md"),
 }
 

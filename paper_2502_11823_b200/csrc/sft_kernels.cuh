@@ -1360,7 +1360,7 @@ __device__ __forceinline__ void finish_fast(const KParams &p, const Tmpl &tm, co
 //      along the SFT axis, and snr = cum_xh / sqrt(cum_hh) (0 where cum_hh == 0).
 // Records: a published entry is ONE 16-byte word {xh, hh} written and read by single 128-bit accesses, with the 16-bit
 // epoch of the call in the low 8 mantissa bits of each double (2^-45 relative: invisible in the fp32 outputs).  A reader that
-// finds the tag has the values, so no fence orders "data before flag" - a release fence here would wait for the 128 KB of
+// finds the tag has the values, so no fence orders "data before flag" - a release fence here would wait for the 4 to 12 KB of
 // output stores of the warp's previous unit to drain, 12 % of the kernel's stall samples when it was there.  Every sum is
 // truncated to the 44-bit mantissa again (scan_trunc) so that a stored value equals the value its writer went on with.
 __device__ __forceinline__ double scan_trunc(double v) {
