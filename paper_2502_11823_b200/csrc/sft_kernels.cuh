@@ -1580,12 +1580,17 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
   // 0.2599 -> 0.2528 ms, config 3 1.2405 -> 1.2166 ms.  (MODE 1: the look-back of scan_store stays free of deadlock - a unit
   // waits only for units with smaller numbers, a warp's current unit has a smaller number than the one it holds in reserve,
   // so the smallest unpublished unit is always some warp's current unit, or the reserve of a warp that has already
-  // published its current one.)
+  // published its current one.)  Single-channel variants only: the others sit at the register cap, and the extra live
+  // register costs more in spills than the hidden latency returns (config 4, 2 channels: 0.4686 -> 0.4724 ms with it).
+  constexpr bool PRECLAIM = CT == 1;
   int nxt = 0;
-  if (lane == 0) nxt = atomicAdd(p.counter, 1);
+  if (PRECLAIM && lane == 0) nxt = atomicAdd(p.counter, 1);
   for (;;) {
     int item = nxt;
-    if (lane == 0) nxt = atomicAdd(p.counter, 1);
+    if (lane == 0) {
+      if (PRECLAIM) nxt = atomicAdd(p.counter, 1);
+      else item = atomicAdd(p.counter, 1);
+    }
     item = __shfl_sync(0xffffffffu, item, 0);
     if (item >= p.n_items) break;
     // MODE 0: latest (most expensive) chunks first; MODE 1: ascending, as the look-back of scan_store needs
