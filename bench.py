@@ -444,10 +444,10 @@ def run_ours(args, rank, world, local_rank):
 # DRAM bytes (read + write) of one main-kernel launch, from the committed ncu --set full captures (dram__bytes_read.sum +
 # dram__bytes_write.sum): NOT measured by this run - the source capture is named in roofline.traffic_source.
 NCU_TRAFFIC = {
-    ("config2-F", "auto"): (2.104832e6 + 84.48e3, "profiles/r02_main_kernel.md"),
-    ("config2-F", "table"): (2.104832e6 + 84.48e3, "profiles/r02_main_kernel.md"),
+    ("config2-F", "auto"): (2.103808e6 + 75.008e3, "profiles/r02_main_kernel.md"),
+    ("config2-F", "table"): (2.103808e6 + 75.008e3, "profiles/r02_main_kernel.md"),
     ("config2-F", "direct"): (8.213504e6 + 10.752e3, "profiles/r01d_kernel_v7_tables.md"),
-    ("config3-F", "auto"): (14.8288e6 + 830.107904e6, "profiles/r02_main_kernel.md"),
+    ("config3-F", "auto"): (38.722304e6 + 831.203584e6, "profiles/r02_main_kernel.md"),
     ("config4", "auto"): (6.319616e6 + 229.888e3, "profiles/r02_main_kernel.md"),
 }
 
