@@ -68,7 +68,8 @@ struct KParams {
   long long nT;
   int chunk, n_chunks;
   int n_tgroups, n_items;  // work units: n_tgroups = ceil(nT/32) template groups x n_chunks
-  int *counter;            // work-unit counter (zeroed before every launch)
+  int *counter;            // work-unit counter (zeroed before every launch): units first_dyn, first_dyn + 1, ... are drawn from it
+  int first_dyn;           // = warps of the grid: warp w of the grid starts on unit w without asking (set by launch_variant)
   unsigned long long *path_counts;   // nullable [PATH_N]: active pairs per evaluator path (diagnostic)
   // moment-table evaluator (sft_table.cuh); mtab == nullptr: direct evaluator only
   const float4 *mtab;      // [C][n_sft][n_node][4]   8 complex64 moments per node, node = kcidx * TAB_R + cell
@@ -1582,15 +1583,18 @@ __global__ void __launch_bounds__(TILE, MINB) sft_main_kernel(const KParams p) {
   // so the smallest unpublished unit is always some warp's current unit, or the reserve of a warp that has already
   // published its current one.)  Single-channel variants only: the others sit at the register cap, and the extra live
   // register costs more in spills than the hidden latency returns (config 4, 2 channels: 0.4686 -> 0.4724 ms with it).
+  // The first unit of every warp is its own number in the grid - no atomic: 2368 warps asking one address at the start of
+  // the kernel cost ~5 us.
   constexpr bool PRECLAIM = CT == 1;
-  int nxt = 0;
-  if (PRECLAIM && lane == 0) nxt = atomicAdd(p.counter, 1);
+  int nxt = (int)blockIdx.x * (TILE / 32) + warp;
+  bool first = true;
   for (;;) {
     int item = nxt;
     if (lane == 0) {
-      if (PRECLAIM) nxt = atomicAdd(p.counter, 1);
-      else item = atomicAdd(p.counter, 1);
+      if (PRECLAIM) nxt = p.first_dyn + atomicAdd(p.counter, 1);
+      else if (!first) item = p.first_dyn + atomicAdd(p.counter, 1);
     }
+    first = false;
     item = __shfl_sync(0xffffffffu, item, 0);
     if (item >= p.n_items) break;
     // MODE 0: latest (most expensive) chunks first; MODE 1: ascending, as the look-back of scan_store needs

@@ -50,7 +50,9 @@ static void launch_variant(const Ctx &c, const sftk::KParams &k) {
   long long blocks = (long long)c.n_sm * per_sm;
   const long long need = ((long long)k.n_items + sftk::TILE / 32 - 1) / (sftk::TILE / 32);
   if (blocks > need) blocks = need;
-  kern<<<(unsigned)blocks, sftk::TILE, 0, c.stream>>>(k);
+  sftk::KParams kk = k;
+  kk.first_dyn = (int)blocks * (sftk::TILE / 32);      // units 0 .. first_dyn - 1 belong to the grid's warps, the rest to the counter
+  kern<<<(unsigned)blocks, sftk::TILE, 0, c.stream>>>(kk);
 }
 
 // One per translation unit: launches and returns true if the unit holds the variant for `key`.
